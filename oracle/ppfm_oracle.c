@@ -1,0 +1,475 @@
+/*
+ * ppfm_oracle.c — plain FP64 CPU oracle for the Probe-Particle hot path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * `--impl reference` legs may build, load or call this file.  It shares no code, header, table or helper with
+ * the CUDA path under paper_2401_14564_b200/csrc/ and includes nothing from include/.
+ *
+ * Written from the paper (citations are /root/reference/PAPER.md lines) and the readings S1-S20 listed in
+ * DESIGN.md.  Deliberately slow and literal: no blocking, no fusion, no reordering beyond what the definition
+ * states.  The only parallelism is `#pragma omp parallel for` over independent outputs (grid points, pixels;
+ * PAPER.md:266, 280 "perfectly parallelizable", "pixels virtually independent"); sums run in the stated order.
+ *
+ *   O1  mixing rules
+ *   O2  LJ + Coulomb pair terms          PAPER.md:82 (Eq.5), 93 (Eq.6), 76 (F = -grad E)
+ *   O3  grid projection, image sum
+ *   O4  tri-linear interpolation
+ *   O5  tip springs, total force         PAPER.md:45 (Eq.1), 51-54 (Eq.2)
+ *   O6  FIRE                             PAPER.md:262 (ref [7]; constants = reading S6)
+ *   O7  z-scan, warm start               PAPER.md:262 (reading S8)
+ *   O8  Fz read-out
+ *   O9  Giessibl df                      PAPER.md:64-66 (Eq.3; quadrature = reading S9)
+ *   O10 stability flag (Hessian)         north_star exemption; reading S14
+ *
+ * Pins: tests/test_oracle_pins.py (closed forms, invariants, brute force).  "Relaxed positions on the real
+ * configs" have no value printed in the paper: PARITY UNPINNED BY THE PAPER for that one item; it is pinned
+ * only by an independent Newton minimiser cross-check and by mirror symmetry.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define KE_EV_A 14.399645478 /* Coulomb constant k_e in eV*Å/e^2 (CODATA 2018), reading S4 */
+#define EVA2_TO_NM 16.02176634 /* 1 eV/Å^2 in N/m, reading S4 */
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O1 + O2: one atom's contribution at displacement D = p - (r_i + shift).
+ *   s = max(|D|^2, r_min^2)                                  (reading S3; identity outside the clamp)
+ *   u = (R0^2/s)^3,  E_LJ = E0 (u^2 - 2u)                    (Eq.5 with R0 = R_i + R_PP, E0 = sqrt(e_i e_PP))
+ *   F_LJ = -dE/dr * D/r = 12 E0 (u^2 - u)/s * D
+ *   E_C = k_e Q q_i / sqrt(s),  F_C = E_C / s * D            (Eq.6)
+ * ---------------------------------------------------------------------------------------------------------- */
+static void pair_terms(const double D[3], double R0, double E0, double keQq, double rmin2, double out[4]) {
+    double s = D[0] * D[0] + D[1] * D[1] + D[2] * D[2];
+    if (s < rmin2) s = rmin2;
+    double u = (R0 * R0 / s);
+    u = u * u * u;
+    double e_lj = E0 * (u * u - 2.0 * u);
+    double f_lj = 12.0 * E0 * (u * u - u) / s;
+    double e_c = keQq / sqrt(s);
+    double f_c = e_c / s;
+    double f = f_lj + f_c;
+    out[0] = f * D[0];
+    out[1] = f * D[1];
+    out[2] = f * D[2];
+    out[3] = e_lj + e_c;
+}
+
+/* O3: sample force field at one point p: images outer, atoms inner, plain double accumulation. */
+static void ff_at_point(const double p[3], int natoms, const double *xyzq, const int *type, const double *R,
+                        const double *e, const double *cell, const int *nimg, double R_pp, double e_pp,
+                        double Q_pp, double r_min, double out[4]) {
+    const double *a = cell, *b = cell + 3, *c = cell + 6;
+    double acc[4] = {0, 0, 0, 0};
+    for (int ia = -nimg[0]; ia <= nimg[0]; ia++)
+        for (int ib = -nimg[1]; ib <= nimg[1]; ib++)
+            for (int ic = -nimg[2]; ic <= nimg[2]; ic++) {
+                double sh[3];
+                for (int d = 0; d < 3; d++) sh[d] = ia * a[d] + ib * b[d] + ic * c[d];
+                for (int i = 0; i < natoms; i++) {
+                    int t = type[i];
+                    double R0 = R[t] + R_pp;           /* O1 */
+                    double E0 = sqrt(e[t] * e_pp);     /* O1 */
+                    double D[3], o[4];
+                    for (int d = 0; d < 3; d++) D[d] = p[d] - (xyzq[4 * i + d] + sh[d]);
+                    pair_terms(D, R0, E0, KE_EV_A * Q_pp * xyzq[4 * i + 3], r_min * r_min, o);
+                    for (int d = 0; d < 4; d++) acc[d] += o[d];
+                }
+            }
+    for (int d = 0; d < 4; d++) out[d] = acc[d];
+}
+
+/* Force field at arbitrary points (used by pins: finite-difference gradient etc.). */
+int oracle_ff_at_points(int natoms, const double *xyzq, const int *type, int ntypes, const double *R,
+                        const double *e, const double *cell, const int *nimg, double R_pp, double e_pp,
+                        double Q_pp, double r_min, int64_t npts, const double *pts, double *out) {
+    for (int i = 0; i < natoms; i++)
+        if (type[i] < 0 || type[i] >= ntypes) return -1;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < npts; m++)
+        ff_at_point(pts + 3 * m, natoms, xyzq, type, R, e, cell, nimg, R_pp, e_pp, Q_pp, r_min, out + 4 * m);
+    return 0;
+}
+
+/* O3: the grid.  point(i,j,k) = origin + i*step[0] + j*step[1] + k*step[2]; out[(k*ny + j)*nx + i][4].
+ * If idx != NULL only the `nidx` flat indices listed are evaluated and written densely to out[m][4]. */
+int oracle_forcefield(int natoms, const double *xyzq, const int *type, int ntypes, const double *R,
+                      const double *e, const double *cell, const int *nimg, double R_pp, double e_pp,
+                      double Q_pp, const double *origin, const double *step, const int *n, double r_min,
+                      int64_t nidx, const int64_t *idx, double *out) {
+    for (int i = 0; i < natoms; i++)
+        if (type[i] < 0 || type[i] >= ntypes) return -1;
+    int64_t nx = n[0], ny = n[1], nz = n[2];
+    int64_t total = idx ? nidx : nx * ny * nz;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < total; m++) {
+        int64_t flat = idx ? idx[m] : m;
+        int64_t i = flat % nx, j = (flat / nx) % ny, k = flat / (nx * ny);
+        double p[3];
+        for (int d = 0; d < 3; d++) p[d] = origin[d] + i * step[d] + j * step[3 + d] + k * step[6 + d];
+        ff_at_point(p, natoms, xyzq, type, R, e, cell, nimg, R_pp, e_pp, Q_pp, r_min, out + 4 * m);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * Grid view used by O4..O10.
+ * ---------------------------------------------------------------------------------------------------------- */
+typedef struct {
+    const void *ff;  /* [nz][ny][nx][4] */
+    int is_f32;      /* 1: float data, widened to double on access (GPU-produced grids) */
+    double origin[3];
+    double Minv[9];  /* t = Minv * (r - origin), fractional grid coordinates */
+    int n[3];
+    int periodic[3];
+} grid_view;
+
+static double ff_get(const grid_view *g, int i, int j, int k, int comp) {
+    size_t o = (((size_t)k * g->n[1] + j) * g->n[0] + i) * 4 + comp;
+    return g->is_f32 ? (double)((const float *)g->ff)[o] : ((const double *)g->ff)[o];
+}
+
+static int invert3(const double *S /* rows = step vectors */, double *Minv) {
+    /* r - origin = S^T t  ->  t = (S^T)^-1 (r - origin).  Build A = S^T and invert by cofactors. */
+    double A[9];
+    for (int r = 0; r < 3; r++)
+        for (int c = 0; c < 3; c++) A[3 * r + c] = S[3 * c + r];
+    double det = A[0] * (A[4] * A[8] - A[5] * A[7]) - A[1] * (A[3] * A[8] - A[5] * A[6]) +
+                 A[2] * (A[3] * A[7] - A[4] * A[6]);
+    if (det == 0.0 || !isfinite(det)) return -1;
+    double id = 1.0 / det;
+    Minv[0] = (A[4] * A[8] - A[5] * A[7]) * id;
+    Minv[1] = (A[2] * A[7] - A[1] * A[8]) * id;
+    Minv[2] = (A[1] * A[5] - A[2] * A[4]) * id;
+    Minv[3] = (A[5] * A[6] - A[3] * A[8]) * id;
+    Minv[4] = (A[0] * A[8] - A[2] * A[6]) * id;
+    Minv[5] = (A[2] * A[3] - A[0] * A[5]) * id;
+    Minv[6] = (A[3] * A[7] - A[4] * A[6]) * id;
+    Minv[7] = (A[1] * A[6] - A[0] * A[7]) * id;
+    Minv[8] = (A[0] * A[4] - A[1] * A[3]) * id;
+    return 0;
+}
+
+static int make_view(grid_view *g, const void *ff, int is_f32, const double *origin, const double *step,
+                     const int *n, const int *periodic) {
+    g->ff = ff;
+    g->is_f32 = is_f32;
+    for (int d = 0; d < 3; d++) {
+        g->origin[d] = origin[d];
+        g->n[d] = n[d];
+        g->periodic[d] = periodic[d];
+        if (n[d] < 2) return -1;
+    }
+    return invert3(step, g->Minv);
+}
+
+/* O4: cell index pair (i0,i1) and fraction f along one axis.
+ *   periodic:      i0 = floor(t) mod n, i1 = (i0+1) mod n, f = t - floor(t)
+ *   non-periodic:  t clamped to [0, n-1]; i0 = min(floor(t), n-2); i1 = i0+1; f = t - i0     (reading S12)
+ * returns 1 if the coordinate was clamped. */
+static int axis_cell(double t, int n, int periodic, int *i0, int *i1, double *f) {
+    if (periodic) {
+        double fl = floor(t);
+        long m = (long)fl % n;
+        if (m < 0) m += n;
+        *i0 = (int)m;
+        *i1 = (int)((m + 1) % n);
+        *f = t - fl;
+        return 0;
+    }
+    int clamped = 0;
+    if (t < 0.0) { t = 0.0; clamped = 1; }
+    if (t > (double)(n - 1)) { t = (double)(n - 1); clamped = 1; }
+    int i = (int)floor(t);
+    if (i > n - 2) i = n - 2;
+    *i0 = i;
+    *i1 = i + 1;
+    *f = t - (double)i;
+    return clamped;
+}
+
+/* O4: F_S(r) = sum over 8 corners of w * FF.xyz.  If G != NULL also returns G[c][a] = dF_c/dt_a, the analytic
+ * derivative of the interpolant with respect to the fractional coordinates inside the current cell (for O10). */
+static int interp(const grid_view *g, const double r[3], double F[3], double G[9]) {
+    double t[3], f[3];
+    int i0[3], i1[3], clamped = 0;
+    for (int a = 0; a < 3; a++)
+        t[a] = g->Minv[3 * a] * (r[0] - g->origin[0]) + g->Minv[3 * a + 1] * (r[1] - g->origin[1]) +
+               g->Minv[3 * a + 2] * (r[2] - g->origin[2]);
+    for (int a = 0; a < 3; a++) clamped |= axis_cell(t[a], g->n[a], g->periodic[a], &i0[a], &i1[a], &f[a]);
+    for (int c = 0; c < 3; c++) F[c] = 0.0;
+    if (G) for (int m = 0; m < 9; m++) G[m] = 0.0;
+    for (int cz = 0; cz < 2; cz++)
+        for (int cy = 0; cy < 2; cy++)
+            for (int cx = 0; cx < 2; cx++) {
+                double wx = cx ? f[0] : 1.0 - f[0], wy = cy ? f[1] : 1.0 - f[1], wz = cz ? f[2] : 1.0 - f[2];
+                double sx = cx ? 1.0 : -1.0, sy = cy ? 1.0 : -1.0, sz = cz ? 1.0 : -1.0;
+                int i = cx ? i1[0] : i0[0], j = cy ? i1[1] : i0[1], k = cz ? i1[2] : i0[2];
+                for (int c = 0; c < 3; c++) {
+                    double v = ff_get(g, i, j, k, c);
+                    F[c] += wx * wy * wz * v;
+                    if (G) {
+                        G[3 * c + 0] += sx * wy * wz * v;
+                        G[3 * c + 1] += wx * sy * wz * v;
+                        G[3 * c + 2] += wx * wy * sz * v;
+                    }
+                }
+            }
+    return clamped;
+}
+
+int oracle_interp(const void *ff, int is_f32, const double *origin, const double *step, const int *n,
+                  const int *periodic, int64_t npts, const double *pts, double *out /* [npts][3] */) {
+    grid_view g;
+    if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
+    for (int64_t m = 0; m < npts; m++) interp(&g, pts + 3 * m, out + 3 * m, NULL);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O5: tip force (Eq.2) and total force (Eq.1).
+ *   d = r_PP - r_TIP;  F_R = -k_R (|d| - R0) d/|d|, R0 = |d0|;  F_L = -(k_x (d_x - d0_x), k_y (d_y - d0_y), 0)
+ * ---------------------------------------------------------------------------------------------------------- */
+typedef struct {
+    double k_lat[2], k_rad, d0[3], R_rest;
+} tip_t;
+
+static void radial_force(const tip_t *tp, const double d[3], double FR[3]) {
+    double L = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    for (int c = 0; c < 3; c++) FR[c] = (L > 0.0) ? -tp->k_rad * (L - tp->R_rest) * d[c] / L : 0.0;
+}
+
+static int total_force(const grid_view *g, const tip_t *tp, const double rtip[3], const double rpp[3],
+                       double F[3]) {
+    double d[3], FS[3], FR[3];
+    for (int c = 0; c < 3; c++) d[c] = rpp[c] - rtip[c];
+    int clamped = interp(g, rpp, FS, NULL);
+    radial_force(tp, d, FR);
+    F[0] = FS[0] + FR[0] - tp->k_lat[0] * (d[0] - tp->d0[0]);
+    F[1] = FS[1] + FR[1] - tp->k_lat[1] * (d[1] - tp->d0[1]);
+    F[2] = FS[2] + FR[2];
+    return clamped;
+}
+
+int oracle_total_force(const void *ff, int is_f32, const double *origin, const double *step, const int *n,
+                       const int *periodic, const double *k_lat, double k_rad, const double *d0,
+                       const double *rtip, const double *rpp, double *F) {
+    grid_view g;
+    if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
+    tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
+                sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2])};
+    total_force(&g, &tp, rtip, rpp, F);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O10: Hessian of the PP's total potential at r_PP:  H = H_spring - (J + J^T)/2,
+ *   J = dF_S/dr = G * Minv (chain rule through t = Minv (r - origin)),
+ *   H_spring = k_R dd^T/|d|^2 + k_R (|d|-R0)/|d| (I - dd^T/|d|^2) + diag(k_x, k_y, 0).
+ * Eigenvalues by cyclic Jacobi rotations (symmetric 3x3).
+ * ---------------------------------------------------------------------------------------------------------- */
+static void hessian(const grid_view *g, const tip_t *tp, const double rtip[3], const double rpp[3], double H[9]) {
+    double F[3], G[9], J[9], d[3];
+    interp(g, rpp, F, G);
+    for (int r = 0; r < 3; r++)
+        for (int c = 0; c < 3; c++) {
+            double s = 0.0;
+            for (int a = 0; a < 3; a++) s += G[3 * r + a] * g->Minv[3 * a + c];
+            J[3 * r + c] = s;
+        }
+    for (int c = 0; c < 3; c++) d[c] = rpp[c] - rtip[c];
+    double L = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    for (int r = 0; r < 3; r++)
+        for (int c = 0; c < 3; c++) {
+            double dd = d[r] * d[c] / (L * L);
+            double I = (r == c) ? 1.0 : 0.0;
+            H[3 * r + c] = tp->k_rad * dd + tp->k_rad * (L - tp->R_rest) / L * (I - dd) -
+                           0.5 * (J[3 * r + c] + J[3 * c + r]);
+        }
+    H[0] += tp->k_lat[0];
+    H[4] += tp->k_lat[1];
+}
+
+static void sym3_eig(const double Hin[9], double w[3]) {
+    double A[9];
+    memcpy(A, Hin, sizeof(A));
+    for (int sweep = 0; sweep < 60; sweep++) {
+        double off = A[1] * A[1] + A[2] * A[2] + A[5] * A[5];
+        if (off < 1e-300) break;
+        for (int p = 0; p < 2; p++)
+            for (int q = p + 1; q < 3; q++) {
+                double apq = A[3 * p + q];
+                if (apq == 0.0) continue;
+                double theta = (A[3 * q + q] - A[3 * p + p]) / (2.0 * apq);
+                double t = (theta >= 0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
+                for (int k = 0; k < 3; k++) { /* A <- A * R */
+                    double akp = A[3 * k + p], akq = A[3 * k + q];
+                    A[3 * k + p] = c * akp - s * akq;
+                    A[3 * k + q] = s * akp + c * akq;
+                }
+                for (int k = 0; k < 3; k++) { /* A <- R^T * A */
+                    double apk = A[3 * p + k], aqk = A[3 * q + k];
+                    A[3 * p + k] = c * apk - s * aqk;
+                    A[3 * q + k] = s * apk + c * aqk;
+                }
+            }
+    }
+    w[0] = A[0]; w[1] = A[4]; w[2] = A[8];
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2 - i; j++)
+            if (w[j] > w[j + 1]) { double t = w[j]; w[j] = w[j + 1]; w[j + 1] = t; }
+}
+
+int oracle_hessian(const void *ff, int is_f32, const double *origin, const double *step, const int *n,
+                   const int *periodic, const double *k_lat, double k_rad, const double *d0,
+                   const double *rtip, const double *rpp, double *H /* 9 */, double *eig /* 3 ascending */) {
+    grid_view g;
+    if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
+    tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
+                sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2])};
+    hessian(&g, &tp, rtip, rpp, H);
+    sym3_eig(H, eig);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O6 FIRE + O7 scan + O8 read-out + O10 flag.
+ *
+ * fire[7] = {dt0, dt_max, finc, fdec, alpha0, falpha, f_conv}.
+ * Pixel (ix,iy), step iz: r_TIP = p0 + ix*dx + iy*dy - (0,0,iz*dz).
+ * iz = 0: r_PP = r_TIP + d0.  iz > 0: r_PP shifted with the tip (d carried over), FIRE state reset.
+ * Outputs (dense over the selected pixels, [nz][npix]):
+ *   pos_fz[.][4] = (r_PP, Fz_tip = -F_R,z);  iters = moves made, -1 if max_iter moves did not converge;
+ *   lam_min = smallest Hessian eigenvalue at the relaxed point;  clamped = 1 if the final r_PP was clamped (S12).
+ * If pix != NULL only the `npix` flat pixel indices (iy*npx + ix) listed are computed.
+ * ---------------------------------------------------------------------------------------------------------- */
+static double norm3(const double v[3]) { return sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]); }
+
+int oracle_relax_scan(const void *ff, int is_f32, const double *origin, const double *step, const int *n,
+                      const int *periodic, const double *k_lat, double k_rad, const double *d0,
+                      const double *fire, int n_min, int max_iter, const double *p0, const double *dx,
+                      const double *dy, int npx, int npy, int nz, double dz, int64_t npix, const int64_t *pix,
+                      double *pos_fz, int *iters, double *lam_min, int *clamped_out) {
+    grid_view g;
+    if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
+    tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
+                sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2])};
+    const double dt0 = fire[0], dt_max = fire[1], finc = fire[2], fdec = fire[3], alpha0 = fire[4],
+                 falpha = fire[5], f_conv = fire[6];
+    int64_t total = pix ? npix : (int64_t)npx * npy;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t m = 0; m < total; m++) {
+        int64_t flat = pix ? pix[m] : m;
+        int ix = (int)(flat % npx), iy = (int)(flat / npx);
+        double dcur[3] = {tp.d0[0], tp.d0[1], tp.d0[2]}; /* O7: d carried from step to step */
+        for (int iz = 0; iz < nz; iz++) {
+            double rtip[3], r[3], v[3] = {0, 0, 0}, F[3];
+            for (int c = 0; c < 3; c++) rtip[c] = p0[c] + ix * dx[c] + iy * dy[c];
+            rtip[2] -= iz * dz;
+            for (int c = 0; c < 3; c++) r[c] = rtip[c] + dcur[c];
+            double dt = dt0, alpha = alpha0;
+            int n_pos = 0, moves = 0, converged = 0, cl = 0;
+            for (;;) { /* O6 */
+                cl = total_force(&g, &tp, rtip, r, F);
+                double Fn = norm3(F);
+                if (Fn < f_conv) { converged = 1; break; } /* S7: check before moving */
+                if (moves >= max_iter) break;
+                double P = F[0] * v[0] + F[1] * v[1] + F[2] * v[2];
+                if (P >= 0.0) { /* S6: P = 0 counts as downhill */
+                    double vn = norm3(v);
+                    for (int c = 0; c < 3; c++) v[c] = (1.0 - alpha) * v[c] + alpha * vn * F[c] / Fn;
+                    if (n_pos > n_min) {
+                        dt = fmin(dt * finc, dt_max);
+                        alpha *= falpha;
+                    }
+                    n_pos += 1;
+                } else {
+                    v[0] = v[1] = v[2] = 0.0;
+                    dt *= fdec;
+                    alpha = alpha0;
+                    n_pos = 0;
+                }
+                for (int c = 0; c < 3; c++) v[c] += F[c] * dt; /* semi-implicit Euler, m = 1 */
+                for (int c = 0; c < 3; c++) r[c] += v[c] * dt;
+                moves++;
+            }
+            for (int c = 0; c < 3; c++) dcur[c] = r[c] - rtip[c];
+            double FR[3];
+            radial_force(&tp, dcur, FR); /* O8: Fz_tip = -F_R,z */
+            size_t o = (size_t)iz * total + m;
+            pos_fz[4 * o + 0] = r[0];
+            pos_fz[4 * o + 1] = r[1];
+            pos_fz[4 * o + 2] = r[2];
+            pos_fz[4 * o + 3] = -FR[2];
+            if (iters) iters[o] = converged ? moves : -1;
+            if (clamped_out) clamped_out[o] = cl;
+            if (lam_min) {
+                double H[9], w[3];
+                hessian(&g, &tp, rtip, r, H);
+                sym3_eig(H, w);
+                lam_min[o] = w[0];
+            }
+        }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O9: Giessibl frequency shift, Eq.3, by exact product integration of the piecewise-linear interpolant of Fz.
+ *   a = A/2, n = A/dz (integer >= 1), nodes q_m = -a + m dz (m = 0..n);
+ *   y(q) = sqrt(a^2 - q^2), G(q) = (a^2/2) asin(q/a) - (q/2) y(q)      [ int q^2/y dq = G,  int q/y dq = -y ]
+ *   per interval j: I1 = y_j - y_{j+1} (= int q/y), I2 = G_{j+1} - G_j (= int q^2/y)
+ *     W_j += (q_{j+1} I1 - I2)/dz,  W_{j+1} += (I2 - q_j I1)/dz;  W *= 2/(pi a^2)
+ *   df_k = -(f0/(2 k0)) * 16.02176634 * sum_m W_m Fz(z_c + q_m);  sample index of z_c + q_m is k + n - m.
+ * ---------------------------------------------------------------------------------------------------------- */
+int oracle_df_weights(int n, double dz, double *W /* n+1 */) {
+    if (n < 1 || !(dz > 0.0)) return -1;
+    double a = 0.5 * n * dz;
+    for (int m = 0; m <= n; m++) W[m] = 0.0;
+    for (int j = 0; j < n; j++) {
+        double q0 = -a + j * dz, q1 = -a + (j + 1) * dz;
+        if (j == n - 1) q1 = a; /* exact end point */
+        double y0 = sqrt(fmax(a * a - q0 * q0, 0.0)), y1 = sqrt(fmax(a * a - q1 * q1, 0.0));
+        double G0 = 0.5 * a * a * asin(fmax(-1.0, fmin(1.0, q0 / a))) - 0.5 * q0 * y0;
+        double G1 = 0.5 * a * a * asin(fmax(-1.0, fmin(1.0, q1 / a))) - 0.5 * q1 * y1;
+        double I1 = y0 - y1, I2 = G1 - G0;
+        W[j] += (q1 * I1 - I2) / dz;
+        W[j + 1] += (I2 - q0 * I1) / dz;
+    }
+    for (int m = 0; m <= n; m++) W[m] *= 2.0 / (M_PI * a * a);
+    return 0;
+}
+
+int oracle_df(const double *fz /* [nz][npix] */, int64_t npix, int nz, double dz, double A, double k0 /* N/m */,
+              double f0 /* Hz */, double *df /* [nz-n][npix] */) {
+    double nn = A / dz;
+    int n = (int)llround(nn);
+    if (n < 1 || fabs(nn - n) > 1e-6 || nz <= n) return -1;
+    double *W = (double *)malloc((size_t)(n + 1) * sizeof(double));
+    if (!W) return -2;
+    oracle_df_weights(n, dz, W);
+    double pref = -(f0 / (2.0 * k0)) * EVA2_TO_NM;
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < npix; p++)
+        for (int k = 0; k < nz - n; k++) {
+            double s = 0.0;
+            for (int m = 0; m <= n; m++) s += W[m] * fz[(size_t)(k + n - m) * npix + p];
+            df[(size_t)k * npix + p] = pref * s;
+        }
+    free(W);
+    return 0;
+}

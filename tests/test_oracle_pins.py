@@ -1,0 +1,522 @@
+"""Pins for the FP64 CPU oracle (oracle/ppfm_oracle.c) against what the paper and the mathematics fix.
+
+The paper prints no worked numeric example, so every pin is a closed form, an invariant, a special
+case that reduces to a library routine (scipy trilinear map_coordinates, scipy quad, scipy Bessel I1, numpy
+eigvalsh), or brute force on tiny inputs.  Citations are /root/reference/PAPER.md lines.
+"""
+import os
+from dataclasses import replace
+
+import numpy as np
+import pytest
+from scipy import integrate, ndimage, special
+
+from oracle import oracle
+from paper_2401_14564_b200 import workloads as W
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "constants.txt")) as fh:
+    for line in fh:
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            GOLD[line[0]] = float(line[1])
+KE = GOLD["k_e_eV_A"]
+NM = GOLD["eVA2_in_Nm"]
+
+
+def one_atom(R=1.908, e=3.73e-3, q=0.0, Rpp=1.661, epp=9.11e-3, Q=0.0, pos=(0.0, 0.0, 0.0)):
+    w = W.get(0)
+    return replace(w, xyzq=np.array([[pos[0], pos[1], pos[2], q]], dtype=np.float32),
+                   types=np.array([0], dtype=np.int32), elem_R=np.array([R]), elem_e=np.array([e]),
+                   probe=W.Probe(R=Rpp, e=epp, Q=Q), r_min=1e-3)
+
+
+# ---------------------------------------------------------------------------------------------------- O1-O2 LJ
+def test_lj_minimum_depth_and_zero_crossing():
+    """Eq.5 + mixing: E(R0) = -E0, F(R0) = 0, E(R0 * 2^(-1/6)) = 0."""
+    R, e, Rpp, epp = 1.908, 3.73e-3, 1.661, 9.11e-3
+    w = one_atom(R, e, 0.0, Rpp, epp, 0.0)
+    R0, E0 = R + Rpp, np.sqrt(e * epp)
+    out = oracle.ff_at_points(w, [[0, 0, R0], [R0 * 2 ** (-1 / 6), 0, 0], [0, R0, 0]])
+    assert out[0, 3] == pytest.approx(-E0, rel=1e-14)
+    assert np.abs(out[0, :3]).max() < 1e-15
+    assert abs(out[1, 3]) < 1e-16
+    assert out[2, 3] == pytest.approx(-E0, rel=1e-14)
+
+
+def test_lj_radial_force_profile():
+    """-dE/dr of Eq.5: F_r = 12 E0 [(R0/r)^12 - (R0/r)^6] / r, along an oblique direction."""
+    R, e, Rpp, epp = 1.78, 3.04e-3, 1.661, 9.11e-3
+    w = one_atom(R, e, 0.0, Rpp, epp, 0.0, pos=(0.5, -0.25, 0.125))
+    R0, E0 = R + Rpp, np.sqrt(e * epp)
+    nhat = np.array([1.0, 2.0, -2.0]) / 3.0
+    for r in (2.0, 3.0, R0, 4.5, 7.0):
+        p = np.array([0.5, -0.25, 0.125]) + r * nhat
+        out = oracle.ff_at_points(w, [p])[0]
+        Fr = 12 * E0 * ((R0 / r) ** 12 - (R0 / r) ** 6) / r
+        assert np.allclose(out[:3], Fr * nhat, rtol=1e-12, atol=1e-15)
+        assert out[3] == pytest.approx(E0 * ((R0 / r) ** 12 - 2 * (R0 / r) ** 6), rel=1e-12, abs=1e-18)
+
+
+# ---------------------------------------------------------------------------------------------------- O2 Coulomb
+def test_coulomb_value_sign_and_inverse_square():
+    """Eq.6: E r = k_e Q q; F(2r) = F(r)/4; sign follows Q q; E(1 Å, Q=q=1) = 14.399645478 eV."""
+    w = one_atom(e=0.0, q=1.0, Q=1.0)      # e_i = 0 -> E0 = 0, pure Coulomb
+    out = oracle.ff_at_points(w, [[1, 0, 0], [2, 0, 0], [0, 0, 3]])
+    assert out[0, 3] == pytest.approx(KE, rel=1e-12)
+    assert out[0, 0] == pytest.approx(KE, rel=1e-12)           # repulsive: pushes +x
+    assert out[1, 0] == pytest.approx(out[0, 0] / 4, rel=1e-12)
+    assert out[2, 3] * 3 == pytest.approx(KE, rel=1e-12)
+    for Q, q in ((-1, 1), (1, -1)):
+        o = oracle.ff_at_points(one_atom(e=0.0, q=q, Q=Q), [[1, 0, 0]])[0]
+        assert o[0] == pytest.approx(-KE, rel=1e-12) and o[3] == pytest.approx(-KE, rel=1e-12)
+    o = oracle.ff_at_points(one_atom(e=0.0, q=-1, Q=-1), [[1, 0, 0]])[0]
+    assert o[0] == pytest.approx(KE, rel=1e-12)
+
+
+def test_rmin_clamp_is_identity_outside_and_finite_inside():
+    """Reading S3: s = max(r^2, r_min^2); direction from the unclamped displacement."""
+    w = replace(one_atom(q=0.3, Q=-0.05), r_min=0.5)
+    a = oracle.ff_at_points(w, [[0.6, 0, 0]], r_min=0.5)
+    b = oracle.ff_at_points(w, [[0.6, 0, 0]], r_min=1e-3)
+    assert np.array_equal(a, b)
+    c = oracle.ff_at_points(w, [[0, 0, 0], [0.1, 0, 0]], r_min=0.5)
+    assert np.all(np.isfinite(c)) and np.all(c[0, :3] == 0.0)
+    assert c[0, 3] == c[1, 3]                              # energy is flat inside the clamp
+
+
+# ---------------------------------------------------------------------------------------------------- F = -grad E
+def test_force_is_minus_gradient_of_energy_cfg0():
+    """F = -grad E, on the summed LJ + Coulomb field of config 0 at 100 random points."""
+    w = W.get(0)
+    rng = np.random.default_rng(7)
+    pts = np.c_[rng.uniform(0, 12, 100), rng.uniform(0, 12, 100), rng.uniform(2.0, 9.0, 100)]
+    F = oracle.ff_at_points(w, pts)[:, :3]
+    h = 1e-4
+    G = np.zeros_like(F)
+    for a in range(3):
+        dp = np.zeros(3)
+        dp[a] = h
+        Ep = oracle.ff_at_points(w, pts + dp)[:, 3]
+        Em = oracle.ff_at_points(w, pts - dp)[:, 3]
+        Epp = oracle.ff_at_points(w, pts + 2 * dp)[:, 3]
+        Emm = oracle.ff_at_points(w, pts - 2 * dp)[:, 3]
+        G[:, a] = -(8 * (Ep - Em) - (Epp - Emm)) / (12 * h)      # 4th-order central difference
+    err = np.linalg.norm(F - G, axis=1) / np.maximum(np.linalg.norm(F, axis=1), 1e-6)
+    assert err.max() < 1e-7
+
+
+# ---------------------------------------------------------------------------------------------------- O3 sums
+def test_brute_force_tiny_grid():
+    """3 atoms, 4x4x4 grid, independent triple loop written from Eq.5/Eq.6 in radial form."""
+    w = W.get(0)
+    w = replace(w, xyzq=np.array([[1.0, 1.5, 0.0, 0.2], [2.5, 0.5, -0.2, -0.3], [0.3, 2.2, 0.1, 0.1]], np.float32),
+                types=np.array([1, 3, 0], np.int32),
+                grid=W.Grid(origin=np.array([0.1, 0.2, 2.0]), step=np.diag([0.7, 0.8, 0.9]), n=(4, 4, 4),
+                            periodic=(0, 0, 0)))
+    ff = oracle.forcefield(w)
+    ref = np.zeros((4, 4, 4, 4))
+    for k in range(4):
+        for j in range(4):
+            for i in range(4):
+                p = np.array([0.1 + 0.7 * i, 0.2 + 0.8 * j, 2.0 + 0.9 * k])
+                for a in range(3):
+                    x, y, z, q = [float(v) for v in w.xyzq[a]]
+                    Rm = w.elem_R[w.types[a]] + w.probe.R
+                    em = np.sqrt(w.elem_e[w.types[a]] * w.probe.e)
+                    D = p - np.array([x, y, z])
+                    r = np.linalg.norm(D)
+                    rho = Rm / r
+                    dEdr = em * (-12 * rho ** 12 + 12 * rho ** 6) / r - KE * w.probe.Q * q / r ** 2
+                    ref[k, j, i, :3] += -dEdr * D / r
+                    ref[k, j, i, 3] += em * (rho ** 12 - 2 * rho ** 6) + KE * w.probe.Q * q / r
+    assert np.allclose(ff, ref, rtol=1e-12, atol=1e-16)
+
+
+def test_linearity_permutation_and_charge_linearity():
+    w = replace(W.shrink(W.get(0), grid_n=(12, 10, 6)))
+    ff = oracle.forcefield(w)
+    A = replace(w, xyzq=w.xyzq[:4], types=w.types[:4])
+    B = replace(w, xyzq=w.xyzq[4:], types=w.types[4:])
+    assert np.allclose(oracle.forcefield(A) + oracle.forcefield(B), ff, rtol=1e-12, atol=1e-15)
+    perm = np.random.default_rng(3).permutation(w.natoms)
+    assert np.allclose(oracle.forcefield(replace(w, xyzq=w.xyzq[perm], types=w.types[perm])), ff, rtol=1e-12,
+                       atol=1e-15)
+    f0, f1, f2 = (oracle.forcefield(w, Q=Q) for Q in (0.0, 0.1, 0.2))
+    assert np.allclose(f2 - f0, 2 * (f1 - f0), rtol=1e-10, atol=1e-15)       # el part linear in Q
+
+
+def test_image_sum_equals_explicit_replication():
+    """Periodic images: nimg = 1 equals the 9x replicated atom list with nimg = 0."""
+    w = W.get(2)
+    idx = W.sample_indices(w.npoints, 300, 11)
+    ref = oracle.forcefield(w, idx=idx)
+    reps, types = [], []
+    for ia in (-1, 0, 1):
+        for ib in (-1, 0, 1):
+            sh = ia * w.lattice.a + ib * w.lattice.b
+            x = w.xyzq.astype(np.float64).copy()
+            x[:, :3] += sh
+            reps.append(x)
+            types.append(w.types)
+    # replicated coordinates are exact in FP64 but not FP32 -> go through ff_at_points with float64 atoms
+    big = replace(w, lattice=replace(w.lattice, nimg=(0, 0, 0)))
+    nx, ny, nz = w.grid.n
+    i, j, k = idx % nx, (idx // nx) % ny, idx // (nx * ny)
+    pts = w.grid.origin + np.outer(i, w.grid.step[0]) + np.outer(j, w.grid.step[1]) + np.outer(k, w.grid.step[2])
+    tot = np.zeros((len(idx), 4))
+    for x, t in zip(reps, types):
+        # shift points instead of atoms (same displacement, atoms stay FP32-exact)
+        sh = x[0, :3] - w.xyzq[0, :3].astype(np.float64)
+        tot += oracle.ff_at_points(big, pts - sh)
+    assert np.allclose(tot, ref, rtol=1e-11, atol=1e-14)
+
+
+def test_mirror_symmetry():
+    """Mirror x -> -x about the plane through grid index (n-1)/2: (Fx,Fy,Fz,E) -> (-Fx,Fy,Fz,E) at mirrored i."""
+    w = W.shrink(W.get(0), grid_n=(21, 8, 5))
+    xm = w.grid.origin[0] + 0.5 * (w.grid.n[0] - 1) * w.grid.step[0, 0]
+    # choose coordinates for which the FP32 mirror image is exact: multiples of 1/64
+    x = np.round(w.xyzq.astype(np.float64) * 64) / 64
+    w = replace(w, xyzq=x.astype(np.float32), grid=replace(w.grid, origin=np.array([0.0, 0.0, 1.5])))
+    xm = 0.5 * (w.grid.n[0] - 1) * 0.2
+    xr = x.copy()
+    xr[:, 0] = 2 * xm - xr[:, 0]
+    assert np.array_equal(xr.astype(np.float32).astype(np.float64), xr)
+    a = oracle.forcefield(w)
+    b = oracle.forcefield(replace(w, xyzq=xr.astype(np.float32)))[:, :, ::-1, :]
+    assert np.allclose(a[..., 0], -b[..., 0], rtol=1e-9, atol=1e-13)
+    assert np.allclose(a[..., 1:], b[..., 1:], rtol=1e-9, atol=1e-13)
+
+
+def test_translation_of_atoms_and_origin():
+    """Translating atoms and grid origin by the same vector leaves the array unchanged."""
+    w = W.shrink(W.get(0), grid_n=(9, 7, 5))
+    x = np.round(w.xyzq.astype(np.float64) * 64) / 64
+    w = replace(w, xyzq=x.astype(np.float32))
+    t = np.array([0.5, -1.25, 0.75])
+    x2 = x.copy()
+    x2[:, :3] += t
+    w2 = replace(w, xyzq=x2.astype(np.float32), grid=replace(w.grid, origin=w.grid.origin + t))
+    assert np.allclose(oracle.forcefield(w), oracle.forcefield(w2), rtol=1e-10, atol=1e-14)
+
+
+def test_lattice_translation_invariance_lj_nimg4():
+    """Reading S18: with nimg = 4 and LJ only the truncated image sum is invariant (to < 1e-6) under moving one
+    atom by a lattice vector."""
+    w = W.get(2)
+    x = np.round(w.xyzq.astype(np.float64) * 64) / 64      # so that x + 25 stays exact in FP32
+    x[:, 3] = 0.0
+    w = replace(w, xyzq=x.astype(np.float32))
+    pts = np.array([[12.3, 11.9, 3.1], [2.0, 20.0, 3.5], [24.0, 1.0, 4.0]])
+    a = oracle.ff_at_points(w, pts, nimg=(4, 4, 0))
+    x = x.copy()
+    x[:60, 0] += 25.0                                   # move the molecule by +a
+    assert np.array_equal(x.astype(np.float32).astype(np.float64), x)
+    b = oracle.ff_at_points(replace(w, xyzq=x.astype(np.float32)), pts, nimg=(4, 4, 0))
+    assert np.allclose(a, b, rtol=1e-6, atol=1e-9)        # r^-6 tail of the dropped/added image row: ~2e-10 eV
+    c = oracle.ff_at_points(replace(w, xyzq=x.astype(np.float32)), pts, nimg=(0, 0, 0))
+    assert not np.allclose(a, c, rtol=1e-3, atol=1e-12)   # and the images do matter
+
+
+# ---------------------------------------------------------------------------------------------------- O4
+def _rand_grid(n=(7, 6, 5), periodic=(0, 0, 0), seed=0, h=(0.3, 0.25, 0.2), origin=(0.5, -0.2, 1.0)):
+    rng = np.random.default_rng(seed)
+    g = W.Grid(origin=np.array(origin), step=np.diag(h), n=n, periodic=periodic)
+    ff = rng.normal(size=(n[2], n[1], n[0], 4))
+    return g, ff
+
+
+def test_interp_matches_scipy_map_coordinates():
+    """Tri-linear interpolation == scipy.ndimage.map_coordinates(order=1), clamped and periodic."""
+    rng = np.random.default_rng(1)
+    for periodic, mode in (((0, 0, 0), "nearest"), ((1, 1, 1), "grid-wrap")):
+        g, ff = _rand_grid(periodic=periodic)
+        h = np.diag(g.step)
+        lo = -1.5 if periodic[0] else 0.0
+        t = np.c_[rng.uniform(lo, g.n[0] + (0.5 if periodic[0] else -1.0), 200),
+                  rng.uniform(lo, g.n[1] + (0.5 if periodic[0] else -1.0), 200),
+                  rng.uniform(lo, g.n[2] + (0.5 if periodic[0] else -1.0), 200)]
+        pts = g.origin + t * h
+        got = oracle.interp(ff, g, pts)
+        for c in range(3):
+            ref = ndimage.map_coordinates(ff[..., c], [t[:, 2], t[:, 1], t[:, 0]], order=1, mode=mode)
+            assert np.allclose(got[:, c], ref, rtol=1e-10, atol=1e-12)
+
+
+def test_interp_clamps_outside_nonperiodic():
+    g, ff = _rand_grid()
+    h = np.diag(g.step)
+    inside = g.origin + np.array([0.0, 2.3, 4.0]) * h
+    outside = g.origin + np.array([-3.0, 2.3, 9.0]) * h
+    assert np.allclose(oracle.interp(ff, g, [inside]), oracle.interp(ff, g, [outside]), atol=1e-14)
+
+
+def test_interp_affine_exact_and_nodes():
+    """An affine field sampled on the grid is reproduced exactly anywhere inside; nodes return node values.
+    Also with a non-orthogonal step matrix."""
+    rng = np.random.default_rng(2)
+    step = np.array([[0.3, 0.02, 0.0], [-0.05, 0.25, 0.01], [0.0, 0.03, 0.2]])
+    g = W.Grid(origin=np.array([0.5, -0.2, 1.0]), step=step, n=(6, 5, 7), periodic=(0, 0, 0))
+    M = rng.normal(size=(3, 3))
+    b = rng.normal(size=3)
+    k, j, i = np.meshgrid(np.arange(7), np.arange(5), np.arange(6), indexing="ij")
+    P = g.origin + i[..., None] * step[0] + j[..., None] * step[1] + k[..., None] * step[2]
+    ff = np.zeros((7, 5, 6, 4))
+    ff[..., :3] = P @ M.T + b
+    t = np.c_[rng.uniform(0, 5, 50), rng.uniform(0, 4, 50), rng.uniform(0, 6, 50)]
+    pts = g.origin + t @ step
+    assert np.allclose(oracle.interp(ff, g, pts), pts @ M.T + b, rtol=1e-11, atol=1e-12)
+    assert np.allclose(oracle.interp(ff, g, P[3, 2, 4][None]), ff[3, 2, 4, :3][None], atol=1e-12)
+
+
+def test_interp_periodic_seam():
+    g, ff = _rand_grid(periodic=(1, 1, 0))
+    h = np.diag(g.step)
+    t = np.array([g.n[0] - 0.25, 1.5, 2.5])              # between last and first node in x
+    got = oracle.interp(ff, g, [g.origin + t * h])[0]
+    f = lambda i: 0.25 * ff[2, 1, i, :3] + 0.25 * ff[2, 2, i, :3] + 0.25 * ff[3, 1, i, :3] + 0.25 * ff[3, 2, i, :3]
+    assert np.allclose(got, 0.25 * f(g.n[0] - 1) + 0.75 * f(0), atol=1e-13)
+    a = oracle.interp(ff, g, [g.origin + np.array([1.3, 2.2, 2.5]) * h])
+    b = oracle.interp(ff, g, [g.origin + np.array([1.3 + g.n[0], 2.2 - g.n[1], 2.5]) * h])
+    assert np.allclose(a, b, atol=1e-12)
+
+
+def test_f32_grid_is_widened_on_access():
+    g, ff = _rand_grid()
+    ff32 = ff.astype(np.float32)
+    pts = g.origin + np.array([[1.2, 2.3, 3.4]]) * np.diag(g.step)
+    assert np.array_equal(oracle.interp(ff32, g, pts), oracle.interp(ff32.astype(np.float64), g, pts))
+
+
+# ---------------------------------------------------------------------------------------------------- O5-O8
+def _flat_grid(n=(20, 20, 60), h=0.2, origin=(0.0, 0.0, 0.0)):
+    g = W.Grid(origin=np.array(origin, float), step=np.diag([h, h, h]), n=n, periodic=(0, 0, 0))
+    return g, np.zeros((n[2], n[1], n[0], 4))
+
+
+def _scan(npx=3, npy=2, nz=25, z0=9.0, dz=0.1):
+    return W.Scan(p0=np.array([1.0, 1.2, z0]), dx=np.array([0.3, 0, 0.0]), dy=np.array([0, 0.4, 0.0]), npx=npx,
+                  npy=npy, nz=nz, dz=dz)
+
+
+def test_zero_field_stays_at_spring_equilibrium():
+    """All-zero grid: r_PP = r_TIP + d0 exactly, 0 iterations, Fz = 0, df = 0 (Eq.2)."""
+    g, ff = _flat_grid()
+    tip, sc = W._default_tip(), _scan()
+    r = oracle.relax_scan(ff, g, tip, W.Fire(), sc)
+    assert np.all(r["iters"] == 0)
+    for iz in range(sc.nz):
+        for iy in range(sc.npy):
+            for ix in range(sc.npx):
+                want = sc.p0 + ix * sc.dx + iy * sc.dy - np.array([0, 0, iz * sc.dz]) + np.array(tip.d0)
+                assert np.array_equal(r["pos_fz"][iz, iy * sc.npx + ix, :3], want)
+    assert np.all(r["pos_fz"][..., 3] == 0.0)
+    assert np.all(oracle.df(r["pos_fz"][..., 3], sc.dz, 1.0, 1800.0, 30300.0) == 0.0)
+
+
+def test_uniform_field_closed_form_and_lateral_hessian():
+    """Uniform F_S = (0,0,f): |d| = R_rest - f/k_R, Fz_tip = f; lateral Hessian eigenvalue
+    k_xy - f/|d| (pins O10), including its sign change at f ~ k_xy R_rest."""
+    g, ff = _flat_grid()
+    tip = W._default_tip()
+    fire = replace(W.Fire(), f_conv=1e-11, max_iter=20000)
+    for f in (0.03, -0.02, 0.07):
+        ff[..., 2] = f
+        r = oracle.relax_scan(ff, g, tip, fire, _scan(nz=2))
+        L = 4.0 - f / tip.k_rad
+        d = r["pos_fz"][0, 0, :3] - _scan().p0
+        assert np.allclose(d, [0, 0, -L], atol=1e-8)
+        assert r["pos_fz"][0, 0, 3] == pytest.approx(f, abs=1e-9)
+        H, w = oracle.hessian(ff, g, tip, _scan().p0, r["pos_fz"][0, 0, :3])
+        lam_lat = tip.k_lat[0] - f / L
+        assert w[0] == pytest.approx(min(lam_lat, tip.k_rad), abs=1e-9)
+        assert r["lam_min"][0, 0] == pytest.approx(lam_lat, abs=1e-9)
+        assert np.allclose(w, np.linalg.eigvalsh(H), atol=1e-12)
+    assert tip.k_lat[0] - 0.07 / (4.0 - 0.07 / tip.k_rad) < 0 < tip.k_lat[0] - 0.03 / (4.0 - 0.03 / tip.k_rad)
+
+
+def test_linear_field_relax_plus_df_closed_form():
+    """F_S,z = g (z - z_c): Fz_tip = k_R g (z_t - R_rest - z_c)/(k_R - g);
+    df = -(f0/2k0) * 16.0218 * k_R g/(k_R - g) for every window (Eq.2 + Eq.3 end to end)."""
+    grid, ff = _flat_grid()
+    gsl, zc = 0.37, 4.1
+    zk = grid.origin[2] + 0.2 * np.arange(grid.n[2])
+    ff[..., 2] = (gsl * (zk - zc))[:, None, None]
+    tip = W._default_tip()
+    fire = replace(W.Fire(), f_conv=1e-12, max_iter=50000)
+    for dz, nz in ((0.1, 25), (0.05, 45)):
+        sc = _scan(nz=nz, dz=dz)
+        r = oracle.relax_scan(ff, grid, tip, fire, sc)
+        zt = sc.p0[2] - dz * np.arange(nz)
+        want = tip.k_rad * gsl * (zt - 4.0 - zc) / (tip.k_rad - gsl)
+        assert np.allclose(r["pos_fz"][:, 0, 3], want, atol=1e-9)
+        df = oracle.df(r["pos_fz"][..., 3], dz, 1.0, 1800.0, 30300.0)
+        assert df.shape[0] == nz - int(round(1.0 / dz))
+        assert np.allclose(df, -(30300.0 / 3600.0) * NM * tip.k_rad * gsl / (tip.k_rad - gsl), rtol=1e-7)
+
+
+def test_fire_finds_a_true_minimum_newton_crosscheck_cfg0():
+    """O6: on config 0 the FIRE end point is a stationary point with positive-definite Hessian, and a damped
+    Newton iteration (analytic Jacobian) started there does not move it by more than 1e-6 Å (non-flagged)."""
+    w = W.get(0)
+    ff = oracle.forcefield(w)
+    pix = W.sample_indices(w.scan.npx * w.scan.npy, 40, 5)
+    r = oracle.relax_scan(ff, w.grid, w.tip, w.fire, w.scan, pix=pix)
+    assert np.all(r["iters"] >= 0)
+    flagged = oracle.near_unstable(r["lam_min"])
+    worst = 0.0
+    for iz in range(0, w.scan.nz, 3):
+        for m, p in enumerate(pix):
+            ix, iy = p % w.scan.npx, p // w.scan.npx
+            rtip = w.scan.p0 + ix * w.scan.dx + iy * w.scan.dy - np.array([0, 0, iz * w.scan.dz])
+            x = r["pos_fz"][iz, m, :3].copy()
+            F = oracle.total_force(ff, w.grid, w.tip, rtip, x)
+            assert np.linalg.norm(F) < w.fire.f_conv
+            if flagged[iz, m]:
+                continue
+            x0 = x.copy()
+            for _ in range(20):
+                H, ev = oracle.hessian(ff, w.grid, w.tip, rtip, x)
+                assert ev[0] > 0
+                x = x + np.linalg.solve(H, oracle.total_force(ff, w.grid, w.tip, rtip, x))
+            worst = max(worst, np.linalg.norm(x - x0))
+            assert np.linalg.norm(oracle.total_force(ff, w.grid, w.tip, rtip, x)) < 1e-9
+    assert worst < 1e-6 / 1e-3 * 1e-3 + 1e-3     # |dx| <= f_conv / lam_min <= 1e-3 Å for non-flagged samples
+    assert worst < 1e-3
+
+
+def test_relaxed_positions_mirror_symmetric_molecule():
+    """A mirror-symmetric sample scanned on a mirror-symmetric pixel set gives mirror-symmetric relaxed positions
+    and equal Fz (pins the whole O3-O8 chain without a reference value)."""
+    w = W.get(0)
+    half = np.round(w.xyzq[:5].astype(np.float64) * 64) / 64
+    half[:, 0] = 4.0 + np.abs(half[:, 0] - 6.0) * 0.5            # x in [4, 5.5]
+    mir = half.copy()
+    mir[:, 0] = 12.0 - mir[:, 0]
+    w = replace(w, xyzq=np.r_[half, mir].astype(np.float32), types=np.r_[w.types[:5], w.types[:5]],
+                grid=replace(w.grid, n=(61, 60, 40)),                 # nodes at 0..12 -> symmetric about x = 6
+                scan=replace(w.scan, p0=np.array([4.0, 5.0, 10.0]), npx=21, npy=3, nz=30))
+    ff = oracle.forcefield(w)
+    assert np.allclose(ff[..., 0], -ff[:, :, ::-1, 0], rtol=1e-9, atol=1e-12)
+    r = oracle.relax_scan(ff, w.grid, w.tip, replace(w.fire, f_conv=1e-9, max_iter=20000), w.scan)
+    pos = r["pos_fz"].reshape(w.scan.nz, w.scan.npy, w.scan.npx, 4)
+    ok = ~oracle.near_unstable(r["lam_min"]).reshape(w.scan.nz, w.scan.npy, w.scan.npx)
+    ok &= ok[:, :, ::-1]
+    assert ok.mean() > 0.9
+    assert np.allclose((pos[..., 0] + pos[:, :, ::-1, 0])[ok], 12.0, atol=1e-5)
+    assert np.allclose((pos[..., 1:] - pos[:, :, ::-1, 1:])[ok], 0.0, atol=1e-5)
+
+
+def test_max_iter_flag():
+    g, ff = _flat_grid()
+    ff[..., 2] = 0.03
+    r = oracle.relax_scan(ff, g, W._default_tip(), replace(W.Fire(), max_iter=3), _scan(nz=1))
+    assert np.all(r["iters"] == -1)
+
+
+def test_fire_first_step_matches_hand_computation():
+    """One FIRE move from rest (v = 0, P = 0 counts as downhill, reading S6): v = F dt, r += v dt = F dt^2."""
+    g, ff = _flat_grid()
+    ff[..., 2] = 0.03
+    ff[..., 0] = -0.01
+    tip = W._default_tip()
+    sc = _scan(nz=1)
+    r = oracle.relax_scan(ff, g, tip, replace(W.Fire(), max_iter=1), sc, pix=np.array([0]))
+    want = sc.p0 + np.array(tip.d0) + np.array([-0.01, 0, 0.03]) * 0.25
+    assert np.allclose(r["pos_fz"][0, 0, :3], want, atol=1e-15)
+    # second move: P > 0, n_pos = 1 <= n_min so dt stays 0.5; v = (1-a) v + a |v| F/|F| then v += F dt
+    r2 = oracle.relax_scan(ff, g, tip, replace(W.Fire(), max_iter=2), sc, pix=np.array([0]))
+    x1 = want
+    d = x1 - sc.p0
+    L = np.linalg.norm(d)
+    F1 = np.array([-0.01, 0, 0.03]) - tip.k_rad * (L - 4.0) * d / L - np.array(
+        [tip.k_lat[0] * d[0], tip.k_lat[1] * d[1], 0.0])
+    v = np.array([-0.01, 0, 0.03]) * 0.5
+    v = 0.9 * v + 0.1 * np.linalg.norm(v) * F1 / np.linalg.norm(F1)
+    v = v + F1 * 0.5
+    assert np.allclose(r2["pos_fz"][0, 0, :3], x1 + v * 0.5, atol=1e-14)
+
+
+# ---------------------------------------------------------------------------------------------------- O9
+def test_df_weights_sum_to_zero_and_match_numerical_quadrature():
+    """Eq.3: W_m = (2/(pi a^2)) int q hat_m(q)/sqrt(a^2-q^2) dq, checked with scipy.quad using
+    the algebraic end-point weight; sum W = 0 (a constant force gives df = 0)."""
+    for n, dz in ((10, 0.1), (20, 0.05), (1, 1.0), (2, 0.5), (7, 0.13)):
+        Wt = oracle.df_weights(n, dz)
+        a = 0.5 * n * dz
+        assert abs(Wt.sum()) < 1e-13
+        assert np.allclose(Wt, -Wt[::-1], atol=1e-13)                   # odd kernel
+        for m in range(n + 1):
+            qm = -a + m * dz
+            tot = 0.0
+            for lo, hi in ((qm - dz, qm), (qm, qm + dz)):
+                if lo < -a - 1e-12 or hi > a + 1e-12:
+                    continue
+                hat = lambda q: q * (1 - abs(q - qm) / dz)
+                # int f(q) (q+a)^(-1/2) (a-q)^(-1/2) dq  via quad's 'alg' weight on [-a, a] restricted by hat
+                val, _ = integrate.quad(lambda q: hat(q) if lo <= q <= hi else 0.0, -a, a, weight="alg",
+                                        wvar=(-0.5, -0.5), points=None, limit=400)
+                tot += val
+            assert Wt[m] == pytest.approx(2 / (np.pi * a * a) * tot, abs=2e-6)
+
+
+def test_df_linear_exact_cubic_and_exponential():
+    pref = (30300.0 / 3600.0) * NM
+    for n in (1, 2, 10, 20):
+        dz = 1.0 / n
+        a = 0.5
+        nz = n + 6
+        z = 8.0 - dz * np.arange(nz)
+        g = 0.37
+        df = oracle.df((g * (z - 5.0))[:, None], dz, 1.0, 1800.0, 30300.0)
+        assert np.allclose(df, -pref * g, rtol=1e-12)                       # linear: exact for any n
+        zc = z[0] - (np.arange(nz - n) + n / 2) * dz
+        kappa, F0 = 1.3, 0.2
+        dfe = oracle.df((F0 * np.exp(-kappa * z))[:, None], dz, 1.0, 1800.0, 30300.0)[:, 0]
+        # int q e^{-kq}/sqrt(a^2-q^2) = -pi a I1(k a)  ->  df = (f0/(k0 a)) * 16.02 * F0 e^{-k zc} I1(k a)
+        want = 2 * pref / a * F0 * np.exp(-kappa * zc) * special.i1(kappa * a)
+        tol = {1: 0.2, 2: 0.05, 10: 2e-3, 20: 6e-4}[n]
+        assert np.allclose(dfe, want, rtol=tol)
+        h3 = 0.11
+        dfc = oracle.df((h3 * (z - zc[2]) ** 3)[:, None], dz, 1.0, 1800.0, 30300.0)[2, 0]
+        wantc = -pref * 0.75 * h3 * a * a
+        tolc = {1: 0.34, 2: 0.34, 10: 0.03, 20: 0.01}[n]      # n = 1, 2: the interpolant is the chord, error exactly 1/3
+        assert dfc == pytest.approx(wantc, rel=tolc)
+    # n = 1 is the two-point finite difference (small-amplitude limit, reading S10)
+    fz = np.array([[0.3], [0.5], [0.9]])
+    assert np.allclose(oracle.df(fz, 0.1, 0.1, 1800.0, 30300.0)[:, 0], -pref * (fz[:-1, 0] - fz[1:, 0]) / 0.1)
+
+
+def test_df_rejects_bad_amplitude():
+    with pytest.raises(ValueError):
+        oracle.df(np.zeros((20, 1)), 0.1, 0.55, 1800.0, 30300.0)       # A/dz not an integer
+    with pytest.raises(ValueError):
+        oracle.df(np.zeros((5, 1)), 0.1, 1.0, 1800.0, 30300.0)         # nz <= n
+
+
+# ---------------------------------------------------------------------------------------------------- O10
+def test_hessian_matches_finite_difference_of_force():
+    w = W.get(0)
+    ff = oracle.forcefield(w)
+    rtip = np.array([5.03, 6.41, 7.52])
+    rpp = rtip + np.array([0.213, -0.117, -3.93])         # interior of a cell (not on a face)
+    H, ev = oracle.hessian(ff, w.grid, w.tip, rtip, rpp)
+    J = np.zeros((3, 3))
+    h = 1e-6
+    for a in range(3):
+        dp = np.zeros(3)
+        dp[a] = h
+        J[:, a] = (oracle.total_force(ff, w.grid, w.tip, rtip, rpp + dp) -
+                   oracle.total_force(ff, w.grid, w.tip, rtip, rpp - dp)) / (2 * h)
+    assert np.allclose(H, -(J + J.T) / 2, rtol=1e-6, atol=1e-8)
+    assert np.allclose(ev, np.linalg.eigvalsh(H), atol=1e-12)
+
+
+def test_golden_constants_are_what_the_generators_use():
+    assert W.EVA2_PER_NM == pytest.approx(1.0 / NM, rel=1e-15)
+    assert W.ELEM_R[:4].tolist() == [GOLD["R_H"], GOLD["R_C"], GOLD["R_N"], GOLD["R_O"]]
+    assert W.ELEM_E[:4].tolist() == [GOLD["e_H"], GOLD["e_C"], GOLD["e_N"], GOLD["e_O"]]
+    w = W.get(0)
+    assert w.tip.k_lat[0] == pytest.approx(GOLD["k_xy_Nm"] / NM) and w.tip.d0 == (0.0, 0.0, -GOLD["R_rest_A"])
+    assert (w.df.A, w.df.k0, w.df.f0) == (GOLD["A_A"], GOLD["k0_Nm"], GOLD["f0_Hz"])
