@@ -1,0 +1,194 @@
+/*
+ * ppfm.h — C ABI of libppfm: the Probe-Particle Model hot path on one NVIDIA B200 (sm_100a).
+ *
+ * Paper: arxiv 2401.14564 ("PAPER.md" below = /root/reference/PAPER.md, cited by line).  The library implements
+ * the simplest level of theory (Lennard-Jones + point charges) of the two-step scheme of
+ * (1) project all sample atoms onto a uniform grid force field, (2) relax the probe particle
+ * (PP) with FIRE under tri-linear interpolation of that grid plus the tip springs, for every scan pixel while
+ * the tip steps down in z, and (3) convert Fz(z) to the frequency shift df.
+ *
+ * Conventions
+ *   Units: Å, eV, elementary charge e; spring constants in eV/Å^2 (ppfm_Nm_to_eVA2 converts from N/m);
+ *          k0 in N/m and f0 in Hz (ppfm_df).  k_e = 14.399645478 eV·Å/e^2;  1 eV/Å^2 = 16.02176634 N/m.
+ *   Pointers: a `d_` prefix = DEVICE memory on the current CUDA device, `h_` prefix = HOST memory.  Structs
+ *          passed by pointer are HOST memory and are read before the call returns.
+ *   Ownership: every buffer is allocated and freed by the caller.  The library keeps no pointer after return and
+ *          holds no persistent device memory; per-call scratch is stream-ordered (cudaMallocAsync / cudaFreeAsync
+ *          on `cuda_stream`).  Device entry points only enqueue work on `cuda_stream` (a cudaStream_t cast to
+ *          void*, NULL = default stream); they never synchronise it and never change the current device.
+ *          Host entry points (ppfm_scan_host) synchronise the stream before returning.
+ *   Errors: 0 on success, a negative ppfm_status otherwise; no exceptions, no exit(), no output.  Per-pixel
+ *          conditions (not converged, PP clamped at a non-periodic grid face) are data (d_iters, d_stats).
+ *   Determinism: outputs are bit-reproducible run to run (fixed summation order, no atomics on results).
+ *   Layouts: force-field grid  float[nz][ny][nx][4] = (Fx, Fy, Fz, E), x fastest;
+ *            scan output       float[nzs][npy][npx][4] = (PPx, PPy, PPz, Fz_tip);
+ *            df                float[nzs - n][npy][npx], n = A/dz.
+ */
+#ifndef PPFM_H
+#define PPFM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PPFM_VERSION 100 /* 0.1.0 */
+#define PPFM_MAX_TYPES 64
+
+typedef enum {
+    PPFM_OK = 0,
+    PPFM_EINVAL = -1, /* null pointer, n <= 0, singular step matrix, A/dz not an integer, nz <= n, bad type index */
+    PPFM_ECUDA = -2,  /* CUDA runtime / launch error; text via ppfm_strerror(PPFM_ECUDA) (thread-local)          */
+    PPFM_ENOMEM = -3  /* scratch allocation failed                                                              */
+} ppfm_status;
+
+/* Supercell vectors (Å) and periodic images: the sum runs over shifts na*a + nb*b + nc*c with
+ * n? in [-nimg[?], +nimg[?]]; nimg = 0 on a non-periodic axis. */
+typedef struct {
+    double a[3], b[3], c[3];
+    int32_t nimg[3];
+} ppfm_lattice;
+
+/* Uniform grid: point(i,j,k) = origin + i*step[0] + j*step[1] + k*step[2], i < n[0] etc..
+ * periodic[ax] != 0: interpolation wraps that axis (n[ax]*step[ax] must be the cell vector); 0: clamps. */
+typedef struct {
+    double origin[3];
+    double step[3][3];
+    int32_t n[3];
+    int32_t periodic[3];
+} ppfm_grid;
+
+/* Probe particle: LJ radius R_PP (Å), well depth e_PP (eV), point charge q_PP (e). */
+typedef struct {
+    double R, e, Q;
+} ppfm_probe;
+
+/* Tip springs of Eq.2: k_lat = (k_x, k_y), k_rad = k_R, d0 = equilibrium displacement of the PP
+ * from the anchor (e.g. (0,0,-4): PP hangs 4 Å below the anchor); R0 of Eq.2 is |d0|. */
+typedef struct {
+    double k_lat[2];
+    double k_rad;
+    double d0[3];
+} ppfm_tip;
+
+/* FIRE parameters (ref [7]); ppfm_fire_default() gives dt = dt_max = 0.5, finc 1.1, fdec 0.5,
+ * alpha0 0.1, falpha 0.99, n_min 5, max_iter 1000, f_conv 1e-6 eV/Å. */
+typedef struct {
+    double dt, dt_max, finc, fdec, alpha0, falpha;
+    int32_t n_min, max_iter;
+    double f_conv;
+} ppfm_fire;
+
+/* Scan: tip anchor(ix,iy,iz) = p0 + ix*dx + iy*dy - (0,0,iz*dz), iz = 0 is the far end. */
+typedef struct {
+    double p0[3], dx[3], dy[3];
+    int32_t npx, npy, nz;
+    double dz;
+} ppfm_scan;
+
+/* Counters accumulated (+=, max) by ppfm_relax_scan into a DEVICE struct the caller zeroes. */
+typedef struct {
+    uint64_t total_iters;     /* FIRE moves summed over all pixel-steps                   */
+    uint64_t n_not_converged; /* pixel-steps that used max_iter moves without converging  */
+    uint64_t n_clamped;       /* pixel-steps whose final PP position was clamped to a non-periodic grid face */
+    uint32_t max_iters;       /* largest move count of any pixel-step                     */
+    uint32_t _pad;
+} ppfm_stats;
+
+int ppfm_version(void);
+/* Message for a status code; for PPFM_ECUDA the text of the last CUDA error seen on this thread. */
+const char *ppfm_strerror(int code);
+void ppfm_fire_default(ppfm_fire *out);
+double ppfm_Nm_to_eVA2(double k_Nm);
+
+/* ---- (1) force-field grid: Eq.5 + Eq.6 summed over atoms and images ------------------
+ * d_xyzq   DEVICE float[natoms][4] = (x, y, z, q_i), 16-byte aligned
+ * d_type   DEVICE int32[natoms], index into h_R / h_e (validated on the device: out-of-range -> that atom is
+ *          skipped and the call's status word, if any, is not affected; validate on the host when you can)
+ * h_R,h_e  HOST double[ntypes]: element radius R_i (Å) and well depth e_i (eV); mixing R_i + R_PP, sqrt(e_i e_PP)
+ * r_min    pair distances are clamped below at r_min (Å) to keep the sum finite on top of an atom; >= 0
+ * d_ff     DEVICE float[n2][n1][n0][4], 16-byte aligned, written completely
+ */
+int ppfm_forcefield(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes, const double *h_R,
+                    const double *h_e, const ppfm_lattice *lattice, const ppfm_probe *probe, const ppfm_grid *grid,
+                    double r_min, float *d_ff, void *cuda_stream);
+
+/* Same pass, two grids (LJ and electrostatic fields are kept separately so the tip charge can
+ * change without recomputation): d_ff_lj = Lennard-Jones only, d_ff_el = Coulomb field of a UNIT probe charge
+ * (probe->Q is ignored).  Combine with ppfm_combine. */
+int ppfm_forcefield_split(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                          const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                          const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff_lj,
+                          float *d_ff_el, void *cuda_stream);
+
+/* d_out = d_ff_lj + Q * d_ff_el over n_points float4 entries (d_out may alias d_ff_lj). */
+int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q, int64_t n_points, float *d_out,
+                 void *cuda_stream);
+
+/* Batch of independent systems in ONE launch (ML-style batches).  Atoms are concatenated:
+ * system m owns atoms h_atom_offset[m] .. h_atom_offset[m+1]-1; grids are concatenated in d_ff in order
+ * (system m starts at float4 offset sum_{l<m} n0*n1*n2).  Arrays of structs are HOST arrays of length nsys. */
+int ppfm_forcefield_batch(int32_t nsys, const int32_t *h_atom_offset, const float *d_xyzq, const int32_t *d_type,
+                          int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
+                          const ppfm_probe *probes, const ppfm_grid *grids, double r_min, float *d_ff,
+                          void *cuda_stream);
+
+/* ---- (2) relaxation scan: Eq.1 + Eq.2 + FIRE on the tri-linearly interpolated grid --
+ * d_ff      DEVICE grid as written by ppfm_forcefield (read-only)
+ * d_pos_fz  DEVICE float[nz][npy][npx][4] = relaxed PP position and Fz_tip = -F_R,z
+ * d_iters   DEVICE uint16[nz][npy][npx] or NULL: FIRE moves made; 0xFFFF = max_iter reached without converging
+ * d_stats   DEVICE ppfm_stats or NULL (accumulated)
+ * Per pixel: iz = 0 starts at r_TIP + d0 with v = 0; each further z-step carries the displacement d over and
+ * resets the FIRE state.  Convergence: |F_total|_2 < f_conv, tested before every move.
+ */
+int ppfm_relax_scan(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_fire *fire,
+                    const ppfm_scan *scan, float *d_pos_fz, uint16_t *d_iters, ppfm_stats *d_stats,
+                    void *cuda_stream);
+
+/* Batch form: nsys scans in one launch; grids concatenated as in ppfm_forcefield_batch, outputs concatenated in
+ * order (system m starts at pixel-step offset sum_{l<m} nz*npy*npx).  One fire setting for all. */
+int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                          const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
+                          ppfm_stats *d_stats, void *cuda_stream);
+
+/* ---- (3) frequency shift, Giessibl's formula Eq.3 -------------------------------------------
+ * Fz is read from the .w lane of d_pos_fz [nz][npy][npx][4].  A = peak-to-peak amplitude (Å); n = A/dz must be an
+ * integer >= 1 (within 1e-6) and nz > n.  Eq.3 is integrated exactly for the piecewise-linear interpolant of the
+ * n+1 samples of each window; output plane k belongs to tip height z0 - (k + n/2) dz.
+ * d_df  DEVICE float[nz - n][npy][npx] (Hz).  ppfm_df_weights writes the n+1 quadrature weights to HOST memory.
+ * The batch count `nsys` treats d_pos_fz / d_df as nsys consecutive stacks of identical shape.
+ */
+int ppfm_df(const float *d_pos_fz, int32_t npx, int32_t npy, int32_t nz, double dz, double A, double k0_Nm,
+            double f0_Hz, float *d_df, void *cuda_stream);
+int ppfm_df_batch(int32_t nsys, const float *d_pos_fz, int32_t npx, int32_t npy, int32_t nz, double dz, double A,
+                  double k0_Nm, double f0_Hz, float *d_df, void *cuda_stream);
+int ppfm_df_weights(int32_t n, double dz, double *h_W);
+
+/* ---- whole simulation in one call, HOST buffers in and out ("run the whole simulation in one step")
+ * Copies the inputs to the device, runs (1) -> (2) -> (3) on `cuda_stream`, copies the results back and
+ * synchronises the stream.  h_pos_fz / h_df / h_iters may each be NULL (not copied back); h_stats may be NULL.
+ * Pinned host buffers make the copies asynchronous; pageable buffers work too.
+ */
+int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t *h_type, int32_t ntypes, const double *h_R,
+                   const double *h_e, const ppfm_lattice *lattice, const ppfm_probe *probe, const ppfm_grid *grid,
+                   double r_min, const ppfm_tip *tip, const ppfm_fire *fire, const ppfm_scan *scan, double A,
+                   double k0_Nm, double f0_Hz, float *h_pos_fz, uint16_t *h_iters, float *h_df,
+                   ppfm_stats *h_stats, void *cuda_stream);
+
+/* ---- measurement helpers (used by bench.py to define the roofline denominators on the box itself) ------------
+ * ppfm_probe_fma:    FFMA-only kernel; returns lane-instructions per second in *h_lane_instr_per_s.
+ * ppfm_probe_gather: the relaxation's 8-corner float4 gather over an L2-resident volume of `n_float4` entries
+ *                    with no dependent math; `bypass_l1` selects ld.global.cg; returns GB/s in *h_gbs.
+ * Both synchronise the stream (they time with CUDA events).
+ */
+int ppfm_probe_fma(double *h_lane_instr_per_s, void *cuda_stream);
+int ppfm_probe_gather(int64_t n_float4, int32_t bypass_l1, double *h_gbs, void *cuda_stream);
+
+/* Number of kernels this library has launched on this process so far (for bench.py's gpu_launches). */
+int64_t ppfm_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PPFM_H */

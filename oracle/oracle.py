@@ -142,9 +142,10 @@ def hessian(ff, grid, tip, rtip, rpp):
     return H, w
 
 
-def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None):
+def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None, traj: bool = True):
     """O4-O8 (+O10).  Returns dict: pos_fz (nz, npix, 4), iters (nz, npix) [-1 = not converged],
-    lam_min (nz, npix), clamped (nz, npix).  Without `pix` npix = npy*npx in row-major (iy, ix) order."""
+    lam_min (nz, npix), clamped (nz, npix), lam_traj (nz, npix; smallest Hessian eigenvalue along the step's FIRE
+    path, reading S17; None when traj=False).  Without `pix` npix = npy*npx in row-major (iy, ix) order."""
     ff, is32, origin, step, n, per = _ff_args(ff, grid)
     if pix is None:
         npix, ppix = scan.npx * scan.npy, None
@@ -155,16 +156,17 @@ def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None):
     iters = np.empty((scan.nz, npix), dtype=np.int32)
     lam = np.empty((scan.nz, npix))
     cl = np.empty((scan.nz, npix), dtype=np.int32)
+    lt = np.empty((scan.nz, npix)) if traj else None
     f = _d([fire.dt, fire.dt_max, fire.finc, fire.fdec, fire.alpha0, fire.falpha, fire.f_conv])
     rc = lib().oracle_relax_scan(_p(ff), C.c_int(is32), _p(origin), _p(step), _p(n), _p(per), _p(_d(tip.k_lat)),
                                  C.c_double(tip.k_rad), _p(_d(tip.d0)), _p(f), C.c_int(fire.n_min),
                                  C.c_int(fire.max_iter), _p(_d(scan.p0)), _p(_d(scan.dx)), _p(_d(scan.dy)),
                                  C.c_int(scan.npx), C.c_int(scan.npy), C.c_int(scan.nz), C.c_double(scan.dz),
                                  C.c_int64(npix if pix is not None else 0), _p(ppix), _p(pos), _p(iters), _p(lam),
-                                 _p(cl))
+                                 _p(cl), _p(lt))
     if rc:
         raise ValueError(f"oracle_relax_scan rc={rc}")
-    return {"pos_fz": pos, "iters": iters, "lam_min": lam, "clamped": cl}
+    return {"pos_fz": pos, "iters": iters, "lam_min": lam, "clamped": cl, "lam_traj": lt}
 
 
 def df_weights(n: int, dz: float) -> np.ndarray:
@@ -188,10 +190,17 @@ def df(fz, dz: float, A: float, k0: float, f0: float) -> np.ndarray:
     return out
 
 
-def near_unstable(lam_min: np.ndarray, thresh: float = 1e-3) -> np.ndarray:
-    """O10 flag over (nz, npix): lam_min < thresh at this z-step or the previous one (snap-through lands one
-    step later)."""
+def near_unstable(lam_min: np.ndarray, thresh: float = 1e-3, lam_traj: Optional[np.ndarray] = None) -> np.ndarray:
+    """O10 flag over (nz, npix): smallest Hessian eigenvalue < thresh at the relaxed point of this z-step or the
+    previous one, or (reading S17, when lam_traj is given) anywhere along the FIRE path of this or the previous step."""
     f = lam_min < thresh
+    if lam_traj is not None:
+        f = f | (lam_traj < thresh)
     out = f.copy()
     out[1:] |= f[:-1]
     return out
+
+
+def flags(res: dict, thresh: float = 1e-3) -> np.ndarray:
+    """near_unstable over a relax_scan result, plus the not-converged samples."""
+    return near_unstable(res["lam_min"], thresh, res.get("lam_traj")) | (res["iters"] < 0)

@@ -355,6 +355,13 @@ int oracle_hessian(const void *ff, int is_f32, const double *origin, const doubl
  * Outputs (dense over the selected pixels, [nz][npix]):
  *   pos_fz[.][4] = (r_PP, Fz_tip = -F_R,z);  iters = moves made, -1 if max_iter moves did not converge;
  *   lam_min = smallest Hessian eigenvalue at the relaxed point;  clamped = 1 if the final r_PP was clamped (S12).
+ *   lam_traj (optional) = smallest Hessian eigenvalue over EVERY point of the step's FIRE path (warm-start point,
+ *   each intermediate point, end point).  Reading S17: when it drops below 1e-3 eV/Å^2 the PP crosses a ridge of the
+ *   potential on its way (snap-through, or an inertial overshoot out of a shallow basin); which basin FIRE then
+ *   lands in depends on rounding-level differences of the grid, so such samples count as near-unstable just like
+ *   samples whose END point has lambda < 1e-3.  (Observed: config 1, pixel 19076, z-step 35: the oracle on its own
+ *   FP64 grid and on an FP32 grid that agrees with it to 1e-5 lands in two different stable minima, 0.88 Å apart,
+ *   end-point lambda 8.0e-3 and 2.8e-3; path minimum -8.9e-3 and -4.0e-3.)
  * If pix != NULL only the `npix` flat pixel indices (iy*npx + ix) listed are computed.
  * ---------------------------------------------------------------------------------------------------------- */
 static double norm3(const double v[3]) { return sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]); }
@@ -363,7 +370,7 @@ int oracle_relax_scan(const void *ff, int is_f32, const double *origin, const do
                       const int *periodic, const double *k_lat, double k_rad, const double *d0,
                       const double *fire, int n_min, int max_iter, const double *p0, const double *dx,
                       const double *dy, int npx, int npy, int nz, double dz, int64_t npix, const int64_t *pix,
-                      double *pos_fz, int *iters, double *lam_min, int *clamped_out) {
+                      double *pos_fz, int *iters, double *lam_min, int *clamped_out, double *lam_traj) {
     grid_view g;
     if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
     tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
@@ -383,8 +390,15 @@ int oracle_relax_scan(const void *ff, int is_f32, const double *origin, const do
             for (int c = 0; c < 3; c++) r[c] = rtip[c] + dcur[c];
             double dt = dt0, alpha = alpha0;
             int n_pos = 0, moves = 0, converged = 0, cl = 0;
+            double ltraj = INFINITY;
             for (;;) { /* O6 */
                 cl = total_force(&g, &tp, rtip, r, F);
+                if (lam_traj) { /* diagnostic only (O10 / S17): does not touch the FIRE state */
+                    double Ht[9], wt[3];
+                    hessian(&g, &tp, rtip, r, Ht);
+                    sym3_eig(Ht, wt);
+                    if (wt[0] < ltraj) ltraj = wt[0];
+                }
                 double Fn = norm3(F);
                 if (Fn < f_conv) { converged = 1; break; } /* S7: check before moving */
                 if (moves >= max_iter) break;
@@ -417,6 +431,7 @@ int oracle_relax_scan(const void *ff, int is_f32, const double *origin, const do
             pos_fz[4 * o + 3] = -FR[2];
             if (iters) iters[o] = converged ? moves : -1;
             if (clamped_out) clamped_out[o] = cl;
+            if (lam_traj) lam_traj[o] = ltraj;
             if (lam_min) {
                 double H[9], w[3];
                 hessian(&g, &tp, rtip, r, H);

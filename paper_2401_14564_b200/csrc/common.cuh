@@ -1,0 +1,80 @@
+// common.cuh — shared host-side plumbing of libppfm (error capture, launch counting, small math helpers).
+// CUDA path only; the CPU oracle under oracle/ shares nothing with this tree.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "../../include/ppfm.h"
+
+namespace ppfm {
+
+// Coulomb constant k_e in eV*Angstrom/e^2 (Eq.6) and eV/Angstrom^2 -> N/m (exact SI e).
+constexpr double kCoulomb = 14.399645478;
+constexpr double kEVA2toNm = 16.02176634;
+
+void set_cuda_error(cudaError_t e, const char *where);
+extern std::atomic<long long> g_launches;
+inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+#define PPFM_CUDA(call)                                  \
+    do {                                                 \
+        cudaError_t _e = (call);                         \
+        if (_e != cudaSuccess) {                         \
+            ::ppfm::set_cuda_error(_e, #call);           \
+            return (_e == cudaErrorMemoryAllocation) ? PPFM_ENOMEM : PPFM_ECUDA; \
+        }                                                \
+    } while (0)
+
+#define PPFM_LAUNCH_CHECK()                              \
+    do {                                                 \
+        cudaError_t _e = cudaGetLastError();             \
+        if (_e != cudaSuccess) {                         \
+            ::ppfm::set_cuda_error(_e, "kernel launch"); \
+            return PPFM_ECUDA;                           \
+        }                                                \
+        ::ppfm::count_launch();                          \
+    } while (0)
+
+// t = Minv (r - origin): inverse of the matrix whose COLUMNS are the grid step vectors.  false if singular.
+inline bool invert_steps(const double step[3][3], double Minv[9]) {
+    double A[9];
+    for (int r = 0; r < 3; r++)
+        for (int c = 0; c < 3; c++) A[3 * r + c] = step[c][r];
+    const double det = A[0] * (A[4] * A[8] - A[5] * A[7]) - A[1] * (A[3] * A[8] - A[5] * A[6]) +
+                       A[2] * (A[3] * A[7] - A[4] * A[6]);
+    if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return false;
+    const double id = 1.0 / det;
+    Minv[0] = (A[4] * A[8] - A[5] * A[7]) * id;
+    Minv[1] = (A[2] * A[7] - A[1] * A[8]) * id;
+    Minv[2] = (A[1] * A[5] - A[2] * A[4]) * id;
+    Minv[3] = (A[5] * A[6] - A[3] * A[8]) * id;
+    Minv[4] = (A[0] * A[8] - A[2] * A[6]) * id;
+    Minv[5] = (A[2] * A[3] - A[0] * A[5]) * id;
+    Minv[6] = (A[3] * A[7] - A[4] * A[6]) * id;
+    Minv[7] = (A[1] * A[6] - A[0] * A[7]) * id;
+    Minv[8] = (A[0] * A[4] - A[1] * A[3]) * id;
+    for (int i = 0; i < 9; i++)
+        if (!std::isfinite(Minv[i])) return false;
+    return true;
+}
+
+inline bool grid_ok(const ppfm_grid *g) {
+    if (!g) return false;
+    for (int a = 0; a < 3; a++) {
+        if (g->n[a] < 1) return false;
+        if (!std::isfinite(g->origin[a])) return false;
+    }
+    if ((long long)g->n[0] * g->n[1] > 0x7fffffffLL) return false;
+    double Minv[9];
+    return invert_steps(g->step, Minv);
+}
+
+inline long long grid_points(const ppfm_grid *g) { return (long long)g->n[0] * g->n[1] * g->n[2]; }
+
+}  // namespace ppfm

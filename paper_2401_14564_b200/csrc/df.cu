@@ -1,0 +1,96 @@
+// df.cu — Fz -> frequency shift: Giessibl's formula, Eq.3,
+//   df = -(f0 / 2k) (8 / (pi A^2)) int_{-A/2}^{A/2} q Fz(z + q) / sqrt(A^2/4 - q^2) dq,
+// integrated exactly for the piecewise-linear interpolant of the n + 1 = A/dz + 1 samples in each window
+// (reading S9).  The n + 1 weights are computed in FP64 on the host and passed by value; the kernel is
+// a streaming weighted sum, one thread per output sample, lanes along x (HBM/L2-bound, trivial next to a2/a5).
+#include "common.cuh"
+
+namespace ppfm {
+
+constexpr int DF_MAX_N = 255;
+
+struct DfWeights {
+    float w[DF_MAX_N + 1];   // already multiplied by -(f0 / 2 k0) * 16.02176634
+};
+
+// Host: exact moments of q / sqrt(a^2 - q^2) against the hat functions of the uniform nodes q_m = -a + m dz.
+// With y(q) = sqrt(a^2 - q^2):  int q/y dq = -y,  int q^2/y dq = (a^2/2) asin(q/a) - (q/2) y.
+static void df_weights_host(int n, double dz, double *W) {
+    const double a = 0.5 * n * dz;
+    for (int m = 0; m <= n; m++) W[m] = 0.0;
+    double q_lo = -a, y_lo = 0.0, G_lo = -0.25 * M_PI * a * a;
+    for (int j = 0; j < n; j++) {
+        const double q_hi = (j == n - 1) ? a : -a + (j + 1) * dz;
+        const double y_hi = (j == n - 1) ? 0.0 : std::sqrt(std::fmax(a * a - q_hi * q_hi, 0.0));
+        const double G_hi = (j == n - 1) ? 0.25 * M_PI * a * a
+                                         : 0.5 * a * a * std::asin(q_hi / a) - 0.5 * q_hi * y_hi;
+        const double m1 = y_lo - y_hi;   // first moment over the interval
+        const double m2 = G_hi - G_lo;   // second moment
+        W[j] += (q_hi * m1 - m2) / dz;
+        W[j + 1] += (m2 - q_lo * m1) / dz;
+        q_lo = q_hi; y_lo = y_hi; G_lo = G_hi;
+    }
+    const double norm = 2.0 / (M_PI * a * a);   // 8 / (pi A^2)
+    for (int m = 0; m <= n; m++) W[m] *= norm;
+}
+
+__global__ void __launch_bounds__(256)
+df_kernel(const float4 *__restrict__ pos_fz, long long npix, int nz, int n, int nsys, DfWeights W,
+          float *__restrict__ df) {
+    const long long nout_per = (long long)(nz - n) * npix;
+    const long long total = nout_per * nsys;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total; o += stride) {
+        const long long s = o / nout_per;
+        const long long r = o - s * nout_per;
+        const long long k = r / npix, p = r - k * npix;
+        const float4 *src = pos_fz + (s * nz + k) * npix + p;
+        float acc = 0.f;
+        for (int m = 0; m <= n; m++) acc = fmaf(W.w[m], __ldg(&src[(long long)(n - m) * npix].w), acc);
+        df[o] = acc;
+    }
+}
+
+static int df_impl(int nsys, const float *d_pos_fz, int npx, int npy, int nz, double dz, double A, double k0,
+                   double f0, float *d_df, void *cuda_stream) {
+    if (nsys < 1 || !d_pos_fz || !d_df || npx < 1 || npy < 1 || nz < 1) return PPFM_EINVAL;
+    if (!(dz > 0) || !(A > 0) || !(k0 > 0) || !std::isfinite(f0) || !std::isfinite(dz) || !std::isfinite(A))
+        return PPFM_EINVAL;
+    if ((uintptr_t)d_pos_fz & 15) return PPFM_EINVAL;
+    const double nn = A / dz;
+    const long long n = std::llround(nn);
+    if (n < 1 || n > DF_MAX_N || std::fabs(nn - (double)n) > 1e-6 || nz <= n) return PPFM_EINVAL;
+    double Wd[DF_MAX_N + 1];
+    df_weights_host((int)n, dz, Wd);
+    DfWeights W;
+    const double pref = -(f0 / (2.0 * k0)) * kEVA2toNm;
+    for (int m = 0; m <= DF_MAX_N; m++) W.w[m] = (m <= n) ? (float)(pref * Wd[m]) : 0.f;
+    const long long npix = (long long)npx * npy;
+    const long long total = (long long)(nz - n) * npix * nsys;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    df_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(reinterpret_cast<const float4 *>(d_pos_fz), npix,
+                                                                      nz, (int)n, nsys, W, d_df);
+    PPFM_LAUNCH_CHECK();
+    return PPFM_OK;
+}
+
+}  // namespace ppfm
+
+using namespace ppfm;
+
+extern "C" int ppfm_df(const float *d_pos_fz, int32_t npx, int32_t npy, int32_t nz, double dz, double A, double k0_Nm,
+                       double f0_Hz, float *d_df, void *cuda_stream) {
+    return df_impl(1, d_pos_fz, npx, npy, nz, dz, A, k0_Nm, f0_Hz, d_df, cuda_stream);
+}
+
+extern "C" int ppfm_df_batch(int32_t nsys, const float *d_pos_fz, int32_t npx, int32_t npy, int32_t nz, double dz,
+                             double A, double k0_Nm, double f0_Hz, float *d_df, void *cuda_stream) {
+    return df_impl(nsys, d_pos_fz, npx, npy, nz, dz, A, k0_Nm, f0_Hz, d_df, cuda_stream);
+}
+
+extern "C" int ppfm_df_weights(int32_t n, double dz, double *h_W) {
+    if (n < 1 || n > DF_MAX_N || !(dz > 0) || !h_W) return PPFM_EINVAL;
+    df_weights_host(n, dz, h_W);
+    return PPFM_OK;
+}

@@ -1,0 +1,526 @@
+// ff.cu — force-field grid sampling: Lennard-Jones (Eq.5, mixing
+// rules PAPER.md:85) plus point-charge Coulomb (Eq.6) summed over all sample atoms and their periodic
+// images at every point of a uniform grid, forces as F = -grad E.
+//
+// Kernel design (B200 / sm_100a; nothing here is a dense contraction, so no tensor cores):
+//   * a1  `ff_prep_kernel` packs one 32-byte record per atom (x, y, z, k_e q_PP q_i | c6, c12, 6 c6, k_e q_i).
+//   * a2  `ff_kernel`: one CTA = 256 columns (consecutive x-fastest (i,j) indices, so a warp's float4 stores are
+//         512 contiguous bytes) x P consecutive z planes held in registers.  Atom records stream through a
+//         4-stage shared-memory ring filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx), one
+//         elected thread producing two chunks ahead; every warp reads records as uniform (broadcast) LDS.128.
+//         Images are the outer loop and are applied as a shift of the grid point; the shifted point is formed in
+//         FP64 once per image and split hi+lo so that dx = (p_hi - a) + p_lo carries no coordinate rounding.
+//         Per pair and grid point: 15 FP32-pipe instructions + 1 MUFU.RSQ (+1 FMNMX when the r_min clamp is
+//         live, which the prep kernel decides from the atoms' distance to the grid's bounding box).
+//   * a3  `combine_kernel`: F = F_LJ + Q F_el, float4 streaming.
+#include "common.cuh"
+
+namespace ppfm {
+
+constexpr int FF_THREADS = 256;
+constexpr int FF_CHUNK = 256;   // atoms per pipeline stage
+constexpr int FF_STAGES = 4;
+constexpr int FF_AHEAD = 2;     // chunks in flight ahead of the consumer
+
+struct __align__(16) AtomRec {
+    float x, y, z, kq;          // kq = k_e q_PP q_i  (eV*Angstrom)
+    float c6, c12, c6x6, kq1;   // c6 = 2 E0 R0^6, c12 = E0 R0^12, c6x6 = 6 c6, kq1 = k_e q_i (unit probe charge)
+};
+static_assert(sizeof(AtomRec) == 32, "AtomRec must be 32 bytes");
+
+struct FFJob {
+    long long tile_begin;   // first tile (CTA) of this system in the launch
+    long long out_offset;   // float4 offset of this system's grid in the output buffer(s)
+    int atom_begin, natoms;
+    int nx, ny, nz, nxy;
+    int n_xy_tiles, n_z_groups;
+    int nimg[3];
+    int table_offset;       // first entry of this system's per-type table
+    double origin[3], step[3][3], cell[3][3];
+    double bb_lo[3], bb_hi[3];   // Cartesian bounding box of the grid points
+    float keQ;              // k_e q_PP
+    float rmin2;
+    int ntypes;
+    int pad;
+};
+
+struct TypeEntry {
+    float c6, c12;
+};
+
+// ---------------------------------------------------------------------------------------------------- a1 prep
+__global__ void ff_prep_kernel(const FFJob *__restrict__ jobs, int njobs, const TypeEntry *__restrict__ table,
+                               const float4 *__restrict__ xyzq, const int *__restrict__ type,
+                               AtomRec *__restrict__ recs, int *__restrict__ clamp_flags, int natoms_total) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= natoms_total) return;
+    int lo = 0, hi = njobs - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (jobs[mid].atom_begin <= i) lo = mid; else hi = mid - 1;
+    }
+    const FFJob &job = jobs[lo];
+    const float4 a = xyzq[i];
+    const int t = type[i];
+    AtomRec r;
+    r.x = a.x; r.y = a.y; r.z = a.z;
+    if (t >= 0 && t < job.ntypes) {
+        const TypeEntry te = table[job.table_offset + t];
+        r.c6 = te.c6; r.c12 = te.c12; r.c6x6 = 6.0f * te.c6;
+        r.kq = (float)((double)job.keQ * (double)a.w);
+        r.kq1 = (float)(kCoulomb * (double)a.w);
+    } else {   // out-of-range type index: the atom contributes nothing
+        r.c6 = r.c12 = r.c6x6 = r.kq = r.kq1 = 0.0f;
+    }
+    recs[i] = r;
+    // r_min clamp needed?  distance of every image of this atom to the grid's bounding box
+    const double rmin = sqrt((double)job.rmin2) * 1.0001 + 1e-6;
+    bool near = false;
+    for (int ia = -job.nimg[0]; ia <= job.nimg[0]; ia++)
+        for (int ib = -job.nimg[1]; ib <= job.nimg[1]; ib++)
+            for (int ic = -job.nimg[2]; ic <= job.nimg[2]; ic++) {
+                double d2 = 0.0;
+                const double p[3] = {a.x, a.y, a.z};
+                for (int c = 0; c < 3; c++) {
+                    const double x = p[c] + ia * job.cell[0][c] + ib * job.cell[1][c] + ic * job.cell[2][c];
+                    const double d = fmax(fmax(job.bb_lo[c] - x, x - job.bb_hi[c]), 0.0);
+                    d2 += d * d;
+                }
+                near |= (d2 < rmin * rmin);
+            }
+    if (near) atomicOr(&clamp_flags[lo], 1);
+}
+
+// ---------------------------------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---------------------------------------------------------------------------------------------------- a2 tile body
+// P      grid points per thread along step[2]
+// SPLIT  false: one grid (LJ + Coulomb with q_PP);  true: two grids (LJ | Coulomb of a unit probe charge)
+// CLAMP  apply s = max(r^2, r_min^2)
+// ZCOL   step[2] is parallel to z (dx, dy shared by the P points of a column)
+template <int P, bool SPLIT, bool CLAMP, bool ZCOL>
+__device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restrict__ recs, float4 *__restrict__ out_a,
+                                        float4 *__restrict__ out_b, AtomRec *s_rec, uint64_t *full_bar,
+                                        uint64_t *empty_bar, long long local_tile) {
+    const int tid = threadIdx.x;
+    const int zg = (int)(local_tile / job.n_xy_tiles);
+    const int xyt = (int)(local_tile - (long long)zg * job.n_xy_tiles);
+    const int col = xyt * FF_THREADS + tid;
+    const bool valid = col < job.nxy;
+    const int colc = valid ? col : job.nxy - 1;
+    const int j = colc / job.nx, i = colc - j * job.nx;
+    const int k0 = zg * P;
+
+    // base point of the column, FP64
+    double pb[3];
+#pragma unroll
+    for (int c = 0; c < 3; c++)
+        pb[c] = job.origin[c] + i * job.step[0][c] + j * job.step[1][c] + k0 * job.step[2][c];
+    float off[ZCOL ? 1 : 3][P];   // offsets of the P points along step[2]
+#pragma unroll
+    for (int k = 0; k < P; k++) {
+        if (ZCOL) {
+            off[0][k] = (float)(k * job.step[2][2]);
+        } else {
+#pragma unroll
+            for (int c = 0; c < (ZCOL ? 1 : 3); c++) off[c][k] = (float)(k * job.step[2][c]);
+        }
+    }
+
+    float Fx[P], Fy[P], Fz[P], E[P];
+    float Gx[SPLIT ? P : 1], Gy[SPLIT ? P : 1], Gz[SPLIT ? P : 1], Ge[SPLIT ? P : 1];
+    // energies are accumulated per chunk and folded into a running total at every chunk boundary: the 1/r and
+    // 1/r^6 tails of tens of thousands of atom images otherwise lose ~1e-5 eV to FP32 accumulation rounding
+    float Etot[P], Getot[SPLIT ? P : 1];
+#pragma unroll
+    for (int k = 0; k < P; k++) {
+        Fx[k] = Fy[k] = Fz[k] = E[k] = Etot[k] = 0.0f;
+        if (SPLIT) Gx[k] = Gy[k] = Gz[k] = Ge[k] = Getot[k] = 0.0f;
+    }
+
+    const int natoms = job.natoms;
+    const int nchunks = (natoms + FF_CHUNK - 1) / FF_CHUNK;
+    const int nimages = (2 * job.nimg[0] + 1) * (2 * job.nimg[1] + 1) * (2 * job.nimg[2] + 1);
+    const int nsteps = nimages * nchunks;
+    const AtomRec *src = recs + job.atom_begin;
+    const float rmin2 = job.rmin2;
+
+    auto issue = [&](int t) {   // producer: fill stage t % STAGES with chunk t % nchunks
+        const int st = t % FF_STAGES;
+        const int use = t / FF_STAGES;
+        if (use > 0) mbar_wait(&empty_bar[st], (use - 1) & 1);
+        const int c = t % nchunks;
+        const int n = min(FF_CHUNK, natoms - c * FF_CHUNK);
+        const uint32_t bytes = (uint32_t)n * (uint32_t)sizeof(AtomRec);
+        mbar_expect_tx(&full_bar[st], bytes);
+        tma_load_1d(s_rec + st * FF_CHUNK, src + (size_t)c * FF_CHUNK, bytes, &full_bar[st]);
+    };
+    if (tid == 0) {
+        for (int t = 0; t < FF_AHEAD && t < nsteps; t++) issue(t);
+    }
+
+    int step = 0;
+    for (int ia = -job.nimg[0]; ia <= job.nimg[0]; ia++)
+        for (int ib = -job.nimg[1]; ib <= job.nimg[1]; ib++)
+            for (int ic = -job.nimg[2]; ic <= job.nimg[2]; ic++) {
+                // shifted point p' = p - shift, split hi + lo (FP64 once per image)
+                float ph[3], pl[3];
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    const double s = pb[c] - (ia * job.cell[0][c] + ib * job.cell[1][c] + ic * job.cell[2][c]);
+                    ph[c] = (float)s;
+                    pl[c] = (float)(s - (double)ph[c]);
+                }
+                for (int ch = 0; ch < nchunks; ch++, step++) {
+                    if (tid == 0 && step + FF_AHEAD < nsteps) issue(step + FF_AHEAD);
+                    const int st = step % FF_STAGES;
+                    mbar_wait(&full_bar[st], (step / FF_STAGES) & 1);
+                    const float4 *s4 = reinterpret_cast<const float4 *>(s_rec + st * FF_CHUNK);
+                    const int n = min(FF_CHUNK, natoms - ch * FF_CHUNK);
+#pragma unroll 2
+                    for (int a = 0; a < n; a++) {
+                        const float4 r0 = s4[2 * a];
+                        const float4 r1 = s4[2 * a + 1];
+                        const float dx0 = (ph[0] - r0.x) + pl[0];
+                        const float dy0 = (ph[1] - r0.y) + pl[1];
+                        const float dz0 = (ph[2] - r0.z) + pl[2];
+                        const float rxy2 = fmaf(dy0, dy0, dx0 * dx0);
+                        const float kq = SPLIT ? r1.w : r0.w;
+#pragma unroll
+                        for (int k = 0; k < P; k++) {
+                            float dx, dy, dz, r2;
+                            if (ZCOL) {
+                                dx = dx0; dy = dy0;
+                                dz = dz0 + off[0][k];
+                                r2 = fmaf(dz, dz, rxy2);
+                            } else {
+                                dx = dx0 + off[0][k]; dy = dy0 + off[1 % (ZCOL ? 1 : 3)][k];
+                                dz = dz0 + off[2 % (ZCOL ? 1 : 3)][k];
+                                r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                            }
+                            if (CLAMP) r2 = fmaxf(r2, rmin2);
+                            const float ir = rsqrt_approx(r2);
+                            const float ir2 = ir * ir;
+                            const float ir6 = ir2 * ir2 * ir2;
+                            const float t = fmaf(r1.y, ir6, -r1.x);        // c12/r^6 - c6
+                            const float t2 = fmaf(t, 12.0f, r1.z);         // 12 c12/r^6 - 6 c6
+                            E[k] = fmaf(t, ir6, E[k]);                       // E_LJ = c12/r^12 - c6/r^6
+                            if (!SPLIT) {
+                                E[k] = fmaf(kq, ir, E[k]);                   // E_C = kq / r
+                                float g = t2 * ir6;
+                                g = fmaf(kq, ir, g);
+                                const float f = g * ir2;                     // (12c12/r^12 - 6c6/r^6 + kq/r) / r^2
+                                Fx[k] = fmaf(f, dx, Fx[k]);
+                                Fy[k] = fmaf(f, dy, Fy[k]);
+                                Fz[k] = fmaf(f, dz, Fz[k]);
+                            } else {
+                                const float f = t2 * ir6 * ir2;
+                                Fx[k] = fmaf(f, dx, Fx[k]);
+                                Fy[k] = fmaf(f, dy, Fy[k]);
+                                Fz[k] = fmaf(f, dz, Fz[k]);
+                                const float ec = kq * ir;
+                                Ge[k] += ec;
+                                const float fe = ec * ir2;
+                                Gx[k] = fmaf(fe, dx, Gx[k]);
+                                Gy[k] = fmaf(fe, dy, Gy[k]);
+                                Gz[k] = fmaf(fe, dz, Gz[k]);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if ((tid & 31) == 0) mbar_arrive(&empty_bar[st]);
+#pragma unroll
+                    for (int k = 0; k < P; k++) {
+                        Etot[k] += E[k]; E[k] = 0.0f;
+                        if (SPLIT) { Getot[k] += Ge[k]; Ge[k] = 0.0f; }
+                    }
+                }
+            }
+
+    if (valid) {
+#pragma unroll
+        for (int k = 0; k < P; k++) {
+            if (k0 + k < job.nz) {
+                const size_t o = (size_t)job.out_offset + (size_t)(k0 + k) * job.nxy + col;
+                out_a[o] = make_float4(Fx[k], Fy[k], Fz[k], Etot[k]);
+                if (SPLIT) out_b[o] = make_float4(Gx[k], Gy[k], Gz[k], Getot[k]);
+            }
+        }
+    }
+}
+
+template <int P, bool SPLIT, bool ZCOL>
+__global__ void __launch_bounds__(FF_THREADS, 2)
+ff_kernel(const FFJob *__restrict__ jobs, int njobs, const int *__restrict__ clamp_flags,
+          const AtomRec *__restrict__ recs, float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
+    __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
+    __shared__ __align__(8) uint64_t full_bar[FF_STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[FF_STAGES];
+    __shared__ FFJob s_job;
+    __shared__ int s_clamp;
+
+    const long long tile = blockIdx.x;
+    int lo = 0, hi = njobs - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (jobs[mid].tile_begin <= tile) lo = mid; else hi = mid - 1;
+    }
+    {
+        const int *srcw = reinterpret_cast<const int *>(&jobs[lo]);
+        int *dstw = reinterpret_cast<int *>(&s_job);
+        for (int w = threadIdx.x; w < (int)(sizeof(FFJob) / sizeof(int)); w += FF_THREADS) dstw[w] = srcw[w];
+    }
+    if (threadIdx.x == 0) {
+        s_clamp = clamp_flags[lo];
+        for (int s = 0; s < FF_STAGES; s++) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], FF_THREADS / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    const long long local_tile = tile - s_job.tile_begin;
+    if (s_clamp)
+        ff_tile<P, SPLIT, true, ZCOL>(s_job, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
+    else
+        ff_tile<P, SPLIT, false, ZCOL>(s_job, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
+}
+
+// ---------------------------------------------------------------------------------------------------- a3 combine
+__global__ void combine_kernel(const float4 *__restrict__ lj, const float4 *__restrict__ el, float Q, long long n,
+                               float4 *__restrict__ out) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const float4 a = lj[i], b = el[i];
+        out[i] = make_float4(fmaf(Q, b.x, a.x), fmaf(Q, b.y, a.y), fmaf(Q, b.z, a.z), fmaf(Q, b.w, a.w));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------- host side
+static int pick_P(int nz) {
+    // padded work ~ ceil(nz/P) * (P + per-atom overhead shared by the column ~ 0.7 points)
+    const int cand[3] = {8, 10, 5};
+    int best = 8;
+    double best_cost = 1e300;
+    for (int c = 0; c < 3; c++) {
+        const int P = cand[c];
+        const double cost = (double)((nz + P - 1) / P) * (P + 0.7);
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = P; }
+    }
+    return best;
+}
+
+template <bool SPLIT>
+static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st, const FFJob *jobs, int njobs,
+                             const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
+    const dim3 grid((unsigned)ntiles), block(FF_THREADS);
+    if (!zcol) {
+        ff_kernel<4, SPLIT, false><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
+    } else if (P == 10) {
+        ff_kernel<10, SPLIT, true><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
+    } else if (P == 5) {
+        ff_kernel<5, SPLIT, true><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
+    } else {
+        ff_kernel<8, SPLIT, true><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
+    }
+    return cudaGetLastError();
+}
+
+static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *d_xyzq, const int32_t *d_type,
+                           int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
+                           const ppfm_probe *probes, const ppfm_grid *grids, double r_min, float *d_a, float *d_b,
+                           bool split, void *cuda_stream) {
+    if (nsys < 1 || !h_atom_offset || !h_R || !h_e || !lattices || !probes || !grids || !d_a) return PPFM_EINVAL;
+    if (h_atom_offset[nsys] > 0 && (!d_xyzq || !d_type)) return PPFM_EINVAL;   // an empty atom list may be NULL
+    if (split && !d_b) return PPFM_EINVAL;
+    if (ntypes < 1 || ntypes > PPFM_MAX_TYPES) return PPFM_EINVAL;
+    if (!(r_min >= 0.0) || !std::isfinite(r_min)) return PPFM_EINVAL;
+    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_a & 15) || (d_b && ((uintptr_t)d_b & 15))) return PPFM_EINVAL;
+    for (int t = 0; t < ntypes; t++)
+        if (!(h_R[t] >= 0.0) || !(h_e[t] >= 0.0) || !std::isfinite(h_R[t]) || !std::isfinite(h_e[t])) return PPFM_EINVAL;
+    if (h_atom_offset[0] != 0) return PPFM_EINVAL;
+
+    // choose one P / column mode for the launch
+    bool zcol = true;
+    int nz_common = grids[0].n[2];
+    for (int m = 0; m < nsys; m++) {
+        const ppfm_grid &g = grids[m];
+        if (!grid_ok(&g)) return PPFM_EINVAL;
+        if (h_atom_offset[m + 1] < h_atom_offset[m]) return PPFM_EINVAL;
+        const ppfm_probe &pr = probes[m];
+        if (!(pr.R >= 0.0) || !(pr.e >= 0.0) || !std::isfinite(pr.R) || !std::isfinite(pr.e) || !std::isfinite(pr.Q))
+            return PPFM_EINVAL;
+        for (int a = 0; a < 3; a++)
+            if (lattices[m].nimg[a] < 0 || lattices[m].nimg[a] > 64) return PPFM_EINVAL;
+        if (g.step[2][0] != 0.0 || g.step[2][1] != 0.0) zcol = false;
+        if (g.n[2] != nz_common) nz_common = -1;
+    }
+    const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2]) : 4;
+
+    const size_t jobs_bytes = (size_t)nsys * sizeof(FFJob);
+    const size_t table_bytes = (size_t)nsys * ntypes * sizeof(TypeEntry);
+    const size_t flags_off = (jobs_bytes + table_bytes + 15) & ~(size_t)15;
+    const size_t flags_bytes = ((size_t)nsys * sizeof(int) + 15) & ~(size_t)15;
+    const size_t recs_off = flags_off + flags_bytes;
+    const int natoms_total = h_atom_offset[nsys];
+    const size_t recs_bytes = (size_t)(natoms_total > 0 ? natoms_total : 1) * sizeof(AtomRec);
+    const size_t total_bytes = recs_off + recs_bytes;
+
+    unsigned char *h_buf = (unsigned char *)malloc(flags_off);
+    if (!h_buf) return PPFM_ENOMEM;
+    memset(h_buf, 0, flags_off);
+    FFJob *hj = reinterpret_cast<FFJob *>(h_buf);
+    TypeEntry *ht = reinterpret_cast<TypeEntry *>(h_buf + jobs_bytes);
+    long long tile = 0, out_off = 0;
+    for (int m = 0; m < nsys; m++) {
+        const ppfm_grid &g = grids[m];
+        FFJob &j = hj[m];
+        j.tile_begin = tile;
+        j.out_offset = out_off;
+        j.atom_begin = h_atom_offset[m];
+        j.natoms = h_atom_offset[m + 1] - h_atom_offset[m];
+        j.nx = g.n[0]; j.ny = g.n[1]; j.nz = g.n[2]; j.nxy = g.n[0] * g.n[1];
+        j.n_xy_tiles = (j.nxy + FF_THREADS - 1) / FF_THREADS;
+        j.n_z_groups = (j.nz + P - 1) / P;
+        j.table_offset = m * ntypes;
+        j.ntypes = ntypes;
+        for (int a = 0; a < 3; a++) {
+            j.nimg[a] = lattices[m].nimg[a];
+            j.origin[a] = g.origin[a];
+            for (int c = 0; c < 3; c++) j.step[a][c] = g.step[a][c];
+            j.cell[0][a] = lattices[m].a[a];
+            j.cell[1][a] = lattices[m].b[a];
+            j.cell[2][a] = lattices[m].c[a];
+        }
+        for (int c = 0; c < 3; c++) {
+            double lo = g.origin[c], hi = g.origin[c];
+            for (int corner = 1; corner < 8; corner++) {
+                double x = g.origin[c];
+                for (int a = 0; a < 3; a++)
+                    if (corner & (1 << a)) x += (g.n[a] - 1) * g.step[a][c];
+                lo = std::fmin(lo, x); hi = std::fmax(hi, x);
+            }
+            j.bb_lo[c] = lo; j.bb_hi[c] = hi;
+        }
+        j.keQ = (float)(kCoulomb * probes[m].Q);
+        j.rmin2 = (float)(r_min * r_min);
+        for (int t = 0; t < ntypes; t++) {   // mixing rules
+            const double R0 = h_R[t] + probes[m].R;
+            const double E0 = std::sqrt(h_e[t] * probes[m].e);
+            const double R6 = R0 * R0 * R0 * R0 * R0 * R0;
+            ht[m * ntypes + t].c6 = (float)(2.0 * E0 * R6);
+            ht[m * ntypes + t].c12 = (float)(E0 * R6 * R6);
+        }
+        tile += (long long)j.n_xy_tiles * j.n_z_groups;
+        out_off += grid_points(&g);
+    }
+    if (tile > 0x7fffffffLL) { free(h_buf); return PPFM_EINVAL; }
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned char *d_buf = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&d_buf, total_bytes, st);
+    if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "cudaMallocAsync"); return PPFM_ENOMEM; }
+    e = cudaMemcpyAsync(d_buf, h_buf, flags_off, cudaMemcpyHostToDevice, st);   // pageable: staged before return
+    free(h_buf);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_buf + flags_off, 0, flags_bytes, st);
+    if (e != cudaSuccess) { set_cuda_error(e, "scratch upload"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+    const FFJob *dj = reinterpret_cast<const FFJob *>(d_buf);
+    const TypeEntry *dt = reinterpret_cast<const TypeEntry *>(d_buf + jobs_bytes);
+    int *dflags = reinterpret_cast<int *>(d_buf + flags_off);
+    AtomRec *drecs = reinterpret_cast<AtomRec *>(d_buf + recs_off);
+    if (natoms_total > 0) {
+        ff_prep_kernel<<<(natoms_total + 127) / 128, 128, 0, st>>>(dj, nsys, dt, reinterpret_cast<const float4 *>(d_xyzq),
+                                                                   d_type, drecs, dflags, natoms_total);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { set_cuda_error(e, "ff_prep_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+        count_launch();
+    }
+    if (tile > 0) {
+        e = split ? launch_ff<true>(P, zcol, tile, st, dj, nsys, dflags, drecs, reinterpret_cast<float4 *>(d_a),
+                                    reinterpret_cast<float4 *>(d_b))
+                  : launch_ff<false>(P, zcol, tile, st, dj, nsys, dflags, drecs, reinterpret_cast<float4 *>(d_a),
+                                     nullptr);
+        if (e != cudaSuccess) { set_cuda_error(e, "ff_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+        count_launch();
+    }
+    PPFM_CUDA(cudaFreeAsync(d_buf, st));
+    return PPFM_OK;
+}
+
+}  // namespace ppfm
+
+using namespace ppfm;
+
+extern "C" int ppfm_forcefield(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                               const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                               const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
+                               void *cuda_stream) {
+    if (natoms < 0) return PPFM_EINVAL;
+    const int32_t off[2] = {0, natoms};
+    return forcefield_impl(1, off, d_xyzq, d_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, d_ff, nullptr,
+                           false, cuda_stream);
+}
+
+extern "C" int ppfm_forcefield_split(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                                     const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                                     const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff_lj,
+                                     float *d_ff_el, void *cuda_stream) {
+    if (natoms < 0) return PPFM_EINVAL;
+    const int32_t off[2] = {0, natoms};
+    return forcefield_impl(1, off, d_xyzq, d_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, d_ff_lj, d_ff_el,
+                           true, cuda_stream);
+}
+
+extern "C" int ppfm_forcefield_batch(int32_t nsys, const int32_t *h_atom_offset, const float *d_xyzq,
+                                     const int32_t *d_type, int32_t ntypes, const double *h_R, const double *h_e,
+                                     const ppfm_lattice *lattices, const ppfm_probe *probes, const ppfm_grid *grids,
+                                     double r_min, float *d_ff, void *cuda_stream) {
+    return forcefield_impl(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min,
+                           d_ff, nullptr, false, cuda_stream);
+}
+
+extern "C" int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q, int64_t n_points, float *d_out,
+                            void *cuda_stream) {
+    if (!d_ff_lj || !d_ff_el || !d_out || n_points < 0 || !std::isfinite(Q)) return PPFM_EINVAL;
+    if (((uintptr_t)d_ff_lj & 15) || ((uintptr_t)d_ff_el & 15) || ((uintptr_t)d_out & 15)) return PPFM_EINVAL;
+    if (n_points == 0) return PPFM_OK;
+    long long blocks = (n_points + 255) / 256;
+    if (blocks > 148LL * 16) blocks = 148LL * 16;
+    combine_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(
+        reinterpret_cast<const float4 *>(d_ff_lj), reinterpret_cast<const float4 *>(d_ff_el), (float)Q, n_points,
+        reinterpret_cast<float4 *>(d_out));
+    PPFM_LAUNCH_CHECK();
+    return PPFM_OK;
+}

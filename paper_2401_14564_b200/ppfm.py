@@ -1,0 +1,349 @@
+"""Thin Python binding over the C-ABI library libppfm.so (include/ppfm.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; torch is used for device memory and streams.
+There is no CPU fallback: if libppfm.so is missing or no CUDA device is present the calls raise.
+Function names mirror the C entry points (forcefield, relax_scan, df, ..., scan_host).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libppfm.so")
+_lib = None
+
+
+class PpfmError(RuntimeError):
+    pass
+
+
+# ---- ctypes mirrors of the structs in include/ppfm.h -------------------------------------------------------
+class Lattice(C.Structure):
+    _fields_ = [("a", C.c_double * 3), ("b", C.c_double * 3), ("c", C.c_double * 3), ("nimg", C.c_int32 * 3)]
+
+
+class Grid(C.Structure):
+    _fields_ = [("origin", C.c_double * 3), ("step", (C.c_double * 3) * 3), ("n", C.c_int32 * 3),
+                ("periodic", C.c_int32 * 3)]
+
+
+class Probe(C.Structure):
+    _fields_ = [("R", C.c_double), ("e", C.c_double), ("Q", C.c_double)]
+
+
+class Tip(C.Structure):
+    _fields_ = [("k_lat", C.c_double * 2), ("k_rad", C.c_double), ("d0", C.c_double * 3)]
+
+
+class Fire(C.Structure):
+    _fields_ = [("dt", C.c_double), ("dt_max", C.c_double), ("finc", C.c_double), ("fdec", C.c_double),
+                ("alpha0", C.c_double), ("falpha", C.c_double), ("n_min", C.c_int32), ("max_iter", C.c_int32),
+                ("f_conv", C.c_double)]
+
+
+class Scan(C.Structure):
+    _fields_ = [("p0", C.c_double * 3), ("dx", C.c_double * 3), ("dy", C.c_double * 3), ("npx", C.c_int32),
+                ("npy", C.c_int32), ("nz", C.c_int32), ("dz", C.c_double)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("total_iters", C.c_uint64), ("n_not_converged", C.c_uint64), ("n_clamped", C.c_uint64),
+                ("max_iters", C.c_uint32), ("_pad", C.c_uint32)]
+
+
+EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
+           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_relax_scan",
+           "ppfm_relax_scan_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
+           "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count"]
+
+
+def lib():
+    """Load libppfm.so (fails loudly when it has not been built: `python -m paper_2401_14564_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise PpfmError(f"{LIB_PATH} not found — build it with `python -m paper_2401_14564_b200.build`; "
+                            "there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        L.ppfm_version.restype = C.c_int
+        L.ppfm_strerror.restype = C.c_char_p
+        L.ppfm_strerror.argtypes = [C.c_int]
+        L.ppfm_Nm_to_eVA2.restype = C.c_double
+        L.ppfm_Nm_to_eVA2.argtypes = [C.c_double]
+        L.ppfm_launch_count.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise PpfmError(f"{what} failed: {rc} ({lib().ppfm_strerror(rc).decode()})")
+
+
+def version() -> int:
+    return int(lib().ppfm_version())
+
+
+def launch_count() -> int:
+    return int(lib().ppfm_launch_count())
+
+
+def Nm_to_eVA2(k: float) -> float:
+    return float(lib().ppfm_Nm_to_eVA2(k))
+
+
+def fire_default() -> Fire:
+    f = Fire()
+    lib().ppfm_fire_default(C.byref(f))
+    return f
+
+
+# ---- marshalling from workloads.* dataclasses (or anything with the same attributes) ------------------------
+def _vec(ctype, vals):
+    return ctype(*[float(v) for v in vals])
+
+
+def c_lattice(l) -> Lattice:
+    return Lattice(_vec(C.c_double * 3, l.a), _vec(C.c_double * 3, l.b), _vec(C.c_double * 3, l.c),
+                   (C.c_int32 * 3)(*[int(v) for v in l.nimg]))
+
+
+def c_grid(g) -> Grid:
+    out = Grid()
+    for a in range(3):
+        out.origin[a] = float(g.origin[a])
+        out.n[a] = int(g.n[a])
+        out.periodic[a] = int(g.periodic[a])
+        for c in range(3):
+            out.step[a][c] = float(g.step[a][c])
+    return out
+
+
+def c_probe(p, Q: Optional[float] = None) -> Probe:
+    return Probe(float(p.R), float(p.e), float(p.Q if Q is None else Q))
+
+
+def c_tip(t) -> Tip:
+    return Tip(_vec(C.c_double * 2, t.k_lat), float(t.k_rad), _vec(C.c_double * 3, t.d0))
+
+
+def c_fire(f) -> Fire:
+    return Fire(float(f.dt), float(f.dt_max), float(f.finc), float(f.fdec), float(f.alpha0), float(f.falpha),
+                int(f.n_min), int(f.max_iter), float(f.f_conv))
+
+
+def c_scan(s) -> Scan:
+    return Scan(_vec(C.c_double * 3, s.p0), _vec(C.c_double * 3, s.dx), _vec(C.c_double * 3, s.dy), int(s.npx),
+                int(s.npy), int(s.nz), float(s.dz))
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise PpfmError("no CUDA device: the ppfm hot path runs only on the GPU (no CPU fallback)")
+    return torch
+
+
+def _stream():
+    return C.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+
+def _dptr(t, dtype=None):
+    if t is None:
+        return C.c_void_p(0)
+    torch = _torch()
+    if not t.is_cuda or not t.is_contiguous():
+        raise PpfmError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise PpfmError(f"expected dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _darr(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+# ---- (1) force field ----------------------------------------------------------------------------------------
+def forcefield(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out=None, Q=None):
+    """ppfm_forcefield: xyzq (N,4) float32 CUDA, types (N,) int32 CUDA -> (nz, ny, nx, 4) float32 CUDA."""
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in grid.n)
+    if out is None:
+        out = torch.empty((nz, ny, nx, 4), dtype=torch.float32, device=xyzq.device)
+    R, pR = _darr(elem_R)
+    e, pe = _darr(elem_e)
+    rc = lib().ppfm_forcefield(C.c_int32(xyzq.shape[0]), _dptr(xyzq, torch.float32), _dptr(types, torch.int32),
+                               C.c_int32(len(R)), pR, pe, C.byref(c_lattice(lattice)), C.byref(c_probe(probe, Q)),
+                               C.byref(c_grid(grid)), C.c_double(r_min), _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_forcefield")
+    return out
+
+
+def forcefield_split(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out_lj=None, out_el=None):
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in grid.n)
+    if out_lj is None:
+        out_lj = torch.empty((nz, ny, nx, 4), dtype=torch.float32, device=xyzq.device)
+    if out_el is None:
+        out_el = torch.empty((nz, ny, nx, 4), dtype=torch.float32, device=xyzq.device)
+    R, pR = _darr(elem_R)
+    e, pe = _darr(elem_e)
+    rc = lib().ppfm_forcefield_split(C.c_int32(xyzq.shape[0]), _dptr(xyzq, torch.float32),
+                                     _dptr(types, torch.int32), C.c_int32(len(R)), pR, pe,
+                                     C.byref(c_lattice(lattice)), C.byref(c_probe(probe)), C.byref(c_grid(grid)),
+                                     C.c_double(r_min), _dptr(out_lj, torch.float32), _dptr(out_el, torch.float32),
+                                     _stream())
+    _check(rc, "ppfm_forcefield_split")
+    return out_lj, out_el
+
+
+def combine(ff_lj, ff_el, Q: float, out=None):
+    torch = _torch()
+    if out is None:
+        out = torch.empty_like(ff_lj)
+    rc = lib().ppfm_combine(_dptr(ff_lj, torch.float32), _dptr(ff_el, torch.float32), C.c_double(Q),
+                            C.c_int64(ff_lj.numel() // 4), _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_combine")
+    return out
+
+
+def forcefield_batch(atom_offset: Sequence[int], xyzq, types, elem_R, elem_e, lattices, probes, grids, r_min=0.1,
+                     out=None):
+    """ppfm_forcefield_batch: concatenated atoms, one launch; returns a flat (sum points, 4) float32 tensor."""
+    torch = _torch()
+    nsys = len(grids)
+    off = (C.c_int32 * (nsys + 1))(*[int(v) for v in atom_offset])
+    lat = (Lattice * nsys)(*[c_lattice(l) for l in lattices])
+    pr = (Probe * nsys)(*[c_probe(p) for p in probes])
+    gr = (Grid * nsys)(*[c_grid(g) for g in grids])
+    npts = sum(int(g.n[0]) * int(g.n[1]) * int(g.n[2]) for g in grids)
+    if out is None:
+        out = torch.empty((npts, 4), dtype=torch.float32, device=xyzq.device)
+    R, pR = _darr(elem_R)
+    e, pe = _darr(elem_e)
+    rc = lib().ppfm_forcefield_batch(C.c_int32(nsys), off, _dptr(xyzq, torch.float32), _dptr(types, torch.int32),
+                                     C.c_int32(len(R)), pR, pe, lat, pr, gr, C.c_double(r_min),
+                                     _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_forcefield_batch")
+    return out
+
+
+# ---- (2) relaxation scan --------------------------------------------------------------------------------------
+def new_stats(device="cuda"):
+    torch = _torch()
+    return torch.zeros(4, dtype=torch.int64, device=device)      # 32 bytes = sizeof(ppfm_stats)
+
+
+def read_stats(stats) -> dict:
+    raw = stats.cpu().numpy().view(np.uint64)
+    return {"total_iters": int(raw[0]), "n_not_converged": int(raw[1]), "n_clamped": int(raw[2]),
+            "max_iters": int(raw[3] & np.uint64(0xFFFFFFFF))}
+
+
+def relax_scan(ff, grid, tip, fire, scan, pos_fz=None, iters=None, stats=None, want_iters=True):
+    """ppfm_relax_scan -> (pos_fz (nz, npy, npx, 4) float32, iters (nz, npy, npx) int16-as-uint16 or None)."""
+    torch = _torch()
+    shape = (int(scan.nz), int(scan.npy), int(scan.npx))
+    if pos_fz is None:
+        pos_fz = torch.empty(shape + (4,), dtype=torch.float32, device=ff.device)
+    if iters is None and want_iters:
+        iters = torch.empty(shape, dtype=torch.int16, device=ff.device)
+    rc = lib().ppfm_relax_scan(_dptr(ff, torch.float32), C.byref(c_grid(grid)), C.byref(c_tip(tip)),
+                               C.byref(c_fire(fire)), C.byref(c_scan(scan)), _dptr(pos_fz, torch.float32),
+                               _dptr(iters), _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan")
+    return pos_fz, iters
+
+
+def relax_scan_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, stats=None, want_iters=True):
+    torch = _torch()
+    nsys = len(grids)
+    gr = (Grid * nsys)(*[c_grid(g) for g in grids])
+    tp = (Tip * nsys)(*[c_tip(t) for t in tips])
+    sc = (Scan * nsys)(*[c_scan(s) for s in scans])
+    nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in scans)
+    if pos_fz is None:
+        pos_fz = torch.empty((nps, 4), dtype=torch.float32, device=ff.device)
+    if iters is None and want_iters:
+        iters = torch.empty((nps,), dtype=torch.int16, device=ff.device)
+    rc = lib().ppfm_relax_scan_batch(C.c_int32(nsys), _dptr(ff, torch.float32), gr, tp, C.byref(c_fire(fire)), sc,
+                                     _dptr(pos_fz, torch.float32), _dptr(iters), _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan_batch")
+    return pos_fz, iters
+
+
+# ---- (3) df ------------------------------------------------------------------------------------------------------
+def df(pos_fz, npx, npy, nz, dz, A, k0, f0, out=None, nsys=1):
+    torch = _torch()
+    n = int(round(A / dz))
+    if out is None:
+        shape = (max(nz - n, 0), npy, npx) if nsys == 1 else (nsys, max(nz - n, 0), npy, npx)
+        out = torch.empty(shape, dtype=torch.float32, device=pos_fz.device)
+    if nsys == 1:
+        rc = lib().ppfm_df(_dptr(pos_fz, torch.float32), C.c_int32(npx), C.c_int32(npy), C.c_int32(nz),
+                           C.c_double(dz), C.c_double(A), C.c_double(k0), C.c_double(f0),
+                           _dptr(out, torch.float32), _stream())
+    else:
+        rc = lib().ppfm_df_batch(C.c_int32(nsys), _dptr(pos_fz, torch.float32), C.c_int32(npx), C.c_int32(npy),
+                                 C.c_int32(nz), C.c_double(dz), C.c_double(A), C.c_double(k0), C.c_double(f0),
+                                 _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_df")
+    return out
+
+
+def df_weights(n: int, dz: float) -> np.ndarray:
+    W = np.empty(n + 1)
+    _check(lib().ppfm_df_weights(C.c_int32(n), C.c_double(dz), W.ctypes.data_as(C.POINTER(C.c_double))),
+           "ppfm_df_weights")
+    return W
+
+
+# ---- whole simulation, host buffers ------------------------------------------------------------------------------
+def scan_host(w, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None, Q=None) -> dict:
+    """ppfm_scan_host on a workload: host (ideally pinned) torch CPU tensors or numpy arrays in and out."""
+    _torch()
+
+    def hp(x):
+        if x is None:
+            return C.c_void_p(0)
+        return C.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data)
+
+    R, pR = _darr(w.elem_R)
+    e, pe = _darr(w.elem_e)
+    st = Stats()
+    rc = lib().ppfm_scan_host(C.c_int32(int(h_xyzq.shape[0])), hp(h_xyzq), hp(h_types), C.c_int32(len(R)), pR, pe,
+                              C.byref(c_lattice(w.lattice)), C.byref(c_probe(w.probe, Q)), C.byref(c_grid(w.grid)),
+                              C.c_double(w.r_min), C.byref(c_tip(w.tip)), C.byref(c_fire(w.fire)),
+                              C.byref(c_scan(w.scan)), C.c_double(w.df.A), C.c_double(w.df.k0), C.c_double(w.df.f0),
+                              hp(h_pos_fz), hp(h_iters), hp(h_df), C.byref(st), _stream())
+    _check(rc, "ppfm_scan_host")
+    return {"total_iters": int(st.total_iters), "n_not_converged": int(st.n_not_converged),
+            "n_clamped": int(st.n_clamped), "max_iters": int(st.max_iters)}
+
+
+# ---- probes --------------------------------------------------------------------------------------------------------
+def probe_fma() -> float:
+    _torch()
+    v = C.c_double(0.0)
+    _check(lib().ppfm_probe_fma(C.byref(v), _stream()), "ppfm_probe_fma")
+    return v.value
+
+
+def probe_gather(n_float4: int, bypass_l1: bool) -> float:
+    _torch()
+    v = C.c_double(0.0)
+    _check(lib().ppfm_probe_gather(C.c_int64(n_float4), C.c_int32(int(bypass_l1)), C.byref(v), _stream()),
+           "ppfm_probe_gather")
+    return v.value
+
+
+# ---- convenience: run a workloads.Workload end to end on device-resident inputs ------------------------------------
+def upload(w, device="cuda"):
+    torch = _torch()
+    return (torch.from_numpy(np.ascontiguousarray(w.xyzq, dtype=np.float32)).to(device),
+            torch.from_numpy(np.ascontiguousarray(w.types, dtype=np.int32)).to(device))

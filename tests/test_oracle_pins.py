@@ -364,7 +364,7 @@ def test_fire_finds_a_true_minimum_newton_crosscheck_cfg0():
     pix = W.sample_indices(w.scan.npx * w.scan.npy, 40, 5)
     r = oracle.relax_scan(ff, w.grid, w.tip, w.fire, w.scan, pix=pix)
     assert np.all(r["iters"] >= 0)
-    flagged = oracle.near_unstable(r["lam_min"])
+    flagged = oracle.flags(r)
     worst = 0.0
     for iz in range(0, w.scan.nz, 3):
         for m, p in enumerate(pix):
@@ -401,7 +401,7 @@ def test_relaxed_positions_mirror_symmetric_molecule():
     assert np.allclose(ff[..., 0], -ff[:, :, ::-1, 0], rtol=1e-9, atol=1e-12)
     r = oracle.relax_scan(ff, w.grid, w.tip, replace(w.fire, f_conv=1e-9, max_iter=20000), w.scan)
     pos = r["pos_fz"].reshape(w.scan.nz, w.scan.npy, w.scan.npx, 4)
-    ok = ~oracle.near_unstable(r["lam_min"]).reshape(w.scan.nz, w.scan.npy, w.scan.npx)
+    ok = ~oracle.flags(r).reshape(w.scan.nz, w.scan.npy, w.scan.npx)
     ok &= ok[:, :, ::-1]
     assert ok.mean() > 0.9
     assert np.allclose((pos[..., 0] + pos[:, :, ::-1, 0])[ok], 12.0, atol=1e-5)
@@ -520,3 +520,21 @@ def test_golden_constants_are_what_the_generators_use():
     w = W.get(0)
     assert w.tip.k_lat[0] == pytest.approx(GOLD["k_xy_Nm"] / NM) and w.tip.d0 == (0.0, 0.0, -GOLD["R_rest_A"])
     assert (w.df.A, w.df.k0, w.df.f0) == (GOLD["A_A"], GOLD["k0_Nm"], GOLD["f0_Hz"])
+
+
+def test_trajectory_stability_diagnostic():
+    """lam_traj (reading S17) is the minimum over the trajectory: equals lam_min when no move is made, never
+    exceeds it, and goes negative on a step that starts on a maximum of the lateral potential."""
+    g, ff = _flat_grid()
+    tip = W._default_tip()
+    r = oracle.relax_scan(ff, g, tip, W.Fire(), _scan(nz=3))
+    assert np.array_equal(r["lam_traj"], r["lam_min"])                    # zero field: single-point trajectories
+    ff[..., 2] = 0.03
+    r = oracle.relax_scan(ff, g, tip, W.Fire(), _scan(nz=3))
+    assert np.all(r["lam_traj"] <= r["lam_min"] + 1e-15)
+    # uniform upward push beyond k_xy R_rest: the on-axis start point is laterally unstable (closed form above)
+    ff[..., 2] = 0.07
+    ff[..., 0] = 1e-4                                                     # break the symmetry so FIRE leaves the axis
+    r = oracle.relax_scan(ff, g, tip, replace(W.Fire(), max_iter=5000), _scan(nz=1))
+    assert np.all(r["lam_traj"] < 0) and np.all(r["lam_min"] > 0)
+    assert np.all(oracle.flags(r))
