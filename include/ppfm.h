@@ -12,9 +12,10 @@
  *          k0 in N/m and f0 in Hz (ppfm_df).  k_e = 14.399645478 eV·Å/e^2;  1 eV/Å^2 = 16.02176634 N/m.
  *   Pointers: a `d_` prefix = DEVICE memory on the current CUDA device, `h_` prefix = HOST memory.  Structs
  *          passed by pointer are HOST memory and are read before the call returns.
- *   Ownership: every buffer is allocated and freed by the caller.  The library keeps no pointer after return and
- *          holds no persistent device memory; per-call scratch is stream-ordered (cudaMallocAsync / cudaFreeAsync
- *          on `cuda_stream`).  Device entry points only enqueue work on `cuda_stream` (a cudaStream_t cast to
+ *   Ownership: every buffer is allocated and freed by the caller.  The library keeps no pointer to caller memory
+ *          after return; per-call scratch is stream-ordered (allocated and freed on `cuda_stream` inside the call)
+ *          from a library-private pool that caches freed blocks until ppfm_release_scratch().
+ *          Device entry points only enqueue work on `cuda_stream` (a cudaStream_t cast to
  *          void*, NULL = default stream); they never synchronise it and never change the current device.
  *          Host entry points (ppfm_scan_host) synchronise the stream before returning.
  *   Errors: 0 on success, a negative ppfm_status otherwise; no exceptions, no exit(), no output.  Per-pixel
@@ -187,6 +188,28 @@ int ppfm_probe_gather(int64_t n_float4, int32_t bypass_l1, double *h_gbs, void *
 
 /* Number of kernels this library has launched on this process so far (for bench.py's gpu_launches). */
 int64_t ppfm_launch_count(void);
+
+/* Per-kernel device timing for the roofline legs of bench.py: while enabled, every launch of the kernels below is
+ * bracketed by CUDA events recorded on the launching stream directly around the launch (no host work in between).
+ * ppfm_timing_enable(on) clears the accumulators; ppfm_timing_read waits for the recorded events of `kernel_id`
+ * (it synchronises on them, not on the stream) and returns the summed milliseconds and the number of launches.
+ * Off by default; process-wide. */
+typedef enum {
+    PPFM_K_FF_PREP = 0, /* a1 atom-record packing            */
+    PPFM_K_FF = 1,      /* a2 force-field grid               */
+    PPFM_K_COMBINE = 2, /* a3 F_LJ + Q F_el                  */
+    PPFM_K_RELAX = 3,   /* a4+a5 relaxation scan             */
+    PPFM_K_DF = 4,      /* a6 frequency shift                */
+    PPFM_K_COUNT = 5
+} ppfm_kernel_id;
+int ppfm_timing_enable(int on);
+int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);
+
+/* Scratch memory.  Per-call scratch (packed atom records, job tables; for ppfm_scan_host also the grid and the
+ * scan buffers) comes from a library-private stream-ordered pool of the current device, so steady-state calls make
+ * no driver allocation.  Freed blocks stay cached in that pool; ppfm_release_scratch() returns them to the driver
+ * (call it when the stream work has completed). */
+int ppfm_release_scratch(void);
 
 #ifdef __cplusplus
 }

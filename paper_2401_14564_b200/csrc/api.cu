@@ -2,13 +2,86 @@
 // two measurement probes that define the roofline denominators on the box.
 #include "common.cuh"
 
+#include <mutex>
+#include <vector>
+
 namespace ppfm {
 
 std::atomic<long long> g_launches{0};
+std::atomic<int> g_timing_on{0};
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
 void set_cuda_error(cudaError_t e, const char *where) {
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), where);
+}
+
+// ---- private scratch pool (one per device, created on first use) ---------------------------------------------------
+static std::mutex g_pool_mu;
+static cudaMemPool_t g_pools[64] = {};
+
+static cudaError_t get_pool(cudaMemPool_t *out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        e = cudaMemPoolCreate(&g_pools[dev], &props);
+        if (e != cudaSuccess) { g_pools[dev] = nullptr; return e; }
+        unsigned long long keep = ~0ull;          // keep freed blocks until ppfm_release_scratch()
+        cudaMemPoolSetAttribute(g_pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    *out = g_pools[dev];
+    return cudaSuccess;
+}
+
+cudaError_t scratch_alloc(void **ptr, size_t bytes, cudaStream_t st) {
+    cudaMemPool_t pool;
+    cudaError_t e = get_pool(&pool);
+    if (e != cudaSuccess) return e;
+    return cudaMallocFromPoolAsync(ptr, bytes ? bytes : 1, pool, st);
+}
+
+// ---- per-kernel timing ---------------------------------------------------------------------------------------------
+struct PendingTiming { int id; cudaEvent_t e0, e1; };
+static std::mutex g_tm_mu;
+static std::vector<PendingTiming> g_tm_pending;
+static double g_tm_ms[PPFM_K_COUNT] = {};
+static long long g_tm_n[PPFM_K_COUNT] = {};
+
+void timing_begin(int, cudaStream_t st, cudaEvent_t *e0) {
+    if (cudaEventCreate(e0) != cudaSuccess) { *e0 = nullptr; return; }
+    cudaEventRecord(*e0, st);
+}
+
+void timing_end(int kernel_id, cudaStream_t st, cudaEvent_t e0) {
+    if (!e0) return;
+    cudaEvent_t e1;
+    if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return; }
+    cudaEventRecord(e1, st);
+    std::lock_guard<std::mutex> lk(g_tm_mu);
+    g_tm_pending.push_back({kernel_id, e0, e1});
+}
+
+static void timing_drain(bool accumulate) {
+    std::lock_guard<std::mutex> lk(g_tm_mu);
+    for (auto &p : g_tm_pending) {
+        if (accumulate && cudaEventSynchronize(p.e1) == cudaSuccess) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, p.e0, p.e1) == cudaSuccess && p.id >= 0 && p.id < PPFM_K_COUNT) {
+                g_tm_ms[p.id] += ms;
+                g_tm_n[p.id] += 1;
+            }
+        }
+        cudaEventDestroy(p.e0);
+        cudaEventDestroy(p.e1);
+    }
+    g_tm_pending.clear();
 }
 
 // ---- probe 1: FP32 FMA issue rate (the denominator of the force-field kernel's pipe utilisation) ----------------
@@ -93,6 +166,33 @@ extern "C" double ppfm_Nm_to_eVA2(double k_Nm) { return k_Nm / kEVA2toNm; }
 
 extern "C" int64_t ppfm_launch_count(void) { return (int64_t)g_launches.load(); }
 
+extern "C" int ppfm_timing_enable(int on) {
+    timing_drain(false);
+    {
+        std::lock_guard<std::mutex> lk(g_tm_mu);
+        for (int k = 0; k < PPFM_K_COUNT; k++) { g_tm_ms[k] = 0.0; g_tm_n[k] = 0; }
+    }
+    g_timing_on.store(on ? 1 : 0);
+    return PPFM_OK;
+}
+
+extern "C" int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches) {
+    if (kernel_id < 0 || kernel_id >= PPFM_K_COUNT || !h_ms_total || !h_launches) return PPFM_EINVAL;
+    timing_drain(true);
+    std::lock_guard<std::mutex> lk(g_tm_mu);
+    *h_ms_total = g_tm_ms[kernel_id];
+    *h_launches = (int64_t)g_tm_n[kernel_id];
+    return PPFM_OK;
+}
+
+extern "C" int ppfm_release_scratch(void) {
+    int dev = 0;
+    PPFM_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    if (dev >= 0 && dev < 64 && g_pools[dev]) PPFM_CUDA(cudaMemPoolTrimTo(g_pools[dev], 0));
+    return PPFM_OK;
+}
+
 extern "C" int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t *h_type, int32_t ntypes,
                               const double *h_R, const double *h_e, const ppfm_lattice *lattice,
                               const ppfm_probe *probe, const ppfm_grid *grid, double r_min, const ppfm_tip *tip,
@@ -117,13 +217,13 @@ extern "C" int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t
     auto fail = [&](cudaError_t e, const char *w) { set_cuda_error(e, w); rc = (e == cudaErrorMemoryAllocation) ? PPFM_ENOMEM : PPFM_ECUDA; };
     cudaError_t e;
 #define TRY(x) if (rc == PPFM_OK && (e = (x)) != cudaSuccess) fail(e, #x)
-    TRY(cudaMallocAsync((void **)&d_xyzq, na * 16, st));
-    TRY(cudaMallocAsync((void **)&d_type, na * 4, st));
-    TRY(cudaMallocAsync((void **)&d_ff, npts * 16, st));
-    TRY(cudaMallocAsync((void **)&d_pos, nps * 16, st));
-    TRY(cudaMallocAsync((void **)&d_it, nps * 2, st));
-    TRY(cudaMallocAsync((void **)&d_stats, sizeof(ppfm_stats), st));
-    if (h_df) TRY(cudaMallocAsync((void **)&d_df, ndf * 4, st));
+    TRY(scratch_alloc((void **)&d_xyzq, na * 16, st));
+    TRY(scratch_alloc((void **)&d_type, na * 4, st));
+    TRY(scratch_alloc((void **)&d_ff, npts * 16, st));
+    TRY(scratch_alloc((void **)&d_pos, nps * 16, st));
+    TRY(scratch_alloc((void **)&d_it, nps * 2, st));
+    TRY(scratch_alloc((void **)&d_stats, sizeof(ppfm_stats), st));
+    if (h_df) TRY(scratch_alloc((void **)&d_df, ndf * 4, st));
     if (natoms > 0) {
         TRY(cudaMemcpyAsync(d_xyzq, h_xyzq, (size_t)natoms * 16, cudaMemcpyHostToDevice, st));
         TRY(cudaMemcpyAsync(d_type, h_type, (size_t)natoms * 4, cudaMemcpyHostToDevice, st));

@@ -22,6 +22,29 @@ void set_cuda_error(cudaError_t e, const char *where);
 extern std::atomic<long long> g_launches;
 inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+// Stream-ordered scratch from the library's private memory pool of the current device (api.cu): freed blocks stay
+// in the pool across calls (no driver allocation on the steady-state path) until ppfm_release_scratch().
+cudaError_t scratch_alloc(void **ptr, size_t bytes, cudaStream_t st);
+
+// Optional per-kernel device timing (ppfm_timing_enable / ppfm_timing_read): CUDA events recorded on the launching
+// stream immediately around one kernel launch.  Costs nothing when timing is off.
+extern std::atomic<int> g_timing_on;
+void timing_begin(int kernel_id, cudaStream_t st, cudaEvent_t *e0);
+void timing_end(int kernel_id, cudaStream_t st, cudaEvent_t e0);
+struct KernelTimer {
+    int id;
+    cudaStream_t st;
+    cudaEvent_t e0 = nullptr;
+    bool on;
+    KernelTimer(int kernel_id, cudaStream_t stream) : id(kernel_id), st(stream) {
+        on = g_timing_on.load(std::memory_order_relaxed) != 0;
+        if (on) timing_begin(id, st, &e0);
+    }
+    ~KernelTimer() {
+        if (on) timing_end(id, st, e0);
+    }
+};
+
 #define PPFM_CUDA(call)                                  \
     do {                                                 \
         cudaError_t _e = (call);                         \

@@ -69,8 +69,11 @@ static int df_impl(int nsys, const float *d_pos_fz, int npx, int npy, int nz, do
     const long long total = (long long)(nz - n) * npix * nsys;
     long long blocks = (total + 255) / 256;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
-    df_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(reinterpret_cast<const float4 *>(d_pos_fz), npix,
-                                                                      nz, (int)n, nsys, W, d_df);
+    {
+        KernelTimer kt(PPFM_K_DF, (cudaStream_t)cuda_stream);
+        df_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(reinterpret_cast<const float4 *>(d_pos_fz),
+                                                                          npix, nz, (int)n, nsys, W, d_df);
+    }
     PPFM_LAUNCH_CHECK();
     return PPFM_OK;
 }

@@ -49,17 +49,14 @@ struct TypeEntry {
 };
 
 // ---------------------------------------------------------------------------------------------------- a1 prep
-__global__ void ff_prep_kernel(const FFJob *__restrict__ jobs, int njobs, const TypeEntry *__restrict__ table,
-                               const float4 *__restrict__ xyzq, const int *__restrict__ type,
-                               AtomRec *__restrict__ recs, int *__restrict__ clamp_flags, int natoms_total) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= natoms_total) return;
-    int lo = 0, hi = njobs - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (jobs[mid].atom_begin <= i) lo = mid; else hi = mid - 1;
-    }
-    const FFJob &job = jobs[lo];
+struct FFSingle {               // one system: job and per-type table travel as a kernel parameter (constant bank)
+    FFJob job;
+    TypeEntry table[PPFM_MAX_TYPES];
+};
+
+__device__ __forceinline__ void prep_atom(const FFJob &job, const TypeEntry *__restrict__ table, int job_index,
+                                          const float4 *__restrict__ xyzq, const int *__restrict__ type,
+                                          AtomRec *__restrict__ recs, int *__restrict__ clamp_flags, int i) {
     const float4 a = xyzq[i];
     const int t = type[i];
     AtomRec r;
@@ -88,7 +85,28 @@ __global__ void ff_prep_kernel(const FFJob *__restrict__ jobs, int njobs, const 
                 }
                 near |= (d2 < rmin * rmin);
             }
-    if (near) atomicOr(&clamp_flags[lo], 1);
+    if (near) atomicOr(&clamp_flags[job_index], 1);
+}
+
+__global__ void ff_prep_kernel(const __grid_constant__ FFSingle one, const float4 *__restrict__ xyzq,
+                               const int *__restrict__ type, AtomRec *__restrict__ recs,
+                               int *__restrict__ clamp_flags, int natoms_total) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= natoms_total) return;
+    prep_atom(one.job, one.table, 0, xyzq, type, recs, clamp_flags, i);
+}
+
+__global__ void ff_prep_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const TypeEntry *__restrict__ table,
+                                     const float4 *__restrict__ xyzq, const int *__restrict__ type,
+                                     AtomRec *__restrict__ recs, int *__restrict__ clamp_flags, int natoms_total) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= natoms_total) return;
+    int lo = 0, hi = njobs - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (jobs[mid].atom_begin <= i) lo = mid; else hi = mid - 1;
+    }
+    prep_atom(jobs[lo], table, lo, xyzq, type, recs, clamp_flags, i);
 }
 
 // ---------------------------------------------------------------------------------------------------- PTX helpers
@@ -280,10 +298,40 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restr
     }
 }
 
+__device__ __forceinline__ void ff_init_barriers(uint64_t *full_bar, uint64_t *empty_bar) {
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < FF_STAGES; s++) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], FF_THREADS / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+}
+
+// One system: job in the constant bank (kernel parameter).
 template <int P, bool SPLIT, bool ZCOL>
 __global__ void __launch_bounds__(FF_THREADS, 2)
-ff_kernel(const FFJob *__restrict__ jobs, int njobs, const int *__restrict__ clamp_flags,
-          const AtomRec *__restrict__ recs, float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
+ff_kernel(const __grid_constant__ FFJob job, const int *__restrict__ clamp_flags, const AtomRec *__restrict__ recs,
+          float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
+    __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
+    __shared__ __align__(8) uint64_t full_bar[FF_STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[FF_STAGES];
+    __shared__ int s_clamp;
+    if (threadIdx.x == 0) s_clamp = clamp_flags[0];
+    ff_init_barriers(full_bar, empty_bar);
+    __syncthreads();
+    if (s_clamp)
+        ff_tile<P, SPLIT, true, ZCOL>(job, recs, out_a, out_b, s_rec, full_bar, empty_bar, (long long)blockIdx.x);
+    else
+        ff_tile<P, SPLIT, false, ZCOL>(job, recs, out_a, out_b, s_rec, full_bar, empty_bar, (long long)blockIdx.x);
+}
+
+// Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
+template <int P, bool SPLIT, bool ZCOL>
+__global__ void __launch_bounds__(FF_THREADS, 2)
+ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const int *__restrict__ clamp_flags,
+                const AtomRec *__restrict__ recs, float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
     __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
     __shared__ __align__(8) uint64_t full_bar[FF_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[FF_STAGES];
@@ -301,15 +349,8 @@ ff_kernel(const FFJob *__restrict__ jobs, int njobs, const int *__restrict__ cla
         int *dstw = reinterpret_cast<int *>(&s_job);
         for (int w = threadIdx.x; w < (int)(sizeof(FFJob) / sizeof(int)); w += FF_THREADS) dstw[w] = srcw[w];
     }
-    if (threadIdx.x == 0) {
-        s_clamp = clamp_flags[lo];
-        for (int s = 0; s < FF_STAGES; s++) {
-            mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], FF_THREADS / 32);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
+    if (threadIdx.x == 0) s_clamp = clamp_flags[lo];
+    ff_init_barriers(full_bar, empty_bar);
     __syncthreads();
     const long long local_tile = tile - s_job.tile_begin;
     if (s_clamp)
@@ -342,19 +383,22 @@ static int pick_P(int nz) {
     return best;
 }
 
-template <bool SPLIT>
-static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st, const FFJob *jobs, int njobs,
-                             const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
+template <bool SPLIT, int P, bool ZCOL>
+static void launch_ff_one(long long ntiles, cudaStream_t st, const FFJob *hj, const FFJob *dj, int njobs,
+                          const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
     const dim3 grid((unsigned)ntiles), block(FF_THREADS);
-    if (!zcol) {
-        ff_kernel<4, SPLIT, false><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
-    } else if (P == 10) {
-        ff_kernel<10, SPLIT, true><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
-    } else if (P == 5) {
-        ff_kernel<5, SPLIT, true><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
-    } else {
-        ff_kernel<8, SPLIT, true><<<grid, block, 0, st>>>(jobs, njobs, flags, recs, a, b);
-    }
+    if (njobs == 1) ff_kernel<P, SPLIT, ZCOL><<<grid, block, 0, st>>>(hj[0], flags, recs, a, b);
+    else ff_batch_kernel<P, SPLIT, ZCOL><<<grid, block, 0, st>>>(dj, njobs, flags, recs, a, b);
+}
+
+template <bool SPLIT>
+static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st, const FFJob *hj, const FFJob *dj,
+                             int njobs, const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
+    KernelTimer kt(PPFM_K_FF, st);
+    if (!zcol) launch_ff_one<SPLIT, 4, false>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 10) launch_ff_one<SPLIT, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 5) launch_ff_one<SPLIT, 5, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else launch_ff_one<SPLIT, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     return cudaGetLastError();
 }
 
@@ -389,18 +433,21 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
     }
     const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2]) : 4;
 
+    const bool single = (nsys == 1);
     const size_t jobs_bytes = (size_t)nsys * sizeof(FFJob);
     const size_t table_bytes = (size_t)nsys * ntypes * sizeof(TypeEntry);
-    const size_t flags_off = (jobs_bytes + table_bytes + 15) & ~(size_t)15;
+    const size_t host_bytes = (jobs_bytes + table_bytes + 15) & ~(size_t)15;
+    // device scratch: [jobs | tables] (batch only) [clamp flags] [atom records]
+    const size_t flags_off = single ? 0 : host_bytes;
     const size_t flags_bytes = ((size_t)nsys * sizeof(int) + 15) & ~(size_t)15;
     const size_t recs_off = flags_off + flags_bytes;
     const int natoms_total = h_atom_offset[nsys];
     const size_t recs_bytes = (size_t)(natoms_total > 0 ? natoms_total : 1) * sizeof(AtomRec);
     const size_t total_bytes = recs_off + recs_bytes;
 
-    unsigned char *h_buf = (unsigned char *)malloc(flags_off);
+    unsigned char *h_buf = (unsigned char *)malloc(host_bytes);
     if (!h_buf) return PPFM_ENOMEM;
-    memset(h_buf, 0, flags_off);
+    memset(h_buf, 0, host_bytes);
     FFJob *hj = reinterpret_cast<FFJob *>(h_buf);
     TypeEntry *ht = reinterpret_cast<TypeEntry *>(h_buf + jobs_bytes);
     long long tile = 0, out_off = 0;
@@ -450,31 +497,43 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     unsigned char *d_buf = nullptr;
-    cudaError_t e = cudaMallocAsync((void **)&d_buf, total_bytes, st);
-    if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "cudaMallocAsync"); return PPFM_ENOMEM; }
-    e = cudaMemcpyAsync(d_buf, h_buf, flags_off, cudaMemcpyHostToDevice, st);   // pageable: staged before return
-    free(h_buf);
+    cudaError_t e = scratch_alloc((void **)&d_buf, total_bytes, st);
+    if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "scratch_alloc"); return PPFM_ENOMEM; }
+    if (!single) e = cudaMemcpyAsync(d_buf, h_buf, host_bytes, cudaMemcpyHostToDevice, st);   // pageable: staged before return
     if (e == cudaSuccess) e = cudaMemsetAsync(d_buf + flags_off, 0, flags_bytes, st);
-    if (e != cudaSuccess) { set_cuda_error(e, "scratch upload"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+    if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "scratch upload"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
     const FFJob *dj = reinterpret_cast<const FFJob *>(d_buf);
     const TypeEntry *dt = reinterpret_cast<const TypeEntry *>(d_buf + jobs_bytes);
     int *dflags = reinterpret_cast<int *>(d_buf + flags_off);
     AtomRec *drecs = reinterpret_cast<AtomRec *>(d_buf + recs_off);
     if (natoms_total > 0) {
-        ff_prep_kernel<<<(natoms_total + 127) / 128, 128, 0, st>>>(dj, nsys, dt, reinterpret_cast<const float4 *>(d_xyzq),
-                                                                   d_type, drecs, dflags, natoms_total);
+        {
+            KernelTimer kt(PPFM_K_FF_PREP, st);
+            if (single) {
+                FFSingle one;
+                memset(&one, 0, sizeof(one));
+                one.job = hj[0];
+                memcpy(one.table, ht, (size_t)ntypes * sizeof(TypeEntry));
+                ff_prep_kernel<<<(natoms_total + 127) / 128, 128, 0, st>>>(one, reinterpret_cast<const float4 *>(d_xyzq),
+                                                                           d_type, drecs, dflags, natoms_total);
+            } else {
+                ff_prep_batch_kernel<<<(natoms_total + 127) / 128, 128, 0, st>>>(
+                    dj, nsys, dt, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs, dflags, natoms_total);
+            }
+        }
         e = cudaGetLastError();
-        if (e != cudaSuccess) { set_cuda_error(e, "ff_prep_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+        if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "ff_prep_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
         count_launch();
     }
     if (tile > 0) {
-        e = split ? launch_ff<true>(P, zcol, tile, st, dj, nsys, dflags, drecs, reinterpret_cast<float4 *>(d_a),
+        e = split ? launch_ff<true>(P, zcol, tile, st, hj, dj, nsys, dflags, drecs, reinterpret_cast<float4 *>(d_a),
                                     reinterpret_cast<float4 *>(d_b))
-                  : launch_ff<false>(P, zcol, tile, st, dj, nsys, dflags, drecs, reinterpret_cast<float4 *>(d_a),
+                  : launch_ff<false>(P, zcol, tile, st, hj, dj, nsys, dflags, drecs, reinterpret_cast<float4 *>(d_a),
                                      nullptr);
-        if (e != cudaSuccess) { set_cuda_error(e, "ff_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+        if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "ff_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
         count_launch();
     }
+    free(h_buf);
     PPFM_CUDA(cudaFreeAsync(d_buf, st));
     return PPFM_OK;
 }
@@ -518,9 +577,12 @@ extern "C" int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q
     if (n_points == 0) return PPFM_OK;
     long long blocks = (n_points + 255) / 256;
     if (blocks > 148LL * 16) blocks = 148LL * 16;
-    combine_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(
-        reinterpret_cast<const float4 *>(d_ff_lj), reinterpret_cast<const float4 *>(d_ff_el), (float)Q, n_points,
-        reinterpret_cast<float4 *>(d_out));
+    {
+        KernelTimer kt(PPFM_K_COMBINE, (cudaStream_t)cuda_stream);
+        combine_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(
+            reinterpret_cast<const float4 *>(d_ff_lj), reinterpret_cast<const float4 *>(d_ff_el), (float)Q, n_points,
+            reinterpret_cast<float4 *>(d_out));
+    }
     PPFM_LAUNCH_CHECK();
     return PPFM_OK;
 }

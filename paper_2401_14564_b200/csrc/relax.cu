@@ -4,10 +4,18 @@
 // FIRE (ref [7]; constants and loop order = DESIGN.md reading S6).  Read-out Fz_tip = -F_R,z
 // (PAPER.md:62).
 //
-// Kernel design: one thread per pixel, the whole z stroke inside the kernel (state carried in registers); a warp
-// covers an 8 x 4 pixel patch so that the 8-corner float4 gathers of neighbouring lanes fall into the same
-// 128-byte lines (L1/L2 hits) and iteration counts within a warp stay similar; the FIRE loop is warp-converged by
-// an __all_sync vote on (converged || max_iter), so the eight LDG.128 of an iteration issue warp-wide.
+// Kernel design.  One thread per pixel, the whole z stroke inside the kernel (state in registers);
+// a warp covers an 8 x 4 pixel patch so that the 8-corner float4 gathers of neighbouring lanes fall into the same
+// 128-byte lines (L1 hit rate > 99 %).  A FIRE iteration is a strictly dependent chain (position -> cell -> 8 loads
+// -> force -> step), so with few pixels the kernel runs at the speed of that chain and with many pixels at the
+// speed of instruction issue; both want the fewest instructions on the chain:
+//   * cell index and fraction by the magic-number trick (t - 0.5 + 1.5*2^23 rounds to floor(t) in the low mantissa
+//     bits; clamps are two FMNMX in that domain, the fraction is one saturating subtract) — no F2I/I2F, no branches;
+//   * all eight LDG.128 are issued back to back (asm volatile) before any use, weights are formed while they fly,
+//     and the spring force seeds the interpolation accumulators;
+//   * FIRE is branch-free: everything that depends only on the old velocity (|v|, (1-a)v, both dt candidates) is
+//     computed under the loads; after F arrives the chain is F.F -> rsqrt -> one select -> two FMA per component;
+//   * the loop exit is one __all_sync vote placed after the (predicated) move, so it overlaps the update.
 // FP32 with two precautions that keep |F| < 1e-6 eV/Å reachable:
 //   * the state is the displacement u = d - d0 from the spring equilibrium, and the radial extension is
 //     |d| - R0 = (|u|^2 + 2 d0.u)/(|d| + R0) (no cancellation);
@@ -19,6 +27,9 @@ namespace ppfm {
 
 constexpr int RX_THREADS = 128;     // 4 warps = 2 x 2 patches of 8 x 4 pixels -> 16 x 8 pixels per CTA
 constexpr int RX_TILE_X = 16, RX_TILE_Y = 8;
+constexpr float RX_MAGIC = 12582912.0f;      // 1.5 * 2^23: floats in [2^23, 2^24) are the integers
+constexpr int RX_MAGIC_BITS = 0x4B400000;
+constexpr int RX_MAX_N = 1 << 21;            // per-axis grid size limit of the magic-number cell index
 
 struct RelaxJob {
     long long ff_offset;     // float4 offset of this system's grid
@@ -44,54 +55,70 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-__device__ __forceinline__ float lerp(float a, float b, float t) { return fmaf(t, b - a, a); }
-
-// cell index pair and fraction along one axis; `ib` = integer part of the base coordinate (already wrapped into
-// [0, n) on periodic axes), `tf` = fractional base + FP32 offset.
-__device__ __forceinline__ bool axis_cell(float tf, int ib, int n, int periodic, int &i0, int &i1, float &f) {
-    bool clamped = false;
-    if (periodic) {
-        tf = fminf(fmaxf(tf, (float)(1 - n)), (float)(n - 1));   // never more than one cell-length away
-        const float fl = floorf(tf);
-        f = tf - fl;
-        int i = ib + (int)fl;
-        if (i >= n) i -= n;
-        if (i < 0) i += n;
-        i0 = i;
-        i1 = (i + 1 == n) ? 0 : i + 1;
-    } else {
-        const float lo = (float)(-ib), hi = (float)(n - 1 - ib);
-        clamped = (tf < lo) || (tf > hi);
-        tf = fminf(fmaxf(tf, lo), hi);
-        int i = ib + (int)floorf(tf);
-        i = min(i, n - 2);
-        i = max(i, 0);
-        f = tf - (float)(i - ib);
-        i0 = i;
-        i1 = i + 1;
-    }
-    return clamped;
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_fast(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// Read-only 16-byte gather.  volatile keeps the eight corner loads of an iteration in program order, all ahead of
+// their first use, so they are in flight together (ptxas otherwise sinks them pairwise to save registers).
+__device__ __forceinline__ float4 ldg_corner(const float4 *p) {
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
 }
 
-__global__ void __launch_bounds__(RX_THREADS)
-relax_kernel(const RelaxJob *__restrict__ jobs, int njobs, FireParams fp, const float4 *__restrict__ ff,
-             float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats) {
-    __shared__ RelaxJob s_job;
-    const int blk = blockIdx.x;
-    int lo = 0, hi = njobs - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (jobs[mid].block_begin <= blk) lo = mid; else hi = mid - 1;
-    }
-    {
-        const int *srcw = reinterpret_cast<const int *>(&jobs[lo]);
-        int *dstw = reinterpret_cast<int *>(&s_job);
-        for (int w = threadIdx.x; w < (int)(sizeof(RelaxJob) / sizeof(int)); w += RX_THREADS) dstw[w] = srcw[w];
-    }
-    __syncthreads();
-    const RelaxJob &job = s_job;
+// Per z-step constants of one grid axis for the magic-number cell lookup.
+struct AxisBase {
+    float tb, tbm;     // fractional part of the base coordinate, and the same minus 0.5
+    float zlo, zhi;    // clamp bounds in the magic domain
+    int K;             // cell index = float_as_int(zc) - K
+    float lo, hi;      // non-periodic: coordinate range [lo, hi] (relative to the base cell) outside which S12 clamps
+};
 
-    const int lb = blk - job.block_begin;
+__device__ __forceinline__ AxisBase axis_base(double t, int n, int periodic) {
+    AxisBase a;
+    const double fl = floor(t);
+    a.tb = (float)(t - fl);
+    a.tbm = a.tb - 0.5f;
+    int ib;
+    if (periodic) {
+        long long m = (long long)fl % n;
+        if (m < 0) m += n;
+        ib = (int)m;
+        a.zlo = RX_MAGIC - (float)(n - 1);
+        a.zhi = RX_MAGIC + (float)(n - 1);
+        a.lo = -3.0e38f;
+        a.hi = 3.0e38f;
+    } else {
+        ib = (int)fmin(fmax(fl, -(double)(1 << 20)), (double)(1 << 20));
+        a.zlo = RX_MAGIC + (float)(-ib);
+        a.zhi = RX_MAGIC + (float)(n - 2 - ib);
+        a.lo = (float)(-ib);
+        a.hi = (float)(n - 1 - ib);
+    }
+    a.K = RX_MAGIC_BITS - ib;
+    return a;
+}
+
+// cell index i0 (absolute, before periodic wrap) and fraction f in [0,1] from t and t - 0.5
+__device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, int &i0, float &f) {
+    const float z = tm + RX_MAGIC;                       // nearest integer of t - 0.5 = floor(t) (ties are harmless:
+    const float zc = fminf(fmaxf(z, a.zlo), a.zhi);      //   the interpolant is continuous across cell faces)
+    const float fl = zc - RX_MAGIC;
+    f = __saturatef(t - fl);
+    i0 = __float_as_int(zc) - a.K;
+}
+
+template <bool ORTHO, bool ANYPER>
+__device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FireParams &fp, int lb,
+                                             const float4 *__restrict__ ff, float4 *__restrict__ pos_fz,
+                                             uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats) {
     const int by = lb / job.nbx, bx = lb - by * job.nbx;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ix = bx * RX_TILE_X + (warp & 1) * 8 + (lane & 7);
@@ -106,7 +133,9 @@ relax_kernel(const RelaxJob *__restrict__ jobs, int njobs, FireParams fp, const 
     const float m10 = job.Minvf[3], m11 = job.Minvf[4], m12 = job.Minvf[5];
     const float m20 = job.Minvf[6], m21 = job.Minvf[7], m22 = job.Minvf[8];
     const float d0x = job.d0f[0], d0y = job.d0f[1], d0z = job.d0f[2];
+    const float d0x2 = 2.0f * d0x, d0y2 = 2.0f * d0y, d0z2 = 2.0f * d0z;
     const float R_rest = job.R_rest, k_rad = job.k_rad, kx = job.k_lat[0], ky = job.k_lat[1];
+    const long long sy = nx, sz = (long long)nx * ny;       // float4 strides
 
     // r_TIP + d0 - origin at iz = 0, FP64
     double rb[3];
@@ -121,89 +150,104 @@ relax_kernel(const RelaxJob *__restrict__ jobs, int njobs, FireParams fp, const 
     for (int iz = 0; iz < job.nzs; iz++) {
         // a4: exact fractional grid coordinate of the spring equilibrium point, split int + frac
         const double rz = rb[2] - iz * job.dz;
-        int ib[3];
-        float fb[3];
-#pragma unroll
-        for (int a = 0; a < 3; a++) {
-            const double t = job.Minv[3 * a] * rb[0] + job.Minv[3 * a + 1] * rb[1] + job.Minv[3 * a + 2] * rz;
-            const double fl = floor(t);
-            fb[a] = (float)(t - fl);
-            const int n = job.n[a];
-            if (job.periodic[a]) {
-                long long m = (long long)fl % n;
-                if (m < 0) m += n;
-                ib[a] = (int)m;
-            } else {
-                ib[a] = (int)fmin(fmax(fl, -1.0e9), 1.0e9);
-            }
-        }
+        const AxisBase ax = axis_base(job.Minv[0] * rb[0] + job.Minv[1] * rb[1] + job.Minv[2] * rz, nx, perx);
+        const AxisBase ay = axis_base(job.Minv[3] * rb[0] + job.Minv[4] * rb[1] + job.Minv[5] * rz, ny, pery);
+        const AxisBase az = axis_base(job.Minv[6] * rb[0] + job.Minv[7] * rb[1] + job.Minv[8] * rz, nz, perz);
 
         float vx = 0.f, vy = 0.f, vz = 0.f, dt = fp.dt0, alpha = fp.alpha0;
         int npos = 0, moves = 0;
-        bool conv = !valid, clamped = false;
-        float ext = 0.f, invL = 0.f, dzc = d0z;
+        bool conv = !valid;
+        float ext, invL, dzc, tx, ty, tz;
 
         while (true) {
-            // ---- F_S: tri-linear interpolation (8 x LDG.128)
-            const float tx = fb[0] + fmaf(m00, ux, fmaf(m01, uy, m02 * uz));
-            const float ty = fb[1] + fmaf(m10, ux, fmaf(m11, uy, m12 * uz));
-            const float tz = fb[2] + fmaf(m20, ux, fmaf(m21, uy, m22 * uz));
-            int i0, i1, j0, j1, k0, k1;
+            // ---- cell lookup
+            float txm, tym, tzm;
+            if (ORTHO) {
+                tx = fmaf(m00, ux, ax.tb); txm = fmaf(m00, ux, ax.tbm);
+                ty = fmaf(m11, uy, ay.tb); tym = fmaf(m11, uy, ay.tbm);
+                tz = fmaf(m22, uz, az.tb); tzm = fmaf(m22, uz, az.tbm);
+            } else {
+                const float sx = fmaf(m00, ux, fmaf(m01, uy, m02 * uz));
+                const float sy_ = fmaf(m10, ux, fmaf(m11, uy, m12 * uz));
+                const float sz_ = fmaf(m20, ux, fmaf(m21, uy, m22 * uz));
+                tx = sx + ax.tb; txm = sx + ax.tbm;
+                ty = sy_ + ay.tb; tym = sy_ + ay.tbm;
+                tz = sz_ + az.tb; tzm = sz_ + az.tbm;
+            }
+            int i0, j0, k0;
             float fx, fy, fz;
-            clamped = axis_cell(tx, ib[0], nx, perx, i0, i1, fx);
-            clamped |= axis_cell(ty, ib[1], ny, pery, j0, j1, fy);
-            clamped |= axis_cell(tz, ib[2], nz, perz, k0, k1, fz);
-            const int r00 = (k0 * ny + j0) * nx, r01 = (k0 * ny + j1) * nx;
-            const int r10 = (k1 * ny + j0) * nx, r11 = (k1 * ny + j1) * nx;
-            const float4 c000 = __ldg(g + r00 + i0), c001 = __ldg(g + r00 + i1);
-            const float4 c010 = __ldg(g + r01 + i0), c011 = __ldg(g + r01 + i1);
-            const float4 c100 = __ldg(g + r10 + i0), c101 = __ldg(g + r10 + i1);
-            const float4 c110 = __ldg(g + r11 + i0), c111 = __ldg(g + r11 + i1);
-            float Fx = lerp(lerp(lerp(c000.x, c001.x, fx), lerp(c010.x, c011.x, fx), fy),
-                            lerp(lerp(c100.x, c101.x, fx), lerp(c110.x, c111.x, fx), fy), fz);
-            float Fy = lerp(lerp(lerp(c000.y, c001.y, fx), lerp(c010.y, c011.y, fx), fy),
-                            lerp(lerp(c100.y, c101.y, fx), lerp(c110.y, c111.y, fx), fy), fz);
-            float Fz = lerp(lerp(lerp(c000.z, c001.z, fx), lerp(c010.z, c011.z, fx), fy),
-                            lerp(lerp(c100.z, c101.z, fx), lerp(c110.z, c111.z, fx), fy), fz);
-            // ---- F_T: radial + lateral springs (Eq.2), d = d0 + u
+            axis_cell(tx, txm, ax, i0, fx);
+            axis_cell(ty, tym, ay, j0, fy);
+            axis_cell(tz, tzm, az, k0, fz);
+            // ---- F_S: eight LDG.128, issued together
+            float4 c000, c001, c010, c011, c100, c101, c110, c111;
+            if (!ANYPER) {
+                const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
+                c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
+                c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
+                c100 = ldg_corner(p + sz);      c101 = ldg_corner(p + sz + 1);
+                c110 = ldg_corner(p + sz + sy); c111 = ldg_corner(p + sz + sy + 1);
+            } else {
+                if (perx) { i0 -= (i0 >= nx) ? nx : 0; i0 += (i0 < 0) ? nx : 0; }
+                if (pery) { j0 -= (j0 >= ny) ? ny : 0; j0 += (j0 < 0) ? ny : 0; }
+                if (perz) { k0 -= (k0 >= nz) ? nz : 0; k0 += (k0 < 0) ? nz : 0; }
+                const int i1 = (i0 + 1 == nx) ? 0 : i0 + 1;       // non-periodic axes never reach n - 1
+                const int j1 = (j0 + 1 == ny) ? 0 : j0 + 1;
+                const int k1 = (k0 + 1 == nz) ? 0 : k0 + 1;
+                const float4 *r00 = g + (long long)(k0 * ny + j0) * nx, *r01 = g + (long long)(k0 * ny + j1) * nx;
+                const float4 *r10 = g + (long long)(k1 * ny + j0) * nx, *r11 = g + (long long)(k1 * ny + j1) * nx;
+                c000 = ldg_corner(r00 + i0); c001 = ldg_corner(r00 + i1);
+                c010 = ldg_corner(r01 + i0); c011 = ldg_corner(r01 + i1);
+                c100 = ldg_corner(r10 + i0); c101 = ldg_corner(r10 + i1);
+                c110 = ldg_corner(r11 + i0); c111 = ldg_corner(r11 + i1);
+            }
+            // ---- under the loads: F_T, radial + lateral springs (Eq.2) with d = d0 + u
             const float dxc = d0x + ux, dyc = d0y + uy;
             dzc = d0z + uz;
             const float L2 = fmaf(dxc, dxc, fmaf(dyc, dyc, dzc * dzc));
             invL = rsqrt_fast(L2);
-            const float L = L2 * invL;
-            const float num = fmaf(ux, ux, fmaf(uy, uy, uz * uz)) + 2.0f * fmaf(d0x, ux, fmaf(d0y, uy, d0z * uz));
-            ext = __fdividef(num, L + R_rest);           // |d| - R0
+            const float num = fmaf(ux, ux + d0x2, fmaf(uy, uy + d0y2, uz * (uz + d0z2)));   // |u|^2 + 2 d0.u
+            ext = num * rcp_fast(fmaf(L2, invL, R_rest));                                    // |d| - R0
             const float fr = -k_rad * ext * invL;
-            Fx = fmaf(fr, dxc, Fx) - kx * ux;
-            Fy = fmaf(fr, dyc, Fy) - ky * uy;
-            Fz = fmaf(fr, dzc, Fz);
+            const float bx_ = fmaf(fr, dxc, -kx * ux), by_ = fmaf(fr, dyc, -ky * uy), bz_ = fr * dzc;
+            // ---- under the loads: the part of FIRE that needs only the old velocity (reading S6)
+            const float vn = sqrt_fast(fmaf(vx, vx, fmaf(vy, vy, vz * vz)));
+            const float av = alpha * vn, om = 1.0f - alpha;
+            const float ovx = om * vx, ovy = om * vy, ovz = om * vz;
+            const bool grow = npos > fp.n_min;
+            const float dt_pos = grow ? fminf(dt * fp.finc, fp.dt_max) : dt;
+            const float al_pos = grow ? alpha * fp.falpha : alpha;
+            const float dt_neg = dt * fp.fdec;
+            // ---- under the loads: tri-linear weights
+            const float gx = 1.0f - fx, gy = 1.0f - fy, gz = 1.0f - fz;
+            const float w00 = gy * gz, w01 = fy * gz, w10 = gy * fz, w11 = fy * fz;
+            const float w000 = w00 * gx, w001 = w00 * fx, w010 = w01 * gx, w011 = w01 * fx;
+            const float w100 = w10 * gx, w101 = w10 * fx, w110 = w11 * gx, w111 = w11 * fx;
+            // ---- total force: two accumulation chains per component, seeded with the spring force
+            const float Fx = fmaf(w110, c110.x, fmaf(w100, c100.x, fmaf(w010, c010.x, fmaf(w000, c000.x, bx_)))) +
+                             fmaf(w111, c111.x, fmaf(w101, c101.x, fmaf(w011, c011.x, w001 * c001.x)));
+            const float Fy = fmaf(w110, c110.y, fmaf(w100, c100.y, fmaf(w010, c010.y, fmaf(w000, c000.y, by_)))) +
+                             fmaf(w111, c111.y, fmaf(w101, c101.y, fmaf(w011, c011.y, w001 * c001.y)));
+            const float Fz = fmaf(w110, c110.z, fmaf(w100, c100.z, fmaf(w010, c010.z, fmaf(w000, c000.z, bz_)))) +
+                             fmaf(w111, c111.z, fmaf(w101, c101.z, fmaf(w011, c011.z, w001 * c001.z)));
             const float F2 = fmaf(Fx, Fx, fmaf(Fy, Fy, Fz * Fz));
-            if (!conv) conv = F2 < fp.fconv2;            // tested before every move (reading S7)
+            const float Pw = fmaf(Fx, vx, fmaf(Fy, vy, Fz * vz));
+            conv = conv || (F2 < fp.fconv2);                     // tested before every move (reading S7)
             const bool done = conv || (moves >= fp.max_iter);
-            if (__all_sync(0xffffffffu, done)) break;
-            if (!done) {
-                // ---- FIRE (reading S6)
-                const float Pw = fmaf(Fx, vx, fmaf(Fy, vy, Fz * vz));
-                if (Pw >= 0.0f) {
-                    const float v2 = fmaf(vx, vx, fmaf(vy, vy, vz * vz));
-                    const float c = alpha * sqrtf(v2) * rsqrt_fast(F2);
-                    const float om = 1.0f - alpha;
-                    vx = fmaf(om, vx, c * Fx); vy = fmaf(om, vy, c * Fy); vz = fmaf(om, vz, c * Fz);
-                    if (npos > fp.n_min) {
-                        dt = fminf(dt * fp.finc, fp.dt_max);
-                        alpha *= fp.falpha;
-                    }
-                    npos++;
-                } else {
-                    vx = vy = vz = 0.f;
-                    dt *= fp.fdec;
-                    alpha = fp.alpha0;
-                    npos = 0;
-                }
-                vx = fmaf(Fx, dt, vx); vy = fmaf(Fy, dt, vy); vz = fmaf(Fz, dt, vz);
+            // ---- FIRE step, branch-free; P >= 0 counts as downhill
+            const bool down = Pw >= 0.0f;
+            const float s = down ? fmaf(av, rsqrt_fast(F2), dt_pos) : dt_neg;
+            vx = fmaf(s, Fx, down ? ovx : 0.0f);
+            vy = fmaf(s, Fy, down ? ovy : 0.0f);
+            vz = fmaf(s, Fz, down ? ovz : 0.0f);
+            dt = down ? dt_pos : dt_neg;
+            alpha = down ? al_pos : fp.alpha0;
+            npos = down ? npos + 1 : 0;
+            if (!done) {                                         // finished lanes stay where they are
                 ux = fmaf(vx, dt, ux); uy = fmaf(vy, dt, uy); uz = fmaf(vz, dt, uz);
                 moves++;
             }
+            if (__all_sync(0xffffffffu, done)) break;
         }
 
         if (valid) {
@@ -215,6 +259,7 @@ relax_kernel(const RelaxJob *__restrict__ jobs, int njobs, FireParams fp, const 
             outv.w = k_rad * ext * invL * dzc;            // Fz_tip = -F_R,z
             pos_fz[o] = outv;
             if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
+            const bool clamped = (tx < ax.lo) | (tx > ax.hi) | (ty < ay.lo) | (ty > ay.hi) | (tz < az.lo) | (tz > az.hi);
             my_iters += (unsigned)moves;
             my_notconv += conv ? 0u : 1u;
             my_clamped += clamped ? 1u : 0u;
@@ -239,6 +284,46 @@ relax_kernel(const RelaxJob *__restrict__ jobs, int njobs, FireParams fp, const 
     }
 }
 
+// One system: the job travels as a kernel parameter (constant bank), no scratch and no copy.
+template <bool ORTHO, bool ANYPER>
+__global__ void __launch_bounds__(RX_THREADS)
+relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireParams fp,
+             const float4 *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
+             ppfm_stats *__restrict__ stats) {
+    relax_pixels<ORTHO, ANYPER>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats);
+}
+
+// Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
+template <bool ORTHO, bool ANYPER>
+__global__ void __launch_bounds__(RX_THREADS)
+relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_constant__ FireParams fp,
+                   const float4 *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
+                   ppfm_stats *__restrict__ stats) {
+    __shared__ RelaxJob s_job;
+    const int blk = blockIdx.x;
+    int lo = 0, hi = njobs - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (jobs[mid].block_begin <= blk) lo = mid; else hi = mid - 1;
+    }
+    {
+        const int *srcw = reinterpret_cast<const int *>(&jobs[lo]);
+        int *dstw = reinterpret_cast<int *>(&s_job);
+        for (int w = threadIdx.x; w < (int)(sizeof(RelaxJob) / sizeof(int)); w += RX_THREADS) dstw[w] = srcw[w];
+    }
+    __syncthreads();
+    relax_pixels<ORTHO, ANYPER>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats);
+}
+
+template <bool ORTHO, bool ANYPER>
+static void launch_relax(int nsys, long long blocks, cudaStream_t st, const RelaxJob *hj, const RelaxJob *dj,
+                         const FireParams &fp, const float4 *ff, float4 *pos, uint16_t *it, ppfm_stats *stats) {
+    if (nsys == 1)
+        relax_kernel<ORTHO, ANYPER><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats);
+    else
+        relax_batch_kernel<ORTHO, ANYPER><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
+}
+
 static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                       const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
                       ppfm_stats *d_stats, void *cuda_stream) {
@@ -252,13 +337,15 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
     RelaxJob *hj = (RelaxJob *)calloc((size_t)nsys, sizeof(RelaxJob));
     if (!hj) return PPFM_ENOMEM;
     long long blocks = 0, ff_off = 0, out_off = 0;
+    bool ortho = true, anyper = false;
     for (int m = 0; m < nsys; m++) {
         const ppfm_grid &g = grids[m];
         const ppfm_scan &s = scans[m];
         const ppfm_tip &t = tips[m];
         RelaxJob &j = hj[m];
-        bool ok = grid_ok(&g) && g.n[0] >= 2 && g.n[1] >= 2 && g.n[2] >= 2 && s.npx >= 1 && s.npy >= 1 && s.nz >= 1 &&
-                  std::isfinite(s.dz) && invert_steps(g.step, j.Minv) && grid_points(&g) <= 0x7fffffffLL;
+        bool ok = grid_ok(&g) && g.n[0] >= 2 && g.n[1] >= 2 && g.n[2] >= 2 && g.n[0] <= RX_MAX_N && g.n[1] <= RX_MAX_N &&
+                  g.n[2] <= RX_MAX_N && s.npx >= 1 && s.npy >= 1 && s.nz >= 1 && std::isfinite(s.dz) &&
+                  invert_steps(g.step, j.Minv) && grid_points(&g) <= 0x7fffffffLL;
         const double R0 = std::sqrt(t.d0[0] * t.d0[0] + t.d0[1] * t.d0[1] + t.d0[2] * t.d0[2]);
         ok = ok && (R0 > 0) && std::isfinite(R0) && (t.k_rad >= 0) && (t.k_lat[0] >= 0) && (t.k_lat[1] >= 0) &&
              std::isfinite(t.k_rad) && std::isfinite(t.k_lat[0]) && std::isfinite(t.k_lat[1]);
@@ -271,10 +358,13 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
         for (int a = 0; a < 3; a++) {
             j.n[a] = g.n[a];
             j.periodic[a] = g.periodic[a] ? 1 : 0;
+            anyper = anyper || (g.periodic[a] != 0);
             j.origin[a] = g.origin[a];
             j.p0[a] = s.p0[a]; j.dx[a] = s.dx[a]; j.dy[a] = s.dy[a];
             j.d0[a] = t.d0[a];
             j.d0f[a] = (float)t.d0[a];
+            for (int c = 0; c < 3; c++)
+                if (a != c && g.step[a][c] != 0.0) ortho = false;
         }
         for (int i = 0; i < 9; i++) j.Minvf[i] = (float)j.Minv[i];
         j.dz = s.dz;
@@ -294,17 +384,27 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     RelaxJob *dj = nullptr;
-    cudaError_t e = cudaMallocAsync((void **)&dj, (size_t)nsys * sizeof(RelaxJob), st);
-    if (e != cudaSuccess) { free(hj); set_cuda_error(e, "cudaMallocAsync"); return PPFM_ENOMEM; }
-    e = cudaMemcpyAsync(dj, hj, (size_t)nsys * sizeof(RelaxJob), cudaMemcpyHostToDevice, st);
+    cudaError_t e;
+    if (nsys > 1) {
+        e = scratch_alloc((void **)&dj, (size_t)nsys * sizeof(RelaxJob), st);
+        if (e != cudaSuccess) { free(hj); set_cuda_error(e, "scratch_alloc"); return PPFM_ENOMEM; }
+        e = cudaMemcpyAsync(dj, hj, (size_t)nsys * sizeof(RelaxJob), cudaMemcpyHostToDevice, st);   // pageable: staged
+        if (e != cudaSuccess) { free(hj); set_cuda_error(e, "job upload"); cudaFreeAsync(dj, st); return PPFM_ECUDA; }
+    }
+    const float4 *ff4 = reinterpret_cast<const float4 *>(d_ff);
+    float4 *pos4 = reinterpret_cast<float4 *>(d_pos_fz);
+    {
+        KernelTimer kt(PPFM_K_RELAX, st);
+        if (ortho && !anyper) launch_relax<true, false>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
+        else if (ortho) launch_relax<true, true>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
+        else if (!anyper) launch_relax<false, false>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
+        else launch_relax<false, true>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
+    }
     free(hj);
-    if (e != cudaSuccess) { set_cuda_error(e, "job upload"); cudaFreeAsync(dj, st); return PPFM_ECUDA; }
-    relax_kernel<<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, reinterpret_cast<const float4 *>(d_ff),
-                                                         reinterpret_cast<float4 *>(d_pos_fz), d_iters, d_stats);
     e = cudaGetLastError();
-    if (e != cudaSuccess) { set_cuda_error(e, "relax_kernel"); cudaFreeAsync(dj, st); return PPFM_ECUDA; }
+    if (e != cudaSuccess) { set_cuda_error(e, "relax_kernel"); if (dj) cudaFreeAsync(dj, st); return PPFM_ECUDA; }
     count_launch();
-    PPFM_CUDA(cudaFreeAsync(dj, st));
+    if (dj) PPFM_CUDA(cudaFreeAsync(dj, st));
     return PPFM_OK;
 }
 

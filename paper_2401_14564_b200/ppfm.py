@@ -58,7 +58,9 @@ class Stats(C.Structure):
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_relax_scan",
            "ppfm_relax_scan_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
-           "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count"]
+           "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
+           "ppfm_release_scratch"]
+KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4}
 
 
 def lib():
@@ -92,6 +94,25 @@ def launch_count() -> int:
     return int(lib().ppfm_launch_count())
 
 
+def timing_enable(on: bool = True) -> None:
+    """ppfm_timing_enable: bracket every kernel launch with CUDA events inside the library (clears the totals)."""
+    _check(lib().ppfm_timing_enable(C.c_int(int(on))), "ppfm_timing_enable")
+
+
+def timing_read() -> dict:
+    """ppfm_timing_read for every kernel: {name: (total ms, launches)}."""
+    out = {}
+    for name, kid in KERNEL_IDS.items():
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        _check(lib().ppfm_timing_read(C.c_int(kid), C.byref(ms), C.byref(n)), "ppfm_timing_read")
+        out[name] = (ms.value, int(n.value))
+    return out
+
+
+def release_scratch() -> None:
+    _check(lib().ppfm_release_scratch(), "ppfm_release_scratch")
+
+
 def Nm_to_eVA2(k: float) -> float:
     return float(lib().ppfm_Nm_to_eVA2(k))
 
@@ -108,11 +129,15 @@ def _vec(ctype, vals):
 
 
 def c_lattice(l) -> Lattice:
+    if isinstance(l, Lattice):
+        return l
     return Lattice(_vec(C.c_double * 3, l.a), _vec(C.c_double * 3, l.b), _vec(C.c_double * 3, l.c),
                    (C.c_int32 * 3)(*[int(v) for v in l.nimg]))
 
 
 def c_grid(g) -> Grid:
+    if isinstance(g, Grid):
+        return g
     out = Grid()
     for a in range(3):
         out.origin[a] = float(g.origin[a])
@@ -124,21 +149,37 @@ def c_grid(g) -> Grid:
 
 
 def c_probe(p, Q: Optional[float] = None) -> Probe:
+    if isinstance(p, Probe) and Q is None:
+        return p
     return Probe(float(p.R), float(p.e), float(p.Q if Q is None else Q))
 
 
 def c_tip(t) -> Tip:
+    if isinstance(t, Tip):
+        return t
     return Tip(_vec(C.c_double * 2, t.k_lat), float(t.k_rad), _vec(C.c_double * 3, t.d0))
 
 
 def c_fire(f) -> Fire:
+    if isinstance(f, Fire):
+        return f
     return Fire(float(f.dt), float(f.dt_max), float(f.finc), float(f.fdec), float(f.alpha0), float(f.falpha),
                 int(f.n_min), int(f.max_iter), float(f.f_conv))
 
 
 def c_scan(s) -> Scan:
+    if isinstance(s, Scan):
+        return s
     return Scan(_vec(C.c_double * 3, s.p0), _vec(C.c_double * 3, s.dx), _vec(C.c_double * 3, s.dy), int(s.npx),
                 int(s.npy), int(s.nz), float(s.dz))
+
+
+def c_array(items, conv):
+    """ctypes array of converted structs, e.g. c_array(grids, c_grid); a ready ctypes array passes through."""
+    if isinstance(items, C.Array):
+        return items
+    cs = [conv(x) for x in items]
+    return (type(cs[0]) * len(cs))(*cs)
 
 
 def _torch():
@@ -217,12 +258,10 @@ def forcefield_batch(atom_offset: Sequence[int], xyzq, types, elem_R, elem_e, la
     """ppfm_forcefield_batch: concatenated atoms, one launch; returns a flat (sum points, 4) float32 tensor."""
     torch = _torch()
     nsys = len(grids)
-    off = (C.c_int32 * (nsys + 1))(*[int(v) for v in atom_offset])
-    lat = (Lattice * nsys)(*[c_lattice(l) for l in lattices])
-    pr = (Probe * nsys)(*[c_probe(p) for p in probes])
-    gr = (Grid * nsys)(*[c_grid(g) for g in grids])
-    npts = sum(int(g.n[0]) * int(g.n[1]) * int(g.n[2]) for g in grids)
+    off = atom_offset if isinstance(atom_offset, C.Array) else (C.c_int32 * (nsys + 1))(*[int(v) for v in atom_offset])
+    lat, pr, gr = c_array(lattices, c_lattice), c_array(probes, c_probe), c_array(grids, c_grid)
     if out is None:
+        npts = sum(int(g.n[0]) * int(g.n[1]) * int(g.n[2]) for g in gr)
         out = torch.empty((npts, 4), dtype=torch.float32, device=xyzq.device)
     R, pR = _darr(elem_R)
     e, pe = _darr(elem_e)
@@ -263,10 +302,8 @@ def relax_scan(ff, grid, tip, fire, scan, pos_fz=None, iters=None, stats=None, w
 def relax_scan_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, stats=None, want_iters=True):
     torch = _torch()
     nsys = len(grids)
-    gr = (Grid * nsys)(*[c_grid(g) for g in grids])
-    tp = (Tip * nsys)(*[c_tip(t) for t in tips])
-    sc = (Scan * nsys)(*[c_scan(s) for s in scans])
-    nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in scans)
+    gr, tp, sc = c_array(grids, c_grid), c_array(tips, c_tip), c_array(scans, c_scan)
+    nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in sc)
     if pos_fz is None:
         pos_fz = torch.empty((nps, 4), dtype=torch.float32, device=ff.device)
     if iters is None and want_iters:
