@@ -473,7 +473,10 @@ def run_ours(args):
                       "s_per_full_scan": t_step, "kernel_ms": ms, "kernel_launches_per_step": n_launch,
                       "call_ms_incl_host_gaps": seg_ms, "wall_s_timed_region": wall_s,
                       "not_converged": stats["n_not_converged"], "clamped": stats["n_clamped"],
-                      "max_iters": stats["max_iters"]},
+                      "max_iters": stats["max_iters"],
+                      "relax_warp_loop_trips": stats["warp_iters"],
+                      "relax_lane_utilisation": stats["total_iters"] / max(1, 32 * stats["warp_iters"]),
+                      "relax_cell_gathers_per_iteration": stats["cell_gathers"] / max(1, stats["total_iters"])},
             "e2e": {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
                     "d2h_bytes_per_step": host.d2h, "ms_per_step": e2e_t * 1e3, "steps": e2e_steps,
                     "api": "ppfm_scan_host (pinned host buffers)"},

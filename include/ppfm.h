@@ -95,6 +95,10 @@ typedef struct {
     uint64_t n_clamped;       /* pixel-steps whose final PP position was clamped to a non-periodic grid face */
     uint32_t max_iters;       /* largest move count of any pixel-step                     */
     uint32_t _pad;
+    uint64_t warp_iters;      /* trips of the warp-converged FIRE loop, summed over warps (x32 lanes = issued lane-
+                                 iterations; minus total_iters = divergence cost)             */
+    uint64_t cell_gathers;    /* 8-corner float4 gathers actually issued (a lane gathers only when the PP leaves
+                                 the grid cell it holds in registers)                          */
 } ppfm_stats;
 
 int ppfm_version(void);

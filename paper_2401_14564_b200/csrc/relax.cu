@@ -106,11 +106,12 @@ __device__ __forceinline__ AxisBase axis_base(double t, int n, int periodic) {
     return a;
 }
 
-// cell index i0 (absolute, before periodic wrap) and fraction f in [0,1] from t and t - 0.5
-__device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, int &i0, float &f) {
+// cell offset fl (float, relative to the base cell), absolute cell index i0 (before periodic wrap) and fraction
+// f in [0,1] from t and t - 0.5
+__device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, int &i0, float &f, float &fl) {
     const float z = tm + RX_MAGIC;                       // nearest integer of t - 0.5 = floor(t) (ties are harmless:
     const float zc = fminf(fmaxf(z, a.zlo), a.zhi);      //   the interpolant is continuous across cell faces)
-    const float fl = zc - RX_MAGIC;
+    fl = zc - RX_MAGIC;
     f = __saturatef(t - fl);
     i0 = __float_as_int(zc) - a.K;
 }
@@ -134,7 +135,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
     const float m20 = job.Minvf[6], m21 = job.Minvf[7], m22 = job.Minvf[8];
     const float d0x = job.d0f[0], d0y = job.d0f[1], d0z = job.d0f[2];
     const float d0x2 = 2.0f * d0x, d0y2 = 2.0f * d0y, d0z2 = 2.0f * d0z;
-    const float R_rest = job.R_rest, k_rad = job.k_rad, kx = job.k_lat[0], ky = job.k_lat[1];
+    const float R_rest = job.R_rest, nk_rad = -job.k_rad, nkx = -job.k_lat[0], nky = -job.k_lat[1];
     const long long sy = nx, sz = (long long)nx * ny;       // float4 strides
 
     // r_TIP + d0 - origin at iz = 0, FP64
@@ -145,7 +146,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 
     float ux = 0.f, uy = 0.f, uz = 0.f;
     unsigned long long my_iters = 0;
-    unsigned int my_notconv = 0, my_clamped = 0, my_max = 0;
+    unsigned int my_notconv = 0, my_clamped = 0, my_max = 0, my_reloads = 0, my_witers = 0;
 
     for (int iz = 0; iz < job.nzs; iz++) {
         // a4: exact fractional grid coordinate of the spring equilibrium point, split int + frac
@@ -157,60 +158,90 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         float vx = 0.f, vy = 0.f, vz = 0.f, dt = fp.dt0, alpha = fp.alpha0;
         int npos = 0, moves = 0;
         bool conv = !valid;
-        float ext, invL, dzc, tx, ty, tz;
+        float fr, dzc, tx, ty, tz;
+        // cached cell (relative to this z-step's base cell): corner forces at x0 and their x-differences, for the
+        // four (y,z) edges 00, 10 (y+1), 01 (z+1), 11.  An impossible offset makes the first iteration reload.
+        float flx = 1.0e30f, fly = 1.0e30f, flz = 1.0e30f;
+        float c0[4][3], cd[4][3];
+#pragma unroll
+        for (int e = 0; e < 4; e++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) c0[e][c] = cd[e][c] = 0.0f;
 
         while (true) {
-            // ---- cell lookup
-            float txm, tym, tzm;
+            // ---- fractional position inside the cached cell
             if (ORTHO) {
-                tx = fmaf(m00, ux, ax.tb); txm = fmaf(m00, ux, ax.tbm);
-                ty = fmaf(m11, uy, ay.tb); tym = fmaf(m11, uy, ay.tbm);
-                tz = fmaf(m22, uz, az.tb); tzm = fmaf(m22, uz, az.tbm);
+                tx = fmaf(m00, ux, ax.tb);
+                ty = fmaf(m11, uy, ay.tb);
+                tz = fmaf(m22, uz, az.tb);
             } else {
-                const float sx = fmaf(m00, ux, fmaf(m01, uy, m02 * uz));
-                const float sy_ = fmaf(m10, ux, fmaf(m11, uy, m12 * uz));
-                const float sz_ = fmaf(m20, ux, fmaf(m21, uy, m22 * uz));
-                tx = sx + ax.tb; txm = sx + ax.tbm;
-                ty = sy_ + ay.tb; tym = sy_ + ay.tbm;
-                tz = sz_ + az.tb; tzm = sz_ + az.tbm;
+                tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
+                ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
+                tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
             }
-            int i0, j0, k0;
-            float fx, fy, fz;
-            axis_cell(tx, txm, ax, i0, fx);
-            axis_cell(ty, tym, ay, j0, fy);
-            axis_cell(tz, tzm, az, k0, fz);
-            // ---- F_S: eight LDG.128, issued together
-            float4 c000, c001, c010, c011, c100, c101, c110, c111;
-            if (!ANYPER) {
-                const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
-                c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
-                c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
-                c100 = ldg_corner(p + sz);      c101 = ldg_corner(p + sz + 1);
-                c110 = ldg_corner(p + sz + sy); c111 = ldg_corner(p + sz + sy + 1);
-            } else {
-                if (perx) { i0 -= (i0 >= nx) ? nx : 0; i0 += (i0 < 0) ? nx : 0; }
-                if (pery) { j0 -= (j0 >= ny) ? ny : 0; j0 += (j0 < 0) ? ny : 0; }
-                if (perz) { k0 -= (k0 >= nz) ? nz : 0; k0 += (k0 < 0) ? nz : 0; }
-                const int i1 = (i0 + 1 == nx) ? 0 : i0 + 1;       // non-periodic axes never reach n - 1
-                const int j1 = (j0 + 1 == ny) ? 0 : j0 + 1;
-                const int k1 = (k0 + 1 == nz) ? 0 : k0 + 1;
-                const float4 *r00 = g + (long long)(k0 * ny + j0) * nx, *r01 = g + (long long)(k0 * ny + j1) * nx;
-                const float4 *r10 = g + (long long)(k1 * ny + j0) * nx, *r11 = g + (long long)(k1 * ny + j1) * nx;
-                c000 = ldg_corner(r00 + i0); c001 = ldg_corner(r00 + i1);
-                c010 = ldg_corner(r01 + i0); c011 = ldg_corner(r01 + i1);
-                c100 = ldg_corner(r10 + i0); c101 = ldg_corner(r10 + i1);
-                c110 = ldg_corner(r11 + i0); c111 = ldg_corner(r11 + i1);
+            float fx = tx - flx, fy = ty - fly, fz = tz - flz;
+            // outside [0,1] on any axis?  As unsigned integers, negative floats and floats > 1 both exceed bits(1.0f).
+            const unsigned worst = max(max(__float_as_uint(fx), __float_as_uint(fy)), __float_as_uint(fz));
+            if (worst > 0x3F800000u) {
+                // ---- the PP left the cached cell: locate the new one (magic-number floor, S12 clamp) and gather it
+                int i0, j0, k0;
+                axis_cell(tx, tx - 0.5f, ax, i0, fx, flx);
+                axis_cell(ty, ty - 0.5f, ay, j0, fy, fly);
+                axis_cell(tz, tz - 0.5f, az, k0, fz, flz);
+                float4 c000, c001, c010, c011, c100, c101, c110, c111;
+                if (!ANYPER) {
+                    const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
+                    c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
+                    c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
+                    c100 = ldg_corner(p + sz);      c101 = ldg_corner(p + sz + 1);
+                    c110 = ldg_corner(p + sz + sy); c111 = ldg_corner(p + sz + sy + 1);
+                } else {
+                    if (perx) { i0 -= (i0 >= nx) ? nx : 0; i0 += (i0 < 0) ? nx : 0; }
+                    if (pery) { j0 -= (j0 >= ny) ? ny : 0; j0 += (j0 < 0) ? ny : 0; }
+                    if (perz) { k0 -= (k0 >= nz) ? nz : 0; k0 += (k0 < 0) ? nz : 0; }
+                    const int i1 = (i0 + 1 == nx) ? 0 : i0 + 1;       // non-periodic axes never reach n - 1
+                    const int j1 = (j0 + 1 == ny) ? 0 : j0 + 1;
+                    const int k1 = (k0 + 1 == nz) ? 0 : k0 + 1;
+                    const float4 *r00 = g + (long long)(k0 * ny + j0) * nx, *r01 = g + (long long)(k0 * ny + j1) * nx;
+                    const float4 *r10 = g + (long long)(k1 * ny + j0) * nx, *r11 = g + (long long)(k1 * ny + j1) * nx;
+                    c000 = ldg_corner(r00 + i0); c001 = ldg_corner(r00 + i1);
+                    c010 = ldg_corner(r01 + i0); c011 = ldg_corner(r01 + i1);
+                    c100 = ldg_corner(r10 + i0); c101 = ldg_corner(r10 + i1);
+                    c110 = ldg_corner(r11 + i0); c111 = ldg_corner(r11 + i1);
+                }
+                c0[0][0] = c000.x; c0[0][1] = c000.y; c0[0][2] = c000.z;
+                c0[1][0] = c010.x; c0[1][1] = c010.y; c0[1][2] = c010.z;
+                c0[2][0] = c100.x; c0[2][1] = c100.y; c0[2][2] = c100.z;
+                c0[3][0] = c110.x; c0[3][1] = c110.y; c0[3][2] = c110.z;
+                cd[0][0] = c001.x - c000.x; cd[0][1] = c001.y - c000.y; cd[0][2] = c001.z - c000.z;
+                cd[1][0] = c011.x - c010.x; cd[1][1] = c011.y - c010.y; cd[1][2] = c011.z - c010.z;
+                cd[2][0] = c101.x - c100.x; cd[2][1] = c101.y - c100.y; cd[2][2] = c101.z - c100.z;
+                cd[3][0] = c111.x - c110.x; cd[3][1] = c111.y - c110.y; cd[3][2] = c111.z - c110.z;
+                my_reloads++;
             }
-            // ---- under the loads: F_T, radial + lateral springs (Eq.2) with d = d0 + u
+            // ---- F_S: tri-linear interpolation as nested lerps (x, then y, then z), 10 FP32 ops per component
+            float S[3];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
+                const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
+                const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
+                const float e11 = fmaf(fx, cd[3][c], c0[3][c]);
+                const float g0 = fmaf(fy, e10 - e00, e00);
+                const float g1 = fmaf(fy, e11 - e01, e01);
+                S[c] = fmaf(fz, g1 - g0, g0);
+            }
+            // ---- F_T: radial + lateral springs (Eq.2) with d = d0 + u; (|d| - R0)/|d| = (|u|^2 + 2 d0.u)/(|d|(|d| + R0))
             const float dxc = d0x + ux, dyc = d0y + uy;
             dzc = d0z + uz;
             const float L2 = fmaf(dxc, dxc, fmaf(dyc, dyc, dzc * dzc));
-            invL = rsqrt_fast(L2);
+            const float L = sqrt_fast(L2);
             const float num = fmaf(ux, ux + d0x2, fmaf(uy, uy + d0y2, uz * (uz + d0z2)));   // |u|^2 + 2 d0.u
-            ext = num * rcp_fast(fmaf(L2, invL, R_rest));                                    // |d| - R0
-            const float fr = -k_rad * ext * invL;
-            const float bx_ = fmaf(fr, dxc, -kx * ux), by_ = fmaf(fr, dyc, -ky * uy), bz_ = fr * dzc;
-            // ---- under the loads: the part of FIRE that needs only the old velocity (reading S6)
+            fr = (nk_rad * num) * rcp_fast(fmaf(R_rest, L, L2));                             // -k_R (|d| - R0)/|d|
+            const float Fx = fmaf(fr, dxc, fmaf(nkx, ux, S[0]));
+            const float Fy = fmaf(fr, dyc, fmaf(nky, uy, S[1]));
+            const float Fz = fmaf(fr, dzc, S[2]);
+            // ---- the part of FIRE that needs only the old velocity (reading S6), off the critical path
             const float vn = sqrt_fast(fmaf(vx, vx, fmaf(vy, vy, vz * vz)));
             const float av = alpha * vn, om = 1.0f - alpha;
             const float ovx = om * vx, ovy = om * vy, ovz = om * vz;
@@ -218,18 +249,6 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             const float dt_pos = grow ? fminf(dt * fp.finc, fp.dt_max) : dt;
             const float al_pos = grow ? alpha * fp.falpha : alpha;
             const float dt_neg = dt * fp.fdec;
-            // ---- under the loads: tri-linear weights
-            const float gx = 1.0f - fx, gy = 1.0f - fy, gz = 1.0f - fz;
-            const float w00 = gy * gz, w01 = fy * gz, w10 = gy * fz, w11 = fy * fz;
-            const float w000 = w00 * gx, w001 = w00 * fx, w010 = w01 * gx, w011 = w01 * fx;
-            const float w100 = w10 * gx, w101 = w10 * fx, w110 = w11 * gx, w111 = w11 * fx;
-            // ---- total force: two accumulation chains per component, seeded with the spring force
-            const float Fx = fmaf(w110, c110.x, fmaf(w100, c100.x, fmaf(w010, c010.x, fmaf(w000, c000.x, bx_)))) +
-                             fmaf(w111, c111.x, fmaf(w101, c101.x, fmaf(w011, c011.x, w001 * c001.x)));
-            const float Fy = fmaf(w110, c110.y, fmaf(w100, c100.y, fmaf(w010, c010.y, fmaf(w000, c000.y, by_)))) +
-                             fmaf(w111, c111.y, fmaf(w101, c101.y, fmaf(w011, c011.y, w001 * c001.y)));
-            const float Fz = fmaf(w110, c110.z, fmaf(w100, c100.z, fmaf(w010, c010.z, fmaf(w000, c000.z, bz_)))) +
-                             fmaf(w111, c111.z, fmaf(w101, c101.z, fmaf(w011, c011.z, w001 * c001.z)));
             const float F2 = fmaf(Fx, Fx, fmaf(Fy, Fy, Fz * Fz));
             const float Pw = fmaf(Fx, vx, fmaf(Fy, vy, Fz * vz));
             conv = conv || (F2 < fp.fconv2);                     // tested before every move (reading S7)
@@ -247,6 +266,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 ux = fmaf(vx, dt, ux); uy = fmaf(vy, dt, uy); uz = fmaf(vz, dt, uz);
                 moves++;
             }
+            my_witers++;
             if (__all_sync(0xffffffffu, done)) break;
         }
 
@@ -256,7 +276,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             outv.x = (float)(rb[0] + job.origin[0] + (double)ux);
             outv.y = (float)(rb[1] + job.origin[1] + (double)uy);
             outv.z = (float)(rz + job.origin[2] + (double)uz);
-            outv.w = k_rad * ext * invL * dzc;            // Fz_tip = -F_R,z
+            outv.w = -fr * dzc;                           // Fz_tip = -F_R,z
             pos_fz[o] = outv;
             if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
             const bool clamped = (tx < ax.lo) | (tx > ax.hi) | (ty < ay.lo) | (ty > ay.hi) | (tz < az.lo) | (tz > az.hi);
@@ -275,7 +295,12 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             my_clamped += __shfl_xor_sync(0xffffffffu, my_clamped, s);
             my_max = max(my_max, __shfl_xor_sync(0xffffffffu, my_max, s));
         }
+        unsigned long long rel = my_reloads;
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) rel += __shfl_xor_sync(0xffffffffu, rel, s);
         if (lane == 0) {
+            atomicAdd(reinterpret_cast<unsigned long long *>(&stats->warp_iters), (unsigned long long)my_witers);
+            atomicAdd(reinterpret_cast<unsigned long long *>(&stats->cell_gathers), rel);
             atomicAdd(reinterpret_cast<unsigned long long *>(&stats->total_iters), my_iters);
             if (my_notconv) atomicAdd(reinterpret_cast<unsigned long long *>(&stats->n_not_converged), (unsigned long long)my_notconv);
             if (my_clamped) atomicAdd(reinterpret_cast<unsigned long long *>(&stats->n_clamped), (unsigned long long)my_clamped);
