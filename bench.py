@@ -476,7 +476,8 @@ def run_ours(args):
                       "max_iters": stats["max_iters"],
                       "relax_warp_loop_trips": stats["warp_iters"],
                       "relax_lane_utilisation": stats["total_iters"] / max(1, 32 * stats["warp_iters"]),
-                      "relax_cell_gathers_per_iteration": stats["cell_gathers"] / max(1, stats["total_iters"])},
+                      "relax_cell_changes_per_iteration": stats["cell_gathers"] / max(1, stats["total_iters"]),
+                      "relax_gather_trips_per_loop_trip": stats["warp_gathers"] / max(1, stats["warp_iters"])},
             "e2e": {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
                     "d2h_bytes_per_step": host.d2h, "ms_per_step": e2e_t * 1e3, "steps": e2e_steps,
                     "api": "ppfm_scan_host (pinned host buffers)"},

@@ -97,8 +97,9 @@ typedef struct {
     uint32_t _pad;
     uint64_t warp_iters;      /* trips of the warp-converged FIRE loop, summed over warps (x32 lanes = issued lane-
                                  iterations; minus total_iters = divergence cost)             */
-    uint64_t cell_gathers;    /* 8-corner float4 gathers actually issued (a lane gathers only when the PP leaves
-                                 the grid cell it holds in registers)                          */
+    uint64_t cell_gathers;    /* lane-iterations in which the PP had left the grid cell the lane holds in registers */
+    uint64_t warp_gathers;    /* warp loop trips that executed the 8-corner float4 gather (all 32 lanes gather when
+                                 any lane left its cell)                                        */
 } ppfm_stats;
 
 int ppfm_version(void);

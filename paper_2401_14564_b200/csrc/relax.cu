@@ -106,17 +106,16 @@ __device__ __forceinline__ AxisBase axis_base(double t, int n, int periodic) {
     return a;
 }
 
-// cell offset fl (float, relative to the base cell), absolute cell index i0 (before periodic wrap) and fraction
-// f in [0,1] from t and t - 0.5
-__device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, int &i0, float &f, float &fl) {
+// cell offset fl (float, relative to the base cell) and absolute cell index i0 (before periodic wrap) from t, t - 0.5
+__device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, int &i0, float &fl) {
+    (void)t;
     const float z = tm + RX_MAGIC;                       // nearest integer of t - 0.5 = floor(t) (ties are harmless:
     const float zc = fminf(fmaxf(z, a.zlo), a.zhi);      //   the interpolant is continuous across cell faces)
     fl = zc - RX_MAGIC;
-    f = __saturatef(t - fl);
     i0 = __float_as_int(zc) - a.K;
 }
 
-template <bool ORTHO, bool ANYPER>
+template <bool ORTHO, bool ANYPER, bool SYMTIP>
 __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FireParams &fp, int lb,
                                              const float4 *__restrict__ ff, float4 *__restrict__ pos_fz,
                                              uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats) {
@@ -146,7 +145,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 
     float ux = 0.f, uy = 0.f, uz = 0.f;
     unsigned long long my_iters = 0;
-    unsigned int my_notconv = 0, my_clamped = 0, my_max = 0, my_reloads = 0, my_witers = 0;
+    unsigned int my_notconv = 0, my_clamped = 0, my_max = 0, my_reloads = 0, my_witers = 0, my_wreloads = 0;
 
     for (int iz = 0; iz < job.nzs; iz++) {
         // a4: exact fractional grid coordinate of the spring equilibrium point, split int + frac
@@ -158,36 +157,85 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         float vx = 0.f, vy = 0.f, vz = 0.f, dt = fp.dt0, alpha = fp.alpha0;
         int npos = 0, moves = 0;
         bool conv = !valid;
-        float fr, dzc, tx, ty, tz;
-        // cached cell (relative to this z-step's base cell): corner forces at x0 and their x-differences, for the
-        // four (y,z) edges 00, 10 (y+1), 01 (z+1), 11.  An impossible offset makes the first iteration reload.
-        float flx = 1.0e30f, fly = 1.0e30f, flz = 1.0e30f;
+        float fr = 0.f, dzc = d0z, fx = 0.f, fy = 0.f, fz = 0.f;
+        // cached cell: corner forces at x0 and their x-differences for the four (y,z) edges 00, 10 (y+1), 01 (z+1),
+        // 11, and per axis tbf = (fraction of the z-step's base point) - (offset of the cached cell from the base
+        // cell), so that the position inside the cell is one FFMA: f = Minv u + tbf.  An impossible offset makes the
+        // first iteration gather.
+        float tbfx = -1.0e30f, tbfy = -1.0e30f, tbfz = -1.0e30f;
         float c0[4][3], cd[4][3];
 #pragma unroll
         for (int e = 0; e < 4; e++)
 #pragma unroll
             for (int c = 0; c < 3; c++) c0[e][c] = cd[e][c] = 0.0f;
 
-        while (true) {
-            // ---- fractional position inside the cached cell
-            if (ORTHO) {
-                tx = fmaf(m00, ux, ax.tb);
-                ty = fmaf(m11, uy, ay.tb);
-                tz = fmaf(m22, uz, az.tb);
-            } else {
-                tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
-                ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
-                tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
+        auto interp = [&](float (&S)[3]) {     // nested lerps x, y, z: 10 FP32 ops per component
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
+                const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
+                const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
+                const float e11 = fmaf(fx, cd[3][c], c0[3][c]);
+                const float g0 = fmaf(fy, e10 - e00, e00);
+                const float g1 = fmaf(fy, e11 - e01, e01);
+                S[c] = fmaf(fz, g1 - g0, g0);
             }
-            float fx = tx - flx, fy = ty - fly, fz = tz - flz;
+        };
+
+        auto fire_iteration = [&]() -> bool {
+            // ---- position inside the cached cell
+            if (ORTHO) {
+                fx = fmaf(m00, ux, tbfx);
+                fy = fmaf(m11, uy, tbfy);
+                fz = fmaf(m22, uz, tbfz);
+            } else {
+                fx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, tbfx)));
+                fy = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy)));
+                fz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz)));
+            }
             // outside [0,1] on any axis?  As unsigned integers, negative floats and floats > 1 both exceed bits(1.0f).
             const unsigned worst = max(max(__float_as_uint(fx), __float_as_uint(fy)), __float_as_uint(fz));
-            if (worst > 0x3F800000u) {
-                // ---- the PP left the cached cell: locate the new one (magic-number floor, S12 clamp) and gather it
+            // ---- F_T first (the longest dependency chain: two MUFU): radial + lateral springs (Eq.2) with d = d0 + u;
+            // (|d| - R0)/|d| = (|u|^2 + 2 d0.u)/(|d|(|d| + R0))
+            float dxc = ux, dyc = uy, frk;
+            dzc = d0z + uz;
+            if (SYMTIP) {                      // d0 = (0, 0, d0z) and k_x = k_y: the usual symmetric tip
+                const float w = fmaf(ux, ux, uy * uy);
+                const float L2 = fmaf(dzc, dzc, w);
+                const float num = fmaf(uz, uz + d0z2, w);                                    // |u|^2 + 2 d0.u
+                const float L = sqrt_fast(L2);
+                fr = (nk_rad * num) * rcp_fast(fmaf(R_rest, L, L2));                         // -k_R (|d| - R0)/|d|
+                frk = fr + nkx;
+            } else {
+                dxc = d0x + ux; dyc = d0y + uy;
+                const float L2 = fmaf(dxc, dxc, fmaf(dyc, dyc, dzc * dzc));
+                const float num = fmaf(ux, ux + d0x2, fmaf(uy, uy + d0y2, uz * (uz + d0z2)));
+                const float L = sqrt_fast(L2);
+                fr = (nk_rad * num) * rcp_fast(fmaf(R_rest, L, L2));
+                frk = fr;
+            }
+            // ---- F_S, speculatively from the cached cell (redone below in the rare case that a lane left its cell)
+            float S[3];
+            interp(S);
+            if (__any_sync(0xffffffffu, worst > 0x3F800000u)) {
+                // ---- some lane's PP left its cell.  The block is warp-uniform (no reconvergence barrier on the hot
+                // path): every lane locates its cell again (magic-number floor, S12 clamp) and gathers it; lanes
+                // that had not moved get the cell they already hold, from L1.
+                float tx, ty, tz;
+                if (ORTHO) {
+                    tx = fmaf(m00, ux, ax.tb);
+                    ty = fmaf(m11, uy, ay.tb);
+                    tz = fmaf(m22, uz, az.tb);
+                } else {
+                    tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
+                    ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
+                    tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
+                }
                 int i0, j0, k0;
-                axis_cell(tx, tx - 0.5f, ax, i0, fx, flx);
-                axis_cell(ty, ty - 0.5f, ay, j0, fy, fly);
-                axis_cell(tz, tz - 0.5f, az, k0, fz, flz);
+                float flx, fly, flz;
+                axis_cell(tx, tx - 0.5f, ax, i0, flx);
+                axis_cell(ty, ty - 0.5f, ay, j0, fly);
+                axis_cell(tz, tz - 0.5f, az, k0, flz);
                 float4 c000, c001, c010, c011, c100, c101, c110, c111;
                 if (!ANYPER) {
                     const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
@@ -209,6 +257,16 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                     c100 = ldg_corner(r10 + i0); c101 = ldg_corner(r10 + i1);
                     c110 = ldg_corner(r11 + i0); c111 = ldg_corner(r11 + i1);
                 }
+                tbfx = ax.tb - flx; tbfy = ay.tb - fly; tbfz = az.tb - flz;
+                if (ORTHO) {
+                    fx = __saturatef(fmaf(m00, ux, tbfx));
+                    fy = __saturatef(fmaf(m11, uy, tbfy));
+                    fz = __saturatef(fmaf(m22, uz, tbfz));
+                } else {
+                    fx = __saturatef(fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, tbfx))));
+                    fy = __saturatef(fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy))));
+                    fz = __saturatef(fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz))));
+                }
                 c0[0][0] = c000.x; c0[0][1] = c000.y; c0[0][2] = c000.z;
                 c0[1][0] = c010.x; c0[1][1] = c010.y; c0[1][2] = c010.z;
                 c0[2][0] = c100.x; c0[2][1] = c100.y; c0[2][2] = c100.z;
@@ -217,34 +275,22 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 cd[1][0] = c011.x - c010.x; cd[1][1] = c011.y - c010.y; cd[1][2] = c011.z - c010.z;
                 cd[2][0] = c101.x - c100.x; cd[2][1] = c101.y - c100.y; cd[2][2] = c101.z - c100.z;
                 cd[3][0] = c111.x - c110.x; cd[3][1] = c111.y - c110.y; cd[3][2] = c111.z - c110.z;
-                my_reloads++;
+                my_reloads += (worst > 0x3F800000u) ? 1u : 0u;
+                my_wreloads++;
+                interp(S);
             }
-            // ---- F_S: tri-linear interpolation as nested lerps (x, then y, then z), 10 FP32 ops per component
-            float S[3];
-#pragma unroll
-            for (int c = 0; c < 3; c++) {
-                const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
-                const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
-                const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
-                const float e11 = fmaf(fx, cd[3][c], c0[3][c]);
-                const float g0 = fmaf(fy, e10 - e00, e00);
-                const float g1 = fmaf(fy, e11 - e01, e01);
-                S[c] = fmaf(fz, g1 - g0, g0);
+            float Fx, Fy, Fz;
+            if (SYMTIP) {
+                Fx = fmaf(frk, ux, S[0]);
+                Fy = fmaf(frk, uy, S[1]);
+            } else {
+                Fx = fmaf(fr, dxc, fmaf(nkx, ux, S[0]));
+                Fy = fmaf(fr, dyc, fmaf(nky, uy, S[1]));
             }
-            // ---- F_T: radial + lateral springs (Eq.2) with d = d0 + u; (|d| - R0)/|d| = (|u|^2 + 2 d0.u)/(|d|(|d| + R0))
-            const float dxc = d0x + ux, dyc = d0y + uy;
-            dzc = d0z + uz;
-            const float L2 = fmaf(dxc, dxc, fmaf(dyc, dyc, dzc * dzc));
-            const float L = sqrt_fast(L2);
-            const float num = fmaf(ux, ux + d0x2, fmaf(uy, uy + d0y2, uz * (uz + d0z2)));   // |u|^2 + 2 d0.u
-            fr = (nk_rad * num) * rcp_fast(fmaf(R_rest, L, L2));                             // -k_R (|d| - R0)/|d|
-            const float Fx = fmaf(fr, dxc, fmaf(nkx, ux, S[0]));
-            const float Fy = fmaf(fr, dyc, fmaf(nky, uy, S[1]));
-            const float Fz = fmaf(fr, dzc, S[2]);
+            Fz = fmaf(fr, dzc, S[2]);
             // ---- the part of FIRE that needs only the old velocity (reading S6), off the critical path
             const float vn = sqrt_fast(fmaf(vx, vx, fmaf(vy, vy, vz * vz)));
             const float av = alpha * vn, om = 1.0f - alpha;
-            const float ovx = om * vx, ovy = om * vy, ovz = om * vz;
             const bool grow = npos > fp.n_min;
             const float dt_pos = grow ? fminf(dt * fp.finc, fp.dt_max) : dt;
             const float al_pos = grow ? alpha * fp.falpha : alpha;
@@ -255,10 +301,11 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             const bool done = conv || (moves >= fp.max_iter);
             // ---- FIRE step, branch-free; P >= 0 counts as downhill
             const bool down = Pw >= 0.0f;
+            const float omv = down ? om : 0.0f;
             const float s = down ? fmaf(av, rsqrt_fast(F2), dt_pos) : dt_neg;
-            vx = fmaf(s, Fx, down ? ovx : 0.0f);
-            vy = fmaf(s, Fy, down ? ovy : 0.0f);
-            vz = fmaf(s, Fz, down ? ovz : 0.0f);
+            vx = fmaf(s, Fx, omv * vx);
+            vy = fmaf(s, Fy, omv * vy);
+            vz = fmaf(s, Fz, omv * vz);
             dt = down ? dt_pos : dt_neg;
             alpha = down ? al_pos : fp.alpha0;
             npos = down ? npos + 1 : 0;
@@ -266,7 +313,15 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 ux = fmaf(vx, dt, ux); uy = fmaf(vy, dt, uy); uz = fmaf(vz, dt, uz);
                 moves++;
             }
-            my_witers++;
+            return done;
+        };
+
+        // the convergence vote is taken every second iteration: finished lanes do not move, so an extra iteration
+        // changes nothing but saves one VOTE + branch per iteration
+        while (true) {
+            fire_iteration();
+            const bool done = fire_iteration();
+            my_witers += 2;
             if (__all_sync(0xffffffffu, done)) break;
         }
 
@@ -279,6 +334,14 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             outv.w = -fr * dzc;                           // Fz_tip = -F_R,z
             pos_fz[o] = outv;
             if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
+            float tx, ty, tz;
+            if (ORTHO) {
+                tx = fmaf(m00, ux, ax.tb); ty = fmaf(m11, uy, ay.tb); tz = fmaf(m22, uz, az.tb);
+            } else {
+                tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
+                ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
+                tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
+            }
             const bool clamped = (tx < ax.lo) | (tx > ax.hi) | (ty < ay.lo) | (ty > ay.hi) | (tz < az.lo) | (tz > az.hi);
             my_iters += (unsigned)moves;
             my_notconv += conv ? 0u : 1u;
@@ -301,6 +364,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         if (lane == 0) {
             atomicAdd(reinterpret_cast<unsigned long long *>(&stats->warp_iters), (unsigned long long)my_witers);
             atomicAdd(reinterpret_cast<unsigned long long *>(&stats->cell_gathers), rel);
+            atomicAdd(reinterpret_cast<unsigned long long *>(&stats->warp_gathers), (unsigned long long)my_wreloads);
             atomicAdd(reinterpret_cast<unsigned long long *>(&stats->total_iters), my_iters);
             if (my_notconv) atomicAdd(reinterpret_cast<unsigned long long *>(&stats->n_not_converged), (unsigned long long)my_notconv);
             if (my_clamped) atomicAdd(reinterpret_cast<unsigned long long *>(&stats->n_clamped), (unsigned long long)my_clamped);
@@ -310,16 +374,16 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 }
 
 // One system: the job travels as a kernel parameter (constant bank), no scratch and no copy.
-template <bool ORTHO, bool ANYPER>
+template <bool ORTHO, bool ANYPER, bool SYMTIP>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireParams fp,
              const float4 *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
              ppfm_stats *__restrict__ stats) {
-    relax_pixels<ORTHO, ANYPER>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats);
+    relax_pixels<ORTHO, ANYPER, SYMTIP>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats);
 }
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
-template <bool ORTHO, bool ANYPER>
+template <bool ORTHO, bool ANYPER, bool SYMTIP>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_constant__ FireParams fp,
                    const float4 *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
@@ -337,16 +401,16 @@ relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_co
         for (int w = threadIdx.x; w < (int)(sizeof(RelaxJob) / sizeof(int)); w += RX_THREADS) dstw[w] = srcw[w];
     }
     __syncthreads();
-    relax_pixels<ORTHO, ANYPER>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats);
+    relax_pixels<ORTHO, ANYPER, SYMTIP>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats);
 }
 
-template <bool ORTHO, bool ANYPER>
+template <bool ORTHO, bool ANYPER, bool SYMTIP>
 static void launch_relax(int nsys, long long blocks, cudaStream_t st, const RelaxJob *hj, const RelaxJob *dj,
                          const FireParams &fp, const float4 *ff, float4 *pos, uint16_t *it, ppfm_stats *stats) {
     if (nsys == 1)
-        relax_kernel<ORTHO, ANYPER><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats);
+        relax_kernel<ORTHO, ANYPER, SYMTIP><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats);
     else
-        relax_batch_kernel<ORTHO, ANYPER><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
+        relax_batch_kernel<ORTHO, ANYPER, SYMTIP><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
 }
 
 static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
@@ -362,7 +426,7 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
     RelaxJob *hj = (RelaxJob *)calloc((size_t)nsys, sizeof(RelaxJob));
     if (!hj) return PPFM_ENOMEM;
     long long blocks = 0, ff_off = 0, out_off = 0;
-    bool ortho = true, anyper = false;
+    bool ortho = true, anyper = false, symtip = true;
     for (int m = 0; m < nsys; m++) {
         const ppfm_grid &g = grids[m];
         const ppfm_scan &s = scans[m];
@@ -396,6 +460,7 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
         j.R_rest = (float)R0;
         j.k_lat[0] = (float)t.k_lat[0]; j.k_lat[1] = (float)t.k_lat[1];
         j.k_rad = (float)t.k_rad;
+        if (t.d0[0] != 0.0 || t.d0[1] != 0.0 || j.k_lat[0] != j.k_lat[1]) symtip = false;
         blocks += (long long)j.nbx * ((s.npy + RX_TILE_Y - 1) / RX_TILE_Y);
         ff_off += grid_points(&g);
         out_off += (long long)s.npx * s.npy * s.nz;
@@ -420,10 +485,19 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
     float4 *pos4 = reinterpret_cast<float4 *>(d_pos_fz);
     {
         KernelTimer kt(PPFM_K_RELAX, st);
-        if (ortho && !anyper) launch_relax<true, false>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
-        else if (ortho) launch_relax<true, true>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
-        else if (!anyper) launch_relax<false, false>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
-        else launch_relax<false, true>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats);
+#define PPFM_RX(O, A, S) launch_relax<O, A, S>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats)
+        if (symtip) {
+            if (ortho && !anyper) PPFM_RX(true, false, true);
+            else if (ortho) PPFM_RX(true, true, true);
+            else if (!anyper) PPFM_RX(false, false, true);
+            else PPFM_RX(false, true, true);
+        } else {
+            if (ortho && !anyper) PPFM_RX(true, false, false);
+            else if (ortho) PPFM_RX(true, true, false);
+            else if (!anyper) PPFM_RX(false, false, false);
+            else PPFM_RX(false, true, false);
+        }
+#undef PPFM_RX
     }
     free(hj);
     e = cudaGetLastError();

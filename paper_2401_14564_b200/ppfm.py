@@ -53,7 +53,7 @@ class Scan(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("total_iters", C.c_uint64), ("n_not_converged", C.c_uint64), ("n_clamped", C.c_uint64),
                 ("max_iters", C.c_uint32), ("_pad", C.c_uint32), ("warp_iters", C.c_uint64),
-                ("cell_gathers", C.c_uint64)]
+                ("cell_gathers", C.c_uint64), ("warp_gathers", C.c_uint64)]
 
 
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
@@ -276,13 +276,14 @@ def forcefield_batch(atom_offset: Sequence[int], xyzq, types, elem_R, elem_e, la
 # ---- (2) relaxation scan --------------------------------------------------------------------------------------
 def new_stats(device="cuda"):
     torch = _torch()
-    return torch.zeros(6, dtype=torch.int64, device=device)      # 48 bytes = sizeof(ppfm_stats)
+    return torch.zeros(7, dtype=torch.int64, device=device)      # 56 bytes = sizeof(ppfm_stats)
 
 
 def read_stats(stats) -> dict:
     raw = stats.cpu().numpy().view(np.uint64)
     return {"total_iters": int(raw[0]), "n_not_converged": int(raw[1]), "n_clamped": int(raw[2]),
-            "max_iters": int(raw[3] & np.uint64(0xFFFFFFFF)), "warp_iters": int(raw[4]), "cell_gathers": int(raw[5])}
+            "max_iters": int(raw[3] & np.uint64(0xFFFFFFFF)), "warp_iters": int(raw[4]), "cell_gathers": int(raw[5]),
+            "warp_gathers": int(raw[6])}
 
 
 def relax_scan(ff, grid, tip, fire, scan, pos_fz=None, iters=None, stats=None, want_iters=True):
@@ -362,7 +363,7 @@ def scan_host(w, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None, Q=None
     _check(rc, "ppfm_scan_host")
     return {"total_iters": int(st.total_iters), "n_not_converged": int(st.n_not_converged),
             "n_clamped": int(st.n_clamped), "max_iters": int(st.max_iters), "warp_iters": int(st.warp_iters),
-            "cell_gathers": int(st.cell_gathers)}
+            "cell_gathers": int(st.cell_gathers), "warp_gathers": int(st.warp_gathers)}
 
 
 # ---- probes --------------------------------------------------------------------------------------------------------

@@ -41,7 +41,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(ppfm.Probe) == 24 and C.sizeof(ppfm.Tip) == 48
     assert C.sizeof(ppfm.Fire) == 6 * 8 + 2 * 4 + 8
     assert C.sizeof(ppfm.Scan) == 9 * 8 + 3 * 4 + 4 + 8
-    assert C.sizeof(ppfm.Stats) == 48
+    assert C.sizeof(ppfm.Stats) == 56
 
 
 def test_defaults_and_units(lib):
