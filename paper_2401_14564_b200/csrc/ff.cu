@@ -19,14 +19,17 @@ namespace ppfm {
 
 constexpr int FF_THREADS = 256;
 constexpr int FF_CHUNK = 256;   // atoms per pipeline stage
-constexpr int FF_STAGES = 4;
+constexpr int FF_STAGES = 3;
 constexpr int FF_AHEAD = 2;     // chunks in flight ahead of the consumer
 
+// 48-byte record.  The pair coefficients are stored twice so that one LDS.128 yields the aligned 64-bit register
+// pairs the packed FP32x2 instructions (FFMA2 / FMUL2 / FADD2, new on sm_100) take as operands, with no MOVs.
 struct __align__(16) AtomRec {
-    float x, y, z, kq;          // kq = k_e q_PP q_i  (eV*Angstrom)
-    float c6, c12, c6x6, kq1;   // c6 = 2 E0 R0^6, c12 = E0 R0^12, c6x6 = 6 c6, kq1 = k_e q_i (unit probe charge)
+    float x, y, z, pad;
+    float c12[2], nc6[2];       // c12 = E0 R0^12, nc6 = -2 E0 R0^6
+    float c6x6[2], kq[2];       // 6 c6;  kq = k_e q_PP q_i (eV*Angstrom), or k_e q_i (unit probe charge) in split mode
 };
-static_assert(sizeof(AtomRec) == 32, "AtomRec must be 32 bytes");
+static_assert(sizeof(AtomRec) == 48, "AtomRec must be 48 bytes");
 
 struct FFJob {
     long long tile_begin;   // first tile (CTA) of this system in the launch
@@ -41,7 +44,7 @@ struct FFJob {
     float keQ;              // k_e q_PP
     float rmin2;
     int ntypes;
-    int pad;
+    int split;              // records carry the unit-charge Coulomb factor
 };
 
 struct TypeEntry {
@@ -61,13 +64,15 @@ __device__ __forceinline__ void prep_atom(const FFJob &job, const TypeEntry *__r
     const int t = type[i];
     AtomRec r;
     r.x = a.x; r.y = a.y; r.z = a.z;
+    r.pad = 0.0f;
     if (t >= 0 && t < job.ntypes) {
         const TypeEntry te = table[job.table_offset + t];
-        r.c6 = te.c6; r.c12 = te.c12; r.c6x6 = 6.0f * te.c6;
-        r.kq = (float)((double)job.keQ * (double)a.w);
-        r.kq1 = (float)(kCoulomb * (double)a.w);
+        r.c12[0] = r.c12[1] = te.c12;
+        r.nc6[0] = r.nc6[1] = -te.c6;
+        r.c6x6[0] = r.c6x6[1] = 6.0f * te.c6;
+        r.kq[0] = r.kq[1] = job.split ? (float)(kCoulomb * (double)a.w) : (float)((double)job.keQ * (double)a.w);
     } else {   // out-of-range type index: the atom contributes nothing
-        r.c6 = r.c12 = r.c6x6 = r.kq = r.kq1 = 0.0f;
+        r.c12[0] = r.c12[1] = r.nc6[0] = r.nc6[1] = r.c6x6[0] = r.c6x6[1] = r.kq[0] = r.kq[1] = 0.0f;
     }
     recs[i] = r;
     // r_min clamp needed?  distance of every image of this atom to the grid's bounding box
@@ -165,26 +170,29 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restr
 #pragma unroll
     for (int c = 0; c < 3; c++)
         pb[c] = job.origin[c] + i * job.step[0][c] + j * job.step[1][c] + k0 * job.step[2][c];
-    float off[ZCOL ? 1 : 3][P];   // offsets of the P points along step[2]
+    // P points along step[2], held as P/2 packed pairs (lo = point 2h, hi = point 2h + 1)
+    constexpr int H = P / 2;
+    static_assert(P % 2 == 0, "P must be even: points are processed as FP32x2 pairs");
+    float2 off[ZCOL ? 1 : 3][H];   // offsets of the points along step[2]
 #pragma unroll
-    for (int k = 0; k < P; k++) {
-        if (ZCOL) {
-            off[0][k] = (float)(k * job.step[2][2]);
-        } else {
+    for (int h = 0; h < H; h++) {
 #pragma unroll
-            for (int c = 0; c < (ZCOL ? 1 : 3); c++) off[c][k] = (float)(k * job.step[2][c]);
+        for (int c = 0; c < (ZCOL ? 1 : 3); c++) {
+            const int cc = ZCOL ? 2 : c;
+            off[c][h] = make_float2((float)((2 * h) * job.step[2][cc]), (float)((2 * h + 1) * job.step[2][cc]));
         }
     }
 
-    float Fx[P], Fy[P], Fz[P], E[P];
-    float Gx[SPLIT ? P : 1], Gy[SPLIT ? P : 1], Gz[SPLIT ? P : 1], Ge[SPLIT ? P : 1];
+    float2 Fx[H], Fy[H], Fz[H], E[H];
+    float2 Gx[SPLIT ? H : 1], Gy[SPLIT ? H : 1], Gz[SPLIT ? H : 1], Ge[SPLIT ? H : 1];
     // energies are accumulated per chunk and folded into a running total at every chunk boundary: the 1/r and
     // 1/r^6 tails of tens of thousands of atom images otherwise lose ~1e-5 eV to FP32 accumulation rounding
-    float Etot[P], Getot[SPLIT ? P : 1];
+    float2 Etot[H], Getot[SPLIT ? H : 1];
+    const float2 zero2 = make_float2(0.0f, 0.0f);
 #pragma unroll
-    for (int k = 0; k < P; k++) {
-        Fx[k] = Fy[k] = Fz[k] = E[k] = Etot[k] = 0.0f;
-        if (SPLIT) Gx[k] = Gy[k] = Gz[k] = Ge[k] = Getot[k] = 0.0f;
+    for (int h = 0; h < H; h++) {
+        Fx[h] = Fy[h] = Fz[h] = E[h] = Etot[h] = zero2;
+        if (SPLIT) Gx[h] = Gy[h] = Gz[h] = Ge[h] = Getot[h] = zero2;
     }
 
     const int natoms = job.natoms;
@@ -226,73 +234,84 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restr
                     mbar_wait(&full_bar[st], (step / FF_STAGES) & 1);
                     const float4 *s4 = reinterpret_cast<const float4 *>(s_rec + st * FF_CHUNK);
                     const int n = min(FF_CHUNK, natoms - ch * FF_CHUNK);
+                    const float2 twelve = make_float2(12.0f, 12.0f);
 #pragma unroll 2
                     for (int a = 0; a < n; a++) {
-                        const float4 r0 = s4[2 * a];
-                        const float4 r1 = s4[2 * a + 1];
+                        const float4 r0 = s4[3 * a];          // x, y, z, -
+                        const float4 r1 = s4[3 * a + 1];      // c12, c12, -c6, -c6
+                        const float4 r2_ = s4[3 * a + 2];     // 6 c6, 6 c6, kq, kq
+                        const float2 c12 = make_float2(r1.x, r1.y), nc6 = make_float2(r1.z, r1.w);
+                        const float2 c6x6 = make_float2(r2_.x, r2_.y), kq = make_float2(r2_.z, r2_.w);
                         const float dx0 = (ph[0] - r0.x) + pl[0];
                         const float dy0 = (ph[1] - r0.y) + pl[1];
                         const float dz0 = (ph[2] - r0.z) + pl[2];
-                        const float rxy2 = fmaf(dy0, dy0, dx0 * dx0);
-                        const float kq = SPLIT ? r1.w : r0.w;
+                        const float rxy2s = fmaf(dy0, dy0, dx0 * dx0);
+                        const float2 dxx = make_float2(dx0, dx0), dyy = make_float2(dy0, dy0);
+                        const float2 dzz = make_float2(dz0, dz0), rxy2 = make_float2(rxy2s, rxy2s);
 #pragma unroll
-                        for (int k = 0; k < P; k++) {
-                            float dx, dy, dz, r2;
+                        for (int h = 0; h < H; h++) {
+                            float2 dx, dy, dz, r2;
                             if (ZCOL) {
-                                dx = dx0; dy = dy0;
-                                dz = dz0 + off[0][k];
-                                r2 = fmaf(dz, dz, rxy2);
+                                dx = dxx; dy = dyy;
+                                dz = __fadd2_rn(dzz, off[0][h]);
+                                r2 = __ffma2_rn(dz, dz, rxy2);
                             } else {
-                                dx = dx0 + off[0][k]; dy = dy0 + off[1 % (ZCOL ? 1 : 3)][k];
-                                dz = dz0 + off[2 % (ZCOL ? 1 : 3)][k];
-                                r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                                dx = __fadd2_rn(dxx, off[0][h]);
+                                dy = __fadd2_rn(dyy, off[1 % (ZCOL ? 1 : 3)][h]);
+                                dz = __fadd2_rn(dzz, off[2 % (ZCOL ? 1 : 3)][h]);
+                                r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
                             }
-                            if (CLAMP) r2 = fmaxf(r2, rmin2);
-                            const float ir = rsqrt_approx(r2);
-                            const float ir2 = ir * ir;
-                            const float ir6 = ir2 * ir2 * ir2;
-                            const float t = fmaf(r1.y, ir6, -r1.x);        // c12/r^6 - c6
-                            const float t2 = fmaf(t, 12.0f, r1.z);         // 12 c12/r^6 - 6 c6
-                            E[k] = fmaf(t, ir6, E[k]);                       // E_LJ = c12/r^12 - c6/r^6
+                            if (CLAMP) { r2.x = fmaxf(r2.x, rmin2); r2.y = fmaxf(r2.y, rmin2); }
+                            float2 ir;
+                            ir.x = rsqrt_approx(r2.x);
+                            ir.y = rsqrt_approx(r2.y);
+                            const float2 ir2 = __fmul2_rn(ir, ir);
+                            const float2 ir6 = __fmul2_rn(__fmul2_rn(ir2, ir2), ir2);
+                            const float2 t = __ffma2_rn(c12, ir6, nc6);        // c12/r^6 - c6
+                            const float2 t2 = __ffma2_rn(t, twelve, c6x6);    // 12 c12/r^6 - 6 c6
+                            E[h] = __ffma2_rn(t, ir6, E[h]);                   // E_LJ = c12/r^12 - c6/r^6
                             if (!SPLIT) {
-                                E[k] = fmaf(kq, ir, E[k]);                   // E_C = kq / r
-                                float g = t2 * ir6;
-                                g = fmaf(kq, ir, g);
-                                const float f = g * ir2;                     // (12c12/r^12 - 6c6/r^6 + kq/r) / r^2
-                                Fx[k] = fmaf(f, dx, Fx[k]);
-                                Fy[k] = fmaf(f, dy, Fy[k]);
-                                Fz[k] = fmaf(f, dz, Fz[k]);
+                                E[h] = __ffma2_rn(kq, ir, E[h]);               // E_C = kq / r
+                                const float2 g = __ffma2_rn(kq, ir, __fmul2_rn(t2, ir6));
+                                const float2 f = __fmul2_rn(g, ir2);           // (12c12/r^12 - 6c6/r^6 + kq/r) / r^2
+                                Fx[h] = __ffma2_rn(f, dx, Fx[h]);
+                                Fy[h] = __ffma2_rn(f, dy, Fy[h]);
+                                Fz[h] = __ffma2_rn(f, dz, Fz[h]);
                             } else {
-                                const float f = t2 * ir6 * ir2;
-                                Fx[k] = fmaf(f, dx, Fx[k]);
-                                Fy[k] = fmaf(f, dy, Fy[k]);
-                                Fz[k] = fmaf(f, dz, Fz[k]);
-                                const float ec = kq * ir;
-                                Ge[k] += ec;
-                                const float fe = ec * ir2;
-                                Gx[k] = fmaf(fe, dx, Gx[k]);
-                                Gy[k] = fmaf(fe, dy, Gy[k]);
-                                Gz[k] = fmaf(fe, dz, Gz[k]);
+                                const float2 f = __fmul2_rn(__fmul2_rn(t2, ir6), ir2);
+                                Fx[h] = __ffma2_rn(f, dx, Fx[h]);
+                                Fy[h] = __ffma2_rn(f, dy, Fy[h]);
+                                Fz[h] = __ffma2_rn(f, dz, Fz[h]);
+                                const float2 ec = __fmul2_rn(kq, ir);
+                                Ge[h] = __fadd2_rn(Ge[h], ec);
+                                const float2 fe = __fmul2_rn(ec, ir2);
+                                Gx[h] = __ffma2_rn(fe, dx, Gx[h]);
+                                Gy[h] = __ffma2_rn(fe, dy, Gy[h]);
+                                Gz[h] = __ffma2_rn(fe, dz, Gz[h]);
                             }
                         }
                     }
                     __syncwarp();
                     if ((tid & 31) == 0) mbar_arrive(&empty_bar[st]);
 #pragma unroll
-                    for (int k = 0; k < P; k++) {
-                        Etot[k] += E[k]; E[k] = 0.0f;
-                        if (SPLIT) { Getot[k] += Ge[k]; Ge[k] = 0.0f; }
+                    for (int h = 0; h < H; h++) {
+                        Etot[h] = __fadd2_rn(Etot[h], E[h]); E[h] = zero2;
+                        if (SPLIT) { Getot[h] = __fadd2_rn(Getot[h], Ge[h]); Ge[h] = zero2; }
                     }
                 }
             }
 
     if (valid) {
 #pragma unroll
-        for (int k = 0; k < P; k++) {
-            if (k0 + k < job.nz) {
-                const size_t o = (size_t)job.out_offset + (size_t)(k0 + k) * job.nxy + col;
-                out_a[o] = make_float4(Fx[k], Fy[k], Fz[k], Etot[k]);
-                if (SPLIT) out_b[o] = make_float4(Gx[k], Gy[k], Gz[k], Getot[k]);
+        for (int h = 0; h < H; h++) {
+            const size_t o = (size_t)job.out_offset + (size_t)(k0 + 2 * h) * job.nxy + col;
+            if (k0 + 2 * h < job.nz) {
+                out_a[o] = make_float4(Fx[h].x, Fy[h].x, Fz[h].x, Etot[h].x);
+                if (SPLIT) out_b[o] = make_float4(Gx[h].x, Gy[h].x, Gz[h].x, Getot[h].x);
+            }
+            if (k0 + 2 * h + 1 < job.nz) {
+                out_a[o + job.nxy] = make_float4(Fx[h].y, Fy[h].y, Fz[h].y, Etot[h].y);
+                if (SPLIT) out_b[o + job.nxy] = make_float4(Gx[h].y, Gy[h].y, Gz[h].y, Getot[h].y);
             }
         }
     }
@@ -370,10 +389,12 @@ __global__ void combine_kernel(const float4 *__restrict__ lj, const float4 *__re
 }
 
 // ---------------------------------------------------------------------------------------------------- host side
-static int pick_P(int nz) {
-    // padded work ~ ceil(nz/P) * (P + per-atom overhead shared by the column ~ 0.7 points)
-    const int cand[3] = {8, 10, 5};
-    int best = 8;
+static int pick_P(int nz, bool split) {
+    // padded work ~ ceil(nz/P) * (P + per-atom overhead shared by the column ~ 0.7 points).  The split kernel keeps
+    // two accumulator sets per point, so it takes fewer points per thread (P = 8, 10 would spill at 128 registers).
+    const int cand_one[3] = {8, 10, 6}, cand_two[3] = {8, 6, 4};
+    const int *cand = split ? cand_two : cand_one;
+    int best = cand[0];
     double best_cost = 1e300;
     for (int c = 0; c < 3; c++) {
         const int P = cand[c];
@@ -396,9 +417,11 @@ static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st
                              int njobs, const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
     KernelTimer kt(PPFM_K_FF, st);
     if (!zcol) launch_ff_one<SPLIT, 4, false>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else if (P == 10) launch_ff_one<SPLIT, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else if (P == 5) launch_ff_one<SPLIT, 5, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else launch_ff_one<SPLIT, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 6) launch_ff_one<SPLIT, 6, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 8) launch_ff_one<SPLIT, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (SPLIT) launch_ff_one<SPLIT, 4, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 10) launch_ff_one<false, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else launch_ff_one<false, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     return cudaGetLastError();
 }
 
@@ -431,7 +454,7 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
         if (g.step[2][0] != 0.0 || g.step[2][1] != 0.0) zcol = false;
         if (g.n[2] != nz_common) nz_common = -1;
     }
-    const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2]) : 4;
+    const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2], split) : 4;
 
     const bool single = (nsys == 1);
     const size_t jobs_bytes = (size_t)nsys * sizeof(FFJob);
@@ -463,6 +486,7 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
         j.n_z_groups = (j.nz + P - 1) / P;
         j.table_offset = m * ntypes;
         j.ntypes = ntypes;
+        j.split = split ? 1 : 0;
         for (int a = 0; a < 3; a++) {
             j.nimg[a] = lattices[m].nimg[a];
             j.origin[a] = g.origin[a];
