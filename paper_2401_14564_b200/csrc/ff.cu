@@ -15,6 +15,8 @@
 //   * a3  `combine_kernel`: F = F_LJ + Q F_el, float4 streaming.
 #include "common.cuh"
 
+#include <type_traits>
+
 namespace ppfm {
 
 constexpr int FF_THREADS = 256;
@@ -57,11 +59,14 @@ struct FFSingle {               // one system: job and per-type table travel as 
     TypeEntry table[PPFM_MAX_TYPES];
 };
 
-__device__ __forceinline__ void prep_atom(const FFJob &job, const TypeEntry *__restrict__ table, int job_index,
-                                          const float4 *__restrict__ xyzq, const int *__restrict__ type,
-                                          AtomRec *__restrict__ recs, int *__restrict__ clamp_flags, int i) {
-    const float4 a = xyzq[i];
-    const int t = type[i];
+// Per-system flags written by the prep kernel and read by every tile of that system.
+struct FFFlags {
+    int clamp;      // some atom image lies within r_min of the grid's bounding box: the tile applies the S3 clamp
+    int ncharged;   // records [0, ncharged) carry a Coulomb factor != 0; the rest are LJ-only (e.g. a neutral slab)
+};
+constexpr int PREP_THREADS = 256;
+
+__device__ __forceinline__ AtomRec make_record(const FFJob &job, const TypeEntry *__restrict__ table, float4 a, int t) {
     AtomRec r;
     r.x = a.x; r.y = a.y; r.z = a.z;
     r.pad = 0.0f;
@@ -74,8 +79,11 @@ __device__ __forceinline__ void prep_atom(const FFJob &job, const TypeEntry *__r
     } else {   // out-of-range type index: the atom contributes nothing
         r.c12[0] = r.c12[1] = r.nc6[0] = r.nc6[1] = r.c6x6[0] = r.c6x6[1] = r.kq[0] = r.kq[1] = 0.0f;
     }
-    recs[i] = r;
-    // r_min clamp needed?  distance of every image of this atom to the grid's bounding box
+    return r;
+}
+
+// r_min clamp needed?  distance of every image of this atom to the grid's bounding box
+__device__ __forceinline__ bool atom_near_grid(const FFJob &job, float4 a) {
     const double rmin = sqrt((double)job.rmin2) * 1.0001 + 1e-6;
     bool near = false;
     for (int ia = -job.nimg[0]; ia <= job.nimg[0]; ia++)
@@ -90,28 +98,80 @@ __device__ __forceinline__ void prep_atom(const FFJob &job, const TypeEntry *__r
                 }
                 near |= (d2 < rmin * rmin);
             }
-    if (near) atomicOr(&clamp_flags[job_index], 1);
+    return near;
 }
 
-__global__ void ff_prep_kernel(const __grid_constant__ FFSingle one, const float4 *__restrict__ xyzq,
-                               const int *__restrict__ type, AtomRec *__restrict__ recs,
-                               int *__restrict__ clamp_flags, int natoms_total) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= natoms_total) return;
-    prep_atom(one.job, one.table, 0, xyzq, type, recs, clamp_flags, i);
-}
-
-__global__ void ff_prep_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const TypeEntry *__restrict__ table,
-                                     const float4 *__restrict__ xyzq, const int *__restrict__ type,
-                                     AtomRec *__restrict__ recs, int *__restrict__ clamp_flags, int natoms_total) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= natoms_total) return;
-    int lo = 0, hi = njobs - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (jobs[mid].atom_begin <= i) lo = mid; else hi = mid - 1;
+// One CTA per system.  Packs the records and stable-partitions them (block scan, so the order and therefore the
+// summation order is fixed): atoms with a Coulomb factor first, LJ-only atoms after them.
+__device__ __forceinline__ void prep_system(const FFJob &job, const TypeEntry *__restrict__ table, int job_index,
+                                            const float4 *__restrict__ xyzq, const int *__restrict__ type,
+                                            AtomRec *__restrict__ recs, FFFlags *__restrict__ flags) {
+    __shared__ int s_warp[PREP_THREADS / 32];
+    __shared__ int s_total, s_near;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int n = job.natoms;
+    // pass 1: number of charged atoms
+    int cnt = 0;
+    for (int i = tid; i < n; i += PREP_THREADS) {
+        const AtomRec r = make_record(job, table, xyzq[job.atom_begin + i], type[job.atom_begin + i]);
+        cnt += (r.kq[0] != 0.0f) ? 1 : 0;
     }
-    prep_atom(jobs[lo], table, lo, xyzq, type, recs, clamp_flags, i);
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, s);
+    if (tid == 0) { s_total = 0; s_near = 0; }
+    __syncthreads();
+    if (lane == 0 && cnt) atomicAdd(&s_total, cnt);      // integer sum: order does not matter
+    __syncthreads();
+    const int nq = s_total;
+    // pass 2: stable partition, PREP_THREADS atoms at a time
+    int run_q = 0;
+    bool near = false;
+    for (int base = 0; base < n; base += PREP_THREADS) {
+        const int i = base + tid;
+        const bool live = i < n;
+        AtomRec r;
+        bool charged = false;
+        if (live) {
+            const float4 a = xyzq[job.atom_begin + i];
+            r = make_record(job, table, a, type[job.atom_begin + i]);
+            charged = r.kq[0] != 0.0f;
+            near |= atom_near_grid(job, a);
+        }
+        const unsigned ballot = __ballot_sync(0xffffffffu, charged);
+        const int in_warp = __popc(ballot & ((1u << lane) - 1u));
+        __syncthreads();                                   // s_warp reuse
+        if (lane == 0) s_warp[wid] = __popc(ballot);
+        __syncthreads();
+        int before = 0, chunk_total = 0;
+#pragma unroll
+        for (int w = 0; w < PREP_THREADS / 32; w++) {
+            const int c = s_warp[w];
+            before += (w < wid) ? c : 0;
+            chunk_total += c;
+        }
+        if (live) {
+            const int q_before = run_q + before + in_warp;             // charged atoms ahead of atom i
+            const int pos = charged ? q_before : nq + (i - q_before);
+            recs[job.atom_begin + pos] = r;
+        }
+        run_q += chunk_total;
+    }
+    if (near) atomicOr(&s_near, 1);
+    __syncthreads();
+    if (tid == 0) { flags[job_index].clamp = s_near; flags[job_index].ncharged = nq; }
+}
+
+__global__ void __launch_bounds__(PREP_THREADS)
+ff_prep_kernel(const __grid_constant__ FFSingle one, const float4 *__restrict__ xyzq, const int *__restrict__ type,
+               AtomRec *__restrict__ recs, FFFlags *__restrict__ flags) {
+    prep_system(one.job, one.table, 0, xyzq, type, recs, flags);
+}
+
+__global__ void __launch_bounds__(PREP_THREADS)
+ff_prep_batch_kernel(const FFJob *__restrict__ jobs, const TypeEntry *__restrict__ table,
+                     const float4 *__restrict__ xyzq, const int *__restrict__ type, AtomRec *__restrict__ recs,
+                     FFFlags *__restrict__ flags) {
+    prep_system(jobs[blockIdx.x], table, blockIdx.x, xyzq, type, recs, flags);
 }
 
 // ---------------------------------------------------------------------------------------------------- PTX helpers
@@ -153,7 +213,8 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
 // CLAMP  apply s = max(r^2, r_min^2)
 // ZCOL   step[2] is parallel to z (dx, dy shared by the P points of a column)
 template <int P, bool SPLIT, bool CLAMP, bool ZCOL>
-__device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restrict__ recs, float4 *__restrict__ out_a,
+__device__ __forceinline__ void ff_tile(const FFJob &job, int ncharged, const AtomRec *__restrict__ recs,
+                                        float4 *__restrict__ out_a,
                                         float4 *__restrict__ out_b, AtomRec *s_rec, uint64_t *full_bar,
                                         uint64_t *empty_bar, long long local_tile) {
     const int tid = threadIdx.x;
@@ -195,8 +256,15 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restr
         if (SPLIT) Gx[h] = Gy[h] = Gz[h] = Ge[h] = Getot[h] = zero2;
     }
 
+    // chunks [0, nch_q) hold atoms with a Coulomb factor, chunks [nch_q, nchunks) the LJ-only atoms behind them
     const int natoms = job.natoms;
-    const int nchunks = (natoms + FF_CHUNK - 1) / FF_CHUNK;
+    const int nq = min(max(ncharged, 0), natoms);
+    const int nch_q = (nq + FF_CHUNK - 1) / FF_CHUNK;
+    const int nchunks = nch_q + (natoms - nq + FF_CHUNK - 1) / FF_CHUNK;
+    auto chunk_begin = [&](int c) { return c < nch_q ? c * FF_CHUNK : nq + (c - nch_q) * FF_CHUNK; };
+    auto chunk_count = [&](int c) {
+        return c < nch_q ? min(FF_CHUNK, nq - c * FF_CHUNK) : min(FF_CHUNK, natoms - nq - (c - nch_q) * FF_CHUNK);
+    };
     const int nimages = (2 * job.nimg[0] + 1) * (2 * job.nimg[1] + 1) * (2 * job.nimg[2] + 1);
     const int nsteps = nimages * nchunks;
     const AtomRec *src = recs + job.atom_begin;
@@ -207,21 +275,88 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restr
         const int use = t / FF_STAGES;
         if (use > 0) mbar_wait(&empty_bar[st], (use - 1) & 1);
         const int c = t % nchunks;
-        const int n = min(FF_CHUNK, natoms - c * FF_CHUNK);
-        const uint32_t bytes = (uint32_t)n * (uint32_t)sizeof(AtomRec);
+        const uint32_t bytes = (uint32_t)chunk_count(c) * (uint32_t)sizeof(AtomRec);
         mbar_expect_tx(&full_bar[st], bytes);
-        tma_load_1d(s_rec + st * FF_CHUNK, src + (size_t)c * FF_CHUNK, bytes, &full_bar[st]);
+        tma_load_1d(s_rec + st * FF_CHUNK, src + chunk_begin(c), bytes, &full_bar[st]);
     };
     if (tid == 0) {
         for (int t = 0; t < FF_AHEAD && t < nsteps; t++) issue(t);
     }
+
+    // shifted point p' = p - image shift, split hi + lo; set once per image
+    float ph[3], pl[3];
+    // one chunk of atom records against the thread's P points; NEUTRAL: the records carry no Coulomb factor
+    auto run_chunk = [&](const float4 *s4, int n, auto neutral_tag) {
+        constexpr bool NEUTRAL = decltype(neutral_tag)::value;
+        const float2 twelve = make_float2(12.0f, 12.0f);
+#pragma unroll 2
+        for (int a = 0; a < n; a++) {
+            const float4 r0 = s4[3 * a];          // x, y, z, -
+            const float4 r1 = s4[3 * a + 1];      // c12, c12, -c6, -c6
+            const float4 r2_ = s4[3 * a + 2];     // 6 c6, 6 c6, kq, kq
+            const float2 c12 = make_float2(r1.x, r1.y), nc6 = make_float2(r1.z, r1.w);
+            const float2 c6x6 = make_float2(r2_.x, r2_.y), kq = make_float2(r2_.z, r2_.w);
+            const float dx0 = (ph[0] - r0.x) + pl[0];
+            const float dy0 = (ph[1] - r0.y) + pl[1];
+            const float dz0 = (ph[2] - r0.z) + pl[2];
+            const float rxy2s = fmaf(dy0, dy0, dx0 * dx0);
+            const float2 dxx = make_float2(dx0, dx0), dyy = make_float2(dy0, dy0);
+            const float2 dzz = make_float2(dz0, dz0), rxy2 = make_float2(rxy2s, rxy2s);
+#pragma unroll
+            for (int h = 0; h < H; h++) {
+                float2 dx, dy, dz, r2;
+                if (ZCOL) {
+                    dx = dxx; dy = dyy;
+                    dz = __fadd2_rn(dzz, off[0][h]);
+                    r2 = __ffma2_rn(dz, dz, rxy2);
+                } else {
+                    dx = __fadd2_rn(dxx, off[0][h]);
+                    dy = __fadd2_rn(dyy, off[1 % (ZCOL ? 1 : 3)][h]);
+                    dz = __fadd2_rn(dzz, off[2 % (ZCOL ? 1 : 3)][h]);
+                    r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                }
+                if (CLAMP) { r2.x = fmaxf(r2.x, rmin2); r2.y = fmaxf(r2.y, rmin2); }
+                float2 ir;
+                ir.x = rsqrt_approx(r2.x);
+                ir.y = rsqrt_approx(r2.y);
+                const float2 ir2 = __fmul2_rn(ir, ir);
+                const float2 ir6 = __fmul2_rn(__fmul2_rn(ir2, ir2), ir2);
+                const float2 t = __ffma2_rn(c12, ir6, nc6);        // c12/r^6 - c6
+                const float2 t2 = __ffma2_rn(t, twelve, c6x6);    // 12 c12/r^6 - 6 c6
+                E[h] = __ffma2_rn(t, ir6, E[h]);                   // E_LJ = c12/r^12 - c6/r^6
+                if (!SPLIT) {
+                    float2 g = __fmul2_rn(t2, ir6);
+                    if (!NEUTRAL) {
+                        E[h] = __ffma2_rn(kq, ir, E[h]);           // E_C = kq / r
+                        g = __ffma2_rn(kq, ir, g);
+                    }
+                    const float2 f = __fmul2_rn(g, ir2);           // (12c12/r^12 - 6c6/r^6 + kq/r) / r^2
+                    Fx[h] = __ffma2_rn(f, dx, Fx[h]);
+                    Fy[h] = __ffma2_rn(f, dy, Fy[h]);
+                    Fz[h] = __ffma2_rn(f, dz, Fz[h]);
+                } else {
+                    const float2 f = __fmul2_rn(__fmul2_rn(t2, ir6), ir2);
+                    Fx[h] = __ffma2_rn(f, dx, Fx[h]);
+                    Fy[h] = __ffma2_rn(f, dy, Fy[h]);
+                    Fz[h] = __ffma2_rn(f, dz, Fz[h]);
+                    if (!NEUTRAL) {
+                        const float2 ec = __fmul2_rn(kq, ir);
+                        Ge[h] = __fadd2_rn(Ge[h], ec);
+                        const float2 fe = __fmul2_rn(ec, ir2);
+                        Gx[h] = __ffma2_rn(fe, dx, Gx[h]);
+                        Gy[h] = __ffma2_rn(fe, dy, Gy[h]);
+                        Gz[h] = __ffma2_rn(fe, dz, Gz[h]);
+                    }
+                }
+            }
+        }
+    };
 
     int step = 0;
     for (int ia = -job.nimg[0]; ia <= job.nimg[0]; ia++)
         for (int ib = -job.nimg[1]; ib <= job.nimg[1]; ib++)
             for (int ic = -job.nimg[2]; ic <= job.nimg[2]; ic++) {
                 // shifted point p' = p - shift, split hi + lo (FP64 once per image)
-                float ph[3], pl[3];
 #pragma unroll
                 for (int c = 0; c < 3; c++) {
                     const double s = pb[c] - (ia * job.cell[0][c] + ib * job.cell[1][c] + ic * job.cell[2][c]);
@@ -233,64 +368,9 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, const AtomRec *__restr
                     const int st = step % FF_STAGES;
                     mbar_wait(&full_bar[st], (step / FF_STAGES) & 1);
                     const float4 *s4 = reinterpret_cast<const float4 *>(s_rec + st * FF_CHUNK);
-                    const int n = min(FF_CHUNK, natoms - ch * FF_CHUNK);
-                    const float2 twelve = make_float2(12.0f, 12.0f);
-#pragma unroll 2
-                    for (int a = 0; a < n; a++) {
-                        const float4 r0 = s4[3 * a];          // x, y, z, -
-                        const float4 r1 = s4[3 * a + 1];      // c12, c12, -c6, -c6
-                        const float4 r2_ = s4[3 * a + 2];     // 6 c6, 6 c6, kq, kq
-                        const float2 c12 = make_float2(r1.x, r1.y), nc6 = make_float2(r1.z, r1.w);
-                        const float2 c6x6 = make_float2(r2_.x, r2_.y), kq = make_float2(r2_.z, r2_.w);
-                        const float dx0 = (ph[0] - r0.x) + pl[0];
-                        const float dy0 = (ph[1] - r0.y) + pl[1];
-                        const float dz0 = (ph[2] - r0.z) + pl[2];
-                        const float rxy2s = fmaf(dy0, dy0, dx0 * dx0);
-                        const float2 dxx = make_float2(dx0, dx0), dyy = make_float2(dy0, dy0);
-                        const float2 dzz = make_float2(dz0, dz0), rxy2 = make_float2(rxy2s, rxy2s);
-#pragma unroll
-                        for (int h = 0; h < H; h++) {
-                            float2 dx, dy, dz, r2;
-                            if (ZCOL) {
-                                dx = dxx; dy = dyy;
-                                dz = __fadd2_rn(dzz, off[0][h]);
-                                r2 = __ffma2_rn(dz, dz, rxy2);
-                            } else {
-                                dx = __fadd2_rn(dxx, off[0][h]);
-                                dy = __fadd2_rn(dyy, off[1 % (ZCOL ? 1 : 3)][h]);
-                                dz = __fadd2_rn(dzz, off[2 % (ZCOL ? 1 : 3)][h]);
-                                r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-                            }
-                            if (CLAMP) { r2.x = fmaxf(r2.x, rmin2); r2.y = fmaxf(r2.y, rmin2); }
-                            float2 ir;
-                            ir.x = rsqrt_approx(r2.x);
-                            ir.y = rsqrt_approx(r2.y);
-                            const float2 ir2 = __fmul2_rn(ir, ir);
-                            const float2 ir6 = __fmul2_rn(__fmul2_rn(ir2, ir2), ir2);
-                            const float2 t = __ffma2_rn(c12, ir6, nc6);        // c12/r^6 - c6
-                            const float2 t2 = __ffma2_rn(t, twelve, c6x6);    // 12 c12/r^6 - 6 c6
-                            E[h] = __ffma2_rn(t, ir6, E[h]);                   // E_LJ = c12/r^12 - c6/r^6
-                            if (!SPLIT) {
-                                E[h] = __ffma2_rn(kq, ir, E[h]);               // E_C = kq / r
-                                const float2 g = __ffma2_rn(kq, ir, __fmul2_rn(t2, ir6));
-                                const float2 f = __fmul2_rn(g, ir2);           // (12c12/r^12 - 6c6/r^6 + kq/r) / r^2
-                                Fx[h] = __ffma2_rn(f, dx, Fx[h]);
-                                Fy[h] = __ffma2_rn(f, dy, Fy[h]);
-                                Fz[h] = __ffma2_rn(f, dz, Fz[h]);
-                            } else {
-                                const float2 f = __fmul2_rn(__fmul2_rn(t2, ir6), ir2);
-                                Fx[h] = __ffma2_rn(f, dx, Fx[h]);
-                                Fy[h] = __ffma2_rn(f, dy, Fy[h]);
-                                Fz[h] = __ffma2_rn(f, dz, Fz[h]);
-                                const float2 ec = __fmul2_rn(kq, ir);
-                                Ge[h] = __fadd2_rn(Ge[h], ec);
-                                const float2 fe = __fmul2_rn(ec, ir2);
-                                Gx[h] = __ffma2_rn(fe, dx, Gx[h]);
-                                Gy[h] = __ffma2_rn(fe, dy, Gy[h]);
-                                Gz[h] = __ffma2_rn(fe, dz, Gz[h]);
-                            }
-                        }
-                    }
+                    const int n = chunk_count(ch);
+                    if (ch < nch_q) run_chunk(s4, n, std::false_type{});
+                    else run_chunk(s4, n, std::true_type{});
                     __syncwarp();
                     if ((tid & 31) == 0) mbar_arrive(&empty_bar[st]);
 #pragma unroll
@@ -331,31 +411,33 @@ __device__ __forceinline__ void ff_init_barriers(uint64_t *full_bar, uint64_t *e
 // One system: job in the constant bank (kernel parameter).
 template <int P, bool SPLIT, bool ZCOL>
 __global__ void __launch_bounds__(FF_THREADS, 2)
-ff_kernel(const __grid_constant__ FFJob job, const int *__restrict__ clamp_flags, const AtomRec *__restrict__ recs,
+ff_kernel(const __grid_constant__ FFJob job, const FFFlags *__restrict__ flags, const AtomRec *__restrict__ recs,
           float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
     __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
     __shared__ __align__(8) uint64_t full_bar[FF_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[FF_STAGES];
-    __shared__ int s_clamp;
-    if (threadIdx.x == 0) s_clamp = clamp_flags[0];
+    __shared__ FFFlags s_flags;
+    if (threadIdx.x == 0) s_flags = flags[0];
     ff_init_barriers(full_bar, empty_bar);
     __syncthreads();
-    if (s_clamp)
-        ff_tile<P, SPLIT, true, ZCOL>(job, recs, out_a, out_b, s_rec, full_bar, empty_bar, (long long)blockIdx.x);
+    if (s_flags.clamp)
+        ff_tile<P, SPLIT, true, ZCOL>(job, s_flags.ncharged, recs, out_a, out_b, s_rec, full_bar, empty_bar,
+                                      (long long)blockIdx.x);
     else
-        ff_tile<P, SPLIT, false, ZCOL>(job, recs, out_a, out_b, s_rec, full_bar, empty_bar, (long long)blockIdx.x);
+        ff_tile<P, SPLIT, false, ZCOL>(job, s_flags.ncharged, recs, out_a, out_b, s_rec, full_bar, empty_bar,
+                                       (long long)blockIdx.x);
 }
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
 template <int P, bool SPLIT, bool ZCOL>
 __global__ void __launch_bounds__(FF_THREADS, 2)
-ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const int *__restrict__ clamp_flags,
+ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const FFFlags *__restrict__ flags,
                 const AtomRec *__restrict__ recs, float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
     __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
     __shared__ __align__(8) uint64_t full_bar[FF_STAGES];
     __shared__ __align__(8) uint64_t empty_bar[FF_STAGES];
     __shared__ FFJob s_job;
-    __shared__ int s_clamp;
+    __shared__ FFFlags s_flags;
 
     const long long tile = blockIdx.x;
     int lo = 0, hi = njobs - 1;
@@ -368,14 +450,14 @@ ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const int *__restrict
         int *dstw = reinterpret_cast<int *>(&s_job);
         for (int w = threadIdx.x; w < (int)(sizeof(FFJob) / sizeof(int)); w += FF_THREADS) dstw[w] = srcw[w];
     }
-    if (threadIdx.x == 0) s_clamp = clamp_flags[lo];
+    if (threadIdx.x == 0) s_flags = flags[lo];
     ff_init_barriers(full_bar, empty_bar);
     __syncthreads();
     const long long local_tile = tile - s_job.tile_begin;
-    if (s_clamp)
-        ff_tile<P, SPLIT, true, ZCOL>(s_job, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
+    if (s_flags.clamp)
+        ff_tile<P, SPLIT, true, ZCOL>(s_job, s_flags.ncharged, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
     else
-        ff_tile<P, SPLIT, false, ZCOL>(s_job, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
+        ff_tile<P, SPLIT, false, ZCOL>(s_job, s_flags.ncharged, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
 }
 
 // ---------------------------------------------------------------------------------------------------- a3 combine
@@ -406,7 +488,7 @@ static int pick_P(int nz, bool split) {
 
 template <bool SPLIT, int P, bool ZCOL>
 static void launch_ff_one(long long ntiles, cudaStream_t st, const FFJob *hj, const FFJob *dj, int njobs,
-                          const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
+                          const FFFlags *flags, const AtomRec *recs, float4 *a, float4 *b) {
     const dim3 grid((unsigned)ntiles), block(FF_THREADS);
     if (njobs == 1) ff_kernel<P, SPLIT, ZCOL><<<grid, block, 0, st>>>(hj[0], flags, recs, a, b);
     else ff_batch_kernel<P, SPLIT, ZCOL><<<grid, block, 0, st>>>(dj, njobs, flags, recs, a, b);
@@ -414,7 +496,7 @@ static void launch_ff_one(long long ntiles, cudaStream_t st, const FFJob *hj, co
 
 template <bool SPLIT>
 static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st, const FFJob *hj, const FFJob *dj,
-                             int njobs, const int *flags, const AtomRec *recs, float4 *a, float4 *b) {
+                             int njobs, const FFFlags *flags, const AtomRec *recs, float4 *a, float4 *b) {
     KernelTimer kt(PPFM_K_FF, st);
     if (!zcol) launch_ff_one<SPLIT, 4, false>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else if (P == 6) launch_ff_one<SPLIT, 6, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
@@ -462,7 +544,7 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
     const size_t host_bytes = (jobs_bytes + table_bytes + 15) & ~(size_t)15;
     // device scratch: [jobs | tables] (batch only) [clamp flags] [atom records]
     const size_t flags_off = single ? 0 : host_bytes;
-    const size_t flags_bytes = ((size_t)nsys * sizeof(int) + 15) & ~(size_t)15;
+    const size_t flags_bytes = ((size_t)nsys * sizeof(FFFlags) + 15) & ~(size_t)15;
     const size_t recs_off = flags_off + flags_bytes;
     const int natoms_total = h_atom_offset[nsys];
     const size_t recs_bytes = (size_t)(natoms_total > 0 ? natoms_total : 1) * sizeof(AtomRec);
@@ -528,7 +610,7 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
     if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "scratch upload"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
     const FFJob *dj = reinterpret_cast<const FFJob *>(d_buf);
     const TypeEntry *dt = reinterpret_cast<const TypeEntry *>(d_buf + jobs_bytes);
-    int *dflags = reinterpret_cast<int *>(d_buf + flags_off);
+    FFFlags *dflags = reinterpret_cast<FFFlags *>(d_buf + flags_off);
     AtomRec *drecs = reinterpret_cast<AtomRec *>(d_buf + recs_off);
     if (natoms_total > 0) {
         {
@@ -538,11 +620,11 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
                 memset(&one, 0, sizeof(one));
                 one.job = hj[0];
                 memcpy(one.table, ht, (size_t)ntypes * sizeof(TypeEntry));
-                ff_prep_kernel<<<(natoms_total + 127) / 128, 128, 0, st>>>(one, reinterpret_cast<const float4 *>(d_xyzq),
-                                                                           d_type, drecs, dflags, natoms_total);
+                ff_prep_kernel<<<1, PREP_THREADS, 0, st>>>(one, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs,
+                                                           dflags);
             } else {
-                ff_prep_batch_kernel<<<(natoms_total + 127) / 128, 128, 0, st>>>(
-                    dj, nsys, dt, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs, dflags, natoms_total);
+                ff_prep_batch_kernel<<<nsys, PREP_THREADS, 0, st>>>(
+                    dj, dt, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs, dflags);
             }
         }
         e = cudaGetLastError();
