@@ -158,6 +158,24 @@ int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grid
                           const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
                           ppfm_stats *d_stats, void *cuda_stream);
 
+/* ---- (2b) stiffness map of the relaxed probe particle (IETS module) ------
+ * "This module calculates the change of the stiffness (resp. vibration frequency) of lateral vibration modes of the
+ * CO molecule attached to the AFM tip due to its interaction with the sample."  For every (pixel, z-step) sample the
+ * Hessian of the PP's total potential at the given position,
+ *     H = H_spring - (J + J^T)/2,   J = dF_S/dr  (analytic Jacobian of the tri-linear interpolant in the cell),
+ *     H_spring = k_R dd^T/|d|^2 + k_R (|d| - R0)/|d| (I - dd^T/|d|^2) + diag(k_x, k_y, 0),   d = r_PP - r_TIP,
+ * and its three eigenvalues.
+ * d_ff      DEVICE grid as written by ppfm_forcefield (read-only)
+ * d_pos_fz  DEVICE float[nz][npy][npx][4] as written by ppfm_relax_scan (x, y, z read; .w ignored)
+ * d_eig     DEVICE float[nz][npy][npx][4] = (lambda_1 <= lambda_2 <= lambda_3, 0) in eV/Å^2.  Without sample
+ *           interaction the two small ones are k_x, k_y (the lateral CO modes) and the large one is k_R.
+ * Outside a non-periodic grid the position is clamped (as in the relaxation) before the cell is taken.
+ */
+int ppfm_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_scan *scan,
+                   const float *d_pos_fz, float *d_eig, void *cuda_stream);
+int ppfm_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                         const ppfm_scan *scans, const float *d_pos_fz, float *d_eig, void *cuda_stream);
+
 /* ---- (3) frequency shift, Giessibl's formula Eq.3 -------------------------------------------
  * Fz is read from the .w lane of d_pos_fz [nz][npy][npx][4].  A = peak-to-peak amplitude (Å); n = A/dz must be an
  * integer >= 1 (within 1e-6) and nz > n.  Eq.3 is integrated exactly for the piecewise-linear interpolant of the
@@ -205,7 +223,8 @@ typedef enum {
     PPFM_K_COMBINE = 2, /* a3 F_LJ + Q F_el                  */
     PPFM_K_RELAX = 3,   /* a4+a5 relaxation scan             */
     PPFM_K_DF = 4,      /* a6 frequency shift                */
-    PPFM_K_COUNT = 5
+    PPFM_K_STIFFNESS = 5, /* N2 stiffness map               */
+    PPFM_K_COUNT = 6
 } ppfm_kernel_id;
 int ppfm_timing_enable(int on);
 int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);

@@ -142,6 +142,30 @@ def hessian(ff, grid, tip, rtip, rpp):
     return H, w
 
 
+def stiffness(ff, grid, tip, rtips, rpps) -> np.ndarray:
+    """IETS stiffness map: eigenvalues (ascending, eV/Å^2) of O10's Hessian at each of the
+    (r_TIP, r_PP) pairs; rtips, rpps (..., 3) -> (..., 3)."""
+    ff, is32, origin, step, n, per = _ff_args(ff, grid)
+    rt = np.ascontiguousarray(np.asarray(rtips, dtype=np.float64).reshape(-1, 3))
+    rp = np.ascontiguousarray(np.asarray(rpps, dtype=np.float64).reshape(-1, 3))
+    assert rt.shape == rp.shape
+    out = np.empty_like(rp)
+    rc = lib().oracle_stiffness(_p(ff), C.c_int(is32), _p(origin), _p(step), _p(n), _p(per), _p(_d(tip.k_lat)),
+                                C.c_double(tip.k_rad), _p(_d(tip.d0)), C.c_int64(rt.shape[0]), _p(rt), _p(rp), _p(out))
+    if rc:
+        raise ValueError(f"oracle_stiffness rc={rc}")
+    return out.reshape(np.asarray(rpps).shape)
+
+
+def tip_positions(scan) -> np.ndarray:
+    """Tip anchors of a scan, (nz, npy*npx, 3): p0 + ix dx + iy dy - (0, 0, iz dz)."""
+    iz, iy, ix = np.meshgrid(np.arange(scan.nz), np.arange(scan.npy), np.arange(scan.npx), indexing="ij")
+    r = (np.asarray(scan.p0, float)[None, None, None, :] + ix[..., None] * np.asarray(scan.dx, float) +
+         iy[..., None] * np.asarray(scan.dy, float))
+    r[..., 2] -= iz * scan.dz
+    return r.reshape(scan.nz, scan.npy * scan.npx, 3)
+
+
 def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None, traj: bool = True):
     """O4-O8 (+O10).  Returns dict: pos_fz (nz, npix, 4), iters (nz, npix) [-1 = not converged],
     lam_min (nz, npix), clamped (nz, npix), lam_traj (nz, npix; smallest Hessian eigenvalue along the step's FIRE

@@ -347,6 +347,28 @@ int oracle_hessian(const void *ff, int is_f32, const double *origin, const doubl
 }
 
 /* ------------------------------------------------------------------------------------------------------------
+ * Stiffness map (IETS module: "calculates the change of the stiffness (resp. vibration
+ * frequency) of lateral vibration modes of the CO molecule attached to the AFM tip due to its interaction with the
+ * sample"): O10's Hessian and its three eigenvalues (ascending) at npts given (r_TIP, r_PP) pairs.
+ * ---------------------------------------------------------------------------------------------------------- */
+int oracle_stiffness(const void *ff, int is_f32, const double *origin, const double *step, const int *n,
+                     const int *periodic, const double *k_lat, double k_rad, const double *d0, int64_t npts,
+                     const double *rtip /* [npts][3] */, const double *rpp /* [npts][3] */,
+                     double *eig /* [npts][3] */) {
+    grid_view g;
+    if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
+    tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
+                sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2])};
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < npts; m++) {
+        double H[9];
+        hessian(&g, &tp, rtip + 3 * m, rpp + 3 * m, H);
+        sym3_eig(H, eig + 3 * m);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
  * O6 FIRE + O7 scan + O8 read-out + O10 flag.
  *
  * fire[7] = {dt0, dt_max, finc, fdec, alpha0, falpha, f_conv}.

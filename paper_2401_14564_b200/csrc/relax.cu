@@ -413,16 +413,10 @@ static void launch_relax(int nsys, long long blocks, cudaStream_t st, const Rela
         relax_batch_kernel<ORTHO, ANYPER, SYMTIP><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
 }
 
-static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
-                      const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
-                      ppfm_stats *d_stats, void *cuda_stream) {
-    if (nsys < 1 || !d_ff || !grids || !tips || !fire || !scans || !d_pos_fz) return PPFM_EINVAL;
-    if (((uintptr_t)d_ff & 15) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
-        return PPFM_EINVAL;
-    if (!(fire->dt > 0) || !(fire->dt_max > 0) || !(fire->finc >= 1.0) || !(fire->fdec > 0 && fire->fdec < 1.0) ||
-        !(fire->alpha0 >= 0 && fire->alpha0 <= 1.0) || !(fire->falpha > 0 && fire->falpha <= 1.0) ||
-        fire->n_min < 0 || fire->max_iter < 0 || fire->max_iter > 0xFFFE || !(fire->f_conv > 0))
-        return PPFM_EINVAL;
+// Host side shared by the relaxation and the stiffness map: validate and pack one RelaxJob per system.
+static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *tips, const ppfm_scan *scans,
+                            RelaxJob **hj_out, long long *blocks_out, long long *samples_out, bool *ortho_out,
+                            bool *anyper_out, bool *symtip_out) {
     RelaxJob *hj = (RelaxJob *)calloc((size_t)nsys, sizeof(RelaxJob));
     if (!hj) return PPFM_ENOMEM;
     long long blocks = 0, ff_off = 0, out_off = 0;
@@ -466,6 +460,30 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
         out_off += (long long)s.npx * s.npy * s.nz;
         if (blocks > 0x7fffffffLL) { free(hj); return PPFM_EINVAL; }
     }
+    *hj_out = hj;
+    *blocks_out = blocks;
+    *samples_out = out_off;
+    *ortho_out = ortho; *anyper_out = anyper; *symtip_out = symtip;
+    return PPFM_OK;
+}
+
+static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                      const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
+                      ppfm_stats *d_stats, void *cuda_stream) {
+    if (nsys < 1 || !d_ff || !grids || !tips || !fire || !scans || !d_pos_fz) return PPFM_EINVAL;
+    if (((uintptr_t)d_ff & 15) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
+        return PPFM_EINVAL;
+    if (!(fire->dt > 0) || !(fire->dt_max > 0) || !(fire->finc >= 1.0) || !(fire->fdec > 0 && fire->fdec < 1.0) ||
+        !(fire->alpha0 >= 0 && fire->alpha0 <= 1.0) || !(fire->falpha > 0 && fire->falpha <= 1.0) ||
+        fire->n_min < 0 || fire->max_iter < 0 || fire->max_iter > 0xFFFE || !(fire->f_conv > 0))
+        return PPFM_EINVAL;
+    RelaxJob *hj = nullptr;
+    long long blocks = 0, samples = 0;
+    bool ortho = true, anyper = false, symtip = true;
+    {
+        const int rc = build_relax_jobs(nsys, grids, tips, scans, &hj, &blocks, &samples, &ortho, &anyper, &symtip);
+        if (rc != PPFM_OK) return rc;
+    }
     FireParams fp;
     fp.dt0 = (float)fire->dt; fp.dt_max = (float)fire->dt_max; fp.finc = (float)fire->finc;
     fp.fdec = (float)fire->fdec; fp.alpha0 = (float)fire->alpha0; fp.falpha = (float)fire->falpha;
@@ -507,6 +525,173 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
     return PPFM_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------- stiffness map
+// SURVEY.md 8(f) N2, PAPER.md:202-216 (IETS module): "the change of the stiffness of lateral vibration modes" of the
+// probe particle caused by the curvature of the tip-sample potential.  At every relaxed point the total Hessian of
+// the PP's potential is H = H_spring - (J + J^T)/2, with J = dF_S/dr the analytic Jacobian of the tri-linear
+// interpolant inside the current cell (reading S14: the interpolant is not a gradient field, so J is symmetrised)
+// and H_spring the second derivative of the tip springs of Eq.2.  Output: the three eigenvalues, ascending.
+//
+// One thread per (pixel, z-step) sample, x fastest so that reads, gathers and the float4 store are coalesced.  Cell
+// lookup and the eigenvalues are FP64 (once per sample; the eigenvalues of interest, ~k_xy = 0.016 eV/A^2, sit next
+// to one of ~k_R = 1.9); the Jacobian is formed in FP32 from the FP32 grid.  Eigenvalues by the closed-form
+// trigonometric solution of the characteristic cubic.
+struct StiffCell {
+    int i0, i1;
+    float f;
+};
+
+__device__ __forceinline__ StiffCell stiff_axis(double t, int n, int periodic) {
+    StiffCell c;
+    if (periodic) {
+        const double fl = floor(t);
+        long long m = (long long)fl % n;
+        if (m < 0) m += n;
+        c.i0 = (int)m;
+        c.i1 = (c.i0 + 1 == n) ? 0 : c.i0 + 1;
+        c.f = (float)(t - fl);
+    } else {
+        const double tc = fmin(fmax(t, 0.0), (double)(n - 1));          // S12: clamp the coordinate
+        int i = (int)floor(tc);
+        if (i > n - 2) i = n - 2;
+        c.i0 = i;
+        c.i1 = i + 1;
+        c.f = (float)(tc - (double)i);
+    }
+    return c;
+}
+
+__device__ __forceinline__ void sym3_eigenvalues(double a00, double a11, double a22, double a01, double a02,
+                                                 double a12, double &e0, double &e1, double &e2) {
+    const double p1 = a01 * a01 + a02 * a02 + a12 * a12;
+    const double q = (a00 + a11 + a22) * (1.0 / 3.0);
+    const double b00 = a00 - q, b11 = a11 - q, b22 = a22 - q;
+    const double p2 = b00 * b00 + b11 * b11 + b22 * b22 + 2.0 * p1;
+    if (!(p2 > 0.0)) { e0 = e1 = e2 = q; return; }
+    const double p = sqrt(p2 * (1.0 / 6.0));
+    const double ip = 1.0 / p;
+    const double c00 = b00 * ip, c11 = b11 * ip, c22 = b22 * ip, c01 = a01 * ip, c02 = a02 * ip, c12 = a12 * ip;
+    const double det = c00 * (c11 * c22 - c12 * c12) - c01 * (c01 * c22 - c12 * c02) + c02 * (c01 * c12 - c11 * c02);
+    const double r = fmin(fmax(0.5 * det, -1.0), 1.0);
+    const double phi = acos(r) * (1.0 / 3.0);
+    e2 = q + 2.0 * p * cos(phi);                                          // largest
+    e0 = q + 2.0 * p * cos(phi + 2.0943951023931954923);                 // smallest (phi + 2 pi / 3)
+    e1 = 3.0 * q - e0 - e2;
+}
+
+__global__ void __launch_bounds__(256)
+stiffness_kernel(const RelaxJob *__restrict__ jobs, int njobs, long long nsamples, const float4 *__restrict__ ff,
+                 const float4 *__restrict__ pos_fz, float4 *__restrict__ eig) {
+    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsamples) return;
+    int lo = 0, hi = njobs - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (jobs[mid].out_offset <= s) lo = mid; else hi = mid - 1;
+    }
+    const RelaxJob &job = jobs[lo];
+    const long long ls = s - job.out_offset;
+    const int npix = job.npx * job.npy;
+    const int iz = (int)(ls / npix);
+    const int pix = (int)(ls - (long long)iz * npix);
+    const int iy = pix / job.npx, ix = pix - iy * job.npx;
+
+    const float4 pp = pos_fz[s];
+    const double r[3] = {(double)pp.x, (double)pp.y, (double)pp.z};
+    double d[3], t[3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const double rtip = job.p0[c] + ix * job.dx[c] + iy * job.dy[c] - (c == 2 ? iz * job.dz : 0.0);
+        d[c] = r[c] - rtip;
+    }
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+        t[a] = job.Minv[3 * a] * (r[0] - job.origin[0]) + job.Minv[3 * a + 1] * (r[1] - job.origin[1]) +
+               job.Minv[3 * a + 2] * (r[2] - job.origin[2]);
+    const StiffCell cx = stiff_axis(t[0], job.n[0], job.periodic[0]);
+    const StiffCell cy = stiff_axis(t[1], job.n[1], job.periodic[1]);
+    const StiffCell cz = stiff_axis(t[2], job.n[2], job.periodic[2]);
+    const float4 *g = ff + job.ff_offset;
+    const long long nx = job.n[0], nxy = (long long)job.n[0] * job.n[1];
+    const float4 *r00 = g + cz.i0 * nxy + cy.i0 * nx, *r01 = g + cz.i0 * nxy + cy.i1 * nx;
+    const float4 *r10 = g + cz.i1 * nxy + cy.i0 * nx, *r11 = g + cz.i1 * nxy + cy.i1 * nx;
+    const float4 c000 = __ldg(r00 + cx.i0), c001 = __ldg(r00 + cx.i1), c010 = __ldg(r01 + cx.i0), c011 = __ldg(r01 + cx.i1);
+    const float4 c100 = __ldg(r10 + cx.i0), c101 = __ldg(r10 + cx.i1), c110 = __ldg(r11 + cx.i0), c111 = __ldg(r11 + cx.i1);
+    // G[c][a] = dF_c/dt_a inside the cell (FP32): difference along axis a, tri-linear weights on the other two
+    const float fx = cx.f, fy = cy.f, fz = cz.f, gx = 1.0f - fx, gy = 1.0f - fy, gz = 1.0f - fz;
+    float G[3][3];
+#define PPFM_G(C)                                                                                                  \
+    {                                                                                                              \
+        const float v000 = c000.C, v001 = c001.C, v010 = c010.C, v011 = c011.C;                                    \
+        const float v100 = c100.C, v101 = c101.C, v110 = c110.C, v111 = c111.C;                                    \
+        row[0] = gz * (gy * (v001 - v000) + fy * (v011 - v010)) + fz * (gy * (v101 - v100) + fy * (v111 - v110));   \
+        row[1] = gz * (gx * (v010 - v000) + fx * (v011 - v001)) + fz * (gx * (v110 - v100) + fx * (v111 - v101));   \
+        row[2] = gy * (gx * (v100 - v000) + fx * (v101 - v001)) + fy * (gx * (v110 - v010) + fx * (v111 - v011));   \
+    }
+    { float *row = G[0]; PPFM_G(x) }
+    { float *row = G[1]; PPFM_G(y) }
+    { float *row = G[2]; PPFM_G(z) }
+#undef PPFM_G
+    // J = G Minv (chain rule through t = Minv (r - origin))
+    double J[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; c++)
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+            J[c][a] = (double)(G[c][0] * job.Minvf[a] + G[c][1] * job.Minvf[3 + a] + G[c][2] * job.Minvf[6 + a]);
+    // H_spring = k_R dd^T/|d|^2 + k_R (|d| - R0)/|d| (I - dd^T/|d|^2) + diag(k_x, k_y, 0)
+    const double L2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    const double L = sqrt(L2);
+    const double kR = (double)job.k_rad;
+    const double R0 = sqrt(job.d0[0] * job.d0[0] + job.d0[1] * job.d0[1] + job.d0[2] * job.d0[2]);
+    const double kt = (L > 0.0) ? kR * (L - R0) / L : 0.0;                // transverse stiffness of the radial spring
+    const double iL2 = (L2 > 0.0) ? 1.0 / L2 : 0.0;
+    double H[3][3];
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+#pragma unroll
+        for (int b = 0; b < 3; b++) {
+            const double dd = d[a] * d[b] * iL2;
+            H[a][b] = kR * dd + kt * ((a == b ? 1.0 : 0.0) - dd) - 0.5 * (J[a][b] + J[b][a]);
+        }
+    H[0][0] += (double)job.k_lat[0];
+    H[1][1] += (double)job.k_lat[1];
+    double e0, e1, e2;
+    sym3_eigenvalues(H[0][0], H[1][1], H[2][2], H[0][1], H[0][2], H[1][2], e0, e1, e2);
+    eig[s] = make_float4((float)e0, (float)e1, (float)e2, 0.0f);
+}
+
+static int stiffness_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                          const ppfm_scan *scans, const float *d_pos_fz, float *d_eig, void *cuda_stream) {
+    if (nsys < 1 || !d_ff || !grids || !tips || !scans || !d_pos_fz || !d_eig) return PPFM_EINVAL;
+    if (((uintptr_t)d_ff & 15) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_eig & 15)) return PPFM_EINVAL;
+    RelaxJob *hj = nullptr;
+    long long blocks = 0, samples = 0;
+    bool ortho, anyper, symtip;
+    const int rc = build_relax_jobs(nsys, grids, tips, scans, &hj, &blocks, &samples, &ortho, &anyper, &symtip);
+    if (rc != PPFM_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RelaxJob *dj = nullptr;
+    cudaError_t e = scratch_alloc((void **)&dj, (size_t)nsys * sizeof(RelaxJob), st);
+    if (e != cudaSuccess) { free(hj); set_cuda_error(e, "scratch_alloc"); return PPFM_ENOMEM; }
+    e = cudaMemcpyAsync(dj, hj, (size_t)nsys * sizeof(RelaxJob), cudaMemcpyHostToDevice, st);   // pageable: staged
+    free(hj);
+    if (e != cudaSuccess) { set_cuda_error(e, "job upload"); cudaFreeAsync(dj, st); return PPFM_ECUDA; }
+    const long long nblk = (samples + 255) / 256;
+    if (nblk > 0x7fffffffLL) { cudaFreeAsync(dj, st); return PPFM_EINVAL; }
+    {
+        KernelTimer kt(PPFM_K_STIFFNESS, st);
+        stiffness_kernel<<<(unsigned)nblk, 256, 0, st>>>(dj, nsys, samples, reinterpret_cast<const float4 *>(d_ff),
+                                                         reinterpret_cast<const float4 *>(d_pos_fz),
+                                                         reinterpret_cast<float4 *>(d_eig));
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { set_cuda_error(e, "stiffness_kernel"); cudaFreeAsync(dj, st); return PPFM_ECUDA; }
+    count_launch();
+    PPFM_CUDA(cudaFreeAsync(dj, st));
+    return PPFM_OK;
+}
+
 }  // namespace ppfm
 
 using namespace ppfm;
@@ -521,4 +706,14 @@ extern "C" int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm
                                      const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz,
                                      uint16_t *d_iters, ppfm_stats *d_stats, void *cuda_stream) {
     return relax_impl(nsys, d_ff, grids, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream);
+}
+
+extern "C" int ppfm_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_scan *scan,
+                              const float *d_pos_fz, float *d_eig, void *cuda_stream) {
+    return stiffness_impl(1, d_ff, grid, tip, scan, d_pos_fz, d_eig, cuda_stream);
+}
+
+extern "C" int ppfm_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                                    const ppfm_scan *scans, const float *d_pos_fz, float *d_eig, void *cuda_stream) {
+    return stiffness_impl(nsys, d_ff, grids, tips, scans, d_pos_fz, d_eig, cuda_stream);
 }

@@ -58,10 +58,10 @@ class Stats(C.Structure):
 
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_relax_scan",
-           "ppfm_relax_scan_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
+           "ppfm_relax_scan_batch", "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
            "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
            "ppfm_release_scratch"]
-KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4}
+KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5}
 
 
 def lib():
@@ -314,6 +314,31 @@ def relax_scan_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, stat
                                      _dptr(pos_fz, torch.float32), _dptr(iters), _dptr(stats), _stream())
     _check(rc, "ppfm_relax_scan_batch")
     return pos_fz, iters
+
+
+# ---- (2b) stiffness map (IETS module) -------------------------------------------------------------
+def stiffness(ff, grid, tip, scan, pos_fz, out=None):
+    """ppfm_stiffness -> (nz, npy, npx, 4) float32: Hessian eigenvalues (ascending) of the PP at pos_fz, 4th lane 0."""
+    torch = _torch()
+    if out is None:
+        out = torch.empty((int(scan.nz), int(scan.npy), int(scan.npx), 4), dtype=torch.float32, device=ff.device)
+    rc = lib().ppfm_stiffness(_dptr(ff, torch.float32), C.byref(c_grid(grid)), C.byref(c_tip(tip)),
+                              C.byref(c_scan(scan)), _dptr(pos_fz, torch.float32), _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_stiffness")
+    return out
+
+
+def stiffness_batch(ff, grids, tips, scans, pos_fz, out=None):
+    """ppfm_stiffness_batch over nsys systems laid out as in relax_scan_batch; out is (total pixel-steps, 4)."""
+    torch = _torch()
+    gr, tp, sc = c_array(grids, c_grid), c_array(tips, c_tip), c_array(scans, c_scan)
+    if out is None:
+        nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in sc)
+        out = torch.empty((nps, 4), dtype=torch.float32, device=ff.device)
+    rc = lib().ppfm_stiffness_batch(C.c_int32(len(grids)), _dptr(ff, torch.float32), gr, tp, sc,
+                                    _dptr(pos_fz, torch.float32), _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_stiffness_batch")
+    return out
 
 
 # ---- (3) df ------------------------------------------------------------------------------------------------------

@@ -167,6 +167,38 @@ def test_ff_batch_cfg3_matches_oracle_and_single_calls(P):
         check_ff(got[idx], oracle.forcefield(mols[m], idx=idx), f"cfg3 mol {m}")
 
 
+def test_ff_charged_neutral_partition(P):
+    """The prep kernel moves atoms without a Coulomb factor behind the charged ones (LJ-only inner loop).  Interleave
+    both kinds so that each fills several 256-atom chunks with ragged tails; then all neutral (Q = 0 and q = 0), all
+    charged, and a single charged atom; split grids too."""
+    import torch
+    base = W.get(2)                                          # 60 charged + 500 neutral atoms, 9 images
+    rng = np.random.default_rng(77)
+    n = 700
+    xyzq = np.zeros((n, 4), dtype=np.float32)
+    xyzq[:, 0:2] = rng.uniform(0.0, 25.0, (n, 2))
+    xyzq[:, 2] = rng.uniform(-6.0, -0.5, n)
+    q = rng.normal(0.0, 0.1, n)
+    q[rng.random(n) < 0.55] = 0.0                            # ~385 neutral, ~315 charged, interleaved
+    xyzq[:, 3] = q
+    types = rng.integers(0, len(base.elem_R), n).astype(np.int32)
+    g = replace(base.grid, n=(41, 19, 12), step=np.diag([0.6, 1.3, 0.25]))
+    w = replace(base, xyzq=xyzq, types=types, grid=g)
+    ref = oracle.forcefield(w)
+    check_ff(gpu_ff(P, w).cpu().numpy(), ref, "mixed")
+    xyzq_d, types_d = P.upload(w)
+    lj, el = P.forcefield_split(xyzq_d, types_d, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
+    check_ff(P.combine(lj, el, w.probe.Q).cpu().numpy(), ref, "mixed split+combine")
+    check_ff(gpu_ff(P, w, Q=0.0).cpu().numpy(), oracle.forcefield(w, Q=0.0), "Q = 0: every record LJ-only")
+    x1 = xyzq.copy(); x1[:, 3] = 0.0; x1[n // 2, 3] = 0.3
+    w1 = replace(w, xyzq=x1)
+    check_ff(gpu_ff(P, w1).cpu().numpy(), oracle.forcefield(w1), "one charged atom")
+    x2 = xyzq.copy(); x2[:, 3] = np.where(x2[:, 3] == 0.0, 0.01, x2[:, 3])
+    w2 = replace(w, xyzq=x2)
+    check_ff(gpu_ff(P, w2).cpu().numpy(), oracle.forcefield(w2), "all charged")
+    torch.cuda.synchronize()
+
+
 def test_ff_is_bit_reproducible(P):
     w = W.shrink(W.get(1), grid_n=(200, 40, 20))
     a = gpu_ff(P, w).cpu().numpy()
@@ -367,6 +399,86 @@ def test_relax_max_iter_flag(P):
     st = P.read_stats(stats)
     assert st["n_not_converged"] == 8 * 4 * 4 and st["max_iters"] == 3 and st["total_iters"] == 3 * 128
     assert np.all(iters.cpu().numpy().view(np.uint16) == 0xFFFF)
+
+
+# ------------------------------------------------------------------------------------------------ stiffness map
+def check_stiffness(eig_gpu, ff_h, w, pos_h, what=""):
+    """GPU eigenvalues vs the oracle's at the same positions on the same (FP32, widened) grid.  Tolerance
+    |d lambda| <= 1e-5 eV/Å^2 + 1e-5 |lambda| (the Jacobian is formed in FP32 from corner differences,
+    ~1e-7 eV/Å / h per entry).  Samples within 1e-6 cell of a cell face are skipped: the Jacobian of a tri-linear
+    interpolant jumps there, and which side a point falls on is decided by rounding."""
+    rt = oracle.tip_positions(w.scan)
+    rp = pos_h[..., :3].astype(np.float64)
+    ref = oracle.stiffness(ff_h, w.grid, w.tip, rt, rp)
+    Minv = np.linalg.inv(np.asarray(w.grid.step, float).T)
+    t = (rp - np.asarray(w.grid.origin, float)) @ Minv.T
+    interior = (np.abs(t - np.round(t)) > 1e-6).all(axis=-1)
+    got = np.asarray(eig_gpu, np.float64).reshape(ref.shape[:-1] + (4,))
+    assert np.all(got[..., 3] == 0.0)
+    err = np.abs(got[..., :3] - ref)
+    tol = 1e-5 + 1e-5 * np.abs(ref)
+    assert interior.mean() > 0.99
+    assert (err <= tol)[interior].all(), f"{what}: stiffness error {err[interior].max():.3e} eV/Å^2"
+    assert np.all(np.diff(got[..., :3], axis=-1) >= 0)
+    return err[interior].max()
+
+
+def test_stiffness_map_cfg0_and_cfg1(P):
+    """SURVEY 8(f) N2 (IETS module) on the relaxed scans of configs 0 and 1."""
+    import torch
+    for cfg in (0, 1):
+        w = W.get(cfg)
+        ff, pos, _, _, _ = gpu_scan(P, w)
+        eig = P.stiffness(ff, w.grid, w.tip, w.scan, pos)
+        torch.cuda.synchronize()
+        npix = w.scan.npx * w.scan.npy
+        pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)
+        check_stiffness(eig.cpu().numpy().reshape(w.scan.nz, npix, 4), ff.cpu().numpy(), w, pos_h, f"cfg{cfg}")
+        # the soft (lateral) modes are softened over the molecule in the repulsive regime: the map has contrast
+        lam_min = eig[..., 0].cpu().numpy()
+        assert lam_min.min() < 0.5 * w.tip.k_lat[0] and lam_min.max() > 0.9 * w.tip.k_lat[0]
+
+
+def test_stiffness_zero_field_periodic_nonorthogonal_and_batch(P):
+    import torch
+    # zero field: (k_x, k_y, k_R) exactly, for an anisotropic tip; ragged scan
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(20, 20, 60), periodic=(0, 0, 0))
+    ff = torch.zeros((60, 20, 20, 4), dtype=torch.float32, device="cuda")
+    sc = W.Scan(p0=np.array([1.0, 1.2, 9.0]), dx=np.array([0.1, 0, 0.0]), dy=np.array([0, 0.1, 0.0]), npx=19, npy=11,
+                nz=7, dz=0.1)
+    tip = replace(W._default_tip(), k_lat=np.array([0.011, 0.023]))
+    pos, _ = P.relax_scan(ff, g, tip, W.Fire(), sc)
+    eig = P.stiffness(ff, g, tip, sc, pos).cpu().numpy()
+    assert np.allclose(eig[..., :3], [0.011, 0.023, tip.k_rad], rtol=1e-6, atol=1e-7)
+    # periodic + skewed grid, positions partly outside the cell (wrap) - against the oracle
+    w = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
+    step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
+    w = replace(w, grid=replace(w.grid, step=step), scan=replace(w.scan, p0=np.array([-3.0, 20.0, 9.0])))
+    ffw = gpu_ff(P, w)
+    posw, _ = P.relax_scan(ffw, w.grid, w.tip, w.fire, w.scan)
+    eigw = P.stiffness(ffw, w.grid, w.tip, w.scan, posw)
+    torch.cuda.synchronize()
+    npix = w.scan.npx * w.scan.npy
+    check_stiffness(eigw.cpu().numpy().reshape(w.scan.nz, npix, 4), ffw.cpu().numpy(), w,
+                    posw.cpu().numpy().reshape(w.scan.nz, npix, 4), "periodic skewed")
+    # batch == per-system calls, bit for bit
+    mols = W.get(3)[:3]
+    mols = [W.shrink(m, grid_n=m.grid.n, scan_np=(24, 20), scan_nz=5) for m in mols]
+    off = np.concatenate([[0], np.cumsum([m.natoms for m in mols])])
+    xyzq = torch.from_numpy(np.concatenate([m.xyzq for m in mols])).cuda()
+    types = torch.from_numpy(np.concatenate([m.types for m in mols])).cuda()
+    ffb = P.forcefield_batch(off, xyzq, types, mols[0].elem_R, mols[0].elem_e, [m.lattice for m in mols],
+                             [m.probe for m in mols], [m.grid for m in mols], mols[0].r_min)
+    posb, _ = P.relax_scan_batch(ffb, [m.grid for m in mols], [m.tip for m in mols], mols[0].fire,
+                                 [m.scan for m in mols])
+    eigb = P.stiffness_batch(ffb, [m.grid for m in mols], [m.tip for m in mols], [m.scan for m in mols], posb)
+    torch.cuda.synchronize()
+    nps = mols[0].pixel_steps
+    npts = mols[0].npoints
+    for m in range(3):
+        one = P.stiffness(ffb[m * npts:(m + 1) * npts], mols[m].grid, mols[m].tip, mols[m].scan,
+                          posb[m * nps:(m + 1) * nps])
+        assert torch.equal(one.reshape(-1, 4), eigb[m * nps:(m + 1) * nps])
 
 
 # ------------------------------------------------------------------------------------------------ df, host API

@@ -513,6 +513,55 @@ def test_hessian_matches_finite_difference_of_force():
     assert np.allclose(ev, np.linalg.eigvalsh(H), atol=1e-12)
 
 
+def test_stiffness_map_closed_forms_and_finite_differences():
+    """IETS stiffness map.  (i) No sample interaction: the PP at the spring equilibrium has
+    eigenvalues (k_x, k_y, k_R) exactly - the two lateral CO modes and the radial one.  (ii) A linear field
+    F_S = -K (r - r0) with K symmetric (exactly reproduced by tri-linear interpolation) adds K to the spring Hessian:
+    eigenvalues = eigvalsh(H_spring + K).  (iii) On config 0 the bulk call equals -sym(dF_total/dr) by central
+    differences of the total force at 40 random in-cell points."""
+    g = W.Grid(origin=np.array([0.0, 0.0, 0.0]), step=np.diag([0.2, 0.25, 0.1]), n=(30, 24, 60), periodic=(0, 0, 0))
+    tip = W._default_tip()
+    zero = np.zeros((60, 24, 30, 4))
+    rtip = np.array([[2.9, 3.1, 8.2], [3.3, 2.2, 7.7]])
+    ev = oracle.stiffness(zero, g, tip, rtip, rtip + np.asarray(tip.d0))
+    assert np.allclose(ev, [[tip.k_lat[0], tip.k_lat[1], tip.k_rad]] * 2, rtol=0, atol=1e-12)
+    # (ii) linear restoring field
+    K = np.array([[0.30, 0.05, -0.02], [0.05, -0.11, 0.04], [-0.02, 0.04, 0.21]])
+    r0 = np.array([3.0, 3.0, 4.0])
+    k, j, i = np.meshgrid(np.arange(60), np.arange(24), np.arange(30), indexing="ij")
+    nodes = np.stack([i * 0.2, j * 0.25, k * 0.1], axis=-1)
+    lin = np.zeros((60, 24, 30, 4))
+    lin[..., :3] = -(nodes - r0) @ K.T
+    rpp = rtip + np.array([[0.31, -0.22, -3.9], [-0.4, 0.15, -4.05]])
+    ev = oracle.stiffness(lin, g, tip, rtip, rpp)
+    for m in range(2):
+        d = rpp[m] - rtip[m]
+        L = np.linalg.norm(d)
+        dd = np.outer(d, d) / L**2
+        Hs = tip.k_rad * dd + tip.k_rad * (L - 4.0) / L * (np.eye(3) - dd) + np.diag([tip.k_lat[0], tip.k_lat[1], 0.0])
+        assert np.allclose(ev[m], np.linalg.eigvalsh(Hs + K), rtol=0, atol=1e-10)
+    # (iii) real field, bulk call vs finite differences of the total force
+    w = W.get(0)
+    ff = oracle.forcefield(w)
+    rng = np.random.default_rng(5)
+    rt = np.stack([rng.uniform(4.0, 8.0, 40), rng.uniform(4.0, 8.0, 40), rng.uniform(6.5, 9.5, 40)], axis=1)
+    cell = np.array([0.2, 0.2, 0.2])
+    rp = rt + np.asarray(w.tip.d0) + rng.uniform(-0.3, 0.3, (40, 3))
+    frac = ((rp - np.asarray(w.grid.origin)) / cell) % 1.0
+    rp += (np.clip(frac, 0.05, 0.95) - frac) * cell                      # keep every point inside its cell
+    ev = oracle.stiffness(ff, w.grid, w.tip, rt, rp)
+    h = 1e-6
+    for m in range(40):
+        J = np.zeros((3, 3))
+        for a in range(3):
+            dp = np.zeros(3)
+            dp[a] = h
+            J[:, a] = (oracle.total_force(ff, w.grid, w.tip, rt[m], rp[m] + dp) -
+                       oracle.total_force(ff, w.grid, w.tip, rt[m], rp[m] - dp)) / (2 * h)
+        assert np.allclose(ev[m], np.linalg.eigvalsh(-(J + J.T) / 2), rtol=1e-6, atol=1e-8)
+    assert np.allclose(oracle.tip_positions(_scan())[3, 0], _scan().p0 - np.array([0, 0, 3 * _scan().dz]))
+
+
 def test_golden_constants_are_what_the_generators_use():
     assert W.EVA2_PER_NM == pytest.approx(1.0 / NM, rel=1e-15)
     assert W.ELEM_R[:4].tolist() == [GOLD["R_H"], GOLD["R_C"], GOLD["R_N"], GOLD["R_O"]]
