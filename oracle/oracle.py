@@ -166,6 +166,38 @@ def tip_positions(scan) -> np.ndarray:
     return r.reshape(scan.nz, scan.npy * scan.npx, 3)
 
 
+def tip_density(grid, sigma: float, q_s: float, p_z: float, Q_zz: float) -> np.ndarray:
+    """O12: Gaussian-multipole tip charge density and its analytic gradient at the grid nodes (minimum image by
+    index) -> (4, nz, ny, nx): rho, d rho/dx, d rho/dy, d rho/dz."""
+    step = np.ascontiguousarray(np.asarray(grid.step, dtype=np.float64).reshape(9))
+    n = _i(grid.n)
+    out = np.empty((4, int(grid.n[2]), int(grid.n[1]), int(grid.n[0])))
+    rc = lib().oracle_tip_density(_p(step), _p(n), C.c_double(sigma), C.c_double(q_s), C.c_double(p_z),
+                                  C.c_double(Q_zz), _p(out))
+    if rc:
+        raise ValueError(f"oracle_tip_density rc={rc}")
+    return out
+
+
+def fft_forcefield(V, grid, sigma: float, q_s: float, p_z: float, Q_zz: float) -> np.ndarray:
+    """O12 (Eq.7; reading S21): E_el(R) = sum_r rho(r) V(r + R) dV and F_el = sum_r grad rho(r)
+    V(r + R) dV on the periodic grid, by direct O(N^2) summation.  V (nz, ny, nx) in eV/e -> (nz, ny, nx, 4) =
+    (Fx, Fy, Fz, E).  Small grids only."""
+    V = np.ascontiguousarray(np.asarray(V, dtype=np.float64))
+    rho4 = tip_density(grid, sigma, q_s, p_z, Q_zz)
+    assert V.shape == rho4.shape[1:]
+    dV = abs(float(np.linalg.det(np.asarray(grid.step, dtype=np.float64))))
+    n = _i(grid.n)
+    out = np.empty(V.shape + (4,))
+    tmp = np.empty(V.shape)
+    for c, lane in ((0, 3), (1, 0), (2, 1), (3, 2)):
+        rc = lib().oracle_crosscorr(_p(n), _p(np.ascontiguousarray(rho4[c])), _p(V), C.c_double(dV), _p(tmp))
+        if rc:
+            raise ValueError(f"oracle_crosscorr rc={rc}")
+        out[..., lane] = tmp
+    return out
+
+
 def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None, traj: bool = True):
     """O4-O8 (+O10).  Returns dict: pos_fz (nz, npix, 4), iters (nz, npix) [-1 = not converged],
     lam_min (nz, npix), clamped (nz, npix), lam_traj (nz, npix; smallest Hessian eigenvalue along the step's FIRE

@@ -20,6 +20,8 @@
  *   O8  Fz read-out
  *   O9  Giessibl df                      PAPER.md:64-66 (Eq.3; quadrature = reading S9)
  *   O10 stability flag (Hessian)         north_star exemption; reading S14
+ *   O11 stiffness map (IETS)
+ *   O12 grid electrostatics, Eq.7        PAPER.md:102-111 (cross-correlation), 270 (convolution theorem); reading S21
  *
  * Pins: tests/test_oracle_pins.py (closed forms, invariants, brute force).  "Relaxed positions on the real
  * configs" have no value printed in the paper: PARITY UNPINNED BY THE PAPER for that one item; it is pinned
@@ -365,6 +367,66 @@ int oracle_stiffness(const void *ff, int is_f32, const double *origin, const dou
         hessian(&g, &tp, rtip + 3 * m, rpp + 3 * m, H);
         sym3_eig(H, eig + 3 * m);
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O12: electrostatics of an extended tip charge density on the grid (Eq.7):
+ *     E_el(R) = integral rho_PP(r) V_S(r + R) dr,        F_el(R) = -grad_R E_el = integral grad rho_PP(r) V_S(r + R) dr
+ * (integration by parts on the periodic cell).  Reading S21: the integral is the cyclic sum over the nodes of the
+ * periodic grid times the cell volume element dV = |det(step)|; rho_PP is a Gaussian multipole (PAPER.md:108:
+ * monopole, and "the quadrupolar charge distribution better reproduces contrast observed with a CO-tip")
+ *     g(r) = (2 pi sigma^2)^(-3/2) exp(-r^2 / 2 sigma^2)
+ *     rho  = [ q_s + p_z z / sigma^2 + (Q_zz / 12) (3 z^2 - r^2) / sigma^4 ] g(r)
+ * (total charge q_s, dipole moment p_z, quadrupole moment Q_zz = integral rho (3z^2 - r^2) dr), evaluated with its
+ * analytic gradient at node (i,j,k) -> r = i' s0 + j' s1 + k' s2, i' = i - n0 if i >= n0/2 (minimum image by index).
+ * This function is the definition written out: O(N^2) direct sums, for small grids only.
+ * ---------------------------------------------------------------------------------------------------------- */
+int oracle_tip_density(const double *step /* [3][3] */, const int *n, double sigma, double q_s, double p_z,
+                       double Q_zz, double *rho4 /* [4][nz][ny][nx]: rho, d/dx, d/dy, d/dz */) {
+    if (!(sigma > 0.0) || n[0] < 1 || n[1] < 1 || n[2] < 1) return -1;
+    const int64_t N = (int64_t)n[0] * n[1] * n[2];
+    const double s2 = sigma * sigma, s4 = s2 * s2;
+    const double norm = pow(2.0 * M_PI * s2, -1.5);
+    for (int k = 0; k < n[2]; k++)
+        for (int j = 0; j < n[1]; j++)
+            for (int i = 0; i < n[0]; i++) {
+                const int iw = (2 * i >= n[0]) ? i - n[0] : i;
+                const int jw = (2 * j >= n[1]) ? j - n[1] : j;
+                const int kw = (2 * k >= n[2]) ? k - n[2] : k;
+                double r[3];
+                for (int c = 0; c < 3; c++) r[c] = iw * step[0 + c] + jw * step[3 + c] + kw * step[6 + c];
+                const double rr = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+                const double g = norm * exp(-rr / (2.0 * s2));
+                const double P = q_s + p_z * r[2] / s2 + (Q_zz / 12.0) * (3.0 * r[2] * r[2] - rr) / s4;
+                const double dP[3] = {(Q_zz / 12.0) * (-2.0 * r[0]) / s4, (Q_zz / 12.0) * (-2.0 * r[1]) / s4,
+                                      p_z / s2 + (Q_zz / 12.0) * (4.0 * r[2]) / s4};
+                const int64_t m = ((int64_t)k * n[1] + j) * n[0] + i;
+                rho4[m] = P * g;
+                for (int c = 0; c < 3; c++) rho4[(c + 1) * N + m] = dP[c] * g - P * g * r[c] / s2;
+            }
+    return 0;
+}
+
+/* out[R] = dV * sum_r rho[r] * V[(r + R) mod n]   (cyclic cross-correlation, Eq.7 on the grid) */
+int oracle_crosscorr(const int *n, const double *rho, const double *V, double dV, double *out) {
+    const int nx = n[0], ny = n[1], nz = n[2];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int K = 0; K < nz; K++)
+        for (int J = 0; J < ny; J++)
+            for (int I = 0; I < nx; I++) {
+                double acc = 0.0;
+                for (int k = 0; k < nz; k++) {
+                    const int kk = (k + K) % nz;
+                    for (int j = 0; j < ny; j++) {
+                        const int jj = (j + J) % ny;
+                        const double *pr = rho + ((int64_t)k * ny + j) * nx;
+                        const double *pv = V + ((int64_t)kk * ny + jj) * nx;
+                        for (int i = 0; i < nx; i++) acc += pr[i] * pv[(i + I) % nx];
+                    }
+                }
+                out[((int64_t)K * ny + J) * nx + I] = acc * dV;
+            }
     return 0;
 }
 

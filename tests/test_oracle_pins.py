@@ -562,6 +562,89 @@ def test_stiffness_map_closed_forms_and_finite_differences():
     assert np.allclose(oracle.tip_positions(_scan())[3, 0], _scan().p0 - np.array([0, 0, 3 * _scan().dz]))
 
 
+# ---------------------------------------------------------------------------------------------------- O12 (Eq.7)
+def _fft_grid(n=(24, 20, 16), h=(0.25, 0.3, 0.35)):
+    return W.Grid(origin=np.zeros(3), step=np.diag(h), n=n, periodic=(1, 1, 1))
+
+
+def test_eq7_crosscorrelation_plane_wave_closed_forms():
+    """PAPER.md:102-106, Eq.7.  For V_S = V0 cos(k.r + phi) with k a reciprocal-lattice vector and a Gaussian
+    multipole tip rho = [q + p z/s^2 + (Q/12)(3z^2 - r^2)/s^4] g_s(r), the cross-correlation integral is closed form:
+        E(R) = V0 exp(-s^2 k^2 / 2) [ q cos(k.R + phi) - p k_z sin(k.R + phi) + (Q/12)(k^2 - 3 k_z^2) cos(k.R + phi) ]
+    and F = -grad E.  A dropped term, a wrong sign, a wrong normalisation of g or a missing dV fails this."""
+    g = _fft_grid()
+    n, h = np.array(g.n), np.diag(np.asarray(g.step))
+    L = n * h
+    kvec = 2 * np.pi * np.array([1, -1, 2]) / L
+    V0, phi, s = 0.8, 0.4, 0.4            # 7 sigma = half the shortest cell edge: no tail is lost to the wrap
+    K, J, I = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+    R = np.stack([I * h[0], J * h[1], K * h[2]], axis=-1)
+    arg = R @ kvec + phi
+    V = V0 * np.cos(arg)
+    damp = V0 * np.exp(-0.5 * s * s * kvec @ kvec)
+    k2, kz = kvec @ kvec, kvec[2]
+    for q, pz, Q in [(1.0, 0.0, 0.0), (0.0, 0.3, 0.0), (0.0, 0.0, -0.1), (-0.05, 0.02, -0.12)]:
+        got = oracle.fft_forcefield(V, g, s, q, pz, Q)
+        amp_c = q + (Q / 12.0) * (k2 - 3 * kz * kz)
+        amp_s = -pz * kz
+        E = damp * (amp_c * np.cos(arg) + amp_s * np.sin(arg))
+        dE = damp * (-amp_c * np.sin(arg) + amp_s * np.cos(arg))           # dE/d(arg)
+        F = -dE[..., None] * kvec
+        assert np.allclose(got[..., 3], E, rtol=0, atol=1e-6), (q, pz, Q)     # residual: Gaussian tail beyond 7 sigma
+        assert np.allclose(got[..., :3], F, rtol=0, atol=1e-6), (q, pz, Q)
+    # moments of the sampled density: total charge, dipole, quadrupole
+    rho = oracle.tip_density(g, s, -0.05, 0.02, -0.12)[0]
+    dV = np.prod(h)
+    Rw = np.where(R >= L / 2, R - L, R)
+    assert np.isclose(rho.sum() * dV, -0.05, atol=1e-10)
+    assert np.isclose((rho * Rw[..., 2]).sum() * dV, 0.02, atol=1e-10)
+    assert np.isclose((rho * (3 * Rw[..., 2] ** 2 - (Rw ** 2).sum(-1))).sum() * dV, -0.12, atol=1e-9)
+
+
+def test_eq7_crosscorrelation_equals_numpy_fft_and_brute_force():
+    """The direct sum against (i) the convolution theorem with numpy's FFT ("a product in the Fourier
+    space with an additional complex conjugation") and (ii) a literal Python loop on a 4 x 3 x 2 grid, for a skewed
+    cell and an arbitrary V."""
+    rng = np.random.default_rng(3)
+    step = np.array([[0.3, 0.02, 0.0], [-0.04, 0.28, 0.01], [0.0, 0.03, 0.33]])
+    g = W.Grid(origin=np.zeros(3), step=step, n=(12, 10, 9), periodic=(1, 1, 1))
+    V = rng.normal(size=(9, 10, 12))
+    got = oracle.fft_forcefield(V, g, 0.6, 0.1, -0.05, 0.2)
+    rho4 = oracle.tip_density(g, 0.6, 0.1, -0.05, 0.2)
+    dV = abs(np.linalg.det(step))
+    for c, lane in ((0, 3), (1, 0), (2, 1), (3, 2)):
+        ref = np.fft.ifftn(np.conj(np.fft.fftn(rho4[c])) * np.fft.fftn(V)).real * dV
+        assert np.allclose(got[..., lane], ref, rtol=0, atol=1e-12)
+    # (ii) brute force
+    g2 = W.Grid(origin=np.zeros(3), step=step, n=(4, 3, 2), periodic=(1, 1, 1))
+    V2 = rng.normal(size=(2, 3, 4))
+    got2 = oracle.fft_forcefield(V2, g2, 0.5, 1.0, 0.0, 0.0)
+    rho2 = oracle.tip_density(g2, 0.5, 1.0, 0.0, 0.0)[0]
+    for K in range(2):
+        for J in range(3):
+            for I in range(4):
+                acc = 0.0
+                for k in range(2):
+                    for j in range(3):
+                        for i in range(4):
+                            acc += rho2[k, j, i] * V2[(k + K) % 2, (j + J) % 3, (i + I) % 4]
+                assert np.isclose(got2[K, J, I, 3], acc * dV, atol=1e-13)
+    # gradient lanes: analytic grad rho against central differences of rho in the continuum formula
+    s, q, pz, Q = 0.6, 0.1, -0.05, 0.2
+
+    def rho_at(r):
+        rr = r @ r
+        return (q + pz * r[2] / s**2 + Q / 12 * (3 * r[2]**2 - rr) / s**4) * (2 * np.pi * s * s) ** -1.5 * np.exp(-rr / (2 * s * s))
+    for (k, j, i) in [(1, 2, 3), (8, 9, 11), (4, 0, 5)]:
+        iw, jw, kw = (i - 12 if 2 * i >= 12 else i), (j - 10 if 2 * j >= 10 else j), (k - 9 if 2 * k >= 9 else k)
+        r = iw * step[0] + jw * step[1] + kw * step[2]
+        assert np.isclose(rho4[0, k, j, i], rho_at(r), rtol=1e-12)
+        for a in range(3):
+            d = np.zeros(3); d[a] = 1e-5
+            fd = (rho_at(r + d) - rho_at(r - d)) / 2e-5
+            assert np.isclose(rho4[a + 1, k, j, i], fd, rtol=1e-6, atol=1e-9)
+
+
 def test_golden_constants_are_what_the_generators_use():
     assert W.EVA2_PER_NM == pytest.approx(1.0 / NM, rel=1e-15)
     assert W.ELEM_R[:4].tolist() == [GOLD["R_H"], GOLD["R_C"], GOLD["R_N"], GOLD["R_O"]]
