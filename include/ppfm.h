@@ -158,6 +158,28 @@ int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grid
                           const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
                           ppfm_stats *d_stats, void *cuda_stream);
 
+/* ---- (1b) electrostatics of an extended tip charge density, Eq.7 -----
+ *     E_el(R) = integral rho_PP(r) V_S(r + R) dr,   F_el(R) = -grad_R E_el = integral grad rho_PP(r) V_S(r + R) dr
+ * by the convolution theorem (cuFFT, FP64) on the grid, which is taken as periodic in all three axes: the integral
+ * is the cyclic sum over the nodes times dV = |det(step)|.  rho_PP is a Gaussian multipole centred on the PP,
+ *     rho(r) = [ q_s + p_z z / sigma^2 + (Q_zz / 12) (3 z^2 - r^2) / sigma^4 ] (2 pi sigma^2)^(-3/2) exp(-r^2 / 2 sigma^2)
+ * (charge q_s in e, dipole p_z in e Å, quadrupole Q_zz = integral rho (3z^2 - r^2) in e Å^2; the paper quotes -0.025 to
+ * -0.15 e Å^2 for CO tips), sampled with its analytic gradient at the nodes (minimum image by index).  Keep
+ * sigma >= ~1.5 grid steps and <= ~1/7 of the shortest cell edge.
+ * d_V   DEVICE float[nz][ny][nx]: sample potential V_S in eV per unit charge (e.g. the .w lane of the unit-charge
+ *       grid of ppfm_forcefield_split, or a Hartree potential)
+ * d_ff  DEVICE float[nz][ny][nx][4] = (Fx, Fy, Fz, E_el); add to an LJ grid with ppfm_combine(lj, d_ff, 1.0, ...)
+ * The library caches the cuFFT plans (and their work areas) per grid size until ppfm_release_scratch().
+ */
+typedef struct {
+    double sigma;   /* Gaussian width (Å)        */
+    double q_s;     /* monopole (e)              */
+    double p_z;     /* dipole along z (e Å)      */
+    double Q_zz;    /* quadrupole (e Å^2)        */
+} ppfm_tip_density;
+int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, const ppfm_tip_density *tip, float *d_ff,
+                        void *cuda_stream);
+
 /* ---- (2b) stiffness map of the relaxed probe particle (IETS module) ------
  * "This module calculates the change of the stiffness (resp. vibration frequency) of lateral vibration modes of the
  * CO molecule attached to the AFM tip due to its interaction with the sample."  For every (pixel, z-step) sample the
@@ -224,7 +246,8 @@ typedef enum {
     PPFM_K_RELAX = 3,   /* a4+a5 relaxation scan             */
     PPFM_K_DF = 4,      /* a6 frequency shift                */
     PPFM_K_STIFFNESS = 5, /* N2 stiffness map               */
-    PPFM_K_COUNT = 6
+    PPFM_K_FFT_EL = 6,  /* N3 Eq.7 electrostatics: own kernels + cuFFT, one timed region */
+    PPFM_K_COUNT = 7
 } ppfm_kernel_id;
 int ppfm_timing_enable(int on);
 int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);

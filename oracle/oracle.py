@@ -198,6 +198,23 @@ def fft_forcefield(V, grid, sigma: float, q_s: float, p_z: float, Q_zz: float) -
     return out
 
 
+def fft_forcefield_at(V, grid, sigma: float, q_s: float, p_z: float, Q_zz: float, ijk) -> np.ndarray:
+    """O12 at selected output nodes ijk (npts, 3) = (I, J, K) -> (npts, 4) = (Fx, Fy, Fz, E); O(N) per sample."""
+    V = np.ascontiguousarray(np.asarray(V, dtype=np.float64))
+    rho4 = tip_density(grid, sigma, q_s, p_z, Q_zz)
+    dV = abs(float(np.linalg.det(np.asarray(grid.step, dtype=np.float64))))
+    ijk = np.ascontiguousarray(ijk, dtype=np.int32)
+    out = np.empty((ijk.shape[0], 4))
+    tmp = np.empty(ijk.shape[0])
+    for c, lane in ((0, 3), (1, 0), (2, 1), (3, 2)):
+        rc = lib().oracle_crosscorr_at(_p(_i(grid.n)), _p(np.ascontiguousarray(rho4[c])), _p(V), C.c_double(dV),
+                                       C.c_int64(ijk.shape[0]), _p(ijk), _p(tmp))
+        if rc:
+            raise ValueError(f"oracle_crosscorr_at rc={rc}")
+        out[:, lane] = tmp
+    return out
+
+
 def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None, traj: bool = True):
     """O4-O8 (+O10).  Returns dict: pos_fz (nz, npix, 4), iters (nz, npix) [-1 = not converged],
     lam_min (nz, npix), clamped (nz, npix), lam_traj (nz, npix; smallest Hessian eigenvalue along the step's FIRE

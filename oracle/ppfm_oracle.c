@@ -430,6 +430,28 @@ int oracle_crosscorr(const int *n, const double *rho, const double *V, double dV
     return 0;
 }
 
+/* The same sum at npts selected output nodes (I, J, K) only: full-size grids are checked on samples. */
+int oracle_crosscorr_at(const int *n, const double *rho, const double *V, double dV, int64_t npts,
+                        const int *ijk /* [npts][3] */, double *out /* [npts] */) {
+    const int nx = n[0], ny = n[1], nz = n[2];
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t m = 0; m < npts; m++) {
+        const int I = ijk[3 * m], J = ijk[3 * m + 1], K = ijk[3 * m + 2];
+        double acc = 0.0;
+        for (int k = 0; k < nz; k++) {
+            const int kk = (k + K) % nz;
+            for (int j = 0; j < ny; j++) {
+                const int jj = (j + J) % ny;
+                const double *pr = rho + ((int64_t)k * ny + j) * nx;
+                const double *pv = V + ((int64_t)kk * ny + jj) * nx;
+                for (int i = 0; i < nx; i++) acc += pr[i] * pv[(i + I) % nx];
+            }
+        }
+        out[m] = acc * dV;
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------------------------------------------------------
  * O6 FIRE + O7 scan + O8 read-out + O10 flag.
  *

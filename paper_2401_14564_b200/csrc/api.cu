@@ -186,6 +186,7 @@ extern "C" int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_la
 }
 
 extern "C" int ppfm_release_scratch(void) {
+    release_fft_plans();
     int dev = 0;
     PPFM_CUDA(cudaGetDevice(&dev));
     std::lock_guard<std::mutex> lk(g_pool_mu);

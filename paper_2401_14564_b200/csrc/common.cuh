@@ -25,6 +25,7 @@ inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_
 // Stream-ordered scratch from the library's private memory pool of the current device (api.cu): freed blocks stay
 // in the pool across calls (no driver allocation on the steady-state path) until ppfm_release_scratch().
 cudaError_t scratch_alloc(void **ptr, size_t bytes, cudaStream_t st);
+void release_fft_plans();   // fftel.cu: cached cuFFT plans
 
 // Optional per-kernel device timing (ppfm_timing_enable / ppfm_timing_read): CUDA events recorded on the launching
 // stream immediately around one kernel launch.  Costs nothing when timing is off.

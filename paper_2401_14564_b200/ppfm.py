@@ -50,6 +50,10 @@ class Scan(C.Structure):
                 ("npy", C.c_int32), ("nz", C.c_int32), ("dz", C.c_double)]
 
 
+class TipDensity(C.Structure):
+    _fields_ = [("sigma", C.c_double), ("q_s", C.c_double), ("p_z", C.c_double), ("Q_zz", C.c_double)]
+
+
 class Stats(C.Structure):
     _fields_ = [("total_iters", C.c_uint64), ("n_not_converged", C.c_uint64), ("n_clamped", C.c_uint64),
                 ("max_iters", C.c_uint32), ("_pad", C.c_uint32), ("warp_iters", C.c_uint64),
@@ -57,11 +61,11 @@ class Stats(C.Structure):
 
 
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
-           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_relax_scan",
+           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft", "ppfm_relax_scan",
            "ppfm_relax_scan_batch", "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
            "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
            "ppfm_release_scratch"]
-KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5}
+KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6}
 
 
 def lib():
@@ -270,6 +274,20 @@ def forcefield_batch(atom_offset: Sequence[int], xyzq, types, elem_R, elem_e, la
                                      C.c_int32(len(R)), pR, pe, lat, pr, gr, C.c_double(r_min),
                                      _dptr(out, torch.float32), _stream())
     _check(rc, "ppfm_forcefield_batch")
+    return out
+
+
+# ---- (1b) Eq.7 electrostatics of an extended tip density (cuFFT) -------------------------------------------------
+def forcefield_fft(V, grid, sigma: float, q_s: float = 0.0, p_z: float = 0.0, Q_zz: float = 0.0, out=None):
+    """ppfm_forcefield_fft: V (nz, ny, nx) float32 device tensor in eV/e -> (nz, ny, nx, 4) = (Fx, Fy, Fz, E_el)."""
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in (grid.n if not isinstance(grid, Grid) else grid.n))
+    if out is None:
+        out = torch.empty((nz, ny, nx, 4), dtype=torch.float32, device=V.device)
+    td = TipDensity(float(sigma), float(q_s), float(p_z), float(Q_zz))
+    rc = lib().ppfm_forcefield_fft(_dptr(V, torch.float32), C.byref(c_grid(grid)), C.byref(td),
+                                   _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_forcefield_fft")
     return out
 
 

@@ -401,6 +401,76 @@ def test_relax_max_iter_flag(P):
     assert np.all(iters.cpu().numpy().view(np.uint16) == 0xFFFF)
 
 
+# ------------------------------------------------------------------------------------------------ Eq.7 electrostatics
+def check_fft_ff(got, ref, what=""):
+    """(.., 4) GPU vs oracle.  The FFTs run in FP64 on the FP32 potential; what remains is the FP32 rounding of the
+    output and ~1e-15 N log N of the transform: |d| <= 1e-6 |ref| + 1e-6 max|ref| per lane."""
+    got = np.asarray(got, np.float64).reshape(-1, 4)
+    ref = np.asarray(ref, np.float64).reshape(-1, 4)
+    assert np.all(np.isfinite(got)), what
+    for lane in range(4):
+        scale = np.abs(ref[:, lane]).max()
+        err = np.abs(got[:, lane] - ref[:, lane])
+        assert (err <= 1e-6 * np.abs(ref[:, lane]) + 1e-6 * scale).all(), f"{what}: lane {lane} error {err.max():.3e} of {scale:.3e}"
+
+
+def test_fft_electrostatics_small_grids_full_parity(P):
+    """SURVEY 8(f) N3 (Eq.7, 270): every node of small grids against the O(N^2) definition:
+    odd/even/prime sizes, a skewed cell, monopole / dipole / quadrupole / mixed tips."""
+    import torch
+    rng = np.random.default_rng(11)
+    cases = [((24, 20, 16), np.diag([0.25, 0.3, 0.35]), (0.5, 1.0, 0.0, 0.0)),
+             ((13, 11, 7), np.array([[0.3, 0.02, 0.0], [-0.04, 0.28, 0.01], [0.0, 0.03, 0.33]]), (0.45, 0.0, 0.3, 0.0)),
+             ((16, 16, 16), np.diag([0.2, 0.2, 0.2]), (0.4, -0.05, 0.02, -0.12)),
+             ((36, 32, 24), np.diag([0.2, 0.25, 0.3]), (0.7, 0.0, 0.0, -0.1))]
+    for n, step, (sig, q, pz, Q) in cases:
+        g = W.Grid(origin=np.zeros(3), step=step, n=n, periodic=(1, 1, 1))
+        V = rng.normal(size=(n[2], n[1], n[0])).astype(np.float32)
+        got = P.forcefield_fft(torch.from_numpy(V).cuda(), g, sig, q, pz, Q)
+        torch.cuda.synchronize()
+        check_fft_ff(got.cpu().numpy(), oracle.fft_forcefield(V, g, sig, q, pz, Q), f"n={n}")
+
+
+def test_fft_electrostatics_point_charge_potential_and_full_size_samples(P):
+    """V_S = the unit-charge Coulomb potential of the config-1 molecule from ppfm_forcefield_split (.w lane), on the
+    full 200 x 200 x 100 grid, CO-like quadrupole tip: sampled nodes against the definition, plus the sum rules
+    sum_R E = q_s sum V and sum_R F = 0 that hold at any size; then LJ + Eq.7 grid through combine and a relaxed scan."""
+    import torch
+    w = W.get(1)
+    xyzq, types = P.upload(w)
+    lj, el = P.forcefield_split(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
+    V = el[..., 3].contiguous()
+    sig, q, pz, Q = 0.7, -0.03, 0.0, -0.1
+    got = P.forcefield_fft(V, w.grid, sig, q, pz, Q)
+    torch.cuda.synchronize()
+    Vh = V.cpu().numpy()
+    rng = np.random.default_rng(5)
+    nx, ny, nz = w.grid.n
+    ijk = np.stack([rng.integers(0, nx, 60), rng.integers(0, ny, 60), rng.integers(0, nz, 60)], axis=1)
+    ref = oracle.fft_forcefield_at(Vh, w.grid, sig, q, pz, Q, ijk)
+    check_fft_ff(got.cpu().numpy()[ijk[:, 2], ijk[:, 1], ijk[:, 0]], ref, "cfg1 sampled")
+    gh = got.cpu().numpy().astype(np.float64)
+    assert np.isclose(gh[..., 3].sum(), q * Vh.astype(np.float64).sum(), rtol=1e-5)
+    assert np.abs(gh[..., :3].sum(axis=(0, 1, 2))).max() <= 1e-6 * np.abs(gh[..., :3]).sum()
+    # the Eq.7 grid is a drop-in replacement for Q * F_el(point charge): combine and scan
+    ff = P.combine(lj, got, 1.0)
+    pos, iters = P.relax_scan(ff, w.grid, w.tip, w.fire, W.shrink(w, scan_np=(40, 40)).scan)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(pos).all()) and int((iters.to(torch.int32) < 0).sum()) == 0
+
+
+def test_fft_electrostatics_rejects_bad_arguments(P):
+    import torch
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(8, 8, 8), periodic=(1, 1, 1))
+    V = torch.zeros((8, 8, 8), dtype=torch.float32, device="cuda")
+    with pytest.raises(P.PpfmError):
+        P.forcefield_fft(V, g, 0.0, 1.0)                      # sigma must be > 0
+    with pytest.raises(P.PpfmError):
+        P.forcefield_fft(V, g, float("nan"), 1.0)
+    out = P.forcefield_fft(V, g, 0.4, 1.0, 0.1, -0.1)
+    assert float(out.abs().max()) == 0.0                     # zero potential -> zero field
+
+
 # ------------------------------------------------------------------------------------------------ stiffness map
 def check_stiffness(eig_gpu, ff_h, w, pos_h, what=""):
     """GPU eigenvalues vs the oracle's at the same positions on the same (FP32, widened) grid.  Tolerance

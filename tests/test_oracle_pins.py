@@ -615,6 +615,9 @@ def test_eq7_crosscorrelation_equals_numpy_fft_and_brute_force():
     for c, lane in ((0, 3), (1, 0), (2, 1), (3, 2)):
         ref = np.fft.ifftn(np.conj(np.fft.fftn(rho4[c])) * np.fft.fftn(V)).real * dV
         assert np.allclose(got[..., lane], ref, rtol=0, atol=1e-12)
+    ijk = np.array([[0, 0, 0], [11, 9, 8], [5, 2, 7], [1, 0, 3]])
+    assert np.allclose(oracle.fft_forcefield_at(V, g, 0.6, 0.1, -0.05, 0.2, ijk), got[ijk[:, 2], ijk[:, 1], ijk[:, 0]],
+                       rtol=0, atol=1e-13)
     # (ii) brute force
     g2 = W.Grid(origin=np.zeros(3), step=step, n=(4, 3, 2), periodic=(1, 1, 1))
     V2 = rng.normal(size=(2, 3, 4))
