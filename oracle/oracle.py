@@ -106,7 +106,10 @@ def _ff_args(ff, grid):
     else:
         raise TypeError("ff must be float32 or float64")
     nx, ny, nz = grid.n
-    assert ff.shape == (nz, ny, nx, 4), (ff.shape, grid.n)
+    if ff.shape == (nz, ny, nx):          # O13: energy-only grid -> tri-cubic interpolation of the potential
+        is32 |= 2
+    else:
+        assert ff.shape == (nz, ny, nx, 4), (ff.shape, grid.n)
     return ff, is32, _d(grid.origin), _d(grid.step), _i(grid.n), _i(grid.periodic)
 
 

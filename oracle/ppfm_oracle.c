@@ -21,6 +21,7 @@
  *   O9  Giessibl df                      PAPER.md:64-66 (Eq.3; quadrature = reading S9)
  *   O10 stability flag (Hessian)         north_star exemption; reading S14
  *   O11 stiffness map (IETS)
+ *   O13 tri-cubic interpolation of E     PAPER.md:264 ("tri-cubic interpolation of the potential"); reading S22
  *   O12 grid electrostatics, Eq.7        PAPER.md:102-111 (cross-correlation), 270 (convolution theorem); reading S21
  *
  * Pins: tests/test_oracle_pins.py (closed forms, invariants, brute force).  "Relaxed positions on the real
@@ -131,8 +132,9 @@ int oracle_forcefield(int natoms, const double *xyzq, const int *type, int ntype
  * Grid view used by O4..O10.
  * ---------------------------------------------------------------------------------------------------------- */
 typedef struct {
-    const void *ff;  /* [nz][ny][nx][4] */
+    const void *ff;  /* [nz][ny][nx][4] forces + energy; or, tricubic = 1, [nz][ny][nx] energies only */
     int is_f32;      /* 1: float data, widened to double on access (GPU-produced grids) */
+    int tricubic;    /* O13: the sample force is -grad of the tri-cubic interpolant of an energy grid */
     double origin[3];
     double Minv[9];  /* t = Minv * (r - origin), fractional grid coordinates */
     int n[3];
@@ -140,7 +142,7 @@ typedef struct {
 } grid_view;
 
 static double ff_get(const grid_view *g, int i, int j, int k, int comp) {
-    size_t o = (((size_t)k * g->n[1] + j) * g->n[0] + i) * 4 + comp;
+    size_t o = (((size_t)k * g->n[1] + j) * g->n[0] + i) * (g->tricubic ? 1 : 4) + (g->tricubic ? 0 : comp);
     return g->is_f32 ? (double)((const float *)g->ff)[o] : ((const double *)g->ff)[o];
 }
 
@@ -168,7 +170,8 @@ static int invert3(const double *S /* rows = step vectors */, double *Minv) {
 static int make_view(grid_view *g, const void *ff, int is_f32, const double *origin, const double *step,
                      const int *n, const int *periodic) {
     g->ff = ff;
-    g->is_f32 = is_f32;
+    g->is_f32 = is_f32 & 1;       /* the callers' flag word: bit 0 = float data, bit 1 = tri-cubic energy grid (O13) */
+    g->tricubic = (is_f32 >> 1) & 1;
     for (int d = 0; d < 3; d++) {
         g->origin[d] = origin[d];
         g->n[d] = n[d];
@@ -203,9 +206,79 @@ static int axis_cell(double t, int n, int periodic, int *i0, int *i1, double *f)
     return clamped;
 }
 
+/* O13 (reading S22): F_S = -grad of the tri-cubic interpolant of the energy grid.  Per axis the
+ * interpolating cubic convolution kernel (Catmull-Rom / Keys a = -1/2) on the four nodes i0-1 .. i0+2 around the
+ * cell [i0, i0+1) that O4's axis_cell picks:
+ *     w0 = (-f^3 + 2f^2 - f)/2,  w1 = (3f^3 - 5f^2 + 2)/2,  w2 = (-3f^3 + 4f^2 + f)/2,  w3 = (f^3 - f^2)/2,
+ * tensor product over the three axes; stencil indices wrap on periodic axes and are clamped to [0, n-1] on the
+ * others (edge replication).  E is C^1, reproduces polynomials up to degree 2 in each variable and passes through
+ * the node values.  Returns F = -(dE/dt) Minv and, if G != NULL, G[c][b] = dF_c/dt_b (second derivatives). */
+static void cubic_weights(double f, double w[4], double d1[4], double d2[4]) {
+    w[0] = 0.5 * (-f * f * f + 2.0 * f * f - f);
+    w[1] = 0.5 * (3.0 * f * f * f - 5.0 * f * f + 2.0);
+    w[2] = 0.5 * (-3.0 * f * f * f + 4.0 * f * f + f);
+    w[3] = 0.5 * (f * f * f - f * f);
+    d1[0] = 0.5 * (-3.0 * f * f + 4.0 * f - 1.0);
+    d1[1] = 0.5 * (9.0 * f * f - 10.0 * f);
+    d1[2] = 0.5 * (-9.0 * f * f + 8.0 * f + 1.0);
+    d1[3] = 0.5 * (3.0 * f * f - 2.0 * f);
+    d2[0] = -3.0 * f + 2.0;
+    d2[1] = 9.0 * f - 5.0;
+    d2[2] = -9.0 * f + 4.0;
+    d2[3] = 3.0 * f - 1.0;
+}
+
+static int stencil_index(int i0, int off, int n, int periodic) {
+    int i = i0 + off;
+    if (periodic) { i %= n; if (i < 0) i += n; return i; }
+    if (i < 0) i = 0;
+    if (i > n - 1) i = n - 1;
+    return i;
+}
+
+static int interp_tricubic(const grid_view *g, const double r[3], double F[3], double G[9]) {
+    double t[3], f[3], w[3][4], d1[3][4], d2[3][4];
+    int i0[3], i1[3], idx[3][4], clamped = 0;
+    for (int a = 0; a < 3; a++)
+        t[a] = g->Minv[3 * a] * (r[0] - g->origin[0]) + g->Minv[3 * a + 1] * (r[1] - g->origin[1]) +
+               g->Minv[3 * a + 2] * (r[2] - g->origin[2]);
+    for (int a = 0; a < 3; a++) {
+        clamped |= axis_cell(t[a], g->n[a], g->periodic[a], &i0[a], &i1[a], &f[a]);
+        cubic_weights(f[a], w[a], d1[a], d2[a]);
+        for (int m = 0; m < 4; m++) idx[a][m] = stencil_index(i0[a], m - 1, g->n[a], g->periodic[a]);
+    }
+    double E1[3] = {0, 0, 0}, E2[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}; /* dE/dt_a, d2E/dt_a dt_b */
+    for (int kz = 0; kz < 4; kz++)
+        for (int ky = 0; ky < 4; ky++)
+            for (int kx = 0; kx < 4; kx++) {
+                const double e = ff_get(g, idx[0][kx], idx[1][ky], idx[2][kz], 0);
+                const double W[3] = {w[0][kx], w[1][ky], w[2][kz]};
+                const double D[3] = {d1[0][kx], d1[1][ky], d1[2][kz]};
+                const double S[3] = {d2[0][kx], d2[1][ky], d2[2][kz]};
+                E1[0] += D[0] * W[1] * W[2] * e;
+                E1[1] += W[0] * D[1] * W[2] * e;
+                E1[2] += W[0] * W[1] * D[2] * e;
+                E2[0] += S[0] * W[1] * W[2] * e;
+                E2[4] += W[0] * S[1] * W[2] * e;
+                E2[8] += W[0] * W[1] * S[2] * e;
+                E2[1] += D[0] * D[1] * W[2] * e;
+                E2[2] += D[0] * W[1] * D[2] * e;
+                E2[5] += W[0] * D[1] * D[2] * e;
+            }
+    E2[3] = E2[1]; E2[6] = E2[2]; E2[7] = E2[5];
+    for (int c = 0; c < 3; c++) {
+        F[c] = -(E1[0] * g->Minv[0 + c] + E1[1] * g->Minv[3 + c] + E1[2] * g->Minv[6 + c]);
+        if (G)
+            for (int b = 0; b < 3; b++)
+                G[3 * c + b] = -(E2[0 + b] * g->Minv[0 + c] + E2[3 + b] * g->Minv[3 + c] + E2[6 + b] * g->Minv[6 + c]);
+    }
+    return clamped;
+}
+
 /* O4: F_S(r) = sum over 8 corners of w * FF.xyz.  If G != NULL also returns G[c][a] = dF_c/dt_a, the analytic
  * derivative of the interpolant with respect to the fractional coordinates inside the current cell (for O10). */
 static int interp(const grid_view *g, const double r[3], double F[3], double G[9]) {
+    if (g->tricubic) return interp_tricubic(g, r, F, G);
     double t[3], f[3];
     int i0[3], i1[3], clamped = 0;
     for (int a = 0; a < 3; a++)

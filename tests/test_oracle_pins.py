@@ -648,6 +648,103 @@ def test_eq7_crosscorrelation_equals_numpy_fft_and_brute_force():
             assert np.isclose(rho4[a + 1, k, j, i], fd, rtol=1e-6, atol=1e-9)
 
 
+# ---------------------------------------------------------------------------------------------------- O13 tri-cubic
+def test_tricubic_potential_interpolation_pins():
+    """PAPER.md:264 "tri-cubic interpolation of the potential" (reading S22: Catmull-Rom cubic convolution per axis).
+    (i) a polynomial of degree <= 2 in each variable is reproduced exactly, so F = -grad E is analytic, also across
+    cell faces and the periodic seam of an axis the polynomial does not depend on; (ii) at nodes the interpolant
+    returns the node values (checked through a line integral of F between two nodes); (iii) F is continuous across
+    cell faces (C^1 interpolant) for random data; (iv) the Hessian G is the finite-difference derivative of F;
+    (v) weights: partition of unity and the printed cubic at f = 0.5: (-1/16, 9/16, 9/16, -1/16)."""
+    step = np.array([[0.25, 0.0, 0.0], [0.02, 0.3, 0.0], [0.0, 0.01, 0.2]])
+    g = W.Grid(origin=np.array([0.3, -0.2, 1.0]), step=step, n=(14, 12, 16), periodic=(0, 0, 0))
+    k, j, i = np.meshgrid(np.arange(16), np.arange(12), np.arange(14), indexing="ij")
+    nodes = np.asarray(g.origin) + i[..., None] * step[0] + j[..., None] * step[1] + k[..., None] * step[2]
+    x, y, z = nodes[..., 0], nodes[..., 1], nodes[..., 2]
+
+    def E_of(x, y, z):
+        return 0.3 * x * x * y - 0.2 * y * y * z * z + 0.7 * x * z + 0.1 * z * z - 0.4 * x + 0.05 * x * x * y * y * z
+
+    def F_of(x, y, z):
+        return -np.array([0.6 * x * y + 0.7 * z - 0.4 + 0.1 * x * y * y * z,
+                          0.3 * x * x - 0.4 * y * z * z + 0.1 * x * x * y * z,
+                          -0.4 * y * y * z + 0.7 * x + 0.2 * z + 0.05 * x * x * y * y])
+    rng = np.random.default_rng(9)
+    tfrac = 1.0 + rng.uniform(0, 1, (50, 3)) * (np.array([14, 12, 16]) - 4.0)   # 4-point stencil inside the grid
+    pts = np.asarray(g.origin) + tfrac @ step
+    # orthogonal grid: degree <= 2 in each variable is exact
+    go = replace(g, step=np.diag([0.25, 0.3, 0.2]))
+    no = np.asarray(go.origin) + np.stack([i * 0.25, j * 0.3, k * 0.2], axis=-1)
+    pto = np.asarray(go.origin) + tfrac * np.array([0.25, 0.3, 0.2])
+    got = oracle.interp(E_of(no[..., 0], no[..., 1], no[..., 2]), go, pto)
+    assert np.allclose(got, np.array([F_of(*p) for p in pto]), rtol=1e-11, atol=1e-11)
+    # skewed grid: total degree <= 2 stays within degree 2 of every index variable -> exact
+    A = np.array([[0.3, 0.1, -0.05], [0.1, -0.2, 0.07], [-0.05, 0.07, 0.15]])
+    bq = np.array([0.4, -0.3, 0.2])
+    Eq = np.einsum("...a,ab,...b->...", nodes, A, nodes) + nodes @ bq
+    got = oracle.interp(Eq, g, pts)
+    assert np.allclose(got, -(2 * pts @ A + bq), rtol=1e-11, atol=1e-11)
+    # (ii) line integral of F between two nodes = E(a) - E(b) for ARBITRARY node data (interpolation property)
+    Er = rng.normal(size=Eq.shape)
+    a_idx, b_idx = (5, 4, 6), (9, 4, 6)                                  # (i, j, k): along x, 4 cells
+    ra = np.asarray(g.origin) + a_idx[0] * step[0] + a_idx[1] * step[1] + a_idx[2] * step[2]
+    rb = np.asarray(g.origin) + b_idx[0] * step[0] + b_idx[1] * step[1] + b_idx[2] * step[2]
+    tt, ww = np.polynomial.legendre.leggauss(6)
+    work = 0.0
+    for c in range(4):                                                   # Gauss-Legendre per cell: exact for cubics
+        p0, p1 = ra + (rb - ra) * c / 4, ra + (rb - ra) * (c + 1) / 4
+        ps = p0 + (p1 - p0) * ((tt[:, None] + 1) / 2)
+        Fs = oracle.interp(Er, g, ps)
+        work += (ww * (Fs @ (p1 - p0))).sum() / 2
+    assert np.isclose(work, Er[a_idx[2], a_idx[1], a_idx[0]] - Er[b_idx[2], b_idx[1], b_idx[0]], atol=1e-12)
+    # (iii) continuity of F across a cell face, random data
+    face = np.asarray(g.origin) + 6 * step[0] + 5.3 * step[1] + 7.6 * step[2]
+    eps = 1e-9 * step[0]
+    assert np.allclose(oracle.interp(Er, g, [face - eps]), oracle.interp(Er, g, [face + eps]), atol=1e-6)
+    # (iv) Hessian = -dF/dr by finite differences (zero springs: k = 0 tip)
+    tip0 = W.Tip(k_lat=np.array([0.0, 0.0]), k_rad=0.0, d0=np.array([0.0, 0.0, -4.0]))
+    rpp = np.asarray(g.origin) + 6.37 * step[0] + 5.21 * step[1] + 7.64 * step[2]
+    H, ev = oracle.hessian(Er, g, tip0, rpp + np.array([0, 0, 4.0]), rpp)
+    J = np.zeros((3, 3))
+    for a in range(3):
+        dp = np.zeros(3); dp[a] = 1e-6
+        J[:, a] = (oracle.interp(Er, g, [rpp + dp])[0] - oracle.interp(Er, g, [rpp - dp])[0]) / 2e-6
+    assert np.allclose(H, -(J + J.T) / 2, rtol=1e-6, atol=1e-6)
+    assert np.allclose(J, J.T, atol=1e-6)                                # a true gradient field, unlike tri-linear F (S14)
+    # (v) the printed kernel values at the cell centre, through a 1-D delta function along x
+    d = np.zeros((16, 12, 14)); d[:, :, 7] = 1.0                         # E = 1 on the plane i = 7
+    gx = W.Grid(origin=np.zeros(3), step=np.diag([1.0, 1.0, 1.0]), n=(14, 12, 16), periodic=(0, 0, 0))
+    # F_x = -dE/dx; integrate F_x from x0 to cell centres to recover E there: use E(x) = E(x0) - int F
+    def E_at(xc):
+        xs = np.linspace(2.0, xc, 2001)
+        Fx = oracle.interp(d, gx, np.stack([xs, np.full_like(xs, 5.0), np.full_like(xs, 6.0)], 1))[:, 0]
+        return -np.sum((Fx[1:] + Fx[:-1]) / 2 * np.diff(xs))
+    assert np.isclose(E_at(5.5), -1 / 16, atol=1e-6) and np.isclose(E_at(6.5), 9 / 16, atol=1e-6)
+    assert np.isclose(E_at(7.5), 9 / 16, atol=1e-6) and np.isclose(E_at(8.5), -1 / 16, atol=1e-6)
+
+
+def test_tricubic_relaxation_linear_field_closed_form_and_periodic_seam():
+    """End to end on O13: E = g/2 (z - zc)^2 (reproduced exactly) gives F_z = -g (z - zc), the linear-field closed
+    form of the tri-linear pin with g -> -g: w = -g (z_t - R - zc)/(k_R + g), Fz_tip = k_R w.  And a potential
+    periodic in x is seamless across the periodic boundary."""
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.1]), n=(30, 24, 70), periodic=(1, 1, 0))
+    k, j, i = np.meshgrid(np.arange(70), np.arange(24), np.arange(30), indexing="ij")
+    zc, gg = 3.0, 0.37
+    E = 0.5 * gg * (k * 0.1 - zc) ** 2
+    tip, sc = W._default_tip(), _scan(npx=3, npy=2, nz=12, z0=8.5, dz=0.1)
+    r = oracle.relax_scan(E, g, tip, W.Fire(), sc)
+    zt = 8.5 - 0.1 * np.arange(12)
+    wexp = -gg * (zt - 4.0 - zc) / (tip.k_rad + gg)
+    assert (r["iters"] >= 0).all()
+    assert np.allclose(r["pos_fz"][:, 0, 2], zt - 4.0 + wexp, atol=2e-6)
+    assert np.allclose(r["pos_fz"][:, 0, 3], tip.k_rad * wexp, atol=2e-6)
+    Ex = np.cos(2 * np.pi * i / 30) * np.ones_like(E)
+    pts = np.array([[5.9, 1.0, 3.05], [6.1, 1.0, 3.05], [-0.1, 1.0, 3.05], [0.1, 1.0, 3.05]])
+    F = oracle.interp(Ex, g, pts)
+    assert np.allclose(F[0], F[2], atol=1e-12) and np.allclose(F[1], F[3], atol=1e-12)
+    assert np.allclose(F[0, 0], 2 * np.pi / 6.0 * np.sin(2 * np.pi * 5.9 / 6.0), atol=2e-3)   # cubic accuracy only
+
+
 def test_golden_constants_are_what_the_generators_use():
     assert W.EVA2_PER_NM == pytest.approx(1.0 / NM, rel=1e-15)
     assert W.ELEM_R[:4].tolist() == [GOLD["R_H"], GOLD["R_C"], GOLD["R_N"], GOLD["R_O"]]
