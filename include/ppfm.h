@@ -180,6 +180,24 @@ typedef struct {
 int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, const ppfm_tip_density *tip, float *d_ff,
                         void *cuda_stream);
 
+/* ---- (2a) relaxation scan on an energy-only grid, tri-cubic interpolation -------
+ * "we are experimenting with tri-cubic interpolation of the potential which may allow us to use larger grid spacing
+ * and avoid storage of forces".  Same scan, FIRE and outputs as ppfm_relax_scan; the sample force is
+ * F_S = -grad of the tri-cubic interpolant of E: per axis the interpolating cubic convolution kernel (Catmull-Rom,
+ * a = -1/2) on the nodes i0-1 .. i0+2 around the cell, tensor product; stencil indices wrap on periodic axes and are
+ * clamped to [0, n-1] on the others; the coordinate is clamped as in ppfm_relax_scan.
+ * d_E  DEVICE float[nz][ny][nx]: potential energy of the PP (eV), e.g. from ppfm_energy_grid (the .w lane of a
+ *      force-field grid; 4 bytes per point instead of 16).  Batch form: grids concatenated.
+ */
+int ppfm_relax_scan_tricubic(const float *d_E, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_fire *fire,
+                             const ppfm_scan *scan, float *d_pos_fz, uint16_t *d_iters, ppfm_stats *d_stats,
+                             void *cuda_stream);
+int ppfm_relax_scan_tricubic_batch(int32_t nsys, const float *d_E, const ppfm_grid *grids, const ppfm_tip *tips,
+                                   const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz,
+                                   uint16_t *d_iters, ppfm_stats *d_stats, void *cuda_stream);
+/* d_E[i] = d_ff[i][3] for n_points grid points (both DEVICE). */
+int ppfm_energy_grid(const float *d_ff, int64_t n_points, float *d_E, void *cuda_stream);
+
 /* ---- (2b) stiffness map of the relaxed probe particle (IETS module) ------
  * "This module calculates the change of the stiffness (resp. vibration frequency) of lateral vibration modes of the
  * CO molecule attached to the AFM tip due to its interaction with the sample."  For every (pixel, z-step) sample the
@@ -247,7 +265,8 @@ typedef enum {
     PPFM_K_DF = 4,      /* a6 frequency shift                */
     PPFM_K_STIFFNESS = 5, /* N2 stiffness map               */
     PPFM_K_FFT_EL = 6,  /* N3 Eq.7 electrostatics: own kernels + cuFFT, one timed region */
-    PPFM_K_COUNT = 7
+    PPFM_K_RELAX_TRICUBIC = 7, /* N4 relaxation with tri-cubic interpolation of the potential */
+    PPFM_K_COUNT = 8
 } ppfm_kernel_id;
 int ppfm_timing_enable(int on);
 int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);

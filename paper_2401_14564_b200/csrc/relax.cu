@@ -128,9 +128,9 @@ __device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, 
     i0 = __float_as_int(zc) - a.K;
 }
 
-template <bool ORTHO, bool ANYPER, bool SYMTIP>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FireParams &fp, int lb,
-                                             const float4 *__restrict__ ff, float4 *__restrict__ pos_fz,
+                                             const void *__restrict__ ff, float4 *__restrict__ pos_fz,
                                              uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats) {
     const int by = lb / job.nbx, bx = lb - by * job.nbx;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -139,7 +139,9 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
     const bool valid = (ix < job.npx) && (iy < job.npy);
     const int ixc = min(ix, job.npx - 1), iyc = min(iy, job.npy - 1);
 
-    const float4 *__restrict__ g = ff + job.ff_offset;
+    // tri-linear: float4 (Fx,Fy,Fz,E) grid; TRICUBIC: energy-only float grid
+    const float4 *__restrict__ g = reinterpret_cast<const float4 *>(ff) + (TRICUBIC ? 0 : job.ff_offset);
+    const float *__restrict__ ge = reinterpret_cast<const float *>(ff) + (TRICUBIC ? job.ff_offset : 0);
     const int nx = job.n[0], ny = job.n[1], nz = job.n[2];
     const int perx = job.periodic[0], pery = job.periodic[1], perz = job.periodic[2];
     const float m00 = job.Minvf[0], m01 = job.Minvf[1], m02 = job.Minvf[2];
@@ -181,8 +183,62 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         for (int e = 0; e < 4; e++)
 #pragma unroll
             for (int c = 0; c < 3; c++) c0[e][c] = cd[e][c] = 0.0f;
+        // TRICUBIC: the 4 x 4 x 4 energies around the cell, [z][y][x], minus the value at the cell's own node (the
+        // gradient does not see a constant, and differences of ~|F| h keep FP32 rounding far below f_conv)
+        float en[TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1];
+        if (TRICUBIC) {
+#pragma unroll
+            for (int a = 0; a < (TRICUBIC ? 4 : 1); a++)
+#pragma unroll
+                for (int b = 0; b < (TRICUBIC ? 4 : 1); b++)
+#pragma unroll
+                    for (int c = 0; c < (TRICUBIC ? 4 : 1); c++) en[a][b][c] = 0.0f;
+        }
 
         auto interp = [&](float (&S)[3]) {     // nested lerps x, y, z: 10 FP32 ops per component
+            if (TRICUBIC) {
+                // F_S = -grad of the tri-cubic (Catmull-Rom per axis, reading S22) interpolant of the energies:
+                // weights w and their derivatives d per axis (Horner), x pass per (z,y) row, y pass per z plane, z pass
+                float w[3][4], d[3][4];
+                const float fa[3] = {fx, fy, fz};
+#pragma unroll
+                for (int a = 0; a < 3; a++) {
+                    const float f = fa[a], f2 = f * f;
+                    w[a][0] = fmaf(fmaf(-0.5f, f, 1.0f), f, -0.5f) * f;
+                    w[a][1] = fmaf(fmaf(1.5f, f, -2.5f), f2, 1.0f);
+                    w[a][2] = fmaf(fmaf(-1.5f, f, 2.0f), f, 0.5f) * f;
+                    w[a][3] = fmaf(0.5f, f, -0.5f) * f2;
+                    d[a][0] = fmaf(fmaf(-1.5f, f, 2.0f), f, -0.5f);
+                    d[a][1] = fmaf(4.5f, f, -5.0f) * f;
+                    d[a][2] = fmaf(fmaf(-4.5f, f, 4.0f), f, 0.5f);
+                    d[a][3] = fmaf(1.5f, f, -1.0f) * f;
+                }
+                float Ex = 0.f, Ey = 0.f, Ez = 0.f;            // dE/dt along the three grid axes
+#pragma unroll
+                for (int k = 0; k < (TRICUBIC ? 4 : 1); k++) {
+                    float V = 0.f, DX = 0.f, DY = 0.f;
+#pragma unroll
+                    for (int j = 0; j < (TRICUBIC ? 4 : 1); j++) {
+                        const float *r = en[k][j];
+                        const float v = fmaf(w[0][3], r[TRICUBIC ? 3 : 0], fmaf(w[0][2], r[TRICUBIC ? 2 : 0], fmaf(w[0][1], r[TRICUBIC ? 1 : 0], w[0][0] * r[0])));
+                        const float dxv = fmaf(d[0][3], r[TRICUBIC ? 3 : 0], fmaf(d[0][2], r[TRICUBIC ? 2 : 0], fmaf(d[0][1], r[TRICUBIC ? 1 : 0], d[0][0] * r[0])));
+                        V = fmaf(w[1][j], v, V);
+                        DX = fmaf(w[1][j], dxv, DX);
+                        DY = fmaf(d[1][j], v, DY);
+                    }
+                    Ex = fmaf(w[2][k], DX, Ex);
+                    Ey = fmaf(w[2][k], DY, Ey);
+                    Ez = fmaf(d[2][k], V, Ez);
+                }
+                if (ORTHO) {
+                    S[0] = -m00 * Ex; S[1] = -m11 * Ey; S[2] = -m22 * Ez;
+                } else {                                         // F_c = -sum_a dE/dt_a Minv[a][c]
+                    S[0] = -fmaf(m20, Ez, fmaf(m10, Ey, m00 * Ex));
+                    S[1] = -fmaf(m21, Ez, fmaf(m11, Ey, m01 * Ex));
+                    S[2] = -fmaf(m22, Ez, fmaf(m12, Ey, m02 * Ex));
+                }
+                return;
+            }
 #pragma unroll
             for (int c = 0; c < 3; c++) {
                 const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
@@ -250,7 +306,32 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 axis_cell(ty, ty - 0.5f, ay, j0, fly);
                 axis_cell(tz, tz - 0.5f, az, k0, flz);
                 float4 c000, c001, c010, c011, c100, c101, c110, c111;
-                if (!ANYPER) {
+                if (TRICUBIC) {
+                    // 4 x 4 x 4 stencil i0-1 .. i0+2: wrap on periodic axes, clamp to [0, n-1] on the others (S22)
+                    int xi[4], yj[4], zk[4];
+#pragma unroll
+                    for (int m = 0; m < 4; m++) {
+                        const int a = i0 + m - 1, b = j0 + m - 1, c = k0 + m - 1;
+                        xi[m] = perx ? ((a % nx) + nx) % nx : min(max(a, 0), nx - 1);
+                        yj[m] = pery ? ((b % ny) + ny) % ny : min(max(b, 0), ny - 1);
+                        zk[m] = perz ? ((c % nz) + nz) % nz : min(max(c, 0), nz - 1);
+                    }
+#pragma unroll
+                    for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
+#pragma unroll
+                        for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
+                            const float *row = ge + (long long)(zk[kk] * ny + yj[jj]) * nx;
+#pragma unroll
+                            for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(row + xi[m]);
+                        }
+                    const float ref = en[TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0];
+#pragma unroll
+                    for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
+#pragma unroll
+                        for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++)
+#pragma unroll
+                            for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] -= ref;
+                } else if (!ANYPER) {
                     const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
                     c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
                     c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
@@ -280,6 +361,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                     fy = __saturatef(fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy))));
                     fz = __saturatef(fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz))));
                 }
+                if (!TRICUBIC) {
                 c0[0][0] = c000.x; c0[0][1] = c000.y; c0[0][2] = c000.z;
                 c0[1][0] = c010.x; c0[1][1] = c010.y; c0[1][2] = c010.z;
                 c0[2][0] = c100.x; c0[2][1] = c100.y; c0[2][2] = c100.z;
@@ -288,6 +370,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 cd[1][0] = c011.x - c010.x; cd[1][1] = c011.y - c010.y; cd[1][2] = c011.z - c010.z;
                 cd[2][0] = c101.x - c100.x; cd[2][1] = c101.y - c100.y; cd[2][2] = c101.z - c100.z;
                 cd[3][0] = c111.x - c110.x; cd[3][1] = c111.y - c110.y; cd[3][2] = c111.z - c110.z;
+                }
                 my_reloads += (worst > 0x3F800000u) ? 1u : 0u;
                 my_wreloads++;
                 interp(S);
@@ -387,19 +470,19 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 }
 
 // One system: the job travels as a kernel parameter (constant bank), no scratch and no copy.
-template <bool ORTHO, bool ANYPER, bool SYMTIP>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireParams fp,
-             const float4 *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
+             const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
              ppfm_stats *__restrict__ stats) {
-    relax_pixels<ORTHO, ANYPER, SYMTIP>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats);
+    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats);
 }
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
-template <bool ORTHO, bool ANYPER, bool SYMTIP>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_constant__ FireParams fp,
-                   const float4 *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
+                   const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
                    ppfm_stats *__restrict__ stats) {
     __shared__ RelaxJob s_job;
     const int blk = blockIdx.x;
@@ -414,16 +497,16 @@ relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_co
         for (int w = threadIdx.x; w < (int)(sizeof(RelaxJob) / sizeof(int)); w += RX_THREADS) dstw[w] = srcw[w];
     }
     __syncthreads();
-    relax_pixels<ORTHO, ANYPER, SYMTIP>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats);
+    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats);
 }
 
-template <bool ORTHO, bool ANYPER, bool SYMTIP>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 static void launch_relax(int nsys, long long blocks, cudaStream_t st, const RelaxJob *hj, const RelaxJob *dj,
-                         const FireParams &fp, const float4 *ff, float4 *pos, uint16_t *it, ppfm_stats *stats) {
+                         const FireParams &fp, const void *ff, float4 *pos, uint16_t *it, ppfm_stats *stats) {
     if (nsys == 1)
-        relax_kernel<ORTHO, ANYPER, SYMTIP><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats);
+        relax_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats);
     else
-        relax_batch_kernel<ORTHO, ANYPER, SYMTIP><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
+        relax_batch_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
 }
 
 // Host side shared by the relaxation and the stiffness map: validate and pack one RelaxJob per system.
@@ -482,9 +565,9 @@ static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *ti
 
 static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                       const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
-                      ppfm_stats *d_stats, void *cuda_stream) {
+                      ppfm_stats *d_stats, void *cuda_stream, bool tricubic = false) {
     if (nsys < 1 || !d_ff || !grids || !tips || !fire || !scans || !d_pos_fz) return PPFM_EINVAL;
-    if (((uintptr_t)d_ff & 15) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
+    if (((uintptr_t)d_ff & (tricubic ? 3 : 15)) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
         return PPFM_EINVAL;
     if (!(fire->dt > 0) || !(fire->dt_max > 0) || !(fire->finc >= 1.0) || !(fire->fdec > 0 && fire->fdec < 1.0) ||
         !(fire->alpha0 >= 0 && fire->alpha0 <= 1.0) || !(fire->falpha > 0 && fire->falpha <= 1.0) ||
@@ -512,11 +595,14 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
         e = cudaMemcpyAsync(dj, hj, (size_t)nsys * sizeof(RelaxJob), cudaMemcpyHostToDevice, st);   // pageable: staged
         if (e != cudaSuccess) { free(hj); set_cuda_error(e, "job upload"); cudaFreeAsync(dj, st); return PPFM_ECUDA; }
     }
-    const float4 *ff4 = reinterpret_cast<const float4 *>(d_ff);
     float4 *pos4 = reinterpret_cast<float4 *>(d_pos_fz);
     {
-        KernelTimer kt(PPFM_K_RELAX, st);
-#define PPFM_RX(O, A, S) launch_relax<O, A, S>(nsys, blocks, st, hj, dj, fp, ff4, pos4, d_iters, d_stats)
+        KernelTimer kt(tricubic ? PPFM_K_RELAX_TRICUBIC : PPFM_K_RELAX, st);
+#define PPFM_RX(O, A, S) \
+    do { \
+        if (tricubic) launch_relax<O, A, S, true>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats); \
+        else launch_relax<O, A, S, false>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats); \
+    } while (0)
         if (symtip) {
             if (ortho && !anyper) PPFM_RX(true, false, true);
             else if (ortho) PPFM_RX(true, true, true);
@@ -729,4 +815,36 @@ extern "C" int ppfm_stiffness(const float *d_ff, const ppfm_grid *grid, const pp
 extern "C" int ppfm_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                                     const ppfm_scan *scans, const float *d_pos_fz, float *d_eig, void *cuda_stream) {
     return stiffness_impl(nsys, d_ff, grids, tips, scans, d_pos_fz, d_eig, cuda_stream);
+}
+
+// ---- relaxation on an energy-only grid with tri-cubic interpolation of the potential
+extern "C" int ppfm_relax_scan_tricubic(const float *d_E, const ppfm_grid *grid, const ppfm_tip *tip,
+                                        const ppfm_fire *fire, const ppfm_scan *scan, float *d_pos_fz,
+                                        uint16_t *d_iters, ppfm_stats *d_stats, void *cuda_stream) {
+    return relax_impl(1, d_E, grid, tip, fire, scan, d_pos_fz, d_iters, d_stats, cuda_stream, true);
+}
+
+extern "C" int ppfm_relax_scan_tricubic_batch(int32_t nsys, const float *d_E, const ppfm_grid *grids,
+                                              const ppfm_tip *tips, const ppfm_fire *fire, const ppfm_scan *scans,
+                                              float *d_pos_fz, uint16_t *d_iters, ppfm_stats *d_stats,
+                                              void *cuda_stream) {
+    return relax_impl(nsys, d_E, grids, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream, true);
+}
+
+namespace ppfm {
+__global__ void energy_grid_kernel(const float4 *__restrict__ ff, long long n, float *__restrict__ E) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) E[i] = ff[i].w;
+}
+}  // namespace ppfm
+
+extern "C" int ppfm_energy_grid(const float *d_ff, int64_t n_points, float *d_E, void *cuda_stream) {
+    if (!d_ff || !d_E || n_points < 0 || ((uintptr_t)d_ff & 15) || ((uintptr_t)d_E & 3)) return PPFM_EINVAL;
+    if (n_points == 0) return PPFM_OK;
+    long long blocks = (n_points + 255) / 256;
+    if (blocks > 148LL * 16) blocks = 148LL * 16;
+    energy_grid_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(
+        reinterpret_cast<const float4 *>(d_ff), n_points, d_E);
+    PPFM_LAUNCH_CHECK();
+    return PPFM_OK;
 }

@@ -62,10 +62,11 @@ class Stats(C.Structure):
 
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft", "ppfm_relax_scan",
-           "ppfm_relax_scan_batch", "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
+           "ppfm_relax_scan_batch", "ppfm_relax_scan_tricubic", "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid",
+           "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host",
            "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
            "ppfm_release_scratch"]
-KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6}
+KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6, "relax_tricubic": 7}
 
 
 def lib():
@@ -331,6 +332,47 @@ def relax_scan_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, stat
     rc = lib().ppfm_relax_scan_batch(C.c_int32(nsys), _dptr(ff, torch.float32), gr, tp, C.byref(c_fire(fire)), sc,
                                      _dptr(pos_fz, torch.float32), _dptr(iters), _dptr(stats), _stream())
     _check(rc, "ppfm_relax_scan_batch")
+    return pos_fz, iters
+
+
+# ---- (2a) relaxation on an energy-only grid, tri-cubic interpolation of the potential ---------------
+def energy_grid(ff, out=None):
+    """ppfm_energy_grid: the .w lane of a float4 force-field grid as a contiguous float32 array of the same shape[:-1]."""
+    torch = _torch()
+    if out is None:
+        out = torch.empty(ff.shape[:-1], dtype=torch.float32, device=ff.device)
+    rc = lib().ppfm_energy_grid(_dptr(ff, torch.float32), C.c_int64(out.numel()), _dptr(out, torch.float32), _stream())
+    _check(rc, "ppfm_energy_grid")
+    return out
+
+
+def relax_scan_tricubic(E, grid, tip, fire, scan, pos_fz=None, iters=None, stats=None, want_iters=True):
+    """ppfm_relax_scan_tricubic: as relax_scan, on an energy grid E (nz, ny, nx) float32."""
+    torch = _torch()
+    shape = (int(scan.nz), int(scan.npy), int(scan.npx))
+    if pos_fz is None:
+        pos_fz = torch.empty(shape + (4,), dtype=torch.float32, device=E.device)
+    if iters is None and want_iters:
+        iters = torch.empty(shape, dtype=torch.int16, device=E.device)
+    rc = lib().ppfm_relax_scan_tricubic(_dptr(E, torch.float32), C.byref(c_grid(grid)), C.byref(c_tip(tip)),
+                                        C.byref(c_fire(fire)), C.byref(c_scan(scan)), _dptr(pos_fz, torch.float32),
+                                        _dptr(iters), _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan_tricubic")
+    return pos_fz, iters
+
+
+def relax_scan_tricubic_batch(E, grids, tips, fire, scans, pos_fz=None, iters=None, stats=None, want_iters=True):
+    torch = _torch()
+    gr, tp, sc = c_array(grids, c_grid), c_array(tips, c_tip), c_array(scans, c_scan)
+    nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in sc)
+    if pos_fz is None:
+        pos_fz = torch.empty((nps, 4), dtype=torch.float32, device=E.device)
+    if iters is None and want_iters:
+        iters = torch.empty((nps,), dtype=torch.int16, device=E.device)
+    rc = lib().ppfm_relax_scan_tricubic_batch(C.c_int32(len(grids)), _dptr(E, torch.float32), gr, tp,
+                                              C.byref(c_fire(fire)), sc, _dptr(pos_fz, torch.float32), _dptr(iters),
+                                              _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan_tricubic_batch")
     return pos_fz, iters
 
 

@@ -401,6 +401,71 @@ def test_relax_max_iter_flag(P):
     assert np.all(iters.cpu().numpy().view(np.uint16) == 0xFFFF)
 
 
+# ------------------------------------------------------------------------------------------------ tri-cubic relaxation
+def test_relax_tricubic_cfg0_full_scan(P):
+    """the scan of config 0 on the energy-only grid with tri-cubic interpolation,
+    against the oracle's O13 on the same FP32 energies; positions at the relaxation's tolerance (2e-3 Å on >= 99.9 %,
+    the rest flagged near-unstable), Fz, df; and it stays close to the tri-linear scan of the same system."""
+    import torch
+    w = W.get(0)
+    ff = gpu_ff(P, w)
+    E = P.energy_grid(ff)
+    assert torch.equal(E, ff[..., 3])
+    stats = P.new_stats()
+    pos, iters = P.relax_scan_tricubic(E, w.grid, w.tip, w.fire, w.scan, stats=stats)
+    torch.cuda.synchronize()
+    npix = w.scan.npx * w.scan.npy
+    pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)
+    ref = oracle.relax_scan(E.cpu().numpy(), w.grid, w.tip, w.fire, w.scan)
+    frac, d = check_positions(pos_h, ref, "cfg0 tricubic")
+    ok = d <= 2e-3
+    assert np.abs(pos_h[..., 3] - ref["pos_fz"][..., 3])[ok].max() < 2e-4
+    st = P.read_stats(stats)
+    assert st["n_not_converged"] == int((ref["iters"] < 0).sum())
+    it_h = iters.cpu().numpy().view(np.uint16).reshape(w.scan.nz, npix).astype(np.int64)
+    same = ok & (ref["iters"] >= 0) & ~oracle.flags(ref)
+    assert np.abs(it_h - ref["iters"])[same].mean() < 2.0           # FP32 vs FP64 FIRE: same path, a move or two apart
+    pos_lin, _ = P.relax_scan(ff, w.grid, w.tip, w.fire, w.scan)
+    dl = np.linalg.norm(pos_lin.cpu().numpy().reshape(w.scan.nz, npix, 4)[..., :3] - pos_h[..., :3], axis=-1)
+    assert np.median(dl) < 5e-3                                      # two interpolants of the same field
+
+
+def test_relax_tricubic_periodic_skewed_batch_and_edges(P):
+    import torch
+    # periodic x, y + skewed grid + scan reaching over the seam and past the non-periodic z faces (clamp)
+    w = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
+    step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
+    w = replace(w, grid=replace(w.grid, step=step), scan=replace(w.scan, p0=np.array([-3.0, 20.0, 9.0])))
+    E = P.energy_grid(gpu_ff(P, w))
+    stats = P.new_stats()
+    pos, _ = P.relax_scan_tricubic(E, w.grid, w.tip, w.fire, w.scan, stats=stats)
+    torch.cuda.synchronize()
+    npix = w.scan.npx * w.scan.npy
+    ref = oracle.relax_scan(E.cpu().numpy(), w.grid, w.tip, w.fire, w.scan)
+    check_positions(pos.cpu().numpy().reshape(w.scan.nz, npix, 4), ref, "tricubic periodic skewed")
+    w2 = replace(w, grid=replace(w.grid, periodic=(0, 0, 0)), scan=replace(w.scan, p0=np.array([-1.0, 23.0, 12.5])))
+    stats2 = P.new_stats()
+    pos2, _ = P.relax_scan_tricubic(E, w2.grid, w2.tip, w2.fire, w2.scan, stats=stats2)
+    ref2 = oracle.relax_scan(E.cpu().numpy(), w2.grid, w2.tip, w2.fire, w2.scan)
+    check_positions(pos2.cpu().numpy().reshape(w.scan.nz, npix, 4), ref2, "tricubic clamped")
+    assert P.read_stats(stats2)["n_clamped"] == int(ref2["clamped"].sum()) > 0
+    # batch == single, bit for bit
+    mols = [W.shrink(m, grid_n=m.grid.n, scan_np=(24, 20), scan_nz=5) for m in W.get(3)[:3]]
+    off = np.concatenate([[0], np.cumsum([m.natoms for m in mols])])
+    xyzq = torch.from_numpy(np.concatenate([m.xyzq for m in mols])).cuda()
+    types = torch.from_numpy(np.concatenate([m.types for m in mols])).cuda()
+    ffb = P.forcefield_batch(off, xyzq, types, mols[0].elem_R, mols[0].elem_e, [m.lattice for m in mols],
+                             [m.probe for m in mols], [m.grid for m in mols], mols[0].r_min)
+    Eb = P.energy_grid(ffb)
+    posb, _ = P.relax_scan_tricubic_batch(Eb, [m.grid for m in mols], [m.tip for m in mols], mols[0].fire,
+                                          [m.scan for m in mols])
+    nps, npts = mols[0].pixel_steps, mols[0].npoints
+    for m in range(3):
+        one, _ = P.relax_scan_tricubic(Eb[m * npts:(m + 1) * npts], mols[m].grid, mols[m].tip, mols[m].fire,
+                                       mols[m].scan)
+        assert torch.equal(one.reshape(-1, 4), posb[m * nps:(m + 1) * nps])
+
+
 # ------------------------------------------------------------------------------------------------ Eq.7 electrostatics
 def check_fft_ff(got, ref, what=""):
     """(.., 4) GPU vs oracle.  The FFTs run in FP64 on the FP32 potential; what remains is the FP32 rounding of the
