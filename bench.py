@@ -172,6 +172,16 @@ class DeviceJob:
             tot += float(per_point) * w.nimages * w.npoints
         return tot
 
+    def relax_tricubic(self, E, stats):
+        """The scan of step() on the energy-only grid E with tri-cubic interpolation (last Q of a sweep)."""
+        P = self.P
+        if self.batch:
+            P.relax_scan_tricubic_batch(E, self.c_grid, self.c_tip, self.c_fire, self.c_scan, pos_fz=self.pos,
+                                        iters=self.iters, stats=stats)
+        else:
+            P.relax_scan_tricubic(E, self.c_grid[0], self.c_tip[0], self.c_fire, self.c_scan[0], pos_fz=self.pos,
+                                  iters=self.iters, stats=stats)
+
     def stiffness(self, out):
         """Stiffness map of the scan held in self.pos (last Q of a sweep) on the resident grid."""
         P, ws = self.P, self.ws
@@ -434,6 +444,21 @@ def run_ours(args):
     P.timing_enable(False)
     del eig
 
+    # ---- tri-cubic relaxation of the same scan on the energy-only grid: beside the step
+    E_only = P.energy_grid(job.ff)
+    tri_stats = P.new_stats()
+    for rep in range(2 + 3):
+        if rep == 2:
+            P.timing_enable(True)
+        flush.zero_()
+        tri_stats.zero_()
+        job.relax_tricubic(E_only, tri_stats)
+    torch.cuda.synchronize()
+    tri_ms = P.timing_read()["relax_tricubic"][0] / 3.0
+    tri = P.read_stats(tri_stats)
+    P.timing_enable(False)
+    del E_only
+
     # ---- Eq.7 electrostatics on the first system's grid: V_S = the .w lane of the resident grid
     # (any potential serves for timing), CO-like quadrupole tip; measured beside the step, not part of it
     w0g = ws[0].grid
@@ -552,7 +577,23 @@ def run_ours(args):
                              "cuFFT (library), the three kernels around them are this library's",
               "ms": fft_ms, "points": npts0, "points_per_s": npts0 / (fft_ms * 1e-3), "in_step": False,
               "traffic": NCU_TRAFFIC.get((cfg, "fft_el"))}
-    kernels = {"ff": rl_ff, "relax": rl_relax, "df": rl_df, "stiffness": rl_stiff, "fft_el": rl_fft}
+    # tri-cubic iteration (relax.cu): weights 42 + x pass 128 + y pass 48 + z pass 12 + metric 3 = 233 FP32-pipe
+    # lane-instructions for the field (tri-linear: 33), the rest of the iteration as above (37): 270 = 2 * 244 + 26
+    TRI_INSTR, TRI_FLOPS = 270, 514
+    tri_s = tri_ms * 1e-3
+    rl_tri = {"kernel": "relax_kernel<.,.,.,TRICUBIC>", "bound": "alu", "unit": "TFLOP/s",
+              "achieved": tri["total_iters"] * TRI_FLOPS / tri_s * 1e-12, "peak": 2 * alu_peak * 1e-12,
+              "frac": tri["total_iters"] * TRI_FLOPS / tri_s / (2 * alu_peak),
+              "pipe_frac": tri["total_iters"] * TRI_INSTR / tri_s / alu_peak,
+              "issued_pipe_frac": 32.0 * tri["warp_iters"] * TRI_INSTR / tri_s / alu_peak,
+              "peak_source": f"{SMS} SMs x {LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 (FMA)",
+              "algorithmic": f"{TRI_FLOPS} flops / {TRI_INSTR} FP32-pipe lane-instructions per FIRE iteration (64-point "
+                             f"stencil held in registers) x {tri['total_iters']:.4g} iterations",
+              "ms": tri_ms, "pixel_steps_per_s": job.pos.shape[0] / tri_s,
+              "iters_per_pixel_step": tri["total_iters"] / job.pos.shape[0], "not_converged": tri["n_not_converged"],
+              "grid_bytes_per_point": 4, "in_step": False, "traffic": NCU_TRAFFIC.get((cfg, "relax_tricubic"))}
+    kernels = {"ff": rl_ff, "relax": rl_relax, "df": rl_df, "stiffness": rl_stiff, "fft_el": rl_fft,
+               "relax_tricubic": rl_tri}
     for k in kernels:
         kernels[k]["timing"] = "CUDA events recorded inside libppfm directly around the launch, mean per step"
     dominant = max(("ff", "relax", "df"), key=lambda k: ms[k])
