@@ -284,8 +284,9 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 frk = fr;
             }
             // ---- F_S, speculatively from the cached cell (redone below in the rare case that a lane left its cell)
+            // (the tri-cubic field is 233 instructions: not worth computing twice, it waits for the vote instead)
             float S[3];
-            interp(S);
+            if (!TRICUBIC) interp(S);
             if (__any_sync(0xffffffffu, worst > 0x3F800000u)) {
                 // ---- some lane's PP left its cell.  The block is warp-uniform (no reconvergence barrier on the hot
                 // path): every lane locates its cell again (magic-number floor, S12 clamp) and gathers it; lanes
@@ -307,23 +308,44 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 axis_cell(tz, tz - 0.5f, az, k0, flz);
                 float4 c000, c001, c010, c011, c100, c101, c110, c111;
                 if (TRICUBIC) {
-                    // 4 x 4 x 4 stencil i0-1 .. i0+2: wrap on periodic axes, clamp to [0, n-1] on the others (S22)
-                    int xi[4], yj[4], zk[4];
+                    // 4 x 4 x 4 stencil i0-1 .. i0+2 (reading S22).  Interior cells of the whole warp: 16 row bases and
+                    // immediate offsets.  Otherwise per-axis index lists: wrap on periodic axes, clamp to [0, n-1] on
+                    // the others.
+                    const bool inside = (i0 >= 1) & (i0 + 2 <= nx - 1) & (j0 >= 1) & (j0 + 2 <= ny - 1) & (k0 >= 1) &
+                                        (k0 + 2 <= nz - 1);
+                    if (__all_sync(0xffffffffu, inside)) {
+                        const int base = (int)((k0 - 1) * ny + (j0 - 1)) * nx + (i0 - 1);
 #pragma unroll
-                    for (int m = 0; m < 4; m++) {
-                        const int a = i0 + m - 1, b = j0 + m - 1, c = k0 + m - 1;
-                        xi[m] = perx ? ((a % nx) + nx) % nx : min(max(a, 0), nx - 1);
-                        yj[m] = pery ? ((b % ny) + ny) % ny : min(max(b, 0), ny - 1);
-                        zk[m] = perz ? ((c % nz) + nz) % nz : min(max(c, 0), nz - 1);
-                    }
+                        for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
 #pragma unroll
-                    for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
+                            for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
+                                const float *row = ge + (base + (kk * ny + jj) * nx);
 #pragma unroll
-                        for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
-                            const float *row = ge + (long long)(zk[kk] * ny + yj[jj]) * nx;
+                                for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(row + m);
+                            }
+                    } else {
+                        int xi[4], yo[4], zo[4];
+                        int iw = i0, jw = j0, kw = k0;              // periodic: |index - [0,n)| < n after axis_cell
+                        if (perx) { iw -= (iw >= nx) ? nx : 0; iw += (iw < 0) ? nx : 0; }
+                        if (pery) { jw -= (jw >= ny) ? ny : 0; jw += (jw < 0) ? ny : 0; }
+                        if (perz) { kw -= (kw >= nz) ? nz : 0; kw += (kw < 0) ? nz : 0; }
 #pragma unroll
-                            for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(row + xi[m]);
+                        for (int m = 0; m < 4; m++) {
+                            int a = iw + m - 1, b = jw + m - 1, c = kw + m - 1;
+                            if (perx) { a -= (a >= nx) ? nx : 0; a += (a < 0) ? nx : 0; } else a = min(max(a, 0), nx - 1);
+                            if (pery) { b -= (b >= ny) ? ny : 0; b += (b < 0) ? ny : 0; } else b = min(max(b, 0), ny - 1);
+                            if (perz) { c -= (c >= nz) ? nz : 0; c += (c < 0) ? nz : 0; } else c = min(max(c, 0), nz - 1);
+                            xi[m] = a; yo[m] = b * nx; zo[m] = c * ny * nx;
                         }
+#pragma unroll
+                        for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
+#pragma unroll
+                            for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
+                                const int ro = zo[kk] + yo[jj];
+#pragma unroll
+                                for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(ge + (ro + xi[m]));
+                            }
+                    }
                     const float ref = en[TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0];
 #pragma unroll
                     for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
@@ -373,8 +395,9 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 }
                 my_reloads += (worst > 0x3F800000u) ? 1u : 0u;
                 my_wreloads++;
-                interp(S);
+                if (!TRICUBIC) interp(S);
             }
+            if (TRICUBIC) interp(S);
             float Fx, Fy, Fz;
             if (SYMTIP) {
                 Fx = fmaf(frk, ux, S[0]);
