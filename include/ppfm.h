@@ -232,13 +232,21 @@ int ppfm_df_weights(int32_t n, double dz, double *h_W);
 /* ---- whole simulation in one call, HOST buffers in and out ("run the whole simulation in one step")
  * Copies the inputs to the device, runs (1) -> (2) -> (3) on `cuda_stream`, copies the results back and
  * synchronises the stream.  h_pos_fz / h_df / h_iters may each be NULL (not copied back); h_stats may be NULL.
- * Pinned host buffers make the copies asynchronous; pageable buffers work too.
+ * When the output buffers are pinned (page-locked, UVA-mapped) host memory the kernels store straight into them:
+ * the PCIe writes overlap the computation and no device-to-host copy follows the scan.  Pageable buffers work too
+ * (staged copies after the kernels).  The batch form runs nsys systems in one launch per step (arguments as in the
+ * *_batch entry points, outputs concatenated in order; with h_df all scans must have one shape).
  */
 int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t *h_type, int32_t ntypes, const double *h_R,
                    const double *h_e, const ppfm_lattice *lattice, const ppfm_probe *probe, const ppfm_grid *grid,
                    double r_min, const ppfm_tip *tip, const ppfm_fire *fire, const ppfm_scan *scan, double A,
                    double k0_Nm, double f0_Hz, float *h_pos_fz, uint16_t *h_iters, float *h_df,
                    ppfm_stats *h_stats, void *cuda_stream);
+int ppfm_scan_host_batch(int32_t nsys, const int32_t *h_atom_offset, const float *h_xyzq, const int32_t *h_type,
+                         int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
+                         const ppfm_probe *probes, const ppfm_grid *grids, double r_min, const ppfm_tip *tips,
+                         const ppfm_fire *fire, const ppfm_scan *scans, double A, double k0_Nm, double f0_Hz,
+                         float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream);
 
 /* ---- measurement helpers (used by bench.py to define the roofline denominators on the box itself) ------------
  * ppfm_probe_fma:    FFMA-only kernel; returns lane-instructions per second in *h_lane_instr_per_s.

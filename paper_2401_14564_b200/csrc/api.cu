@@ -194,23 +194,48 @@ extern "C" int ppfm_release_scratch(void) {
     return PPFM_OK;
 }
 
-extern "C" int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t *h_type, int32_t ntypes,
-                              const double *h_R, const double *h_e, const ppfm_lattice *lattice,
-                              const ppfm_probe *probe, const ppfm_grid *grid, double r_min, const ppfm_tip *tip,
-                              const ppfm_fire *fire, const ppfm_scan *scan, double A, double k0_Nm, double f0_Hz,
-                              float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats,
-                              void *cuda_stream) {
-    if (natoms < 0 || !h_xyzq || !h_type || !grid || !scan || !tip || !fire || !lattice || !probe) return PPFM_EINVAL;
-    if (!grid_ok(grid) || scan->npx < 1 || scan->npy < 1 || scan->nz < 1) return PPFM_EINVAL;
+// Device-side alias of a host buffer, if it is pinned/registered (UVA-mapped) memory; nullptr for pageable memory.
+static void *mapped_alias(const void *h) {
+    if (!h) return nullptr;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, h) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return (a.type == cudaMemoryTypeHost) ? a.devicePointer : nullptr;
+}
+
+// One call, host buffers ("run the whole simulation in one step").  When the output buffers are pinned
+// host memory the kernels store straight into them (posted PCIe writes that overlap the computation: no
+// device-to-host copy after the scan); the relaxation then also keeps a plain Fz stack on the device for the df kernel.
+// Pageable outputs take staged cudaMemcpyAsync copies.
+static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h_xyzq, const int32_t *h_type,
+                          int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
+                          const ppfm_probe *probes, const ppfm_grid *grids, double r_min, const ppfm_tip *tips,
+                          const ppfm_fire *fire, const ppfm_scan *scans, double A, double k0_Nm, double f0_Hz,
+                          float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream) {
+    if (nsys < 1 || !h_atom_offset || !grids || !scans || !tips || !fire || !lattices || !probes) return PPFM_EINVAL;
+    const int natoms = h_atom_offset[nsys];
+    if (natoms < 0 || h_atom_offset[0] != 0 || (natoms > 0 && (!h_xyzq || !h_type))) return PPFM_EINVAL;
+    size_t npts = 0, nps = 0;
+    for (int m = 0; m < nsys; m++) {
+        if (!grid_ok(&grids[m]) || scans[m].npx < 1 || scans[m].npy < 1 || scans[m].nz < 1) return PPFM_EINVAL;
+        if (h_df && (scans[m].npx != scans[0].npx || scans[m].npy != scans[0].npy || scans[m].nz != scans[0].nz ||
+                     scans[m].dz != scans[0].dz))
+            return PPFM_EINVAL;                        // the df batch takes stacks of one shape
+        npts += (size_t)grid_points(&grids[m]);
+        nps += (size_t)scans[m].npx * scans[m].npy * scans[m].nz;
+    }
+    const ppfm_scan *scan = &scans[0];
     const double nn = (scan->dz > 0) ? A / scan->dz : -1.0;
     const long long n = std::llround(nn);
     if (h_df && (n < 1 || std::fabs(nn - (double)n) > 1e-6 || scan->nz <= n)) return PPFM_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t npts = (size_t)grid_points(grid);
-    const size_t nps = (size_t)scan->npx * scan->npy * scan->nz;
-    const size_t ndf = h_df ? (size_t)scan->npx * scan->npy * (size_t)(scan->nz - n) : 0;
+    const size_t ndf = h_df ? (size_t)nsys * scan->npx * scan->npy * (size_t)(scan->nz - n) : 0;
     const size_t na = (size_t)(natoms > 0 ? natoms : 1);
-    float *d_xyzq = nullptr, *d_ff = nullptr, *d_pos = nullptr, *d_df = nullptr;
+    // zero-copy outputs?
+    float *m_pos = (float *)mapped_alias(h_pos_fz);
+    uint16_t *m_it = (uint16_t *)mapped_alias(h_iters);
+    float *m_df = (float *)mapped_alias(h_df);
+    const bool zc = h_pos_fz && m_pos && (!h_iters || m_it) && (!h_df || m_df);
+    float *d_xyzq = nullptr, *d_ff = nullptr, *d_pos = nullptr, *d_df = nullptr, *d_fz = nullptr;
     int32_t *d_type = nullptr;
     uint16_t *d_it = nullptr;
     ppfm_stats *d_stats = nullptr;
@@ -221,31 +246,69 @@ extern "C" int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t
     TRY(scratch_alloc((void **)&d_xyzq, na * 16, st));
     TRY(scratch_alloc((void **)&d_type, na * 4, st));
     TRY(scratch_alloc((void **)&d_ff, npts * 16, st));
-    TRY(scratch_alloc((void **)&d_pos, nps * 16, st));
-    TRY(scratch_alloc((void **)&d_it, nps * 2, st));
     TRY(scratch_alloc((void **)&d_stats, sizeof(ppfm_stats), st));
-    if (h_df) TRY(scratch_alloc((void **)&d_df, ndf * 4, st));
+    if (zc) {
+        if (h_df) TRY(scratch_alloc((void **)&d_fz, nps * 4, st));
+    } else {
+        TRY(scratch_alloc((void **)&d_pos, nps * 16, st));
+        TRY(scratch_alloc((void **)&d_it, nps * 2, st));
+        if (h_df) TRY(scratch_alloc((void **)&d_df, ndf * 4, st));
+    }
     if (natoms > 0) {
         TRY(cudaMemcpyAsync(d_xyzq, h_xyzq, (size_t)natoms * 16, cudaMemcpyHostToDevice, st));
         TRY(cudaMemcpyAsync(d_type, h_type, (size_t)natoms * 4, cudaMemcpyHostToDevice, st));
     }
     TRY(cudaMemsetAsync(d_stats, 0, sizeof(ppfm_stats), st));
     if (rc == PPFM_OK)
-        rc = ppfm_forcefield(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, d_ff, cuda_stream);
-    if (rc == PPFM_OK) rc = ppfm_relax_scan(d_ff, grid, tip, fire, scan, d_pos, d_it, d_stats, cuda_stream);
-    if (rc == PPFM_OK && h_df)
-        rc = ppfm_df(d_pos, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, d_df, cuda_stream);
-    if (h_pos_fz) TRY(cudaMemcpyAsync(h_pos_fz, d_pos, nps * 16, cudaMemcpyDeviceToHost, st));
-    if (h_iters) TRY(cudaMemcpyAsync(h_iters, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
-    if (h_df) TRY(cudaMemcpyAsync(h_df, d_df, ndf * 4, cudaMemcpyDeviceToHost, st));
+        rc = (nsys == 1) ? ppfm_forcefield(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min, d_ff,
+                                           cuda_stream)
+                         : ppfm_forcefield_batch(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes,
+                                                 grids, r_min, d_ff, cuda_stream);
+    if (zc) {
+        if (rc == PPFM_OK)
+            rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, m_pos, h_iters ? m_it : nullptr, d_stats, d_fz,
+                               cuda_stream);
+        if (rc == PPFM_OK && h_df)
+            rc = df_from_fz(nsys, d_fz, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, m_df, cuda_stream);
+    } else {
+        if (rc == PPFM_OK)
+            rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, d_pos, d_it, d_stats, nullptr, cuda_stream);
+        if (rc == PPFM_OK && h_df)
+            rc = ppfm_df_batch(nsys, d_pos, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, d_df, cuda_stream);
+        if (h_pos_fz) TRY(cudaMemcpyAsync(h_pos_fz, d_pos, nps * 16, cudaMemcpyDeviceToHost, st));
+        if (h_iters) TRY(cudaMemcpyAsync(h_iters, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
+        if (h_df) TRY(cudaMemcpyAsync(h_df, d_df, ndf * 4, cudaMemcpyDeviceToHost, st));
+    }
     if (h_stats) TRY(cudaMemcpyAsync(h_stats, d_stats, sizeof(ppfm_stats), cudaMemcpyDeviceToHost, st));
 #undef TRY
-    void *bufs[] = {d_xyzq, d_type, d_ff, d_pos, d_it, d_stats, d_df};
+    void *bufs[] = {d_xyzq, d_type, d_ff, d_pos, d_it, d_stats, d_df, d_fz};
     for (void *b : bufs)
         if (b) cudaFreeAsync(b, st);
     e = cudaStreamSynchronize(st);
     if (rc == PPFM_OK && e != cudaSuccess) fail(e, "cudaStreamSynchronize");
     return rc;
+}
+
+extern "C" int ppfm_scan_host(int32_t natoms, const float *h_xyzq, const int32_t *h_type, int32_t ntypes,
+                              const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                              const ppfm_probe *probe, const ppfm_grid *grid, double r_min, const ppfm_tip *tip,
+                              const ppfm_fire *fire, const ppfm_scan *scan, double A, double k0_Nm, double f0_Hz,
+                              float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats,
+                              void *cuda_stream) {
+    if (natoms < 0) return PPFM_EINVAL;
+    const int32_t off[2] = {0, natoms};
+    return scan_host_impl(1, off, h_xyzq, h_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, tip, fire, scan, A,
+                          k0_Nm, f0_Hz, h_pos_fz, h_iters, h_df, h_stats, cuda_stream);
+}
+
+extern "C" int ppfm_scan_host_batch(int32_t nsys, const int32_t *h_atom_offset, const float *h_xyzq,
+                                    const int32_t *h_type, int32_t ntypes, const double *h_R, const double *h_e,
+                                    const ppfm_lattice *lattices, const ppfm_probe *probes, const ppfm_grid *grids,
+                                    double r_min, const ppfm_tip *tips, const ppfm_fire *fire, const ppfm_scan *scans,
+                                    double A, double k0_Nm, double f0_Hz, float *h_pos_fz, uint16_t *h_iters,
+                                    float *h_df, ppfm_stats *h_stats, void *cuda_stream) {
+    return scan_host_impl(nsys, h_atom_offset, h_xyzq, h_type, ntypes, h_R, h_e, lattices, probes, grids, r_min, tips,
+                          fire, scans, A, k0_Nm, f0_Hz, h_pos_fz, h_iters, h_df, h_stats, cuda_stream);
 }
 
 extern "C" int ppfm_probe_fma(double *h_lane_instr_per_s, void *cuda_stream) {

@@ -26,6 +26,14 @@ inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_
 // in the pool across calls (no driver allocation on the steady-state path) until ppfm_release_scratch().
 cudaError_t scratch_alloc(void **ptr, size_t bytes, cudaStream_t st);
 void release_fft_plans();   // fftel.cu: cached cuFFT plans
+// Internal forms used by ppfm_scan_host[_batch] (api.cu) when the caller's output buffers are mapped host memory:
+// the relaxation also writes a plain Fz stack (device) for the df kernel, which then reads that instead of the
+// float4 stack.
+int relax_scan_fz(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips, const ppfm_fire *fire,
+                  const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters, ppfm_stats *d_stats, float *d_fz,
+                  void *cuda_stream);
+int df_from_fz(int nsys, const float *d_fz, int npx, int npy, int nz, double dz, double A, double k0, double f0,
+               float *d_df, void *cuda_stream);
 
 // Optional per-kernel device timing (ppfm_timing_enable / ppfm_timing_read): CUDA events recorded on the launching
 // stream immediately around one kernel launch.  Costs nothing when timing is off.

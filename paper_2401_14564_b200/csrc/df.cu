@@ -34,8 +34,11 @@ static void df_weights_host(int n, double dz, double *W) {
     for (int m = 0; m <= n; m++) W[m] *= norm;
 }
 
+// FZ4: Fz is the .w lane of the float4 (x, y, z, Fz) stack; otherwise a plain float stack (ppfm_scan_host keeps one
+// on the device when the float4 stack itself is written straight to mapped host memory).
+template <bool FZ4>
 __global__ void __launch_bounds__(256)
-df_kernel(const float4 *__restrict__ pos_fz, long long npix, int nz, int n, int nsys, DfWeights W,
+df_kernel(const float *__restrict__ fz, long long npix, int nz, int n, int nsys, DfWeights W,
           float *__restrict__ df) {
     const long long nout_per = (long long)(nz - n) * npix;
     const long long total = nout_per * nsys;
@@ -44,19 +47,19 @@ df_kernel(const float4 *__restrict__ pos_fz, long long npix, int nz, int n, int 
         const long long s = o / nout_per;
         const long long r = o - s * nout_per;
         const long long k = r / npix, p = r - k * npix;
-        const float4 *src = pos_fz + (s * nz + k) * npix + p;
+        const float *src = fz + ((s * nz + k) * npix + p) * (FZ4 ? 4 : 1) + (FZ4 ? 3 : 0);
         float acc = 0.f;
-        for (int m = 0; m <= n; m++) acc = fmaf(W.w[m], __ldg(&src[(long long)(n - m) * npix].w), acc);
+        for (int m = 0; m <= n; m++) acc = fmaf(W.w[m], __ldg(&src[(long long)(n - m) * npix * (FZ4 ? 4 : 1)]), acc);
         df[o] = acc;
     }
 }
 
 static int df_impl(int nsys, const float *d_pos_fz, int npx, int npy, int nz, double dz, double A, double k0,
-                   double f0, float *d_df, void *cuda_stream) {
+                   double f0, float *d_df, void *cuda_stream, bool fz4 = true) {
     if (nsys < 1 || !d_pos_fz || !d_df || npx < 1 || npy < 1 || nz < 1) return PPFM_EINVAL;
     if (!(dz > 0) || !(A > 0) || !(k0 > 0) || !std::isfinite(f0) || !std::isfinite(dz) || !std::isfinite(A))
         return PPFM_EINVAL;
-    if ((uintptr_t)d_pos_fz & 15) return PPFM_EINVAL;
+    if ((uintptr_t)d_pos_fz & (fz4 ? 15 : 3)) return PPFM_EINVAL;
     const double nn = A / dz;
     const long long n = std::llround(nn);
     if (n < 1 || n > DF_MAX_N || std::fabs(nn - (double)n) > 1e-6 || nz <= n) return PPFM_EINVAL;
@@ -71,11 +74,16 @@ static int df_impl(int nsys, const float *d_pos_fz, int npx, int npy, int nz, do
     if (blocks > 148LL * 32) blocks = 148LL * 32;
     {
         KernelTimer kt(PPFM_K_DF, (cudaStream_t)cuda_stream);
-        df_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(reinterpret_cast<const float4 *>(d_pos_fz),
-                                                                          npix, nz, (int)n, nsys, W, d_df);
+        if (fz4) df_kernel<true><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(d_pos_fz, npix, nz, (int)n, nsys, W, d_df);
+        else df_kernel<false><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(d_pos_fz, npix, nz, (int)n, nsys, W, d_df);
     }
     PPFM_LAUNCH_CHECK();
     return PPFM_OK;
+}
+
+int df_from_fz(int nsys, const float *d_fz, int npx, int npy, int nz, double dz, double A, double k0, double f0,
+               float *d_df, void *cuda_stream) {
+    return df_impl(nsys, d_fz, npx, npy, nz, dz, A, k0, f0, d_df, cuda_stream, false);
 }
 
 }  // namespace ppfm

@@ -131,7 +131,8 @@ __device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, 
 template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FireParams &fp, int lb,
                                              const void *__restrict__ ff, float4 *__restrict__ pos_fz,
-                                             uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats) {
+                                             uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats,
+                                             float *__restrict__ fz_out) {
     const int by = lb / job.nbx, bx = lb - by * job.nbx;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ix = bx * RX_TILE_X + (warp & 1) * 8 + (lane & 7);
@@ -237,10 +238,9 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                     S[1] = -fmaf(m21, Ez, fmaf(m11, Ey, m01 * Ex));
                     S[2] = -fmaf(m22, Ez, fmaf(m12, Ey, m02 * Ex));
                 }
-                return;
             }
 #pragma unroll
-            for (int c = 0; c < 3; c++) {
+            for (int c = 0; c < (TRICUBIC ? 0 : 3); c++) {
                 const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
                 const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
                 const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
@@ -452,6 +452,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             outv.z = (float)(rz + job.origin[2] + (double)uz);
             outv.w = -fr * dzc;                           // Fz_tip = -F_R,z
             pos_fz[o] = outv;
+            if (fz_out) fz_out[o] = outv.w;
             if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
             float tx, ty, tz;
             if (ORTHO) {
@@ -497,8 +498,8 @@ template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireParams fp,
              const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
-             ppfm_stats *__restrict__ stats) {
-    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats);
+             ppfm_stats *__restrict__ stats, float *__restrict__ fz_out) {
+    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats, fz_out);
 }
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
@@ -506,7 +507,7 @@ template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_constant__ FireParams fp,
                    const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
-                   ppfm_stats *__restrict__ stats) {
+                   ppfm_stats *__restrict__ stats, float *__restrict__ fz_out) {
     __shared__ RelaxJob s_job;
     const int blk = blockIdx.x;
     int lo = 0, hi = njobs - 1;
@@ -520,16 +521,17 @@ relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_co
         for (int w = threadIdx.x; w < (int)(sizeof(RelaxJob) / sizeof(int)); w += RX_THREADS) dstw[w] = srcw[w];
     }
     __syncthreads();
-    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats);
+    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats, fz_out);
 }
 
 template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
 static void launch_relax(int nsys, long long blocks, cudaStream_t st, const RelaxJob *hj, const RelaxJob *dj,
-                         const FireParams &fp, const void *ff, float4 *pos, uint16_t *it, ppfm_stats *stats) {
+                         const FireParams &fp, const void *ff, float4 *pos, uint16_t *it, ppfm_stats *stats,
+                         float *fz) {
     if (nsys == 1)
-        relax_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats);
+        relax_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats, fz);
     else
-        relax_batch_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats);
+        relax_batch_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats, fz);
 }
 
 // Host side shared by the relaxation and the stiffness map: validate and pack one RelaxJob per system.
@@ -588,7 +590,7 @@ static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *ti
 
 static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                       const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
-                      ppfm_stats *d_stats, void *cuda_stream, bool tricubic = false) {
+                      ppfm_stats *d_stats, void *cuda_stream, bool tricubic = false, float *d_fz = nullptr) {
     if (nsys < 1 || !d_ff || !grids || !tips || !fire || !scans || !d_pos_fz) return PPFM_EINVAL;
     if (((uintptr_t)d_ff & (tricubic ? 3 : 15)) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
         return PPFM_EINVAL;
@@ -623,8 +625,8 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
         KernelTimer kt(tricubic ? PPFM_K_RELAX_TRICUBIC : PPFM_K_RELAX, st);
 #define PPFM_RX(O, A, S) \
     do { \
-        if (tricubic) launch_relax<O, A, S, true>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats); \
-        else launch_relax<O, A, S, false>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats); \
+        if (tricubic) launch_relax<O, A, S, true>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz); \
+        else launch_relax<O, A, S, false>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz); \
     } while (0)
         if (symtip) {
             if (ortho && !anyper) PPFM_RX(true, false, true);
@@ -812,6 +814,12 @@ static int stiffness_impl(int nsys, const float *d_ff, const ppfm_grid *grids, c
     count_launch();
     PPFM_CUDA(cudaFreeAsync(dj, st));
     return PPFM_OK;
+}
+
+int relax_scan_fz(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips, const ppfm_fire *fire,
+                  const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters, ppfm_stats *d_stats, float *d_fz,
+                  void *cuda_stream) {
+    return relax_impl(nsys, d_ff, grids, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream, false, d_fz);
 }
 
 }  // namespace ppfm

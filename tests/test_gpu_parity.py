@@ -631,11 +631,44 @@ def test_scan_host_equals_device_path(P):
     h_pos = torch.empty(pos.shape, dtype=torch.float32).pin_memory()
     h_it = torch.empty(iters.shape, dtype=torch.int16).pin_memory()
     h_df = torch.empty(df.shape, dtype=torch.float32).pin_memory()
-    st2 = P.scan_host(w, h_xyzq, h_types, h_pos, h_it, h_df)
+    st2 = P.scan_host(w, h_xyzq, h_types, h_pos, h_it, h_df)          # pinned: kernels store straight to the host
     assert np.array_equal(h_pos.numpy(), pos.cpu().numpy())
     assert np.array_equal(h_it.numpy(), iters.cpu().numpy())
     assert np.array_equal(h_df.numpy(), df.cpu().numpy())
     assert st2 == st
+    # pageable buffers: staged copies, same bits
+    p_pos, p_it, p_df = np.empty(pos.shape, np.float32), np.empty(iters.shape, np.int16), np.empty(df.shape, np.float32)
+    st3 = P.scan_host(w, w.xyzq.copy(), w.types.copy(), p_pos, p_it, p_df)
+    assert np.array_equal(p_pos, h_pos.numpy()) and np.array_equal(p_it, h_it.numpy()) and np.array_equal(p_df, h_df.numpy())
+    assert st3 == st
+    # only positions wanted
+    h_pos2 = torch.zeros(pos.shape, dtype=torch.float32).pin_memory()
+    P.scan_host(w, h_xyzq, h_types, h_pos2, None, None)
+    assert np.array_equal(h_pos2.numpy(), h_pos.numpy())
+
+
+def test_scan_host_batch_equals_per_system_calls(P):
+    import torch
+    mols = [W.shrink(m, grid_n=m.grid.n, scan_np=(24, 20), scan_nz=14) for m in W.get(3)[:4]]
+    hx = torch.from_numpy(np.concatenate([m.xyzq for m in mols])).pin_memory()
+    ht = torch.from_numpy(np.concatenate([m.types for m in mols])).pin_memory()
+    nps = mols[0].pixel_steps
+    ndf = (14 - mols[0].n_df) * 24 * 20
+    hp = torch.empty((4 * nps, 4), dtype=torch.float32).pin_memory()
+    hi = torch.empty((4 * nps,), dtype=torch.int16).pin_memory()
+    hd = torch.empty((4 * ndf,), dtype=torch.float32).pin_memory()
+    st = P.scan_host_batch(mols, hx, ht, hp, hi, hd)
+    tot = 0
+    for m, w in enumerate(mols):
+        p1 = torch.empty((nps, 4), dtype=torch.float32).pin_memory()
+        i1 = torch.empty((nps,), dtype=torch.int16).pin_memory()
+        d1 = torch.empty((ndf,), dtype=torch.float32).pin_memory()
+        s1 = P.scan_host(w, torch.from_numpy(w.xyzq.copy()).pin_memory(), torch.from_numpy(w.types.copy()).pin_memory(),
+                         p1, i1, d1)
+        assert torch.equal(p1, hp[m * nps:(m + 1) * nps]) and torch.equal(i1, hi[m * nps:(m + 1) * nps])
+        assert torch.equal(d1, hd[m * ndf:(m + 1) * ndf])
+        tot += s1["total_iters"]
+    assert st["total_iters"] == tot
 
 
 def test_probes_run(P):
