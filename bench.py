@@ -244,6 +244,10 @@ class HostJob:
     """The same scan through ppfm_scan_host: pinned host buffers in and out, copies inside the timed region."""
 
     def __init__(self, P, torch, ws):
+        from dataclasses import replace as _replace
+        # argument marshalling done once (as DeviceJob does): ready ctypes structs pass straight through the binding
+        ws = [_replace(w, lattice=P.c_lattice(w.lattice), grid=P.c_grid(w.grid), tip=P.c_tip(w.tip),
+                       fire=P.c_fire(w.fire), scan=P.c_scan(w.scan)) for w in ws]
         self.P, self.ws = P, ws
         self.bufs = []
         self.h2d = self.d2h = 0
