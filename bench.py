@@ -255,11 +255,11 @@ class HostJob:
             s = w.scan
             hx = torch.from_numpy(w.xyzq.astype(np.float32)).pin_memory()
             ht = torch.from_numpy(w.types.astype(np.int32)).pin_memory()
-            hp = torch.empty((s.nz, s.npy, s.npx, 4), dtype=torch.float32).pin_memory()
-            hi = torch.empty((s.nz, s.npy, s.npx), dtype=torch.int16).pin_memory()
-            hd = torch.empty((s.nz - w.n_df, s.npy, s.npx), dtype=torch.float32).pin_memory()
-            self.bufs.append((hx, ht, hp, hi, hd))
             nq = len(w.Q_sweep) if w.Q_sweep else 1
+            hp = torch.empty((nq, s.nz, s.npy, s.npx, 4), dtype=torch.float32).pin_memory()
+            hi = torch.empty((nq, s.nz, s.npy, s.npx), dtype=torch.int16).pin_memory()
+            hd = torch.empty((nq, s.nz - w.n_df, s.npy, s.npx), dtype=torch.float32).pin_memory()
+            self.bufs.append((hx, ht, hp, hi, hd))
             self.h2d += nq * (hx.numel() * 4 + ht.numel() * 4)
             self.d2h += nq * (hp.numel() * 4 + hi.numel() * 2 + hd.numel() * 4 + 32)
 
@@ -278,8 +278,10 @@ class HostJob:
             self.P.scan_host_batch(self.ws, hx, ht, hp, hi, hd)
             return
         for w, (hx, ht, hp, hi, hd) in zip(self.ws, self.bufs):
-            for Q in (w.Q_sweep if w.Q_sweep else [None]):
-                self.P.scan_host(w, hx, ht, hp, hi, hd, Q=Q)
+            if w.Q_sweep:
+                self.P.scan_host_sweep(w, w.Q_sweep, hx, ht, hp, hi, hd)
+            else:
+                self.P.scan_host(w, hx, ht, hp, hi, hd)
 
 
 # ------------------------------------------------------------------------------------------------- oracle legs
@@ -637,7 +639,7 @@ def run_ours(args):
                       "relax_gather_trips_per_loop_trip": stats["warp_gathers"] / max(1, stats["warp_iters"])},
             "e2e": {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
                     "d2h_bytes_per_step": host.d2h, "ms_per_step": e2e_t * 1e3, "steps": e2e_steps,
-                    "api": "ppfm_scan_host[_batch] (pinned host buffers: inputs copied in, outputs stored by the kernels straight into host memory)"},
+                    "api": "ppfm_scan_host[_batch|_sweep] (pinned host buffers: inputs copied in, outputs stored by the kernels straight into host memory)"},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "roofline_kernels": kernels}
     if world == 1 and not args.no_cpu_baseline:
         w0 = ws[0]

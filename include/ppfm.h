@@ -248,6 +248,17 @@ int ppfm_scan_host_batch(int32_t nsys, const int32_t *h_atom_offset, const float
                          const ppfm_fire *fire, const ppfm_scan *scans, double A, double k0_Nm, double f0_Hz,
                          float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream);
 
+/* Tip-charge sweep (the LJ and electrostatic grids are separate so that the tip charge can change
+ * without recomputation; reading S19): F_LJ and the unit-charge F_el are sampled once, then for each of the nQ
+ * charges h_Q[i] the grids are combined and the scan + df run.  Outputs hold nQ consecutive result sets:
+ * h_pos_fz float[nQ][nz][npy][npx][4], h_iters uint16[nQ][nz][npy][npx], h_df float[nQ][nz-n][npy][npx]; h_stats
+ * accumulates over the sweep.  probe->Q is ignored. */
+int ppfm_scan_host_sweep(int32_t nQ, const double *h_Q, int32_t natoms, const float *h_xyzq, const int32_t *h_type,
+                         int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                         const ppfm_probe *probe, const ppfm_grid *grid, double r_min, const ppfm_tip *tip,
+                         const ppfm_fire *fire, const ppfm_scan *scan, double A, double k0_Nm, double f0_Hz,
+                         float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream);
+
 /* ---- measurement helpers (used by bench.py to define the roofline denominators on the box itself) ------------
  * ppfm_probe_fma:    FFMA-only kernel; returns lane-instructions per second in *h_lane_instr_per_s.
  * ppfm_probe_gather: the relaxation's 8-corner float4 gather over an L2-resident volume of `n_float4` entries

@@ -210,8 +210,11 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
                           int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
                           const ppfm_probe *probes, const ppfm_grid *grids, double r_min, const ppfm_tip *tips,
                           const ppfm_fire *fire, const ppfm_scan *scans, double A, double k0_Nm, double f0_Hz,
-                          float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream) {
+                          float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream,
+                          int nQ = 0, const double *h_Q = nullptr) {
     if (nsys < 1 || !h_atom_offset || !grids || !scans || !tips || !fire || !lattices || !probes) return PPFM_EINVAL;
+    if (nQ < 0 || (nQ > 0 && (!h_Q || nsys != 1))) return PPFM_EINVAL;      // the Q sweep is a single-system form
+    const int nrun = nQ > 0 ? nQ : 1;
     const int natoms = h_atom_offset[nsys];
     if (natoms < 0 || h_atom_offset[0] != 0 || (natoms > 0 && (!h_xyzq || !h_type))) return PPFM_EINVAL;
     size_t npts = 0, nps = 0;
@@ -236,6 +239,7 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
     float *m_df = (float *)mapped_alias(h_df);
     const bool zc = h_pos_fz && m_pos && (!h_iters || m_it) && (!h_df || m_df);
     float *d_xyzq = nullptr, *d_ff = nullptr, *d_pos = nullptr, *d_df = nullptr, *d_fz = nullptr;
+    float *d_lj = nullptr, *d_el = nullptr;
     int32_t *d_type = nullptr;
     uint16_t *d_it = nullptr;
     ppfm_stats *d_stats = nullptr;
@@ -246,6 +250,10 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
     TRY(scratch_alloc((void **)&d_xyzq, na * 16, st));
     TRY(scratch_alloc((void **)&d_type, na * 4, st));
     TRY(scratch_alloc((void **)&d_ff, npts * 16, st));
+    if (nQ > 0) {
+        TRY(scratch_alloc((void **)&d_lj, npts * 16, st));
+        TRY(scratch_alloc((void **)&d_el, npts * 16, st));
+    }
     TRY(scratch_alloc((void **)&d_stats, sizeof(ppfm_stats), st));
     if (zc) {
         if (h_df) TRY(scratch_alloc((void **)&d_fz, nps * 4, st));
@@ -259,29 +267,40 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
         TRY(cudaMemcpyAsync(d_type, h_type, (size_t)natoms * 4, cudaMemcpyHostToDevice, st));
     }
     TRY(cudaMemsetAsync(d_stats, 0, sizeof(ppfm_stats), st));
-    if (rc == PPFM_OK)
-        rc = (nsys == 1) ? ppfm_forcefield(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min, d_ff,
-                                           cuda_stream)
-                         : ppfm_forcefield_batch(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes,
-                                                 grids, r_min, d_ff, cuda_stream);
-    if (zc) {
-        if (rc == PPFM_OK)
-            rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, m_pos, h_iters ? m_it : nullptr, d_stats, d_fz,
-                               cuda_stream);
-        if (rc == PPFM_OK && h_df)
-            rc = df_from_fz(nsys, d_fz, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, m_df, cuda_stream);
-    } else {
-        if (rc == PPFM_OK)
-            rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, d_pos, d_it, d_stats, nullptr, cuda_stream);
-        if (rc == PPFM_OK && h_df)
-            rc = ppfm_df_batch(nsys, d_pos, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, d_df, cuda_stream);
-        if (h_pos_fz) TRY(cudaMemcpyAsync(h_pos_fz, d_pos, nps * 16, cudaMemcpyDeviceToHost, st));
-        if (h_iters) TRY(cudaMemcpyAsync(h_iters, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
-        if (h_df) TRY(cudaMemcpyAsync(h_df, d_df, ndf * 4, cudaMemcpyDeviceToHost, st));
+    if (rc == PPFM_OK) {
+        if (nQ > 0)          // S19: F_LJ and unit-charge F_el once, combined per Q
+            rc = ppfm_forcefield_split(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min, d_lj,
+                                       d_el, cuda_stream);
+        else
+            rc = (nsys == 1) ? ppfm_forcefield(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min,
+                                               d_ff, cuda_stream)
+                             : ppfm_forcefield_batch(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices,
+                                                     probes, grids, r_min, d_ff, cuda_stream);
+    }
+    for (int run = 0; run < nrun; run++) {
+        if (rc == PPFM_OK && nQ > 0) rc = ppfm_combine(d_lj, d_el, h_Q[run], (int64_t)npts, d_ff, cuda_stream);
+        const size_t op = (size_t)run * nps, od = (size_t)run * ndf;      // this run's slice of the host outputs
+        if (zc) {
+            if (rc == PPFM_OK)
+                rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, m_pos + 4 * op, h_iters ? m_it + op : nullptr,
+                                   d_stats, d_fz, cuda_stream);
+            if (rc == PPFM_OK && h_df)
+                rc = df_from_fz(nsys, d_fz, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, m_df + od,
+                                cuda_stream);
+        } else {
+            if (rc == PPFM_OK)
+                rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, d_pos, d_it, d_stats, nullptr, cuda_stream);
+            if (rc == PPFM_OK && h_df)
+                rc = ppfm_df_batch(nsys, d_pos, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, d_df,
+                                   cuda_stream);
+            if (h_pos_fz) TRY(cudaMemcpyAsync(h_pos_fz + 4 * op, d_pos, nps * 16, cudaMemcpyDeviceToHost, st));
+            if (h_iters) TRY(cudaMemcpyAsync(h_iters + op, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
+            if (h_df) TRY(cudaMemcpyAsync(h_df + od, d_df, ndf * 4, cudaMemcpyDeviceToHost, st));
+        }
     }
     if (h_stats) TRY(cudaMemcpyAsync(h_stats, d_stats, sizeof(ppfm_stats), cudaMemcpyDeviceToHost, st));
 #undef TRY
-    void *bufs[] = {d_xyzq, d_type, d_ff, d_pos, d_it, d_stats, d_df, d_fz};
+    void *bufs[] = {d_xyzq, d_type, d_ff, d_pos, d_it, d_stats, d_df, d_fz, d_lj, d_el};
     for (void *b : bufs)
         if (b) cudaFreeAsync(b, st);
     e = cudaStreamSynchronize(st);
@@ -390,4 +409,16 @@ extern "C" int ppfm_probe_gather(int64_t n_float4, int32_t bypass_l1, double *h_
     PPFM_CUDA(cudaStreamSynchronize(st));
     *h_gbs = best;
     return PPFM_OK;
+}
+
+extern "C" int ppfm_scan_host_sweep(int32_t nQ, const double *h_Q, int32_t natoms, const float *h_xyzq,
+                                    const int32_t *h_type, int32_t ntypes, const double *h_R, const double *h_e,
+                                    const ppfm_lattice *lattice, const ppfm_probe *probe, const ppfm_grid *grid,
+                                    double r_min, const ppfm_tip *tip, const ppfm_fire *fire, const ppfm_scan *scan,
+                                    double A, double k0_Nm, double f0_Hz, float *h_pos_fz, uint16_t *h_iters,
+                                    float *h_df, ppfm_stats *h_stats, void *cuda_stream) {
+    if (natoms < 0 || nQ < 1) return PPFM_EINVAL;
+    const int32_t off[2] = {0, natoms};
+    return scan_host_impl(1, off, h_xyzq, h_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, tip, fire, scan, A,
+                          k0_Nm, f0_Hz, h_pos_fz, h_iters, h_df, h_stats, cuda_stream, nQ, h_Q);
 }

@@ -63,7 +63,7 @@ class Stats(C.Structure):
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft", "ppfm_relax_scan",
            "ppfm_relax_scan_batch", "ppfm_relax_scan_tricubic", "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid",
-           "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch",
+           "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch", "ppfm_scan_host_sweep",
            "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
            "ppfm_release_scratch"]
 KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6, "relax_tricubic": 7}
@@ -452,6 +452,32 @@ def scan_host(w, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None, Q=None
 
 
 # ---- probes --------------------------------------------------------------------------------------------------------
+def scan_host_sweep(w, Qs, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None) -> dict:
+    """ppfm_scan_host_sweep: one split force-field pass, then combine + scan + df per tip charge in Qs; the host
+    outputs hold len(Qs) consecutive result sets."""
+    _torch()
+
+    def hp(x):
+        if x is None:
+            return C.c_void_p(0)
+        return C.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data)
+
+    R, pR = _darr(w.elem_R)
+    e, pe = _darr(w.elem_e)
+    Q, pQ = _darr(list(Qs))
+    st = Stats()
+    rc = lib().ppfm_scan_host_sweep(C.c_int32(len(Q)), pQ, C.c_int32(int(h_xyzq.shape[0])), hp(h_xyzq), hp(h_types),
+                                    C.c_int32(len(R)), pR, pe, C.byref(c_lattice(w.lattice)), C.byref(c_probe(w.probe)),
+                                    C.byref(c_grid(w.grid)), C.c_double(w.r_min), C.byref(c_tip(w.tip)),
+                                    C.byref(c_fire(w.fire)), C.byref(c_scan(w.scan)), C.c_double(w.df.A),
+                                    C.c_double(w.df.k0), C.c_double(w.df.f0), hp(h_pos_fz), hp(h_iters), hp(h_df),
+                                    C.byref(st), _stream())
+    _check(rc, "ppfm_scan_host_sweep")
+    return {"total_iters": int(st.total_iters), "n_not_converged": int(st.n_not_converged),
+            "n_clamped": int(st.n_clamped), "max_iters": int(st.max_iters), "warp_iters": int(st.warp_iters),
+            "cell_gathers": int(st.cell_gathers), "warp_gathers": int(st.warp_gathers)}
+
+
 def scan_host_batch(ws, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None) -> dict:
     """ppfm_scan_host_batch on a list of workloads (atoms concatenated in h_xyzq / h_types, outputs concatenated)."""
     _torch()

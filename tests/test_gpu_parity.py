@@ -647,6 +647,31 @@ def test_scan_host_equals_device_path(P):
     assert np.array_equal(h_pos2.numpy(), h_pos.numpy())
 
 
+def test_scan_host_sweep_equals_split_combine_scans(P):
+    """ppfm_scan_host_sweep = forcefield_split once + (combine, relax_scan, df) per tip charge, bit for bit."""
+    import torch
+    w = W.shrink(W.get(2), grid_n=(250, 250, 120), scan_np=(40, 24), scan_nz=14)
+    Qs = [-0.1, 0.0, 0.1]
+    s = w.scan
+    hx, ht = torch.from_numpy(w.xyzq.copy()).pin_memory(), torch.from_numpy(w.types.copy()).pin_memory()
+    hp = torch.empty((3, s.nz, s.npy, s.npx, 4), dtype=torch.float32).pin_memory()
+    hi = torch.empty((3, s.nz, s.npy, s.npx), dtype=torch.int16).pin_memory()
+    hd = torch.empty((3, s.nz - w.n_df, s.npy, s.npx), dtype=torch.float32).pin_memory()
+    st = P.scan_host_sweep(w, Qs, hx, ht, hp, hi, hd)
+    xyzq, types = P.upload(w)
+    lj, el = P.forcefield_split(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
+    tot = 0
+    for q, Q in enumerate(Qs):
+        stats = P.new_stats()
+        pos, iters = P.relax_scan(P.combine(lj, el, Q), w.grid, w.tip, w.fire, s, stats=stats)
+        df = P.df(pos, s.npx, s.npy, s.nz, s.dz, w.df.A, w.df.k0, w.df.f0)
+        torch.cuda.synchronize()
+        assert np.array_equal(hp[q].numpy(), pos.cpu().numpy()) and np.array_equal(hi[q].numpy(), iters.cpu().numpy())
+        assert np.array_equal(hd[q].numpy(), df.cpu().numpy())
+        tot += P.read_stats(stats)["total_iters"]
+    assert st["total_iters"] == tot
+
+
 def test_scan_host_batch_equals_per_system_calls(P):
     import torch
     mols = [W.shrink(m, grid_n=m.grid.n, scan_np=(24, 20), scan_nz=14) for m in W.get(3)[:4]]
