@@ -54,9 +54,9 @@ ITER_INSTR, ITER_FLOPS = 70, 114
 SMS, LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/);
 # None where no capture exists for that kernel and config.
-NCU_TRAFFIC = {(1, "ff"): 5.99e6, (1, "relax"): 13.59e6, (1, "df"): 14.41e6, (1, "stiffness"): 27.43e6,
-               (1, "fft_el"): 2.06e9, (2, "ff"): 188.5e6,
-               (3, "ff"): 1.0149e9, (3, "relax"): 512.7e6, (3, "df"): 453.8e6}      # profiles/r01d_full_cfg{1,2,3}*.txt
+NCU_TRAFFIC = {(1, "ff"): 6.59e6, (1, "relax"): 13.59e6, (1, "df"): 14.41e6, (1, "stiffness"): 27.43e6,
+               (1, "fft_el"): 2.06e9, (2, "ff"): 188.8e6,
+               (3, "ff"): 1.0149e9, (3, "relax"): 513.8e6, (3, "df"): 454.7e6}      # profiles/r01e_full_cfg{1,2,3}*.txt
 
 
 def measured_peaks():
