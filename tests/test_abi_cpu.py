@@ -100,6 +100,29 @@ def test_invalid_arguments_are_rejected_on_the_host(lib):
     assert df(*args(40, 0.1, 0.55)) == EINVAL                              # A/dz not an integer
     assert df(*args(10, 0.1, 1.0)) == EINVAL                               # nz <= n
     assert df(*args(40, 0.0, 1.0)) == EINVAL
+    # the 8(f) entry points and the host forms validate before any CUDA call too
+    td = ppfm.TipDensity(0.0, 1.0, 0.0, 0.0)                               # sigma must be > 0
+    assert lib.ppfm_forcefield_fft(fake, C.byref(gr), C.byref(td), fake, null) == EINVAL
+    td = ppfm.TipDensity(0.5, 1.0, 0.0, 0.0)
+    assert lib.ppfm_forcefield_fft(null, C.byref(gr), C.byref(td), fake, null) == EINVAL
+    assert lib.ppfm_stiffness(fake, C.byref(gr), C.byref(tip), C.byref(sc), null, fake, null) == EINVAL
+    assert lib.ppfm_stiffness(fake, C.byref(gr), C.byref(badt), C.byref(sc), fake, fake, null) == EINVAL
+    assert lib.ppfm_relax_scan_tricubic(C.c_void_p(0x1002), C.byref(gr), C.byref(tip), C.byref(fire), C.byref(sc), fake,
+                                        null, null, null) == EINVAL        # misaligned float grid
+    assert lib.ppfm_energy_grid(fake, C.c_int64(-1), fake, null) == EINVAL
+    sweep = lib.ppfm_scan_host_sweep
+    assert sweep(C.c_int32(0), pd(np.zeros(1)), C.c_int32(10), fake, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat),
+                 C.byref(pr), C.byref(gr), C.c_double(0.1), C.byref(tip), C.byref(fire), C.byref(sc), C.c_double(1.0),
+                 C.c_double(1800.0), C.c_double(30300.0), fake, null, null, null, null) == EINVAL     # no charges
+    off = (C.c_int32 * 3)(0, 5, 10)
+    grs, tips = (ppfm.Grid * 2)(gr, gr), (ppfm.Tip * 2)(tip, tip)
+    lats, prs = (ppfm.Lattice * 2)(lat, lat), (ppfm.Probe * 2)(pr, pr)
+    sc2 = ppfm.c_scan(w.scan)
+    sc2.nz = sc.nz + 1
+    scs = (ppfm.Scan * 2)(sc, sc2)
+    assert lib.ppfm_scan_host_batch(C.c_int32(2), off, fake, fake, C.c_int32(5), pd(R), pd(e), lats, prs, grs,
+                                    C.c_double(0.1), tips, C.byref(fire), scs, C.c_double(1.0), C.c_double(1800.0),
+                                    C.c_double(30300.0), fake, null, fake, null, null) == EINVAL      # df needs one shape
     assert lib.ppfm_combine(null, fake, C.c_double(0.1), C.c_int64(4), fake, null) == EINVAL
     assert lib.ppfm_df_weights(C.c_int32(0), C.c_double(0.1), pd(np.zeros(4))) == EINVAL
 
