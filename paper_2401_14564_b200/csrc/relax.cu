@@ -163,278 +163,314 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
     unsigned long long my_iters = 0;
     unsigned int my_notconv = 0, my_clamped = 0, my_max = 0, my_reloads = 0, my_witers = 0, my_wreloads = 0;
 
-    for (int iz = 0; iz < job.nzs; iz++) {
-        // a4: exact fractional grid coordinate of the spring equilibrium point, split int + frac
-        const double rz = rb[2] - iz * job.dz;
-        const AxisBase ax = axis_base(job.Minv[0] * rb[0] + job.Minv[1] * rb[1] + job.Minv[2] * rz, nx, perx);
-        const AxisBase ay = axis_base(job.Minv[3] * rb[0] + job.Minv[4] * rb[1] + job.Minv[5] * rz, ny, pery);
-        const AxisBase az = axis_base(job.Minv[6] * rb[0] + job.Minv[7] * rb[1] + job.Minv[8] * rz, nz, perz);
+    // per z-step state (set by begin_step): axis bases of the spring equilibrium point, FIRE state
+    AxisBase ax, ay, az;
+    float vx = 0.f, vy = 0.f, vz = 0.f, dt = fp.dt0, alpha = fp.alpha0;
+    int npos = 0, moves = 0;
+    bool conv = !valid;
+    float fr = 0.f, dzc = d0z, fx = 0.f, fy = 0.f, fz = 0.f;
+    // cached cell: corner forces at x0 and their x-differences for the four (y,z) edges 00, 10 (y+1), 01 (z+1),
+    // 11, and per axis tbf = (fraction of the z-step's base point) - (offset of the cached cell from the base
+    // cell), so that the position inside the cell is one FFMA: f = Minv u + tbf.  An impossible offset makes the
+    // first iteration gather.
+    float tbfx = -1.0e30f, tbfy = -1.0e30f, tbfz = -1.0e30f;
+    float c0[4][3], cd[4][3];
+#pragma unroll
+    for (int e = 0; e < 4; e++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) c0[e][c] = cd[e][c] = 0.0f;
+    // TRICUBIC: the 4 x 4 x 4 energies around the cell, [z][y][x], minus the value at the cell's own node (the
+    // gradient does not see a constant, and differences of ~|F| h keep FP32 rounding far below f_conv)
+    float en[TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1];
+    if (TRICUBIC) {
+#pragma unroll
+        for (int a = 0; a < (TRICUBIC ? 4 : 1); a++)
+#pragma unroll
+            for (int b = 0; b < (TRICUBIC ? 4 : 1); b++)
+#pragma unroll
+                for (int c = 0; c < (TRICUBIC ? 4 : 1); c++) en[a][b][c] = 0.0f;
+    }
 
-        float vx = 0.f, vy = 0.f, vz = 0.f, dt = fp.dt0, alpha = fp.alpha0;
-        int npos = 0, moves = 0;
-        bool conv = !valid;
-        float fr = 0.f, dzc = d0z, fx = 0.f, fy = 0.f, fz = 0.f;
-        // cached cell: corner forces at x0 and their x-differences for the four (y,z) edges 00, 10 (y+1), 01 (z+1),
-        // 11, and per axis tbf = (fraction of the z-step's base point) - (offset of the cached cell from the base
-        // cell), so that the position inside the cell is one FFMA: f = Minv u + tbf.  An impossible offset makes the
-        // first iteration gather.
-        float tbfx = -1.0e30f, tbfy = -1.0e30f, tbfz = -1.0e30f;
-        float c0[4][3], cd[4][3];
-#pragma unroll
-        for (int e = 0; e < 4; e++)
-#pragma unroll
-            for (int c = 0; c < 3; c++) c0[e][c] = cd[e][c] = 0.0f;
-        // TRICUBIC: the 4 x 4 x 4 energies around the cell, [z][y][x], minus the value at the cell's own node (the
-        // gradient does not see a constant, and differences of ~|F| h keep FP32 rounding far below f_conv)
-        float en[TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1];
+    auto interp = [&](float (&S)[3]) {     // nested lerps x, y, z: 10 FP32 ops per component
         if (TRICUBIC) {
+            // F_S = -grad of the tri-cubic (Catmull-Rom per axis, reading S22) interpolant of the energies:
+            // weights w and their derivatives d per axis (Horner), x pass per (z,y) row, y pass per z plane, z pass
+            float w[3][4], d[3][4];
+            const float fa[3] = {fx, fy, fz};
 #pragma unroll
-            for (int a = 0; a < (TRICUBIC ? 4 : 1); a++)
-#pragma unroll
-                for (int b = 0; b < (TRICUBIC ? 4 : 1); b++)
-#pragma unroll
-                    for (int c = 0; c < (TRICUBIC ? 4 : 1); c++) en[a][b][c] = 0.0f;
-        }
-
-        auto interp = [&](float (&S)[3]) {     // nested lerps x, y, z: 10 FP32 ops per component
-            if (TRICUBIC) {
-                // F_S = -grad of the tri-cubic (Catmull-Rom per axis, reading S22) interpolant of the energies:
-                // weights w and their derivatives d per axis (Horner), x pass per (z,y) row, y pass per z plane, z pass
-                float w[3][4], d[3][4];
-                const float fa[3] = {fx, fy, fz};
-#pragma unroll
-                for (int a = 0; a < 3; a++) {
-                    const float f = fa[a], f2 = f * f;
-                    w[a][0] = fmaf(fmaf(-0.5f, f, 1.0f), f, -0.5f) * f;
-                    w[a][1] = fmaf(fmaf(1.5f, f, -2.5f), f2, 1.0f);
-                    w[a][2] = fmaf(fmaf(-1.5f, f, 2.0f), f, 0.5f) * f;
-                    w[a][3] = fmaf(0.5f, f, -0.5f) * f2;
-                    d[a][0] = fmaf(fmaf(-1.5f, f, 2.0f), f, -0.5f);
-                    d[a][1] = fmaf(4.5f, f, -5.0f) * f;
-                    d[a][2] = fmaf(fmaf(-4.5f, f, 4.0f), f, 0.5f);
-                    d[a][3] = fmaf(1.5f, f, -1.0f) * f;
-                }
-                float Ex = 0.f, Ey = 0.f, Ez = 0.f;            // dE/dt along the three grid axes
-#pragma unroll
-                for (int k = 0; k < (TRICUBIC ? 4 : 1); k++) {
-                    float V = 0.f, DX = 0.f, DY = 0.f;
-#pragma unroll
-                    for (int j = 0; j < (TRICUBIC ? 4 : 1); j++) {
-                        const float *r = en[k][j];
-                        const float v = fmaf(w[0][3], r[TRICUBIC ? 3 : 0], fmaf(w[0][2], r[TRICUBIC ? 2 : 0], fmaf(w[0][1], r[TRICUBIC ? 1 : 0], w[0][0] * r[0])));
-                        const float dxv = fmaf(d[0][3], r[TRICUBIC ? 3 : 0], fmaf(d[0][2], r[TRICUBIC ? 2 : 0], fmaf(d[0][1], r[TRICUBIC ? 1 : 0], d[0][0] * r[0])));
-                        V = fmaf(w[1][j], v, V);
-                        DX = fmaf(w[1][j], dxv, DX);
-                        DY = fmaf(d[1][j], v, DY);
-                    }
-                    Ex = fmaf(w[2][k], DX, Ex);
-                    Ey = fmaf(w[2][k], DY, Ey);
-                    Ez = fmaf(d[2][k], V, Ez);
-                }
-                if (ORTHO) {
-                    S[0] = -m00 * Ex; S[1] = -m11 * Ey; S[2] = -m22 * Ez;
-                } else {                                         // F_c = -sum_a dE/dt_a Minv[a][c]
-                    S[0] = -fmaf(m20, Ez, fmaf(m10, Ey, m00 * Ex));
-                    S[1] = -fmaf(m21, Ez, fmaf(m11, Ey, m01 * Ex));
-                    S[2] = -fmaf(m22, Ez, fmaf(m12, Ey, m02 * Ex));
-                }
+            for (int a = 0; a < 3; a++) {
+                const float f = fa[a], f2 = f * f;
+                w[a][0] = fmaf(fmaf(-0.5f, f, 1.0f), f, -0.5f) * f;
+                w[a][1] = fmaf(fmaf(1.5f, f, -2.5f), f2, 1.0f);
+                w[a][2] = fmaf(fmaf(-1.5f, f, 2.0f), f, 0.5f) * f;
+                w[a][3] = fmaf(0.5f, f, -0.5f) * f2;
+                d[a][0] = fmaf(fmaf(-1.5f, f, 2.0f), f, -0.5f);
+                d[a][1] = fmaf(4.5f, f, -5.0f) * f;
+                d[a][2] = fmaf(fmaf(-4.5f, f, 4.0f), f, 0.5f);
+                d[a][3] = fmaf(1.5f, f, -1.0f) * f;
             }
+            float Ex = 0.f, Ey = 0.f, Ez = 0.f;            // dE/dt along the three grid axes
 #pragma unroll
-            for (int c = 0; c < (TRICUBIC ? 0 : 3); c++) {
-                const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
-                const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
-                const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
-                const float e11 = fmaf(fx, cd[3][c], c0[3][c]);
-                const float g0 = fmaf(fy, e10 - e00, e00);
-                const float g1 = fmaf(fy, e11 - e01, e01);
-                S[c] = fmaf(fz, g1 - g0, g0);
+            for (int k = 0; k < (TRICUBIC ? 4 : 1); k++) {
+                float V = 0.f, DX = 0.f, DY = 0.f;
+#pragma unroll
+                for (int j = 0; j < (TRICUBIC ? 4 : 1); j++) {
+                    const float *r = en[k][j];
+                    const float v = fmaf(w[0][3], r[TRICUBIC ? 3 : 0], fmaf(w[0][2], r[TRICUBIC ? 2 : 0], fmaf(w[0][1], r[TRICUBIC ? 1 : 0], w[0][0] * r[0])));
+                    const float dxv = fmaf(d[0][3], r[TRICUBIC ? 3 : 0], fmaf(d[0][2], r[TRICUBIC ? 2 : 0], fmaf(d[0][1], r[TRICUBIC ? 1 : 0], d[0][0] * r[0])));
+                    V = fmaf(w[1][j], v, V);
+                    DX = fmaf(w[1][j], dxv, DX);
+                    DY = fmaf(d[1][j], v, DY);
+                }
+                Ex = fmaf(w[2][k], DX, Ex);
+                Ey = fmaf(w[2][k], DY, Ey);
+                Ez = fmaf(d[2][k], V, Ez);
             }
-        };
-
-        auto fire_iteration = [&]() -> bool {
-            // ---- position inside the cached cell
             if (ORTHO) {
-                fx = fmaf(m00, ux, tbfx);
-                fy = fmaf(m11, uy, tbfy);
-                fz = fmaf(m22, uz, tbfz);
-            } else {
-                fx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, tbfx)));
-                fy = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy)));
-                fz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz)));
+                S[0] = -m00 * Ex; S[1] = -m11 * Ey; S[2] = -m22 * Ez;
+            } else {                                         // F_c = -sum_a dE/dt_a Minv[a][c]
+                S[0] = -fmaf(m20, Ez, fmaf(m10, Ey, m00 * Ex));
+                S[1] = -fmaf(m21, Ez, fmaf(m11, Ey, m01 * Ex));
+                S[2] = -fmaf(m22, Ez, fmaf(m12, Ey, m02 * Ex));
             }
-            // outside [0,1] on any axis?  As unsigned integers, negative floats and floats > 1 both exceed bits(1.0f).
-            const unsigned worst = max(max(__float_as_uint(fx), __float_as_uint(fy)), __float_as_uint(fz));
-            // ---- F_T first (the longest dependency chain: two MUFU): radial + lateral springs (Eq.2) with d = d0 + u;
-            // (|d| - R0)/|d| = (|u|^2 + 2 d0.u)/(|d|(|d| + R0))
-            float dxc = ux, dyc = uy, frk;
-            dzc = d0z + uz;
-            if (SYMTIP) {                      // d0 = (0, 0, d0z) and k_x = k_y: the usual symmetric tip
-                const float w = fmaf(ux, ux, uy * uy);
-                const float L2 = fmaf(dzc, dzc, w);
-                const float num = fmaf(uz, uz + d0z2, w);                                    // |u|^2 + 2 d0.u
-                const float L = sqrt_pinned(L2);
-                fr = (nk_rad * num) * rcp_pinned(fmaf(R_rest, L, L2));                       // -k_R (|d| - R0)/|d|
-                frk = fr + nkx;
+        }
+#pragma unroll
+        for (int c = 0; c < (TRICUBIC ? 0 : 3); c++) {
+            const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
+            const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
+            const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
+            const float e11 = fmaf(fx, cd[3][c], c0[3][c]);
+            const float g0 = fmaf(fy, e10 - e00, e00);
+            const float g1 = fmaf(fy, e11 - e01, e01);
+            S[c] = fmaf(fz, g1 - g0, g0);
+        }
+    };
+
+    auto fire_iteration = [&]() -> bool {
+        // ---- position inside the cached cell
+        if (ORTHO) {
+            fx = fmaf(m00, ux, tbfx);
+            fy = fmaf(m11, uy, tbfy);
+            fz = fmaf(m22, uz, tbfz);
+        } else {
+            fx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, tbfx)));
+            fy = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy)));
+            fz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz)));
+        }
+        // outside [0,1] on any axis?  As unsigned integers, negative floats and floats > 1 both exceed bits(1.0f).
+        const unsigned worst = max(max(__float_as_uint(fx), __float_as_uint(fy)), __float_as_uint(fz));
+        // ---- F_T first (the longest dependency chain: two MUFU): radial + lateral springs (Eq.2) with d = d0 + u;
+        // (|d| - R0)/|d| = (|u|^2 + 2 d0.u)/(|d|(|d| + R0))
+        float dxc = ux, dyc = uy, frk;
+        dzc = d0z + uz;
+        if (SYMTIP) {                      // d0 = (0, 0, d0z) and k_x = k_y: the usual symmetric tip
+            const float w = fmaf(ux, ux, uy * uy);
+            const float L2 = fmaf(dzc, dzc, w);
+            const float num = fmaf(uz, uz + d0z2, w);                                    // |u|^2 + 2 d0.u
+            const float L = sqrt_pinned(L2);
+            fr = (nk_rad * num) * rcp_pinned(fmaf(R_rest, L, L2));                       // -k_R (|d| - R0)/|d|
+            frk = fr + nkx;
+        } else {
+            dxc = d0x + ux; dyc = d0y + uy;
+            const float L2 = fmaf(dxc, dxc, fmaf(dyc, dyc, dzc * dzc));
+            const float num = fmaf(ux, ux + d0x2, fmaf(uy, uy + d0y2, uz * (uz + d0z2)));
+            const float L = sqrt_pinned(L2);
+            fr = (nk_rad * num) * rcp_pinned(fmaf(R_rest, L, L2));
+            frk = fr;
+        }
+        // ---- F_S, speculatively from the cached cell (redone below in the rare case that a lane left its cell)
+        // (the tri-cubic field is 233 instructions: not worth computing twice, it waits for the vote instead)
+        float S[3];
+        if (!TRICUBIC) interp(S);
+        if (__any_sync(0xffffffffu, worst > 0x3F800000u)) {
+            // ---- some lane's PP left its cell.  The block is warp-uniform (no reconvergence barrier on the hot
+            // path): every lane locates its cell again (magic-number floor, S12 clamp) and gathers it; lanes
+            // that had not moved get the cell they already hold, from L1.
+            float tx, ty, tz;
+            if (ORTHO) {
+                tx = fmaf(m00, ux, ax.tb);
+                ty = fmaf(m11, uy, ay.tb);
+                tz = fmaf(m22, uz, az.tb);
             } else {
-                dxc = d0x + ux; dyc = d0y + uy;
-                const float L2 = fmaf(dxc, dxc, fmaf(dyc, dyc, dzc * dzc));
-                const float num = fmaf(ux, ux + d0x2, fmaf(uy, uy + d0y2, uz * (uz + d0z2)));
-                const float L = sqrt_pinned(L2);
-                fr = (nk_rad * num) * rcp_pinned(fmaf(R_rest, L, L2));
-                frk = fr;
+                tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
+                ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
+                tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
             }
-            // ---- F_S, speculatively from the cached cell (redone below in the rare case that a lane left its cell)
-            // (the tri-cubic field is 233 instructions: not worth computing twice, it waits for the vote instead)
-            float S[3];
-            if (!TRICUBIC) interp(S);
-            if (__any_sync(0xffffffffu, worst > 0x3F800000u)) {
-                // ---- some lane's PP left its cell.  The block is warp-uniform (no reconvergence barrier on the hot
-                // path): every lane locates its cell again (magic-number floor, S12 clamp) and gathers it; lanes
-                // that had not moved get the cell they already hold, from L1.
-                float tx, ty, tz;
-                if (ORTHO) {
-                    tx = fmaf(m00, ux, ax.tb);
-                    ty = fmaf(m11, uy, ay.tb);
-                    tz = fmaf(m22, uz, az.tb);
-                } else {
-                    tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
-                    ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
-                    tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
-                }
-                int i0, j0, k0;
-                float flx, fly, flz;
-                axis_cell(tx, tx - 0.5f, ax, i0, flx);
-                axis_cell(ty, ty - 0.5f, ay, j0, fly);
-                axis_cell(tz, tz - 0.5f, az, k0, flz);
-                float4 c000, c001, c010, c011, c100, c101, c110, c111;
-                if (TRICUBIC) {
-                    // 4 x 4 x 4 stencil i0-1 .. i0+2 (reading S22).  Interior cells of the whole warp: 16 row bases and
-                    // immediate offsets.  Otherwise per-axis index lists: wrap on periodic axes, clamp to [0, n-1] on
-                    // the others.
-                    const bool inside = (i0 >= 1) & (i0 + 2 <= nx - 1) & (j0 >= 1) & (j0 + 2 <= ny - 1) & (k0 >= 1) &
-                                        (k0 + 2 <= nz - 1);
-                    if (__all_sync(0xffffffffu, inside)) {
-                        const int base = (int)((k0 - 1) * ny + (j0 - 1)) * nx + (i0 - 1);
-#pragma unroll
-                        for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
-#pragma unroll
-                            for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
-                                const float *row = ge + (base + (kk * ny + jj) * nx);
-#pragma unroll
-                                for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(row + m);
-                            }
-                    } else {
-                        int xi[4], yo[4], zo[4];
-                        int iw = i0, jw = j0, kw = k0;              // periodic: |index - [0,n)| < n after axis_cell
-                        if (perx) { iw -= (iw >= nx) ? nx : 0; iw += (iw < 0) ? nx : 0; }
-                        if (pery) { jw -= (jw >= ny) ? ny : 0; jw += (jw < 0) ? ny : 0; }
-                        if (perz) { kw -= (kw >= nz) ? nz : 0; kw += (kw < 0) ? nz : 0; }
-#pragma unroll
-                        for (int m = 0; m < 4; m++) {
-                            int a = iw + m - 1, b = jw + m - 1, c = kw + m - 1;
-                            if (perx) { a -= (a >= nx) ? nx : 0; a += (a < 0) ? nx : 0; } else a = min(max(a, 0), nx - 1);
-                            if (pery) { b -= (b >= ny) ? ny : 0; b += (b < 0) ? ny : 0; } else b = min(max(b, 0), ny - 1);
-                            if (perz) { c -= (c >= nz) ? nz : 0; c += (c < 0) ? nz : 0; } else c = min(max(c, 0), nz - 1);
-                            xi[m] = a; yo[m] = b * nx; zo[m] = c * ny * nx;
-                        }
-#pragma unroll
-                        for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
-#pragma unroll
-                            for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
-                                const int ro = zo[kk] + yo[jj];
-#pragma unroll
-                                for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(ge + (ro + xi[m]));
-                            }
-                    }
-                    const float ref = en[TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0];
+            int i0, j0, k0;
+            float flx, fly, flz;
+            axis_cell(tx, tx - 0.5f, ax, i0, flx);
+            axis_cell(ty, ty - 0.5f, ay, j0, fly);
+            axis_cell(tz, tz - 0.5f, az, k0, flz);
+            float4 c000, c001, c010, c011, c100, c101, c110, c111;
+            if (TRICUBIC) {
+                // 4 x 4 x 4 stencil i0-1 .. i0+2 (reading S22).  Interior cells of the whole warp: 16 row bases and
+                // immediate offsets.  Otherwise per-axis index lists: wrap on periodic axes, clamp to [0, n-1] on
+                // the others.
+                const bool inside = (i0 >= 1) & (i0 + 2 <= nx - 1) & (j0 >= 1) & (j0 + 2 <= ny - 1) & (k0 >= 1) &
+                                    (k0 + 2 <= nz - 1);
+                if (__all_sync(0xffffffffu, inside)) {
+                    const int base = (int)((k0 - 1) * ny + (j0 - 1)) * nx + (i0 - 1);
 #pragma unroll
                     for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
 #pragma unroll
-                        for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++)
+                        for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
+                            const float *row = ge + (base + (kk * ny + jj) * nx);
 #pragma unroll
-                            for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] -= ref;
-                } else if (!ANYPER) {
-                    const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
-                    c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
-                    c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
-                    c100 = ldg_corner(p + sz);      c101 = ldg_corner(p + sz + 1);
-                    c110 = ldg_corner(p + sz + sy); c111 = ldg_corner(p + sz + sy + 1);
+                            for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(row + m);
+                        }
                 } else {
-                    if (perx) { i0 -= (i0 >= nx) ? nx : 0; i0 += (i0 < 0) ? nx : 0; }
-                    if (pery) { j0 -= (j0 >= ny) ? ny : 0; j0 += (j0 < 0) ? ny : 0; }
-                    if (perz) { k0 -= (k0 >= nz) ? nz : 0; k0 += (k0 < 0) ? nz : 0; }
-                    const int i1 = (i0 + 1 == nx) ? 0 : i0 + 1;       // non-periodic axes never reach n - 1
-                    const int j1 = (j0 + 1 == ny) ? 0 : j0 + 1;
-                    const int k1 = (k0 + 1 == nz) ? 0 : k0 + 1;
-                    const float4 *r00 = g + (long long)(k0 * ny + j0) * nx, *r01 = g + (long long)(k0 * ny + j1) * nx;
-                    const float4 *r10 = g + (long long)(k1 * ny + j0) * nx, *r11 = g + (long long)(k1 * ny + j1) * nx;
-                    c000 = ldg_corner(r00 + i0); c001 = ldg_corner(r00 + i1);
-                    c010 = ldg_corner(r01 + i0); c011 = ldg_corner(r01 + i1);
-                    c100 = ldg_corner(r10 + i0); c101 = ldg_corner(r10 + i1);
-                    c110 = ldg_corner(r11 + i0); c111 = ldg_corner(r11 + i1);
+                    int xi[4], yo[4], zo[4];
+                    int iw = i0, jw = j0, kw = k0;              // periodic: |index - [0,n)| < n after axis_cell
+                    if (perx) { iw -= (iw >= nx) ? nx : 0; iw += (iw < 0) ? nx : 0; }
+                    if (pery) { jw -= (jw >= ny) ? ny : 0; jw += (jw < 0) ? ny : 0; }
+                    if (perz) { kw -= (kw >= nz) ? nz : 0; kw += (kw < 0) ? nz : 0; }
+#pragma unroll
+                    for (int m = 0; m < 4; m++) {
+                        int a = iw + m - 1, b = jw + m - 1, c = kw + m - 1;
+                        if (perx) { a -= (a >= nx) ? nx : 0; a += (a < 0) ? nx : 0; } else a = min(max(a, 0), nx - 1);
+                        if (pery) { b -= (b >= ny) ? ny : 0; b += (b < 0) ? ny : 0; } else b = min(max(b, 0), ny - 1);
+                        if (perz) { c -= (c >= nz) ? nz : 0; c += (c < 0) ? nz : 0; } else c = min(max(c, 0), nz - 1);
+                        xi[m] = a; yo[m] = b * nx; zo[m] = c * ny * nx;
+                    }
+#pragma unroll
+                    for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
+#pragma unroll
+                        for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++) {
+                            const int ro = zo[kk] + yo[jj];
+#pragma unroll
+                            for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] = __ldg(ge + (ro + xi[m]));
+                        }
                 }
-                tbfx = ax.tb - flx; tbfy = ay.tb - fly; tbfz = az.tb - flz;
-                if (ORTHO) {
-                    fx = __saturatef(fmaf(m00, ux, tbfx));
-                    fy = __saturatef(fmaf(m11, uy, tbfy));
-                    fz = __saturatef(fmaf(m22, uz, tbfz));
-                } else {
-                    fx = __saturatef(fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, tbfx))));
-                    fy = __saturatef(fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy))));
-                    fz = __saturatef(fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz))));
-                }
-                if (!TRICUBIC) {
-                c0[0][0] = c000.x; c0[0][1] = c000.y; c0[0][2] = c000.z;
-                c0[1][0] = c010.x; c0[1][1] = c010.y; c0[1][2] = c010.z;
-                c0[2][0] = c100.x; c0[2][1] = c100.y; c0[2][2] = c100.z;
-                c0[3][0] = c110.x; c0[3][1] = c110.y; c0[3][2] = c110.z;
-                cd[0][0] = c001.x - c000.x; cd[0][1] = c001.y - c000.y; cd[0][2] = c001.z - c000.z;
-                cd[1][0] = c011.x - c010.x; cd[1][1] = c011.y - c010.y; cd[1][2] = c011.z - c010.z;
-                cd[2][0] = c101.x - c100.x; cd[2][1] = c101.y - c100.y; cd[2][2] = c101.z - c100.z;
-                cd[3][0] = c111.x - c110.x; cd[3][1] = c111.y - c110.y; cd[3][2] = c111.z - c110.z;
-                }
-                my_reloads += (worst > 0x3F800000u) ? 1u : 0u;
-                my_wreloads++;
-                if (!TRICUBIC) interp(S);
-            }
-            if (TRICUBIC) interp(S);
-            float Fx, Fy, Fz;
-            if (SYMTIP) {
-                Fx = fmaf(frk, ux, S[0]);
-                Fy = fmaf(frk, uy, S[1]);
+                const float ref = en[TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0][TRICUBIC ? 1 : 0];
+#pragma unroll
+                for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
+#pragma unroll
+                    for (int jj = 0; jj < (TRICUBIC ? 4 : 1); jj++)
+#pragma unroll
+                        for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] -= ref;
+            } else if (!ANYPER) {
+                const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
+                c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
+                c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
+                c100 = ldg_corner(p + sz);      c101 = ldg_corner(p + sz + 1);
+                c110 = ldg_corner(p + sz + sy); c111 = ldg_corner(p + sz + sy + 1);
             } else {
-                Fx = fmaf(fr, dxc, fmaf(nkx, ux, S[0]));
-                Fy = fmaf(fr, dyc, fmaf(nky, uy, S[1]));
+                if (perx) { i0 -= (i0 >= nx) ? nx : 0; i0 += (i0 < 0) ? nx : 0; }
+                if (pery) { j0 -= (j0 >= ny) ? ny : 0; j0 += (j0 < 0) ? ny : 0; }
+                if (perz) { k0 -= (k0 >= nz) ? nz : 0; k0 += (k0 < 0) ? nz : 0; }
+                const int i1 = (i0 + 1 == nx) ? 0 : i0 + 1;       // non-periodic axes never reach n - 1
+                const int j1 = (j0 + 1 == ny) ? 0 : j0 + 1;
+                const int k1 = (k0 + 1 == nz) ? 0 : k0 + 1;
+                const float4 *r00 = g + (long long)(k0 * ny + j0) * nx, *r01 = g + (long long)(k0 * ny + j1) * nx;
+                const float4 *r10 = g + (long long)(k1 * ny + j0) * nx, *r11 = g + (long long)(k1 * ny + j1) * nx;
+                c000 = ldg_corner(r00 + i0); c001 = ldg_corner(r00 + i1);
+                c010 = ldg_corner(r01 + i0); c011 = ldg_corner(r01 + i1);
+                c100 = ldg_corner(r10 + i0); c101 = ldg_corner(r10 + i1);
+                c110 = ldg_corner(r11 + i0); c111 = ldg_corner(r11 + i1);
             }
-            Fz = fmaf(fr, dzc, S[2]);
-            // ---- the part of FIRE that needs only the old velocity (reading S6), off the critical path
-            const float vn = sqrt_fast(fmaf(vx, vx, fmaf(vy, vy, vz * vz)));
-            const float av = alpha * vn, om = 1.0f - alpha;
-            const bool grow = npos > fp.n_min;
-            const float dt_pos = grow ? fminf(dt * fp.finc, fp.dt_max) : dt;
-            const float al_pos = grow ? alpha * fp.falpha : alpha;
-            const float dt_neg = dt * fp.fdec;
-            const float F2 = fmaf(Fx, Fx, fmaf(Fy, Fy, Fz * Fz));
-            const float Pw = fmaf(Fx, vx, fmaf(Fy, vy, Fz * vz));
-            conv = conv || (F2 < fp.fconv2);                     // tested before every move (reading S7)
-            const bool done = conv || (moves >= fp.max_iter);
-            // ---- FIRE step, branch-free; P >= 0 counts as downhill
-            const bool down = Pw >= 0.0f;
-            const float omv = down ? om : 0.0f;
-            const float s = down ? fmaf(av, rsqrt_fast(F2), dt_pos) : dt_neg;
-            vx = fmaf(s, Fx, omv * vx);
-            vy = fmaf(s, Fy, omv * vy);
-            vz = fmaf(s, Fz, omv * vz);
-            dt = down ? dt_pos : dt_neg;
-            alpha = down ? al_pos : fp.alpha0;
-            npos = down ? npos + 1 : 0;
-            if (!done) {                                         // finished lanes stay where they are
-                ux = fmaf(vx, dt, ux); uy = fmaf(vy, dt, uy); uz = fmaf(vz, dt, uz);
-                moves++;
+            tbfx = ax.tb - flx; tbfy = ay.tb - fly; tbfz = az.tb - flz;
+            if (ORTHO) {
+                fx = __saturatef(fmaf(m00, ux, tbfx));
+                fy = __saturatef(fmaf(m11, uy, tbfy));
+                fz = __saturatef(fmaf(m22, uz, tbfz));
+            } else {
+                fx = __saturatef(fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, tbfx))));
+                fy = __saturatef(fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, tbfy))));
+                fz = __saturatef(fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz))));
             }
-            return done;
-        };
+            if (!TRICUBIC) {
+            c0[0][0] = c000.x; c0[0][1] = c000.y; c0[0][2] = c000.z;
+            c0[1][0] = c010.x; c0[1][1] = c010.y; c0[1][2] = c010.z;
+            c0[2][0] = c100.x; c0[2][1] = c100.y; c0[2][2] = c100.z;
+            c0[3][0] = c110.x; c0[3][1] = c110.y; c0[3][2] = c110.z;
+            cd[0][0] = c001.x - c000.x; cd[0][1] = c001.y - c000.y; cd[0][2] = c001.z - c000.z;
+            cd[1][0] = c011.x - c010.x; cd[1][1] = c011.y - c010.y; cd[1][2] = c011.z - c010.z;
+            cd[2][0] = c101.x - c100.x; cd[2][1] = c101.y - c100.y; cd[2][2] = c101.z - c100.z;
+            cd[3][0] = c111.x - c110.x; cd[3][1] = c111.y - c110.y; cd[3][2] = c111.z - c110.z;
+            }
+            my_reloads += (worst > 0x3F800000u) ? 1u : 0u;
+            my_wreloads++;
+            if (!TRICUBIC) interp(S);
+        }
+        if (TRICUBIC) interp(S);
+        float Fx, Fy, Fz;
+        if (SYMTIP) {
+            Fx = fmaf(frk, ux, S[0]);
+            Fy = fmaf(frk, uy, S[1]);
+        } else {
+            Fx = fmaf(fr, dxc, fmaf(nkx, ux, S[0]));
+            Fy = fmaf(fr, dyc, fmaf(nky, uy, S[1]));
+        }
+        Fz = fmaf(fr, dzc, S[2]);
+        // ---- the part of FIRE that needs only the old velocity (reading S6), off the critical path
+        const float vn = sqrt_fast(fmaf(vx, vx, fmaf(vy, vy, vz * vz)));
+        const float av = alpha * vn, om = 1.0f - alpha;
+        const bool grow = npos > fp.n_min;
+        const float dt_pos = grow ? fminf(dt * fp.finc, fp.dt_max) : dt;
+        const float al_pos = grow ? alpha * fp.falpha : alpha;
+        const float dt_neg = dt * fp.fdec;
+        const float F2 = fmaf(Fx, Fx, fmaf(Fy, Fy, Fz * Fz));
+        const float Pw = fmaf(Fx, vx, fmaf(Fy, vy, Fz * vz));
+        conv = conv || (F2 < fp.fconv2);                     // tested before every move (reading S7)
+        const bool done = conv || (moves >= fp.max_iter);
+        // ---- FIRE step, branch-free; P >= 0 counts as downhill
+        const bool down = Pw >= 0.0f;
+        const float omv = down ? om : 0.0f;
+        const float s = down ? fmaf(av, rsqrt_fast(F2), dt_pos) : dt_neg;
+        vx = fmaf(s, Fx, omv * vx);
+        vy = fmaf(s, Fy, omv * vy);
+        vz = fmaf(s, Fz, omv * vz);
+        dt = down ? dt_pos : dt_neg;
+        alpha = down ? al_pos : fp.alpha0;
+        npos = down ? npos + 1 : 0;
+        if (!done) {                                         // finished lanes stay where they are
+            ux = fmaf(vx, dt, ux); uy = fmaf(vy, dt, uy); uz = fmaf(vz, dt, uz);
+            moves++;
+        }
+        return done;
+    };
 
+    // start of a z-step (O7): FIRE state reset, the displacement u is carried over; the cached cell is dropped
+    auto reset_step = [&]() {
+        vx = vy = vz = 0.f; dt = fp.dt0; alpha = fp.alpha0;
+        npos = 0; moves = 0;
+        conv = !valid;
+        tbfx = tbfy = tbfz = -1.0e30f;
+    };
+    // end of a z-step (O8): outputs of this pixel at tip height index iz
+    auto finish_step = [&](int iz) {
+        const double rz = rb[2] - iz * job.dz;
+        const size_t o = (size_t)job.out_offset + ((size_t)iz * job.npy + iy) * job.npx + ix;
+        float4 outv;
+        outv.x = (float)(rb[0] + job.origin[0] + (double)ux);
+        outv.y = (float)(rb[1] + job.origin[1] + (double)uy);
+        outv.z = (float)(rz + job.origin[2] + (double)uz);
+        outv.w = -fr * dzc;                           // Fz_tip = -F_R,z
+        pos_fz[o] = outv;
+        if (fz_out) fz_out[o] = outv.w;
+        if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
+        float tx, ty, tz;
+        if (ORTHO) {
+            tx = fmaf(m00, ux, ax.tb); ty = fmaf(m11, uy, ay.tb); tz = fmaf(m22, uz, az.tb);
+        } else {
+            tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
+            ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
+            tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
+        }
+        const bool clamped = (tx < ax.lo) | (tx > ax.hi) | (ty < ay.lo) | (ty > ay.hi) | (tz < az.lo) | (tz > az.hi);
+        my_iters += (unsigned)moves;
+        my_notconv += conv ? 0u : 1u;
+        my_clamped += clamped ? 1u : 0u;
+        my_max = max(my_max, (unsigned)moves);
+    };
+
+    for (int iz = 0; iz < job.nzs; iz++) {
+        // a4: exact fractional grid coordinate of the spring equilibrium point, split int + frac
+        const double rz = rb[2] - iz * job.dz;
+        ax = axis_base(job.Minv[0] * rb[0] + job.Minv[1] * rb[1] + job.Minv[2] * rz, nx, perx);
+        ay = axis_base(job.Minv[3] * rb[0] + job.Minv[4] * rb[1] + job.Minv[5] * rz, ny, pery);
+        az = axis_base(job.Minv[6] * rb[0] + job.Minv[7] * rb[1] + job.Minv[8] * rz, nz, perz);
+        reset_step();
         // the convergence vote is taken every second iteration: finished lanes do not move, so an extra iteration
         // changes nothing but saves one VOTE + branch per iteration
         while (true) {
@@ -443,31 +479,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             my_witers += 2;
             if (__all_sync(0xffffffffu, done)) break;
         }
-
-        if (valid) {
-            const size_t o = (size_t)job.out_offset + ((size_t)iz * job.npy + iy) * job.npx + ix;
-            float4 outv;
-            outv.x = (float)(rb[0] + job.origin[0] + (double)ux);
-            outv.y = (float)(rb[1] + job.origin[1] + (double)uy);
-            outv.z = (float)(rz + job.origin[2] + (double)uz);
-            outv.w = -fr * dzc;                           // Fz_tip = -F_R,z
-            pos_fz[o] = outv;
-            if (fz_out) fz_out[o] = outv.w;
-            if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
-            float tx, ty, tz;
-            if (ORTHO) {
-                tx = fmaf(m00, ux, ax.tb); ty = fmaf(m11, uy, ay.tb); tz = fmaf(m22, uz, az.tb);
-            } else {
-                tx = fmaf(m00, ux, fmaf(m01, uy, fmaf(m02, uz, ax.tb)));
-                ty = fmaf(m10, ux, fmaf(m11, uy, fmaf(m12, uz, ay.tb)));
-                tz = fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, az.tb)));
-            }
-            const bool clamped = (tx < ax.lo) | (tx > ax.hi) | (ty < ay.lo) | (ty > ay.hi) | (tz < az.lo) | (tz > az.hi);
-            my_iters += (unsigned)moves;
-            my_notconv += conv ? 0u : 1u;
-            my_clamped += clamped ? 1u : 0u;
-            my_max = max(my_max, (unsigned)moves);
-        }
+        if (valid) finish_step(iz);
     }
 
     if (stats) {
