@@ -5,17 +5,23 @@
 // (PAPER.md:62).
 //
 // Kernel design.  One thread per pixel, the whole z stroke inside the kernel (state in registers);
-// a warp covers an 8 x 4 pixel patch so that the 8-corner float4 gathers of neighbouring lanes fall into the same
-// 128-byte lines (L1 hit rate > 99 %).  A FIRE iteration is a strictly dependent chain (position -> cell -> 8 loads
-// -> force -> step), so with few pixels the kernel runs at the speed of that chain and with many pixels at the
-// speed of instruction issue; both want the fewest instructions on the chain:
-//   * cell index and fraction by the magic-number trick (t - 0.5 + 1.5*2^23 rounds to floor(t) in the low mantissa
-//     bits; clamps are two FMNMX in that domain, the fraction is one saturating subtract) — no F2I/I2F, no branches;
-//   * all eight LDG.128 are issued back to back (asm volatile) before any use, weights are formed while they fly,
-//     and the spring force seeds the interpolation accumulators;
-//   * FIRE is branch-free: everything that depends only on the old velocity (|v|, (1-a)v, both dt candidates) is
-//     computed under the loads; after F arrives the chain is F.F -> rsqrt -> one select -> two FMA per component;
-//   * the loop exit is one __all_sync vote placed after the (predicated) move, so it overlaps the update.
+// a warp covers an 8 x 4 pixel patch so that the gathers of neighbouring lanes fall into the same 128-byte lines.
+// A FIRE iteration is a strictly dependent chain (position -> force -> step), so with few pixels the kernel runs at
+// the latency of that chain and with many pixels at the speed of instruction issue; both want the fewest
+// instructions per iteration:
+//   * the lane keeps the 8 corner forces of its current grid cell in registers (corner values + x-differences) and
+//     the per-axis offset that turns the position into the in-cell fraction with one FFMA; the probe particle leaves
+//     its cell in 2-3 % of iterations, and only then the warp (all lanes, one warp-uniform block entered through
+//     __any_sync) re-locates and re-gathers: cell index and fraction by the magic-number trick (t - 0.5 + 1.5*2^23
+//     rounds to floor(t) in the low mantissa bits; clamps are two FMNMX in that domain), eight LDG.128 issued back
+//     to back;
+//   * the interpolation (nested lerps) is computed speculatively from the cached cell ahead of that branch, the
+//     spring chain's two MUFU are pinned ahead of it too (asm volatile: see sqrt_pinned);
+//   * FIRE is branch-free: everything that depends only on the old velocity is computed off the critical path; after
+//     F arrives the chain is F.F -> rsqrt -> one select -> two FMA per component;
+//   * the convergence vote (__all_sync) is taken every second iteration: finished lanes do not move.
+// The same function, templated on the interpolant, serves the tri-cubic energy-only variant: 64
+// energies of the 4 x 4 x 4 stencil in registers instead of the 8 corner forces.
 // FP32 with two precautions that keep |F| < 1e-6 eV/Å reachable:
 //   * the state is the displacement u = d - d0 from the spring equilibrium, and the radial extension is
 //     |d| - R0 = (|u|^2 + 2 d0.u)/(|d| + R0) (no cancellation);
