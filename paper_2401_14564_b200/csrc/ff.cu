@@ -3,14 +3,17 @@
 // images at every point of a uniform grid, forces as F = -grad E.
 //
 // Kernel design (B200 / sm_100a; nothing here is a dense contraction, so no tensor cores):
-//   * a1  `ff_prep_kernel` packs one 32-byte record per atom (x, y, z, k_e q_PP q_i | c6, c12, 6 c6, k_e q_i).
+//   * a1  `ff_prep_kernel` (one CTA per system) packs one 48-byte record per atom (x, y, z, - | c12, c12, -c6, -c6 |
+//         6 c6, 6 c6, kq, kq: the pair coefficients twice, so that LDS.128 yields aligned FP32x2 operand pairs) and
+//         stable-partitions the records: atoms with a Coulomb factor first, LJ-only atoms behind them.
 //   * a2  `ff_kernel`: one CTA = 256 columns (consecutive x-fastest (i,j) indices, so a warp's float4 stores are
-//         512 contiguous bytes) x P consecutive z planes held in registers.  Atom records stream through a
-//         4-stage shared-memory ring filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx), one
-//         elected thread producing two chunks ahead; every warp reads records as uniform (broadcast) LDS.128.
+//         512 contiguous bytes) x P consecutive z planes held in registers as P/2 FP32x2 pairs.  Atom records stream
+//         through a 3-stage shared-memory ring filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx),
+//         one elected thread producing two chunks ahead; every warp reads records as uniform (broadcast) LDS.128.
 //         Images are the outer loop and are applied as a shift of the grid point; the shifted point is formed in
 //         FP64 once per image and split hi+lo so that dx = (p_hi - a) + p_lo carries no coordinate rounding.
-//         Per pair and grid point: 15 FP32-pipe instructions + 1 MUFU.RSQ (+1 FMNMX when the r_min clamp is
+//         The inner loop is sm_100's packed FP32x2 arithmetic (FFMA2 / FMUL2 / FADD2): per pair of grid points and
+//         atom 15 packed instructions + 2 MUFU.RSQ (13 + 2 for an LJ-only atom; +2 FMNMX when the r_min clamp is
 //         live, which the prep kernel decides from the atoms' distance to the grid's bounding box).
 //   * a3  `combine_kernel`: F = F_LJ + Q F_el, float4 streaming.
 #include "common.cuh"
