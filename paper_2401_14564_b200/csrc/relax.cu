@@ -170,7 +170,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
     unsigned int my_notconv = 0, my_clamped = 0, my_max = 0, my_reloads = 0, my_witers = 0, my_wreloads = 0;
 
     // per z-step state (set by begin_step): axis bases of the spring equilibrium point, FIRE state
-    AxisBase ax, ay, az;
+    AxisBase ax = {}, ay = {}, az = {};
     float vx = 0.f, vy = 0.f, vz = 0.f, dt = fp.dt0, alpha = fp.alpha0;
     int npos = 0, moves = 0;
     bool conv = !valid;
