@@ -218,6 +218,27 @@ def fft_forcefield_at(V, grid, sigma: float, q_s: float, p_z: float, Q_zz: float
     return out
 
 
+def pauli_forcefield(rho_S, grid, sigma: float, q: float, A: float, beta: float) -> np.ndarray:
+    """O14 (Eq.8; reading S23): E(R) = A sum_r [rho_PP(r) rho_S(r + R)]^beta dV and F = -grad_R E on
+    the periodic grid by direct O(N^2) sums; rho_PP = q g_sigma.  rho_S (nz, ny, nx) -> (nz, ny, nx, 4)."""
+    S = np.ascontiguousarray(np.maximum(np.asarray(rho_S, dtype=np.float64), 0.0) ** beta)
+    step = np.ascontiguousarray(np.asarray(grid.step, dtype=np.float64).reshape(9))
+    n = _i(grid.n)
+    T4 = np.empty((4,) + S.shape)
+    rc = lib().oracle_pauli_tip(_p(step), _p(n), C.c_double(sigma), C.c_double(q), C.c_double(beta), _p(T4))
+    if rc:
+        raise ValueError(f"oracle_pauli_tip rc={rc}")
+    dV = abs(float(np.linalg.det(np.asarray(grid.step, dtype=np.float64))))
+    out = np.empty(S.shape + (4,))
+    tmp = np.empty(S.shape)
+    for c, lane in ((0, 3), (1, 0), (2, 1), (3, 2)):
+        rc = lib().oracle_crosscorr(_p(n), _p(np.ascontiguousarray(T4[c])), _p(S), C.c_double(dV * A), _p(tmp))
+        if rc:
+            raise ValueError(f"oracle_crosscorr rc={rc}")
+        out[..., lane] = tmp
+    return out
+
+
 def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None, traj: bool = True):
     """O4-O8 (+O10).  Returns dict: pos_fz (nz, npix, 4), iters (nz, npix) [-1 = not converged],
     lam_min (nz, npix), clamped (nz, npix), lam_traj (nz, npix; smallest Hessian eigenvalue along the step's FIRE

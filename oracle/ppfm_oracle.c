@@ -22,6 +22,7 @@
  *   O10 stability flag (Hessian)         north_star exemption; reading S14
  *   O11 stiffness map (IETS)
  *   O13 tri-cubic interpolation of E     PAPER.md:264 ("tri-cubic interpolation of the potential"); reading S22
+ *   O14 FDBM Pauli repulsion, Eq.8       PAPER.md:118-122; reading S23
  *   O12 grid electrostatics, Eq.7        PAPER.md:102-111 (cross-correlation), 270 (convolution theorem); reading S21
  *
  * Pins: tests/test_oracle_pins.py (closed forms, invariants, brute force).  "Relaxed positions on the real
@@ -522,6 +523,40 @@ int oracle_crosscorr_at(const int *n, const double *rho, const double *V, double
         }
         out[m] = acc * dV;
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * O14: Pauli repulsion of the full density-based model (Eq.8):
+ *     E_Pauli(R) = A integral [ rho_PP(r) rho_S(r + R) ]^beta dr,      F = -grad_R E_Pauli.
+ * Reading S23: on the periodic grid as in S21; rho_PP = q g_sigma(r) (a Gaussian electron density of q electrons,
+ * positive, so the power is defined); rho_S is clipped at 0 before the power.  This routine only tabulates the tip
+ * factor literally, T0 = (q g)^beta and its analytic gradient T_a = beta (q g)^(beta-1) q dg/dr_a; the sums are
+ * oracle_crosscorr(T, rho_S^beta) (the integrand factorises: [ab]^beta = a^beta b^beta for a, b >= 0).
+ * ---------------------------------------------------------------------------------------------------------- */
+int oracle_pauli_tip(const double *step /* [3][3] */, const int *n, double sigma, double q, double beta,
+                     double *T4 /* [4][nz][ny][nx]: T0, dT0/dx, dT0/dy, dT0/dz */) {
+    if (!(sigma > 0.0) || !(q > 0.0) || !(beta > 0.0)) return -1;
+    const int64_t N = (int64_t)n[0] * n[1] * n[2];
+    const double s2 = sigma * sigma;
+    const double norm = pow(2.0 * M_PI * s2, -1.5);
+    for (int k = 0; k < n[2]; k++)
+        for (int j = 0; j < n[1]; j++)
+            for (int i = 0; i < n[0]; i++) {
+                const int iw = (2 * i >= n[0]) ? i - n[0] : i;
+                const int jw = (2 * j >= n[1]) ? j - n[1] : j;
+                const int kw = (2 * k >= n[2]) ? k - n[2] : k;
+                double r[3];
+                for (int c = 0; c < 3; c++) r[c] = iw * step[0 + c] + jw * step[3 + c] + kw * step[6 + c];
+                const double rr = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+                const double rho = q * norm * exp(-rr / (2.0 * s2));          /* rho_PP(r) */
+                const int64_t m = ((int64_t)k * n[1] + j) * n[0] + i;
+                T4[m] = pow(rho, beta);
+                for (int c = 0; c < 3; c++) {
+                    const double drho = -rho * r[c] / s2;                     /* d rho_PP / d r_c */
+                    T4[(c + 1) * N + m] = (rho > 0.0) ? beta * pow(rho, beta - 1.0) * drho : 0.0;
+                }
+            }
     return 0;
 }
 

@@ -745,6 +745,58 @@ def test_tricubic_relaxation_linear_field_closed_form_and_periodic_seam():
     assert np.allclose(F[0, 0], 2 * np.pi / 6.0 * np.sin(2 * np.pi * 5.9 / 6.0), atol=2e-3)   # cubic accuracy only
 
 
+# ---------------------------------------------------------------------------------------------------- O14 (Eq.8)
+def test_eq8_pauli_overlap_pins():
+    """PAPER.md:118-122, Eq.8.  (i) A literal loop of A sum_r [rho_PP(r) rho_S(r+R)]^beta dV on a 5 x 4 x 3 grid;
+    (ii) beta = 1 is A times the overlap integral = Eq.7 with V := rho_S and a monopole tip (O12, pinned above);
+    (iii) a Gaussian to the power beta is a Gaussian: (q g_s)^beta = q^beta (2 pi s^2)^(3(1-beta)/2) beta^(-3/2)
+    g_{s/sqrt(beta)}, so Eq.8 equals Eq.7 on rho_S^beta with that tip (closed form of the tip factor);
+    (iv) plane-wave density rho_S^beta = c + a cos(k.r): E and F in closed form."""
+    rng = np.random.default_rng(12)
+    step = np.diag([0.3, 0.35, 0.4])
+    g = W.Grid(origin=np.zeros(3), step=step, n=(5, 4, 3), periodic=(1, 1, 1))
+    rho = rng.uniform(0.0, 0.5, (3, 4, 5))
+    s, q, A, beta = 0.35, 1.7, 12.0, 1.2
+    got = oracle.pauli_forcefield(rho, g, s, q, A, beta)
+    dV = 0.3 * 0.35 * 0.4
+    for K in range(3):
+        for J in range(4):
+            for I in range(5):
+                acc = 0.0
+                for k in range(3):
+                    for j in range(4):
+                        for i in range(5):
+                            r = np.array([(i - 5 if 2 * i >= 5 else i) * 0.3, (j - 4 if 2 * j >= 4 else j) * 0.35,
+                                          (k - 3 if 2 * k >= 3 else k) * 0.4])
+                            rpp = q * (2 * np.pi * s * s) ** -1.5 * np.exp(-(r @ r) / (2 * s * s))
+                            acc += (rpp * rho[(k + K) % 3, (j + J) % 4, (i + I) % 5]) ** beta
+                assert np.isclose(got[K, J, I, 3], A * acc * dV, rtol=1e-12)
+    # (ii), (iii) on a larger grid
+    g2 = _fft_grid()
+    rho2 = rng.uniform(0.0, 0.3, (16, 20, 24))
+    one = oracle.pauli_forcefield(rho2, g2, 0.4, 1.3, 5.0, 1.0)
+    assert np.allclose(one, 5.0 * oracle.fft_forcefield(rho2, g2, 0.4, 1.3, 0.0, 0.0), rtol=1e-12, atol=1e-14)
+    for beta in (0.9, 1.1, 1.3):
+        s, q, A = 0.45, 1.3, 5.0
+        lit = oracle.pauli_forcefield(rho2, g2, s, q, A, beta)
+        qeff = A * q**beta * (2 * np.pi * s * s) ** (1.5 * (1 - beta)) * beta ** -1.5
+        ident = oracle.fft_forcefield(rho2**beta, g2, s / np.sqrt(beta), qeff, 0.0, 0.0)
+        assert np.allclose(lit, ident, rtol=1e-10, atol=1e-12), beta
+    # (iv) closed form for a plane-wave rho_S^beta
+    n, h = np.array(g2.n), np.diag(np.asarray(g2.step))
+    L = n * h
+    kvec = 2 * np.pi * np.array([1, 0, -1]) / L
+    Kz, Jy, Ix = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+    arg = np.stack([Ix * h[0], Jy * h[1], Kz * h[2]], axis=-1) @ kvec
+    beta, s, q, A = 1.2, 0.4, 1.0, 3.0
+    Sb = 0.5 + 0.3 * np.cos(arg)                                          # rho_S^beta
+    got = oracle.pauli_forcefield(Sb ** (1 / beta), g2, s, q, A, beta)
+    qeff = A * q**beta * (2 * np.pi * s * s) ** (1.5 * (1 - beta)) * beta ** -1.5
+    damp = np.exp(-0.5 * (s * s / beta) * kvec @ kvec)
+    assert np.allclose(got[..., 3], qeff * (0.5 + 0.3 * damp * np.cos(arg)), atol=1e-6)
+    assert np.allclose(got[..., :3], qeff * 0.3 * damp * np.sin(arg)[..., None] * kvec, atol=1e-6)
+
+
 def test_golden_constants_are_what_the_generators_use():
     assert W.EVA2_PER_NM == pytest.approx(1.0 / NM, rel=1e-15)
     assert W.ELEM_R[:4].tolist() == [GOLD["R_H"], GOLD["R_C"], GOLD["R_N"], GOLD["R_O"]]
