@@ -180,6 +180,15 @@ typedef struct {
 int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, const ppfm_tip_density *tip, float *d_ff,
                         void *cuda_stream);
 
+/* ---- (1c) Pauli repulsion of the full density-based model, Eq.8 ---------------------------------
+ *     E_Pauli(R) = A integral [ rho_PP(r) rho_S(r + R) ]^beta dr,   F = -grad_R E_Pauli,
+ * on the periodic grid as in (1b), with rho_PP = q_tip g_sigma(r) (a Gaussian electron density of q_tip > 0 electrons).
+ * d_rho_S  DEVICE float[nz][ny][nx]: sample electron density (e/Å^3); negative values are clipped to 0.
+ * d_ff     DEVICE float[nz][ny][nx][4] = (Fx, Fy, Fz, E_Pauli); A in eV Å^(3(2 beta - 1)) e^(-2 beta), beta > 0.
+ */
+int ppfm_forcefield_pauli(const float *d_rho_S, const ppfm_grid *grid, double sigma, double q_tip, double A, double beta,
+                          float *d_ff, void *cuda_stream);
+
 /* ---- (2a) relaxation scan on an energy-only grid, tri-cubic interpolation -------
  * "we are experimenting with tri-cubic interpolation of the potential which may allow us to use larger grid spacing
  * and avoid storage of forces".  Same scan, FIRE and outputs as ppfm_relax_scan; the sample force is

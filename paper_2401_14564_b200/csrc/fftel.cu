@@ -24,6 +24,7 @@ struct FftJob {
     double step[3][3];
     double sigma, q_s, p_z, Q_zz;
     double scale;              // dV / N
+    double vpow;               // Eq.8 (vpow > 0): the input grid is clipped at 0 and raised to this power; 0 = Eq.7: as is
 };
 
 __global__ void __launch_bounds__(256)
@@ -48,7 +49,8 @@ fft_fill_kernel(const __grid_constant__ FftJob job, const float *__restrict__ V,
     const double dPx = -2.0 * q12 * r[0] * is4, dPy = -2.0 * q12 * r[1] * is4;
     const double dPz = job.p_z * is2 + 4.0 * q12 * r[2] * is4;
     const double Pg = P * g;
-    real5[m] = (double)V[m];
+    const double v = (double)V[m];
+    real5[m] = (job.vpow == 0.0) ? v : pow(fmax(v, 0.0), job.vpow);
     real5[job.N + m] = Pg;
     real5[2 * job.N + m] = dPx * g - Pg * r[0] * is2;
     real5[3 * job.N + m] = dPy * g - Pg * r[1] * is2;
@@ -112,8 +114,8 @@ void release_fft_plans() {
 
 using namespace ppfm;
 
-extern "C" int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, const ppfm_tip_density *tip, float *d_ff,
-                                   void *cuda_stream) {
+static int forcefield_fft_impl(const float *d_V, const ppfm_grid *grid, const ppfm_tip_density *tip, double vpow,
+                               float *d_ff, void *cuda_stream) {
     if (!d_V || !grid || !tip || !d_ff) return PPFM_EINVAL;
     if (((uintptr_t)d_V & 3) || ((uintptr_t)d_ff & 15)) return PPFM_EINVAL;
     if (!grid_ok(grid)) return PPFM_EINVAL;
@@ -132,6 +134,7 @@ extern "C" int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, cons
                        s[0][2] * (s[1][0] * s[2][1] - s[1][1] * s[2][0]);
     job.sigma = tip->sigma; job.q_s = tip->q_s; job.p_z = tip->p_z; job.Q_zz = tip->Q_zz;
     job.scale = std::fabs(det) / (double)job.N;
+    job.vpow = vpow;
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cufftHandle fwd, inv;
@@ -165,4 +168,25 @@ extern "C" int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, cons
     cudaFreeAsync(d_cplx, st);
     cudaFreeAsync(d_real, st);
     return rc;
+}
+
+extern "C" int ppfm_forcefield_fft(const float *d_V, const ppfm_grid *grid, const ppfm_tip_density *tip, float *d_ff,
+                                   void *cuda_stream) {
+    return forcefield_fft_impl(d_V, grid, tip, 0.0, d_ff, cuda_stream);
+}
+
+// Eq.8: E_Pauli(R) = A integral [rho_PP(r) rho_S(r + R)]^beta dr with rho_PP = q g_sigma.  A Gaussian
+// to the power beta is a Gaussian, (q g_s)^beta = q^beta (2 pi s^2)^(3(1-beta)/2) beta^(-3/2) g_{s/sqrt(beta)}, so this
+// is the Eq.7 pipeline on rho_S^beta with a monopole tip of that width and weight.
+extern "C" int ppfm_forcefield_pauli(const float *d_rho_S, const ppfm_grid *grid, double sigma, double q_tip, double A,
+                                     double beta, float *d_ff, void *cuda_stream) {
+    if (!(sigma > 0.0) || !(q_tip > 0.0) || !(beta > 0.0) || !std::isfinite(sigma) || !std::isfinite(q_tip) ||
+        !std::isfinite(beta) || !std::isfinite(A))
+        return PPFM_EINVAL;
+    ppfm_tip_density td;
+    td.sigma = sigma / std::sqrt(beta);
+    td.q_s = A * std::pow(q_tip, beta) * std::pow(2.0 * M_PI * sigma * sigma, 1.5 * (1.0 - beta)) * std::pow(beta, -1.5);
+    td.p_z = 0.0;
+    td.Q_zz = 0.0;
+    return forcefield_fft_impl(d_rho_S, grid, &td, beta, d_ff, cuda_stream);
 }

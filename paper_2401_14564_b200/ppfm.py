@@ -61,7 +61,7 @@ class Stats(C.Structure):
 
 
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
-           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft", "ppfm_relax_scan",
+           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft", "ppfm_forcefield_pauli", "ppfm_relax_scan",
            "ppfm_relax_scan_batch", "ppfm_relax_scan_tricubic", "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid",
            "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch", "ppfm_scan_host_sweep",
            "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
@@ -289,6 +289,19 @@ def forcefield_fft(V, grid, sigma: float, q_s: float = 0.0, p_z: float = 0.0, Q_
     rc = lib().ppfm_forcefield_fft(_dptr(V, torch.float32), C.byref(c_grid(grid)), C.byref(td),
                                    _dptr(out, torch.float32), _stream())
     _check(rc, "ppfm_forcefield_fft")
+    return out
+
+
+def forcefield_pauli(rho_S, grid, sigma: float, q_tip: float, A: float, beta: float, out=None):
+    """ppfm_forcefield_pauli (Eq.8): rho_S (nz, ny, nx) float32 device tensor -> (nz, ny, nx, 4) = (Fx, Fy, Fz, E)."""
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in grid.n)
+    if out is None:
+        out = torch.empty((nz, ny, nx, 4), dtype=torch.float32, device=rho_S.device)
+    rc = lib().ppfm_forcefield_pauli(_dptr(rho_S, torch.float32), C.byref(c_grid(grid)), C.c_double(sigma),
+                                     C.c_double(q_tip), C.c_double(A), C.c_double(beta), _dptr(out, torch.float32),
+                                     _stream())
+    _check(rc, "ppfm_forcefield_pauli")
     return out
 
 

@@ -524,6 +524,24 @@ def test_fft_electrostatics_point_charge_potential_and_full_size_samples(P):
     assert bool(torch.isfinite(pos).all()) and int((iters.to(torch.int32) < 0).sum()) == 0
 
 
+def test_fft_pauli_overlap_eq8(P):
+    """PAPER.md:118-122 Eq.8 (FDBM Pauli repulsion) against the oracle's literal sum of [rho_PP rho_S]^beta; the GPU
+    goes through the Gaussian-power identity and the Eq.7 pipeline, the oracle does not."""
+    import torch
+    rng = np.random.default_rng(21)
+    for n, step, (sig, q, A, beta) in [((24, 20, 16), np.diag([0.25, 0.3, 0.35]), (0.45, 1.3, 5.0, 1.2)),
+                                       ((13, 11, 7), np.array([[0.3, 0.02, 0.0], [-0.04, 0.28, 0.01], [0.0, 0.03, 0.33]]),
+                                        (0.4, 2.0, 12.0, 0.9)),
+                                       ((16, 16, 16), np.diag([0.2, 0.2, 0.2]), (0.35, 1.0, 3.0, 1.0))]:
+        g = W.Grid(origin=np.zeros(3), step=step, n=n, periodic=(1, 1, 1))
+        rho = rng.uniform(-0.05, 0.4, (n[2], n[1], n[0])).astype(np.float32)      # a few negatives: clipped
+        got = P.forcefield_pauli(torch.from_numpy(rho).cuda(), g, sig, q, A, beta)
+        torch.cuda.synchronize()
+        check_fft_ff(got.cpu().numpy(), oracle.pauli_forcefield(rho, g, sig, q, A, beta), f"pauli n={n}")
+    with pytest.raises(P.PpfmError):
+        P.forcefield_pauli(torch.from_numpy(rho).cuda(), g, sig, -1.0, A, beta)    # q_tip must be > 0
+
+
 def test_fft_electrostatics_rejects_bad_arguments(P):
     import torch
     g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(8, 8, 8), periodic=(1, 1, 1))
