@@ -5,7 +5,10 @@
  * the simplest level of theory (Lennard-Jones + point charges) of the two-step scheme of
  * (1) project all sample atoms onto a uniform grid force field, (2) relax the probe particle
  * (PP) with FIRE under tri-linear interpolation of that grid plus the tip springs, for every scan pixel while
- * the tip steps down in z, and (3) convert Fz(z) to the frequency shift df.
+ * the tip steps down in z, and (3) convert Fz(z) to the frequency shift df.  Beyond that path:
+ * (1b) Eq.7 electrostatics of an extended tip charge density and (1c) the Eq.8 Pauli overlap, both by the
+ * convolution theorem; (2a) the scan with tri-cubic interpolation of an energy-only grid
+ * (PAPER.md:264); (2b) the stiffness map of the relaxed PP (IETS module).
  *
  * Conventions
  *   Units: Å, eV, elementary charge e; spring constants in eV/Å^2 (ppfm_Nm_to_eVA2 converts from N/m);
@@ -14,10 +17,11 @@
  *          passed by pointer are HOST memory and are read before the call returns.
  *   Ownership: every buffer is allocated and freed by the caller.  The library keeps no pointer to caller memory
  *          after return; per-call scratch is stream-ordered (allocated and freed on `cuda_stream` inside the call)
- *          from a library-private pool that caches freed blocks until ppfm_release_scratch().
+ *          from a library-private pool that caches freed blocks until ppfm_release_scratch(); the cuFFT plans of
+ *          (1b)/(1c) are cached per grid size until then too.
  *          Device entry points only enqueue work on `cuda_stream` (a cudaStream_t cast to
  *          void*, NULL = default stream); they never synchronise it and never change the current device.
- *          Host entry points (ppfm_scan_host) synchronise the stream before returning.
+ *          Host entry points (ppfm_scan_host, _batch, _sweep) synchronise the stream before returning.
  *   Errors: 0 on success, a negative ppfm_status otherwise; no exceptions, no exit(), no output.  Per-pixel
  *          conditions (not converged, PP clamped at a non-periodic grid face) are data (d_iters, d_stats).
  *   Determinism: outputs are bit-reproducible run to run (fixed summation order, no atomics on results).
