@@ -204,7 +204,9 @@ static void *mapped_alias(const void *h) {
 
 // One call, host buffers ("run the whole simulation in one step").  When the output buffers are pinned
 // host memory the kernels store straight into them (posted PCIe writes that overlap the computation: no
-// device-to-host copy after the scan); the relaxation then also keeps a plain Fz stack on the device for the df kernel.
+// device-to-host copy of the float4 stack and of df after the scan); the relaxation then also keeps a plain Fz stack on
+// the device for the df kernel.  The uint16 iteration counts go through a device buffer and one DMA copy: written in
+// place they are 16-byte PCIe writes, which slow the relaxation more than the 2 bytes per sample are worth.
 // Pageable outputs take staged cudaMemcpyAsync copies.
 static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h_xyzq, const int32_t *h_type,
                           int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
@@ -257,6 +259,7 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
     TRY(scratch_alloc((void **)&d_stats, sizeof(ppfm_stats), st));
     if (zc) {
         if (h_df) TRY(scratch_alloc((void **)&d_fz, nps * 4, st));
+        if (h_iters) TRY(scratch_alloc((void **)&d_it, nps * 2, st));
     } else {
         TRY(scratch_alloc((void **)&d_pos, nps * 16, st));
         TRY(scratch_alloc((void **)&d_it, nps * 2, st));
@@ -282,8 +285,9 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
         const size_t op = (size_t)run * nps, od = (size_t)run * ndf;      // this run's slice of the host outputs
         if (zc) {
             if (rc == PPFM_OK)
-                rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, m_pos + 4 * op, h_iters ? m_it + op : nullptr,
+                rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, m_pos + 4 * op, h_iters ? d_it : nullptr,
                                    d_stats, d_fz, cuda_stream);
+            if (h_iters) TRY(cudaMemcpyAsync(h_iters + op, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
             if (rc == PPFM_OK && h_df)
                 rc = df_from_fz(nsys, d_fz, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, m_df + od,
                                 cuda_stream);
