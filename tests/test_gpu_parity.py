@@ -409,8 +409,8 @@ def test_relax_tricubic_cfg0_full_scan(P):
     import torch
     w = W.get(0)
     ff = gpu_ff(P, w)
-    E = P.energy_grid(ff)
-    assert torch.equal(E, ff[..., 3])
+    assert torch.equal(P.energy_grid(ff), ff[..., 3])                  # the extraction kernel
+    E = torch.from_numpy(np.ascontiguousarray(oracle.forcefield(w)[..., 3].astype(np.float32))).cuda()   # oracle's energies
     stats = P.new_stats()
     pos, iters = P.relax_scan_tricubic(E, w.grid, w.tip, w.fire, w.scan, stats=stats)
     torch.cuda.synchronize()
@@ -436,7 +436,7 @@ def test_relax_tricubic_periodic_skewed_batch_and_edges(P):
     w = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
     step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
     w = replace(w, grid=replace(w.grid, step=step), scan=replace(w.scan, p0=np.array([-3.0, 20.0, 9.0])))
-    E = P.energy_grid(gpu_ff(P, w))
+    E = torch.from_numpy(np.ascontiguousarray(oracle.forcefield(w)[..., 3].astype(np.float32))).cuda()   # oracle's energies
     stats = P.new_stats()
     pos, _ = P.relax_scan_tricubic(E, w.grid, w.tip, w.fire, w.scan, stats=stats)
     torch.cuda.synchronize()
@@ -497,27 +497,34 @@ def test_fft_electrostatics_small_grids_full_parity(P):
 
 
 def test_fft_electrostatics_point_charge_potential_and_full_size_samples(P):
-    """V_S = the unit-charge Coulomb potential of the config-1 molecule from ppfm_forcefield_split (.w lane), on the
-    full 200 x 200 x 100 grid, CO-like quadrupole tip: sampled nodes against the definition, plus the sum rules
-    sum_R E = q_s sum V and sum_R F = 0 that hold at any size; then LJ + Eq.7 grid through combine and a relaxed scan."""
+    """Full 200 x 200 x 100 grid of config 1, CO-like quadrupole tip, V_S = a screened point-charge potential built
+    here in numpy: sampled nodes against the definition, plus the sum rules sum_R E = q_s sum V and sum_R F = 0 that
+    hold at any size; then, on the unit-charge potential of ppfm_forcefield_split, LJ + Eq.7 through combine and a scan."""
     import torch
     w = W.get(1)
     xyzq, types = P.upload(w)
     lj, el = P.forcefield_split(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
-    V = el[..., 3].contiguous()
     sig, q, pz, Q = 0.7, -0.03, 0.0, -0.1
-    got = P.forcefield_fft(V, w.grid, sig, q, pz, Q)
-    torch.cuda.synchronize()
-    Vh = V.cpu().numpy()
-    rng = np.random.default_rng(5)
+    # parity input made here, not by the CUDA path: a screened point-charge potential of the molecule's charges
     nx, ny, nz = w.grid.n
+    zz, yy, xx = np.meshgrid(np.arange(nz) * 0.1 + w.grid.origin[2], np.arange(ny) * 0.1, np.arange(nx) * 0.1, indexing="ij")
+    Vh = np.zeros((nz, ny, nx))
+    for (ax_, ay_, az_, aq) in w.xyzq[:12]:
+        r = np.sqrt((xx - ax_) ** 2 + (yy - ay_) ** 2 + (zz - az_) ** 2 + 0.25)
+        Vh += 14.399645478 * aq * np.exp(-r / 6.0) / r
+    Vh = Vh.astype(np.float32)
+    got = P.forcefield_fft(torch.from_numpy(Vh).cuda(), w.grid, sig, q, pz, Q)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
     ijk = np.stack([rng.integers(0, nx, 60), rng.integers(0, ny, 60), rng.integers(0, nz, 60)], axis=1)
     ref = oracle.fft_forcefield_at(Vh, w.grid, sig, q, pz, Q, ijk)
     check_fft_ff(got.cpu().numpy()[ijk[:, 2], ijk[:, 1], ijk[:, 0]], ref, "cfg1 sampled")
     gh = got.cpu().numpy().astype(np.float64)
     assert np.isclose(gh[..., 3].sum(), q * Vh.astype(np.float64).sum(), rtol=1e-5)
     assert np.abs(gh[..., :3].sum(axis=(0, 1, 2))).max() <= 1e-6 * np.abs(gh[..., :3]).sum()
-    # the Eq.7 grid is a drop-in replacement for Q * F_el(point charge): combine and scan
+    # the Eq.7 grid is a drop-in replacement for Q * F_el(point charge): on the unit-charge potential of the split pass,
+    # combine and scan (a smoke run of the whole chain: finite, converged)
+    got = P.forcefield_fft(el[..., 3].contiguous(), w.grid, sig, q, pz, Q)
     ff = P.combine(lj, got, 1.0)
     pos, iters = P.relax_scan(ff, w.grid, w.tip, w.fire, W.shrink(w, scan_np=(40, 40)).scan)
     torch.cuda.synchronize()
@@ -555,6 +562,15 @@ def test_fft_electrostatics_rejects_bad_arguments(P):
 
 
 # ------------------------------------------------------------------------------------------------ stiffness map
+def oracle_inputs(w):
+    """Inputs for the 8(f) kernels made by the ORACLE (none of them comes from the CUDA path): its force-field grid
+    rounded to FP32 and the relaxed scan on that grid, positions rounded to FP32."""
+    ff_o = oracle.forcefield(w).astype(np.float32)
+    ref = oracle.relax_scan(ff_o, w.grid, w.tip, w.fire, w.scan, traj=False)
+    pos_o = np.ascontiguousarray(ref["pos_fz"].astype(np.float32))          # (nz, npix, 4)
+    return ff_o, pos_o
+
+
 def check_stiffness(eig_gpu, ff_h, w, pos_h, what=""):
     """GPU eigenvalues vs the oracle's at the same positions on the same (FP32, widened) grid.  Tolerance
     |d lambda| <= 1e-5 eV/Å^2 + 1e-5 |lambda| (the Jacobian is formed in FP32 from corner differences,
@@ -581,12 +597,11 @@ def test_stiffness_map_cfg0_and_cfg1(P):
     import torch
     for cfg in (0, 1):
         w = W.get(cfg)
-        ff, pos, _, _, _ = gpu_scan(P, w)
-        eig = P.stiffness(ff, w.grid, w.tip, w.scan, pos)
-        torch.cuda.synchronize()
+        ff_o, pos_o = oracle_inputs(w)                       # grid and positions from the oracle, for both sides
         npix = w.scan.npx * w.scan.npy
-        pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)
-        check_stiffness(eig.cpu().numpy().reshape(w.scan.nz, npix, 4), ff.cpu().numpy(), w, pos_h, f"cfg{cfg}")
+        eig = P.stiffness(torch.from_numpy(ff_o).cuda(), w.grid, w.tip, w.scan, torch.from_numpy(pos_o).cuda())
+        torch.cuda.synchronize()
+        check_stiffness(eig.cpu().numpy().reshape(w.scan.nz, npix, 4), ff_o, w, pos_o, f"cfg{cfg}")
         # the soft (lateral) modes are softened over the molecule in the repulsive regime: the map has contrast
         lam_min = eig[..., 0].cpu().numpy()
         assert lam_min.min() < 0.5 * w.tip.k_lat[0] and lam_min.max() > 0.9 * w.tip.k_lat[0]
@@ -607,13 +622,11 @@ def test_stiffness_zero_field_periodic_nonorthogonal_and_batch(P):
     w = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
     step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
     w = replace(w, grid=replace(w.grid, step=step), scan=replace(w.scan, p0=np.array([-3.0, 20.0, 9.0])))
-    ffw = gpu_ff(P, w)
-    posw, _ = P.relax_scan(ffw, w.grid, w.tip, w.fire, w.scan)
-    eigw = P.stiffness(ffw, w.grid, w.tip, w.scan, posw)
+    ff_o, pos_o = oracle_inputs(w)
+    eigw = P.stiffness(torch.from_numpy(ff_o).cuda(), w.grid, w.tip, w.scan, torch.from_numpy(pos_o).cuda())
     torch.cuda.synchronize()
     npix = w.scan.npx * w.scan.npy
-    check_stiffness(eigw.cpu().numpy().reshape(w.scan.nz, npix, 4), ffw.cpu().numpy(), w,
-                    posw.cpu().numpy().reshape(w.scan.nz, npix, 4), "periodic skewed")
+    check_stiffness(eigw.cpu().numpy().reshape(w.scan.nz, npix, 4), ff_o, w, pos_o, "periodic skewed")
     # batch == per-system calls, bit for bit
     mols = W.get(3)[:3]
     mols = [W.shrink(m, grid_n=m.grid.n, scan_np=(24, 20), scan_nz=5) for m in mols]
