@@ -257,8 +257,12 @@ def test_relax_and_df_full_scan(P, cfg):
     # Fz and df
     ok = np.linalg.norm(pos_h[..., :3] - ref64["pos_fz"][..., :3], axis=-1) <= 2e-3
     assert np.abs(pos_h[..., 3] - ref64["pos_fz"][..., 3])[ok].max() < 2e-4
-    df_ref_same = oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0)
-    check_df(df.cpu().numpy().reshape(df_ref_same.shape), df_ref_same, f"cfg{cfg} df kernel")
+    # df kernel alone, on the ORACLE's Fz stack (rounded to FP32) as the input of both sides
+    import torch
+    stack_o = np.ascontiguousarray(ref64["pos_fz"].astype(np.float32))
+    df_o = P.df(torch.from_numpy(stack_o).cuda(), w.scan.npx, w.scan.npy, w.scan.nz, w.scan.dz, w.df.A, w.df.k0, w.df.f0)
+    df_ref_same = oracle.df(stack_o[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0)
+    check_df(df_o.cpu().numpy().reshape(df_ref_same.shape), df_ref_same, f"cfg{cfg} df kernel")
     df_ref = oracle.df(ref64["pos_fz"][..., 3], w.scan.dz, w.df.A, w.df.k0, w.df.f0)
     n = w.n_df
     bad = ~ok            # windows in which all n + 1 positions agree must give the same df
