@@ -22,7 +22,7 @@
 
 namespace ppfm {
 
-constexpr int FF_THREADS = 256;
+constexpr int FF_THREADS = 128;  // columns per CTA
 constexpr int FF_CHUNK = 256;   // atoms per pipeline stage
 constexpr int FF_STAGES = 3;
 constexpr int FF_AHEAD = 2;     // chunks in flight ahead of the consumer
@@ -288,71 +288,119 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, int ncharged, const At
 
     // shifted point p' = p - image shift, split hi + lo; set once per image
     float ph[3], pl[3];
-    // one chunk of atom records against the thread's P points; NEUTRAL: the records carry no Coulomb factor
-    auto run_chunk = [&](const float4 *s4, int n, auto neutral_tag) {
-        constexpr bool NEUTRAL = decltype(neutral_tag)::value;
-        const float2 twelve = make_float2(12.0f, 12.0f);
-#pragma unroll 2
-        for (int a = 0; a < n; a++) {
-            const float4 r0 = s4[3 * a];          // x, y, z, -
-            const float4 r1 = s4[3 * a + 1];      // c12, c12, -c6, -c6
-            const float4 r2_ = s4[3 * a + 2];     // 6 c6, 6 c6, kq, kq
-            const float2 c12 = make_float2(r1.x, r1.y), nc6 = make_float2(r1.z, r1.w);
-            const float2 c6x6 = make_float2(r2_.x, r2_.y), kq = make_float2(r2_.z, r2_.w);
-            const float dx0 = (ph[0] - r0.x) + pl[0];
-            const float dy0 = (ph[1] - r0.y) + pl[1];
-            const float dz0 = (ph[2] - r0.z) + pl[2];
+    const float2 twelve = make_float2(12.0f, 12.0f);
+
+    // The pair body is written in two stages so that the MUFU of atom a + 1 is in flight while the polynomial of
+    // atom a runs (software pipelining), and every stage loops over the H point pairs of the column, which gives
+    // ptxas H independent dependency chains side by side instead of one chain after the other (ncu, round 1: the
+    // serial schedule left the FMA pipe 79 % busy with `wait` and `short_scoreboard` stalls on every link).
+    //   stage A (atom record -> displacement, r^2, 1/r):   per pair of points 1 FADD2 + 1 FFMA2 + 2 MUFU.RSQ
+    //   stage B (1/r -> energy and force accumulation):    13 packed instructions (11 for an LJ-only atom)
+    struct Stage {
+        float2 dx[ZCOL ? 1 : H], dy[ZCOL ? 1 : H], dz[H], ir[H];
+        float2 c12, nc6, c6x6, kq;
+    };
+    auto stage_a = [&](const float4 *s4, int a, Stage &S) {
+        const float4 r0 = s4[3 * a];          // x, y, z, -
+        const float4 r1 = s4[3 * a + 1];      // c12, c12, -c6, -c6
+        const float4 r2_ = s4[3 * a + 2];     // 6 c6, 6 c6, kq, kq
+        S.c12 = make_float2(r1.x, r1.y); S.nc6 = make_float2(r1.z, r1.w);
+        S.c6x6 = make_float2(r2_.x, r2_.y); S.kq = make_float2(r2_.z, r2_.w);
+        const float dx0 = (ph[0] - r0.x) + pl[0];
+        const float dy0 = (ph[1] - r0.y) + pl[1];
+        const float dz0 = (ph[2] - r0.z) + pl[2];
+        const float2 dxx = make_float2(dx0, dx0), dyy = make_float2(dy0, dy0), dzz = make_float2(dz0, dz0);
+        float2 r2[H];
+        if (ZCOL) {
             const float rxy2s = fmaf(dy0, dy0, dx0 * dx0);
-            const float2 dxx = make_float2(dx0, dx0), dyy = make_float2(dy0, dy0);
-            const float2 dzz = make_float2(dz0, dz0), rxy2 = make_float2(rxy2s, rxy2s);
+            const float2 rxy2 = make_float2(rxy2s, rxy2s);
+            S.dx[0] = dxx; S.dy[0] = dyy;
+#pragma unroll
+            for (int h = 0; h < H; h++) S.dz[h] = __fadd2_rn(dzz, off[0][h]);
+#pragma unroll
+            for (int h = 0; h < H; h++) r2[h] = __ffma2_rn(S.dz[h], S.dz[h], rxy2);
+        } else {
 #pragma unroll
             for (int h = 0; h < H; h++) {
-                float2 dx, dy, dz, r2;
-                if (ZCOL) {
-                    dx = dxx; dy = dyy;
-                    dz = __fadd2_rn(dzz, off[0][h]);
-                    r2 = __ffma2_rn(dz, dz, rxy2);
-                } else {
-                    dx = __fadd2_rn(dxx, off[0][h]);
-                    dy = __fadd2_rn(dyy, off[1 % (ZCOL ? 1 : 3)][h]);
-                    dz = __fadd2_rn(dzz, off[2 % (ZCOL ? 1 : 3)][h]);
-                    r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-                }
-                if (CLAMP) { r2.x = fmaxf(r2.x, rmin2); r2.y = fmaxf(r2.y, rmin2); }
-                float2 ir;
-                ir.x = rsqrt_approx(r2.x);
-                ir.y = rsqrt_approx(r2.y);
-                const float2 ir2 = __fmul2_rn(ir, ir);
-                const float2 ir6 = __fmul2_rn(__fmul2_rn(ir2, ir2), ir2);
-                const float2 t = __ffma2_rn(c12, ir6, nc6);        // c12/r^6 - c6
-                const float2 t2 = __ffma2_rn(t, twelve, c6x6);    // 12 c12/r^6 - 6 c6
-                E[h] = __ffma2_rn(t, ir6, E[h]);                   // E_LJ = c12/r^12 - c6/r^6
-                if (!SPLIT) {
-                    float2 g = __fmul2_rn(t2, ir6);
-                    if (!NEUTRAL) {
-                        E[h] = __ffma2_rn(kq, ir, E[h]);           // E_C = kq / r
-                        g = __ffma2_rn(kq, ir, g);
-                    }
-                    const float2 f = __fmul2_rn(g, ir2);           // (12c12/r^12 - 6c6/r^6 + kq/r) / r^2
-                    Fx[h] = __ffma2_rn(f, dx, Fx[h]);
-                    Fy[h] = __ffma2_rn(f, dy, Fy[h]);
-                    Fz[h] = __ffma2_rn(f, dz, Fz[h]);
-                } else {
-                    const float2 f = __fmul2_rn(__fmul2_rn(t2, ir6), ir2);
-                    Fx[h] = __ffma2_rn(f, dx, Fx[h]);
-                    Fy[h] = __ffma2_rn(f, dy, Fy[h]);
-                    Fz[h] = __ffma2_rn(f, dz, Fz[h]);
-                    if (!NEUTRAL) {
-                        const float2 ec = __fmul2_rn(kq, ir);
-                        Ge[h] = __fadd2_rn(Ge[h], ec);
-                        const float2 fe = __fmul2_rn(ec, ir2);
-                        Gx[h] = __ffma2_rn(fe, dx, Gx[h]);
-                        Gy[h] = __ffma2_rn(fe, dy, Gy[h]);
-                        Gz[h] = __ffma2_rn(fe, dz, Gz[h]);
-                    }
-                }
+                S.dx[ZCOL ? 0 : h] = __fadd2_rn(dxx, off[0][h]);
+                S.dy[ZCOL ? 0 : h] = __fadd2_rn(dyy, off[1 % (ZCOL ? 1 : 3)][h]);
+                S.dz[h] = __fadd2_rn(dzz, off[2 % (ZCOL ? 1 : 3)][h]);
+                r2[h] = __ffma2_rn(S.dz[h], S.dz[h], __ffma2_rn(S.dy[ZCOL ? 0 : h], S.dy[ZCOL ? 0 : h],
+                                                                 __fmul2_rn(S.dx[ZCOL ? 0 : h], S.dx[ZCOL ? 0 : h])));
             }
         }
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            if (CLAMP) { r2[h].x = fmaxf(r2[h].x, rmin2); r2[h].y = fmaxf(r2[h].y, rmin2); }
+            S.ir[h].x = rsqrt_approx(r2[h].x);
+            S.ir[h].y = rsqrt_approx(r2[h].y);
+        }
+    };
+    auto stage_b = [&](const Stage &S, auto neutral_tag) {
+        constexpr bool NEUTRAL = decltype(neutral_tag)::value;
+        float2 ir2[H], ir6[H], t[H], g[H];
+#pragma unroll
+        for (int h = 0; h < H; h++) ir2[h] = __fmul2_rn(S.ir[h], S.ir[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) ir6[h] = __fmul2_rn(ir2[h], ir2[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) ir6[h] = __fmul2_rn(ir6[h], ir2[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) t[h] = __ffma2_rn(S.c12, ir6[h], S.nc6);            // c12/r^6 - c6
+#pragma unroll
+        for (int h = 0; h < H; h++) E[h] = __ffma2_rn(t[h], ir6[h], E[h]);              // E_LJ = c12/r^12 - c6/r^6
+#pragma unroll
+        for (int h = 0; h < H; h++) t[h] = __ffma2_rn(t[h], twelve, S.c6x6);            // 12 c12/r^6 - 6 c6
+#pragma unroll
+        for (int h = 0; h < H; h++) g[h] = __fmul2_rn(t[h], ir6[h]);
+        if (!SPLIT) {
+            if (!NEUTRAL) {
+#pragma unroll
+                for (int h = 0; h < H; h++) E[h] = __ffma2_rn(S.kq, S.ir[h], E[h]);     // E_C = kq / r
+#pragma unroll
+                for (int h = 0; h < H; h++) g[h] = __ffma2_rn(S.kq, S.ir[h], g[h]);
+            }
+#pragma unroll
+            for (int h = 0; h < H; h++) g[h] = __fmul2_rn(g[h], ir2[h]);                // (12c12/r^12 - 6c6/r^6 + kq/r)/r^2
+        } else {
+#pragma unroll
+            for (int h = 0; h < H; h++) g[h] = __fmul2_rn(g[h], ir2[h]);
+        }
+#pragma unroll
+        for (int h = 0; h < H; h++) Fx[h] = __ffma2_rn(g[h], S.dx[ZCOL ? 0 : h], Fx[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) Fy[h] = __ffma2_rn(g[h], S.dy[ZCOL ? 0 : h], Fy[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) Fz[h] = __ffma2_rn(g[h], S.dz[h], Fz[h]);
+        if (SPLIT && !NEUTRAL) {
+            float2 ec[SPLIT ? H : 1];
+#pragma unroll
+            for (int h = 0; h < (SPLIT ? H : 0); h++) ec[h] = __fmul2_rn(S.kq, S.ir[h]);
+#pragma unroll
+            for (int h = 0; h < (SPLIT ? H : 0); h++) Ge[h] = __fadd2_rn(Ge[h], ec[h]);
+#pragma unroll
+            for (int h = 0; h < (SPLIT ? H : 0); h++) ec[h] = __fmul2_rn(ec[h], ir2[h]);
+#pragma unroll
+            for (int h = 0; h < (SPLIT ? H : 0); h++) Gx[h] = __ffma2_rn(ec[h], S.dx[ZCOL ? 0 : h], Gx[h]);
+#pragma unroll
+            for (int h = 0; h < (SPLIT ? H : 0); h++) Gy[h] = __ffma2_rn(ec[h], S.dy[ZCOL ? 0 : h], Gy[h]);
+#pragma unroll
+            for (int h = 0; h < (SPLIT ? H : 0); h++) Gz[h] = __ffma2_rn(ec[h], S.dz[h], Gz[h]);
+        }
+    };
+    // one chunk of atom records against the thread's P points; NEUTRAL: the records carry no Coulomb factor
+    auto run_chunk = [&](const float4 *s4, int n, auto neutral_tag) {
+        Stage S0, S1;
+        stage_a(s4, 0, S0);
+        int a = 0;
+#pragma unroll 1
+        for (; a + 2 <= n; a += 2) {
+            stage_a(s4, a + 1, S1);
+            stage_b(S0, neutral_tag);
+            stage_a(s4, min(a + 2, n - 1), S0);      // past the end: the last atom again, not used
+            stage_b(S1, neutral_tag);
+        }
+        if (a < n) stage_b(S0, neutral_tag);
     };
 
     int step = 0;
@@ -411,9 +459,15 @@ __device__ __forceinline__ void ff_init_barriers(uint64_t *full_bar, uint64_t *e
     }
 }
 
+// CTAs per SM the register budget is cut for.  The software-pipelined body keeps ~(18 + 4) registers per point pair
+// plus ~40 (two accumulator sets in split mode: ~28 per pair): P = 20 needs the full 255 registers (2 CTAs of 128
+// threads per SM), P <= 10 fits 168 (3 CTAs).  More warps do not help: the loop is bound by issue slots, not latency.
+template <int P, bool SPLIT>
+constexpr int ff_min_ctas() { return SPLIT ? (P >= 10 ? 2 : 3) : (P >= 16 ? 2 : 3); }
+
 // One system: job in the constant bank (kernel parameter).
 template <int P, bool SPLIT, bool ZCOL>
-__global__ void __launch_bounds__(FF_THREADS, 2)
+__global__ void __launch_bounds__(FF_THREADS, ff_min_ctas<P, SPLIT>())
 ff_kernel(const __grid_constant__ FFJob job, const FFFlags *__restrict__ flags, const AtomRec *__restrict__ recs,
           float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
     __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
@@ -433,7 +487,7 @@ ff_kernel(const __grid_constant__ FFJob job, const FFFlags *__restrict__ flags, 
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
 template <int P, bool SPLIT, bool ZCOL>
-__global__ void __launch_bounds__(FF_THREADS, 2)
+__global__ void __launch_bounds__(FF_THREADS, ff_min_ctas<P, SPLIT>())
 ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const FFFlags *__restrict__ flags,
                 const AtomRec *__restrict__ recs, float4 *__restrict__ out_a, float4 *__restrict__ out_b) {
     __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
@@ -474,16 +528,19 @@ __global__ void combine_kernel(const float4 *__restrict__ lj, const float4 *__re
 }
 
 // ---------------------------------------------------------------------------------------------------- host side
-static int pick_P(int nz, bool split) {
-    // padded work ~ ceil(nz/P) * (P + per-atom overhead shared by the column ~ 0.7 points).  The split kernel keeps
-    // two accumulator sets per point, so it takes fewer points per thread (P = 8, 10 would spill at 128 registers).
-    const int cand_one[3] = {8, 10, 6}, cand_two[3] = {8, 6, 4};
+static int pick_P(int nz, long long nxy_tiles, bool split) {
+    // padded work ~ ceil(nz/P) * (P + per-atom overhead shared by the column, ~1.2 points: 8 scalar FP32 + 3 LDS +
+    // loop control against ~16 issue slots per point).  The split kernel keeps two accumulator sets per point, so
+    // it takes fewer points per thread.  Small grids take the smallest P that still gives every SM two CTAs.
+    const int cand_one[3] = {20, 10, 8}, cand_two[3] = {10, 8, 6};
     const int *cand = split ? cand_two : cand_one;
     int best = cand[0];
     double best_cost = 1e300;
     for (int c = 0; c < 3; c++) {
         const int P = cand[c];
-        const double cost = (double)((nz + P - 1) / P) * (P + 0.7);
+        const long long ctas = nxy_tiles * ((nz + P - 1) / P);
+        double cost = (double)((nz + P - 1) / P) * (P + 1.2);
+        if (ctas < 2 * 148) cost *= 2.0 * 148.0 / (double)(ctas > 0 ? ctas : 1);      // idle SMs
         if (cost < best_cost - 1e-9) { best_cost = cost; best = P; }
     }
     return best;
@@ -502,11 +559,10 @@ static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st
                              int njobs, const FFFlags *flags, const AtomRec *recs, float4 *a, float4 *b) {
     KernelTimer kt(PPFM_K_FF, st);
     if (!zcol) launch_ff_one<SPLIT, 4, false>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else if (P == 6) launch_ff_one<SPLIT, 6, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else if (P == 8) launch_ff_one<SPLIT, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else if (SPLIT) launch_ff_one<SPLIT, 4, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else if (P == 10) launch_ff_one<false, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
-    else launch_ff_one<false, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 10) launch_ff_one<SPLIT, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if constexpr (SPLIT) launch_ff_one<true, 6, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else launch_ff_one<false, 20, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     return cudaGetLastError();
 }
 
@@ -539,7 +595,10 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
         if (g.step[2][0] != 0.0 || g.step[2][1] != 0.0) zcol = false;
         if (g.n[2] != nz_common) nz_common = -1;
     }
-    const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2], split) : 4;
+    long long nxy_tiles_total = 0;
+    for (int m = 0; m < nsys; m++)
+        nxy_tiles_total += ((long long)grids[m].n[0] * grids[m].n[1] + FF_THREADS - 1) / FF_THREADS;
+    const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2], nxy_tiles_total, split) : 4;
 
     const bool single = (nsys == 1);
     const size_t jobs_bytes = (size_t)nsys * sizeof(FFJob);

@@ -439,6 +439,96 @@ def test_fire_first_step_matches_hand_computation():
 
 
 # ---------------------------------------------------------------------------------------------------- O9
+def _fire_reference(force, r0, fire, kmax):
+    """FIRE of ref [7] (Bitzek et al. 2006) in the reading S6 / S7 of DESIGN.md, written out independently of the
+    oracle: check |F| < f_conv BEFORE moving; P = F.v; P >= 0: mix v towards F, and once MORE than n_min downhill
+    moves have been counted grow dt (capped at dt_max) and shrink alpha; P < 0: v = 0, dt halves, alpha = alpha0,
+    counter = 0; then semi-implicit Euler with m = 1.  Returns the positions after 0, 1, 2, ... moves and the event
+    log (kind, dt used for the move, alpha after the update, grew?)."""
+    r, v = np.array(r0, dtype=np.float64), np.zeros(3)
+    dt, alpha, n_pos = fire.dt, fire.alpha0, 0
+    traj, events = [r.copy()], []
+    for _ in range(kmax):
+        F = force(r)
+        Fn = np.sqrt(F @ F)
+        if Fn < fire.f_conv:
+            break
+        if F @ v >= 0.0:
+            v = (1.0 - alpha) * v + alpha * np.sqrt(v @ v) * F / Fn
+            grew = n_pos > fire.n_min
+            if grew:
+                dt = min(dt * fire.finc, fire.dt_max)
+                alpha = alpha * fire.falpha
+            n_pos += 1
+            events.append(("down", dt, alpha, grew))
+        else:
+            v = np.zeros(3)
+            dt = dt * fire.fdec
+            alpha = fire.alpha0
+            n_pos = 0
+            events.append(("up", dt, alpha, False))
+        v = v + F * dt
+        r = r + v * dt
+        traj.append(r.copy())
+    return np.array(traj), events
+
+
+def test_fire_path_move_by_move_against_independent_implementation():
+    """O6 control flow (ref [7]; readings S6, S7), pinned MOVE BY MOVE: an affine sample field (which
+    tri-linear interpolation reproduces exactly, so the total force is analytic) plus the springs of an asymmetric
+    tip gives a relaxation with several P < 0 events, a run of > 14 downhill moves after a halving (so the
+    n_pos > n_min gate opens, dt grows by finc per move and is capped at dt_max, alpha decays by falpha) and a
+    convergence after ~120 moves.  The oracle, stopped after k = 1, 2, ... moves (max_iter = k), must sit where the
+    independent numpy FIRE above sits after k moves, to 1e-13 Å, and must converge in exactly the same number of
+    moves.  A '>=' instead of '>' in the gate, a missing dt cap, a wrong reset in the P < 0 branch or a different
+    integrator order each change the path at the 1e-3 Å level."""
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(20, 20, 60), periodic=(0, 0, 0))
+    zz, yy, xx = np.meshgrid(np.arange(60) * 0.2, np.arange(20) * 0.2, np.arange(20) * 0.2, indexing="ij")
+    b = np.array([0.004, -0.002, -0.08])
+    M = np.array([[-0.004, 0.001, 0.0], [0.0005, -0.006, 0.002], [0.001, 0.0, 0.01]])
+    ff = np.zeros((60, 20, 20, 4))
+    for c in range(3):
+        ff[..., c] = b[c] + M[c, 0] * xx + M[c, 1] * yy + M[c, 2] * zz
+    tip = replace(W._default_tip(), k_lat=(0.012, 0.019), d0=(0.3, -0.2, -3.98))      # asymmetric tip (PAPER.md:54)
+    d0 = np.array(tip.d0)
+    R0 = np.linalg.norm(d0)
+    p0 = np.array([1.5, 1.7, 9.0])
+    sc = W.Scan(p0=p0, dx=np.array([0.3, 0, 0.0]), dy=np.array([0, 0.4, 0.0]), npx=1, npy=1, nz=1, dz=0.1)
+
+    def force(r):       # Eq.1 + Eq.2 with F_S = b + M r
+        d = r - p0
+        L = np.sqrt(d @ d)
+        return (b + M @ r - tip.k_rad * (L - R0) * d / L -
+                np.array([tip.k_lat[0] * (d[0] - d0[0]), tip.k_lat[1] * (d[1] - d0[1]), 0.0]))
+
+    fire = W.Fire()
+    traj, events = _fire_reference(force, p0 + d0, fire, 1000)
+    n_moves = len(traj) - 1
+    assert traj.min() > 0.2 and traj[:, :2].max() < 3.6          # the path stays inside the grid (no clamping)
+    kinds = "".join("d" if e[0] == "down" else "u" for e in events)
+    # the path exercises every branch: >= 3 uphill events, a halving followed by growth back to the dt_max cap,
+    # alpha decay, and a long downhill run
+    assert kinds.count("u") >= 3 and 100 < n_moves < 200
+    first_up = kinds.index("u")
+    assert events[first_up][1] == fire.dt * fire.fdec and events[first_up][2] == fire.alpha0
+    run = len(kinds[first_up + 1:].split("u")[0])
+    assert run > fire.n_min + 9
+    dts = [e[1] for e in events[first_up + 1:first_up + 1 + run]]
+    assert dts[fire.n_min] == fire.dt * fire.fdec and dts[fire.n_min + 1] == pytest.approx(fire.dt * fire.fdec * fire.finc)
+    assert max(dts) == fire.dt_max and dts.count(fire.dt_max) >= 2                   # growth hit the cap and stayed there
+    assert min(e[2] for e in events) < fire.alpha0 * fire.falpha ** 10               # alpha decayed
+    # the oracle, move by move
+    for k in list(range(1, 61)) + list(range(60, n_moves, 7)) + [n_moves - 1]:
+        r = oracle.relax_scan(ff, g, tip, replace(fire, max_iter=k), sc)
+        assert r["iters"][0, 0] == -1                                                # not yet converged
+        assert np.abs(r["pos_fz"][0, 0, :3] - traj[k]).max() < 1e-13, k
+    for k in (n_moves, n_moves + 1, 1000):
+        r = oracle.relax_scan(ff, g, tip, replace(fire, max_iter=k), sc)
+        assert r["iters"][0, 0] == n_moves                                           # exact move count at f_conv
+        assert np.abs(r["pos_fz"][0, 0, :3] - traj[n_moves]).max() < 1e-13
+    assert np.linalg.norm(force(traj[n_moves])) < fire.f_conv <= np.linalg.norm(force(traj[n_moves - 1]))
+
+
 def test_df_weights_sum_to_zero_and_match_numerical_quadrature():
     """Eq.3: W_m = (2/(pi a^2)) int q hat_m(q)/sqrt(a^2-q^2) dq, checked with scipy.quad using
     the algebraic end-point weight; sum W = 0 (a constant force gives df = 0)."""
