@@ -266,6 +266,44 @@ def relax_scan(ff, grid, tip, fire, scan, pix: Optional[np.ndarray] = None, traj
     return {"pos_fz": pos, "iters": iters, "lam_min": lam, "clamped": cl, "lam_traj": lt}
 
 
+def relax_scan_atoms(w, pix: Optional[np.ndarray] = None, traj: bool = True, Q: Optional[float] = None,
+                     tip=None, scan=None, grid=None):
+    """O3-O8 (+O10) end to end WITHOUT a stored grid: the same scan as relax_scan(forcefield(w), ...), every grid node
+    the interpolation touches being evaluated on demand from the atoms (ff_at_point, the value oracle_forcefield would
+    store) and memoised per pixel.  Affordable on sampled pixels of grids whose full FP64 evaluation
+    takes hours.  Returns relax_scan's dict plus `nodes` (npix,) = grid nodes evaluated per pixel."""
+    tip = w.tip if tip is None else tip
+    scan = w.scan if scan is None else scan
+    grid = w.grid if grid is None else grid
+    xyzq, types = _d(w.xyzq), _i(w.types)
+    R, e = _d(w.elem_R), _d(w.elem_e)
+    cell, nimg = _cell(w.lattice), _i(w.lattice.nimg)
+    origin, step, n, per = _d(grid.origin), _d(grid.step), _i(grid.n), _i(grid.periodic)
+    if pix is None:
+        npix, ppix = scan.npx * scan.npy, None
+    else:
+        pix = np.ascontiguousarray(pix, dtype=np.int64)
+        npix, ppix = len(pix), pix
+    pos = np.empty((scan.nz, npix, 4))
+    iters = np.empty((scan.nz, npix), dtype=np.int32)
+    lam = np.empty((scan.nz, npix))
+    cl = np.empty((scan.nz, npix), dtype=np.int32)
+    lt = np.empty((scan.nz, npix)) if traj else None
+    nodes = np.zeros(npix, dtype=np.int64)
+    fire = w.fire
+    f = _d([fire.dt, fire.dt_max, fire.finc, fire.fdec, fire.alpha0, fire.falpha, fire.f_conv])
+    rc = lib().oracle_relax_scan_atoms(
+        C.c_int(len(types)), _p(xyzq), _p(types), C.c_int(len(R)), _p(R), _p(e), _p(cell), _p(nimg),
+        C.c_double(w.probe.R), C.c_double(w.probe.e), C.c_double(w.probe.Q if Q is None else Q), C.c_double(w.r_min),
+        _p(origin), _p(step), _p(n), _p(per), _p(_d(tip.k_lat)), C.c_double(tip.k_rad), _p(_d(tip.d0)), _p(f),
+        C.c_int(fire.n_min), C.c_int(fire.max_iter), _p(_d(scan.p0)), _p(_d(scan.dx)), _p(_d(scan.dy)),
+        C.c_int(scan.npx), C.c_int(scan.npy), C.c_int(scan.nz), C.c_double(scan.dz),
+        C.c_int64(npix if pix is not None else 0), _p(ppix), _p(pos), _p(iters), _p(lam), _p(cl), _p(lt), _p(nodes))
+    if rc:
+        raise ValueError(f"oracle_relax_scan_atoms rc={rc}")
+    return {"pos_fz": pos, "iters": iters, "lam_min": lam, "clamped": cl, "lam_traj": lt, "nodes": nodes}
+
+
 def df_weights(n: int, dz: float) -> np.ndarray:
     W = np.empty(n + 1)
     rc = lib().oracle_df_weights(C.c_int(n), C.c_double(dz), _p(W))

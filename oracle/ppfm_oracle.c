@@ -20,6 +20,7 @@
  *   O8  Fz read-out
  *   O9  Giessibl df                      PAPER.md:64-66 (Eq.3; quadrature = reading S9)
  *   O10 stability flag (Hessian)         north_star exemption; reading S14
+ *   O3+O7 with nodes evaluated lazily     SURVEY.md 8(d) (end-to-end check on sampled pixels of large grids)
  *   O11 stiffness map (IETS)
  *   O13 tri-cubic interpolation of E     PAPER.md:264 ("tri-cubic interpolation of the potential"); reading S22
  *   O14 FDBM Pauli repulsion, Eq.8       PAPER.md:118-122; reading S23
@@ -132,8 +133,11 @@ int oracle_forcefield(int natoms, const double *xyzq, const int *type, int ntype
 /* ------------------------------------------------------------------------------------------------------------
  * Grid view used by O4..O10.
  * ---------------------------------------------------------------------------------------------------------- */
+struct lazy_nodes;   /* defined below: grid nodes evaluated on demand from the atoms (O3) and memoised */
+
 typedef struct {
     const void *ff;  /* [nz][ny][nx][4] forces + energy; or, tricubic = 1, [nz][ny][nx] energies only */
+    struct lazy_nodes *lazy; /* != NULL: ff is not stored; node (i,j,k) = ff_at_point(origin + i s0 + j s1 + k s2) */
     int is_f32;      /* 1: float data, widened to double on access (GPU-produced grids) */
     int tricubic;    /* O13: the sample force is -grad of the tri-cubic interpolant of an energy grid */
     double origin[3];
@@ -142,7 +146,10 @@ typedef struct {
     int periodic[3];
 } grid_view;
 
+static const double *lazy_node(struct lazy_nodes *L, const grid_view *g, int i, int j, int k);
+
 static double ff_get(const grid_view *g, int i, int j, int k, int comp) {
+    if (g->lazy) return lazy_node(g->lazy, g, i, j, k)[comp];
     size_t o = (((size_t)k * g->n[1] + j) * g->n[0] + i) * (g->tricubic ? 1 : 4) + (g->tricubic ? 0 : comp);
     return g->is_f32 ? (double)((const float *)g->ff)[o] : ((const double *)g->ff)[o];
 }
@@ -171,6 +178,7 @@ static int invert3(const double *S /* rows = step vectors */, double *Minv) {
 static int make_view(grid_view *g, const void *ff, int is_f32, const double *origin, const double *step,
                      const int *n, const int *periodic) {
     g->ff = ff;
+    g->lazy = NULL;
     g->is_f32 = is_f32 & 1;       /* the callers' flag word: bit 0 = float data, bit 1 = tri-cubic energy grid (O13) */
     g->tricubic = (is_f32 >> 1) & 1;
     for (int d = 0; d < 3; d++) {
@@ -580,6 +588,88 @@ int oracle_pauli_tip(const double *step /* [3][3] */, const int *n, double sigma
  * ---------------------------------------------------------------------------------------------------------- */
 static double norm3(const double v[3]) { return sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]); }
 
+typedef struct {
+    double dt0, dt_max, finc, fdec, alpha0, falpha, f_conv;
+    int n_min, max_iter;
+} fire_t;
+
+typedef struct {
+    double p0[3], dx[3], dy[3], dz;
+    int npx, npy, nz;
+} scan_t;
+
+/* One pixel (ix, iy), all z-steps (O6 + O7 + O8 + O10); output column m of `total` columns. */
+static void relax_pixel(const grid_view *g, const tip_t *tp, const fire_t *fp, const scan_t *sc, int ix, int iy,
+                        int64_t m, int64_t total, double *pos_fz, int *iters, double *lam_min, int *clamped_out,
+                        double *lam_traj) {
+    double dcur[3] = {tp->d0[0], tp->d0[1], tp->d0[2]}; /* O7: d carried from step to step */
+    for (int iz = 0; iz < sc->nz; iz++) {
+        double rtip[3], r[3], v[3] = {0, 0, 0}, F[3];
+        for (int c = 0; c < 3; c++) rtip[c] = sc->p0[c] + ix * sc->dx[c] + iy * sc->dy[c];
+        rtip[2] -= iz * sc->dz;
+        for (int c = 0; c < 3; c++) r[c] = rtip[c] + dcur[c];
+        double dt = fp->dt0, alpha = fp->alpha0;
+        int n_pos = 0, moves = 0, converged = 0, cl = 0;
+        double ltraj = INFINITY;
+        for (;;) { /* O6 */
+            cl = total_force(g, tp, rtip, r, F);
+            if (lam_traj) { /* diagnostic only (O10 / S17): does not touch the FIRE state */
+                double Ht[9], wt[3];
+                hessian(g, tp, rtip, r, Ht);
+                sym3_eig(Ht, wt);
+                if (wt[0] < ltraj) ltraj = wt[0];
+            }
+            double Fn = norm3(F);
+            if (Fn < fp->f_conv) { converged = 1; break; } /* S7: check before moving */
+            if (moves >= fp->max_iter) break;
+            double P = F[0] * v[0] + F[1] * v[1] + F[2] * v[2];
+            if (P >= 0.0) { /* S6: P = 0 counts as downhill */
+                double vn = norm3(v);
+                for (int c = 0; c < 3; c++) v[c] = (1.0 - alpha) * v[c] + alpha * vn * F[c] / Fn;
+                if (n_pos > fp->n_min) {
+                    dt = fmin(dt * fp->finc, fp->dt_max);
+                    alpha *= fp->falpha;
+                }
+                n_pos += 1;
+            } else {
+                v[0] = v[1] = v[2] = 0.0;
+                dt *= fp->fdec;
+                alpha = fp->alpha0;
+                n_pos = 0;
+            }
+            for (int c = 0; c < 3; c++) v[c] += F[c] * dt; /* semi-implicit Euler, m = 1 */
+            for (int c = 0; c < 3; c++) r[c] += v[c] * dt;
+            moves++;
+        }
+        for (int c = 0; c < 3; c++) dcur[c] = r[c] - rtip[c];
+        double FR[3];
+        radial_force(tp, dcur, FR); /* O8: Fz_tip = -F_R,z */
+        size_t o = (size_t)iz * total + m;
+        pos_fz[4 * o + 0] = r[0];
+        pos_fz[4 * o + 1] = r[1];
+        pos_fz[4 * o + 2] = r[2];
+        pos_fz[4 * o + 3] = -FR[2];
+        if (iters) iters[o] = converged ? moves : -1;
+        if (clamped_out) clamped_out[o] = cl;
+        if (lam_traj) lam_traj[o] = ltraj;
+        if (lam_min) {
+            double H[9], w[3];
+            hessian(g, tp, rtip, r, H);
+            sym3_eig(H, w);
+            lam_min[o] = w[0];
+        }
+    }
+}
+
+static void pack_scan(fire_t *fp, scan_t *sc, const double *fire, int n_min, int max_iter, const double *p0,
+                      const double *dx, const double *dy, int npx, int npy, int nz, double dz) {
+    fp->dt0 = fire[0]; fp->dt_max = fire[1]; fp->finc = fire[2]; fp->fdec = fire[3]; fp->alpha0 = fire[4];
+    fp->falpha = fire[5]; fp->f_conv = fire[6];
+    fp->n_min = n_min; fp->max_iter = max_iter;
+    for (int c = 0; c < 3; c++) { sc->p0[c] = p0[c]; sc->dx[c] = dx[c]; sc->dy[c] = dy[c]; }
+    sc->dz = dz; sc->npx = npx; sc->npy = npy; sc->nz = nz;
+}
+
 int oracle_relax_scan(const void *ff, int is_f32, const double *origin, const double *step, const int *n,
                       const int *periodic, const double *k_lat, double k_rad, const double *d0,
                       const double *fire, int n_min, int max_iter, const double *p0, const double *dx,
@@ -589,70 +679,100 @@ int oracle_relax_scan(const void *ff, int is_f32, const double *origin, const do
     if (make_view(&g, ff, is_f32, origin, step, n, periodic)) return -1;
     tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
                 sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2])};
-    const double dt0 = fire[0], dt_max = fire[1], finc = fire[2], fdec = fire[3], alpha0 = fire[4],
-                 falpha = fire[5], f_conv = fire[6];
+    fire_t fp;
+    scan_t sc;
+    pack_scan(&fp, &sc, fire, n_min, max_iter, p0, dx, dy, npx, npy, nz, dz);
     int64_t total = pix ? npix : (int64_t)npx * npy;
 #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t m = 0; m < total; m++) {
         int64_t flat = pix ? pix[m] : m;
-        int ix = (int)(flat % npx), iy = (int)(flat / npx);
-        double dcur[3] = {tp.d0[0], tp.d0[1], tp.d0[2]}; /* O7: d carried from step to step */
-        for (int iz = 0; iz < nz; iz++) {
-            double rtip[3], r[3], v[3] = {0, 0, 0}, F[3];
-            for (int c = 0; c < 3; c++) rtip[c] = p0[c] + ix * dx[c] + iy * dy[c];
-            rtip[2] -= iz * dz;
-            for (int c = 0; c < 3; c++) r[c] = rtip[c] + dcur[c];
-            double dt = dt0, alpha = alpha0;
-            int n_pos = 0, moves = 0, converged = 0, cl = 0;
-            double ltraj = INFINITY;
-            for (;;) { /* O6 */
-                cl = total_force(&g, &tp, rtip, r, F);
-                if (lam_traj) { /* diagnostic only (O10 / S17): does not touch the FIRE state */
-                    double Ht[9], wt[3];
-                    hessian(&g, &tp, rtip, r, Ht);
-                    sym3_eig(Ht, wt);
-                    if (wt[0] < ltraj) ltraj = wt[0];
-                }
-                double Fn = norm3(F);
-                if (Fn < f_conv) { converged = 1; break; } /* S7: check before moving */
-                if (moves >= max_iter) break;
-                double P = F[0] * v[0] + F[1] * v[1] + F[2] * v[2];
-                if (P >= 0.0) { /* S6: P = 0 counts as downhill */
-                    double vn = norm3(v);
-                    for (int c = 0; c < 3; c++) v[c] = (1.0 - alpha) * v[c] + alpha * vn * F[c] / Fn;
-                    if (n_pos > n_min) {
-                        dt = fmin(dt * finc, dt_max);
-                        alpha *= falpha;
-                    }
-                    n_pos += 1;
-                } else {
-                    v[0] = v[1] = v[2] = 0.0;
-                    dt *= fdec;
-                    alpha = alpha0;
-                    n_pos = 0;
-                }
-                for (int c = 0; c < 3; c++) v[c] += F[c] * dt; /* semi-implicit Euler, m = 1 */
-                for (int c = 0; c < 3; c++) r[c] += v[c] * dt;
-                moves++;
+        relax_pixel(&g, &tp, &fp, &sc, (int)(flat % npx), (int)(flat / npx), m, total, pos_fz, iters, lam_min,
+                    clamped_out, lam_traj);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------
+ * The same scan with the grid NOT stored: every node the interpolation touches is evaluated on demand from the
+ * atoms with ff_at_point (O3, exactly the value oracle_forcefield would have stored there) and memoised per pixel.
+ * This is what makes an end-to-end check (the oracle on its own FP64 grid) affordable on grids whose full
+ * evaluation would take hours ("lazily evaluated, memoised FP64 nodes"); no arithmetic differs
+ * from oracle_forcefield + oracle_relax_scan.  nodes_out[m] (optional) = nodes evaluated for pixel m.
+ * ---------------------------------------------------------------------------------------------------------- */
+struct lazy_nodes {
+    int natoms;
+    const double *xyzq;
+    const int *type;
+    const double *R, *e, *cell;
+    const int *nimg;
+    double R_pp, e_pp, Q_pp, r_min;
+    const double *origin, *step;
+    /* open-addressing table: key = flat node index + 1 (0 = empty), value = 4 doubles */
+    int64_t cap, used;
+    int64_t *keys;
+    double *vals;
+};
+
+static const double *lazy_node(struct lazy_nodes *L, const grid_view *g, int i, int j, int k) {
+    const int64_t key = (((int64_t)k * g->n[1] + j) * g->n[0] + i) + 1;
+    if (2 * (L->used + 1) > L->cap) { /* grow and re-insert */
+        int64_t ncap = L->cap ? 2 * L->cap : 1024;
+        int64_t *nk = (int64_t *)calloc((size_t)ncap, sizeof(int64_t));
+        double *nv = (double *)malloc((size_t)ncap * 4 * sizeof(double));
+        for (int64_t s = 0; s < L->cap; s++)
+            if (L->keys[s]) {
+                int64_t h = (int64_t)(((uint64_t)L->keys[s] * 0x9E3779B97F4A7C15ull) >> 11) & (ncap - 1);
+                while (nk[h]) h = (h + 1) & (ncap - 1);
+                nk[h] = L->keys[s];
+                memcpy(nv + 4 * h, L->vals + 4 * s, 4 * sizeof(double));
             }
-            for (int c = 0; c < 3; c++) dcur[c] = r[c] - rtip[c];
-            double FR[3];
-            radial_force(&tp, dcur, FR); /* O8: Fz_tip = -F_R,z */
-            size_t o = (size_t)iz * total + m;
-            pos_fz[4 * o + 0] = r[0];
-            pos_fz[4 * o + 1] = r[1];
-            pos_fz[4 * o + 2] = r[2];
-            pos_fz[4 * o + 3] = -FR[2];
-            if (iters) iters[o] = converged ? moves : -1;
-            if (clamped_out) clamped_out[o] = cl;
-            if (lam_traj) lam_traj[o] = ltraj;
-            if (lam_min) {
-                double H[9], w[3];
-                hessian(&g, &tp, rtip, r, H);
-                sym3_eig(H, w);
-                lam_min[o] = w[0];
-            }
-        }
+        free(L->keys);
+        free(L->vals);
+        L->keys = nk; L->vals = nv; L->cap = ncap;
+    }
+    int64_t h = (int64_t)(((uint64_t)key * 0x9E3779B97F4A7C15ull) >> 11) & (L->cap - 1);
+    while (L->keys[h] && L->keys[h] != key) h = (h + 1) & (L->cap - 1);
+    if (!L->keys[h]) {
+        double p[3];
+        for (int d = 0; d < 3; d++) p[d] = L->origin[d] + i * L->step[d] + j * L->step[3 + d] + k * L->step[6 + d];
+        ff_at_point(p, L->natoms, L->xyzq, L->type, L->R, L->e, L->cell, L->nimg, L->R_pp, L->e_pp, L->Q_pp,
+                    L->r_min, L->vals + 4 * h);
+        L->keys[h] = key;
+        L->used++;
+    }
+    return L->vals + 4 * h;
+}
+
+int oracle_relax_scan_atoms(int natoms, const double *xyzq, const int *type, int ntypes, const double *R,
+                            const double *e, const double *cell, const int *nimg, double R_pp, double e_pp,
+                            double Q_pp, double r_min, const double *origin, const double *step, const int *n,
+                            const int *periodic, const double *k_lat, double k_rad, const double *d0,
+                            const double *fire, int n_min, int max_iter, const double *p0, const double *dx,
+                            const double *dy, int npx, int npy, int nz, double dz, int64_t npix, const int64_t *pix,
+                            double *pos_fz, int *iters, double *lam_min, int *clamped_out, double *lam_traj,
+                            int64_t *nodes_out) {
+    for (int i = 0; i < natoms; i++)
+        if (type[i] < 0 || type[i] >= ntypes) return -1;
+    grid_view g0;
+    if (make_view(&g0, NULL, 0, origin, step, n, periodic)) return -1;
+    tip_t tp = {{k_lat[0], k_lat[1]}, k_rad, {d0[0], d0[1], d0[2]},
+                sqrt(d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2])};
+    fire_t fp;
+    scan_t sc;
+    pack_scan(&fp, &sc, fire, n_min, max_iter, p0, dx, dy, npx, npy, nz, dz);
+    int64_t total = pix ? npix : (int64_t)npx * npy;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t m = 0; m < total; m++) {
+        int64_t flat = pix ? pix[m] : m;
+        struct lazy_nodes L = {natoms, xyzq, type, R, e, cell, nimg, R_pp, e_pp, Q_pp, r_min, origin, step,
+                               0, 0, NULL, NULL};
+        grid_view g = g0;
+        g.lazy = &L;
+        relax_pixel(&g, &tp, &fp, &sc, (int)(flat % npx), (int)(flat / npx), m, total, pos_fz, iters, lam_min,
+                    clamped_out, lam_traj);
+        if (nodes_out) nodes_out[m] = L.used;
+        free(L.keys);
+        free(L.vals);
     }
     return 0;
 }

@@ -12,6 +12,31 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
 
 
+# Exemption accounting of the relaxation parity tests (tests/test_gpu_parity.py appends one record per comparison):
+# how many (pixel, z-step) samples missed the 2e-3 Å tolerance, how many of those carry north_star's end-point flag
+# (smallest Hessian eigenvalue < 1e-3 eV/Å^2 at the relaxed point of this or the previous z-step, or not converged),
+# and how many are exempt ONLY through the trajectory flag of reading S17.  Printed at the end of the session.
+PARITY_LOG = []
+
+
+def pytest_terminal_summary(terminalreporter, exitstatus, config):
+    if not PARITY_LOG:
+        return
+    tr = terminalreporter
+    tr.write_sep("-", "relaxation parity: samples outside 2e-3 Å and how they are exempt (reading S17)")
+    tr.write_line(f"{'case':58s} {'samples':>9s} {'fail':>6s} {'end-point flag':>15s} {'trajectory flag only':>21s} "
+                  f"{'max |dr| ok (Å)':>16s}")
+    for r in PARITY_LOG:
+        tr.write_line(f"{r['what'][:58]:58s} {r['samples']:9d} {r['fail']:6d} {r['fail_endpoint_flag']:15d} "
+                      f"{r['fail_traj_only']:21d} {r['max_ok_dist']:16.2e}")
+    out = os.path.join(ROOT, "gpurun_out")
+    if os.path.isdir(out):
+        import json
+        with open(os.path.join(out, "parity_exemptions.jsonl"), "w") as fh:
+            for r in PARITY_LOG:
+                fh.write(json.dumps(r) + "\n")
+
+
 def pytest_collection_modifyitems(config, items):
     # GPU tests must never pass silently on a box without a device: they are deselected by `-m "not gpu"`;
     # when explicitly selected without a GPU they fail loudly inside the binding (no CPU fallback exists).

@@ -9,15 +9,27 @@ Tolerances (BASELINE.json north_star; readings S13, S16, S17 in DESIGN.md):
                the FIRE trajectory of that or the previous z-step, readings S17)
   df           within 1e-2 Hz or 0.5 %
 """
+import math
+import os
 from dataclasses import replace
 
 import numpy as np
 import pytest
 
+from conftest import PARITY_LOG
 from oracle import oracle
 from paper_2401_14564_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
+
+# Seeds of the sampled grid points / pixels are offset by PPFM_TEST_SEED (default 0), so that a different sample of
+# the large configs can be drawn: PPFM_TEST_SEED=7 python -m pytest tests -m gpu
+SEED0 = int(os.environ.get("PPFM_TEST_SEED", "0"))
+
+
+def sample(n_total, n_sample, seed):
+    return W.sample_indices(n_total, n_sample, seed + 1000 * SEED0)
+
 
 # Energy lane (float4.w, not used by the relaxation; north_star states no tolerance for it).  DESIGN.md
 # "Tolerances": FP32 accumulation of N = atoms x images Coulomb terms of random sign whose partial sums reach
@@ -59,16 +71,43 @@ def check_ff(got, ref, what=""):
     return (rel.max() if rel.size else 0.0), (dF[~big].max() if (~big).any() else 0.0)
 
 
-def check_positions(pos_gpu, ref, what=""):
-    """pos_gpu (nz, npix, 4) vs oracle dict; returns fraction within 2e-3 Å."""
+def check_positions(pos_gpu, ref, what="", max_traj_only=None):
+    """pos_gpu (nz, npix, 4) vs oracle dict; returns (fraction within 2e-3 Å, distances).
+
+    north_star: within 2e-3 Å on >= 99.9 % of samples, the rest limited to samples the oracle flags near-unstable.
+    The failing samples are counted by the way they are exempt and logged (conftest.PARITY_LOG): `end-point flag` =
+    north_star's own criterion (lambda_min < 1e-3 eV/Å^2 at the relaxed point of this or the previous z-step, or not
+    converged); `trajectory flag only` = exempt only because lambda_min < 1e-3 somewhere along the FIRE path
+    (reading S17).  The latter is bounded: at most max(2, 2e-5 x samples) per comparison unless a test states
+    another number."""
     d = np.linalg.norm(np.asarray(pos_gpu, np.float64)[..., :3] - ref["pos_fz"][..., :3], axis=-1)
     ok = d <= 2e-3
+    end_flag = oracle.near_unstable(ref["lam_min"]) | (ref["iters"] < 0)
     flagged = oracle.flags(ref)
+    bad = ~ok
+    rec = {"what": what, "samples": int(d.size), "fail": int(bad.sum()), "fail_endpoint_flag": int((bad & end_flag).sum()),
+           "fail_traj_only": int((bad & flagged & ~end_flag).sum()), "fail_unflagged": int((bad & ~flagged).sum()),
+           "flagged_endpoint": int(end_flag.sum()), "flagged_any": int(flagged.sum()),
+           "max_ok_dist": float(d[ok].max()) if ok.any() else 0.0}
+    PARITY_LOG.append(rec)
+    print("parity", rec)
     frac = ok.mean()
     assert frac >= 0.999, f"{what}: only {frac:.5f} of samples within 2e-3 Å (max {d.max():.3e})"
-    bad = ~ok
-    assert not np.any(bad & ~flagged), f"{what}: {int((bad & ~flagged).sum())} failing samples are not flagged near-unstable"
+    assert rec["fail_unflagged"] == 0, f"{what}: {rec['fail_unflagged']} failing samples are not flagged near-unstable"
+    bound = max(2, math.ceil(2e-5 * d.size)) if max_traj_only is None else max_traj_only
+    assert rec["fail_traj_only"] <= bound, f"{what}: {rec['fail_traj_only']} samples exempt only by the trajectory flag (> {bound})"
     return frac, d
+
+
+def check_iters(it_gpu, ref, d, what=""):
+    """FIRE move counts of the FP32 kernel against the FP64 oracle on samples that agree and are not flagged: the same
+    path, a move or two apart (mean |difference| < 2)."""
+    it = np.asarray(it_gpu).view(np.uint16).astype(np.int64).reshape(ref["iters"].shape)
+    comparable = (ref["iters"] >= 0) & ~oracle.flags(ref)
+    same = (d <= 2e-3) & comparable & (it != 0xFFFF)
+    assert same.sum() >= 0.99 * comparable.sum() and same.sum() >= 100, what
+    diff = np.abs(it - ref["iters"])[same]
+    assert diff.mean() < 2.0, f"{what}: mean |iters_gpu - iters_oracle| = {diff.mean():.2f}"
 
 
 def check_df(got, ref, what=""):
@@ -138,7 +177,7 @@ def test_ff_rmin_clamp_grid_point_on_atom(P):
 def test_ff_sampled_cfg2_and_Q_sweep_split_combine(P):
     import torch
     w = W.get(2)
-    idx = W.sample_indices(w.npoints, 4000, 21)
+    idx = sample(w.npoints, 4000, 21)
     xyzq, types = P.upload(w)
     lj, el = P.forcefield_split(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
     for Q in w.Q_sweep:
@@ -163,7 +202,7 @@ def test_ff_batch_cfg3_matches_oracle_and_single_calls(P):
         got = out[m * npts:(m + 1) * npts].cpu().numpy()
         single = gpu_ff(P, mols[m]).reshape(-1, 4).cpu().numpy()
         assert np.array_equal(got, single)                    # bit-reproducible, batch == single
-        idx = W.sample_indices(npts, 20000, 31 + m)
+        idx = sample(npts, 20000, 31 + m)
         check_ff(got[idx], oracle.forcefield(mols[m], idx=idx), f"cfg3 mol {m}")
 
 
@@ -223,7 +262,7 @@ def cfg4(P):
 def test_ff_full_size_cfg4_sampled(cfg4):
     import torch
     w, ff = cfg4[0], cfg4[1]
-    idx = W.sample_indices(w.npoints, 1500, 41)
+    idx = sample(w.npoints, 1500, 41)
     got = ff.reshape(-1, 4)[torch.from_numpy(idx).cuda()].cpu().numpy()
     check_ff(got, oracle.forcefield(w, idx=idx), "cfg4 sampled")
     assert bool(torch.isfinite(ff).all())
@@ -282,25 +321,66 @@ def test_relax_and_df_full_scan(P, cfg):
     assert abs(it_h[conv].mean() - ref64["iters"][ref64["iters"] >= 0].mean()) < 0.05 * ref64["iters"].mean()
 
 
-def test_relax_sampled_cfg2_periodic(P):
+def check_df_end_to_end(df_gpu, ref, d, w, what=""):
+    """GPU df against the oracle's df of ITS OWN Fz stack, in every window whose n + 1 relaxed positions agree."""
+    df_ref = oracle.df(ref["pos_fz"][..., 3], w.scan.dz, w.df.A, w.df.k0, w.df.f0)
+    n = w.n_df
+    bad = d > 2e-3
+    win_ok = np.stack([~bad[k:k + n + 1].any(axis=0) for k in range(df_ref.shape[0])])
+    g = np.asarray(df_gpu, np.float64).reshape(df_ref.shape)
+    err = np.abs(g - df_ref)
+    assert ((err <= 1e-2) | (err <= 5e-3 * np.abs(df_ref)))[win_ok].all(), f"{what}: end-to-end df {err[win_ok].max():.3e} Hz"
+    assert win_ok.mean() > 0.99, what
+
+
+def test_relax_cfg2_all_three_tip_charges_gpu_grid_and_end_to_end(P):
+    """Config 2 (periodic slab, 9 images) at all three tip charges of its sweep, in the launch configuration bench.py
+    times (one split force-field pass, then combine + scan + df per Q): (ii) the oracle on the GPU's combined grid,
+    400 sampled pixels; (i) END TO END: the oracle relaxing on its own FP64 force field (nodes evaluated from the atoms
+    on demand), 200 sampled pixels; df both ways; FIRE move counts."""
+    import torch
     w = W.get(2)
-    ff, pos, iters, df, st = gpu_scan(P, w)
-    pix = W.sample_indices(w.scan.npx * w.scan.npy, 400, 51)
-    ref = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan, pix=pix)
-    pos_h = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix]
-    check_positions(pos_h, ref, "cfg2 sampled")
-    dfh = df.cpu().numpy().reshape(df.shape[0], -1)[:, pix]
-    check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0), "cfg2 df")
+    xyzq, types = P.upload(w)
+    lj, el = P.forcefield_split(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
+    npix = w.scan.npx * w.scan.npy
+    for q, Q in enumerate(w.Q_sweep):
+        ff = P.combine(lj, el, Q)
+        ff, pos, iters, df, st = gpu_scan(P, w, ff=ff)
+        pix = sample(npix, 400, 51 + q)
+        ref = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan, pix=pix)
+        pos_h = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix]
+        frac, d = check_positions(pos_h, ref, f"cfg2 Q={Q:+.1f} (GPU grid, 400 px)")
+        check_iters(iters.cpu().numpy().reshape(w.scan.nz, -1)[:, pix], ref, d, f"cfg2 Q={Q}")
+        dfh = df.cpu().numpy().reshape(df.shape[0], -1)[:, pix]
+        check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0), f"cfg2 df Q={Q}")
+        pix2 = sample(npix, 200, 151 + q)
+        ref2 = oracle.relax_scan_atoms(w, pix=pix2, Q=Q)
+        pos2 = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix2]
+        frac2, d2 = check_positions(pos2, ref2, f"cfg2 Q={Q:+.1f} (end to end, 200 px)")
+        assert np.abs(pos2[..., 3] - ref2["pos_fz"][..., 3])[d2 <= 2e-3].max() < 2e-4
+        check_df_end_to_end(df.cpu().numpy().reshape(df.shape[0], -1)[:, pix2], ref2, d2, w, f"cfg2 Q={Q}")
+        assert st["n_clamped"] == 0 and int(ref2["clamped"].sum()) == 0
+    torch.cuda.synchronize()
 
 
-def test_relax_full_size_cfg4_sampled(cfg4):
+def test_relax_full_size_cfg4_sampled_gpu_grid_and_end_to_end(cfg4):
+    """Config 4 at full size: (ii) 150 sampled pixels, oracle on the GPU's 1.9 GiB grid; (i) END TO END on 96 sampled
+    pixels, the oracle evaluating its own FP64 grid nodes from the 45 000 atom images on demand."""
     w, ff, pos, iters, df, st = cfg4
-    pix = W.sample_indices(w.scan.npx * w.scan.npy, 150, 61)
+    npix = w.scan.npx * w.scan.npy
+    pix = sample(npix, 150, 61)
     ref = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan, pix=pix)
     pos_h = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix]
-    check_positions(pos_h, ref, "cfg4 sampled")
+    frac, d = check_positions(pos_h, ref, "cfg4 (GPU grid, 150 px)")
+    check_iters(iters.cpu().numpy().reshape(w.scan.nz, -1)[:, pix], ref, d, "cfg4")
     dfh = df.cpu().numpy().reshape(df.shape[0], -1)[:, pix]
     check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0), "cfg4 df")
+    pix2 = sample(npix, 96, 161)
+    ref2 = oracle.relax_scan_atoms(w, pix=pix2)
+    pos2 = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix2]
+    frac2, d2 = check_positions(pos2, ref2, "cfg4 (end to end, 96 px)")
+    assert np.abs(pos2[..., 3] - ref2["pos_fz"][..., 3])[d2 <= 2e-3].max() < 2e-4
+    check_df_end_to_end(df.cpu().numpy().reshape(df.shape[0], -1)[:, pix2], ref2, d2, w, "cfg4")
     assert st["n_clamped"] == 0
     assert st["n_not_converged"] <= 1e-3 * w.pixel_steps
 
@@ -322,14 +402,99 @@ def test_relax_batch_cfg3(P):
     nps = s.npx * s.npy * s.nz
     npts = mols[0].npoints
     for m in (0, 3):
-        pix = W.sample_indices(s.npx * s.npy, 300, 71 + m)
+        pix = sample(s.npx * s.npy, 300, 71 + m)
         grid_h = ff[m * npts:(m + 1) * npts].cpu().numpy().reshape(mols[m].grid.n[2], mols[m].grid.n[1],
                                                                   mols[m].grid.n[0], 4)
         ref = oracle.relax_scan(grid_h, mols[m].grid, mols[m].tip, mols[m].fire, mols[m].scan, pix=pix)
         pos_h = pos[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1, 4)[:, pix]
-        check_positions(pos_h, ref, f"cfg3 mol {m}")
+        frac, d = check_positions(pos_h, ref, f"cfg3 mol {m} (GPU grid, 300 px)")
+        check_iters(iters[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1)[:, pix], ref, d, f"cfg3 mol {m}")
         dfh = df[m].cpu().numpy().reshape(df.shape[1], -1)[:, pix]
         check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), s.dz, 1.0, 1800.0, 30300.0), f"cfg3 df {m}")
+        # end to end: the oracle on its own FP64 field of this molecule
+        pix2 = sample(s.npx * s.npy, 300, 171 + m)
+        ref2 = oracle.relax_scan_atoms(mols[m], pix=pix2)
+        pos2 = pos[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1, 4)[:, pix2]
+        frac2, d2 = check_positions(pos2, ref2, f"cfg3 mol {m} (end to end, 300 px)")
+        check_df_end_to_end(df[m].cpu().numpy().reshape(df.shape[1], -1)[:, pix2], ref2, d2, mols[m], f"cfg3 mol {m}")
+
+
+# Every relax kernel instance the dispatcher can pick (relax.cu: ORTHO x ANYPER x SYMTIP x TRICUBIC, single and batch
+# form) against the oracle on a small system: the grid data are the ORACLE's (its FP64 grid rounded to FP32), so both
+# sides read the same numbers.  SYMTIP = false is the asymmetric tip of PAPER.md:54 ("may be deflected in x, y to
+# simulate an asymmetric CO tip"): d0 = (0.3, -0.2, -3.98), k_x != k_y.
+@pytest.fixture(scope="module")
+def small_system():
+    w = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
+    out = {}
+    for ortho in (True, False):
+        step = np.diag([0.5, 0.5, 0.25]) if ortho else np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
+        wg = replace(w, grid=replace(w.grid, step=step))
+        out[ortho] = (wg, oracle.forcefield(wg).astype(np.float32))
+    return out
+
+
+@pytest.mark.parametrize("tricubic", [False, True], ids=["trilinear", "tricubic"])
+@pytest.mark.parametrize("symtip", [True, False], ids=["symtip", "asymtip"])
+@pytest.mark.parametrize("anyper", [False, True], ids=["clamped", "periodic"])
+@pytest.mark.parametrize("ortho", [True, False], ids=["ortho", "skewed"])
+def test_relax_every_kernel_instance(P, small_system, ortho, anyper, symtip, tricubic):
+    """relax_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC> and relax_batch_kernel<...> for all 16 combinations."""
+    import torch
+    w, ff_o = small_system[ortho]
+    tip = w.tip if symtip else replace(w.tip, k_lat=(0.012, 0.019), d0=(0.3, -0.2, -3.98))
+    if anyper:      # periodic x, y; the scan reaches over the seam
+        grid, scan = replace(w.grid, periodic=(1, 1, 0)), replace(w.scan, p0=np.array([-3.0, 20.0, 9.0]))
+    else:           # non-periodic; part of the scan hangs over the grid faces (clamped, reading S12)
+        grid, scan = replace(w.grid, periodic=(0, 0, 0)), replace(w.scan, p0=np.array([-1.8, 17.0, 9.0]))
+    data = np.ascontiguousarray(ff_o[..., 3]) if tricubic else ff_o
+    run = P.relax_scan_tricubic if tricubic else P.relax_scan
+    run_b = P.relax_scan_tricubic_batch if tricubic else P.relax_scan_batch
+    name = f"relax_kernel<{int(ortho)},{int(anyper)},{int(symtip)},{int(tricubic)}>"
+    dev = torch.from_numpy(data).cuda()
+    stats = P.new_stats()
+    pos, iters = run(dev, grid, tip, w.fire, scan, stats=stats)
+    torch.cuda.synchronize()
+    npix = scan.npx * scan.npy
+    ref = oracle.relax_scan(data, grid, tip, w.fire, scan)
+    assert np.abs(ref["pos_fz"][..., :2] - (oracle.tip_positions(scan) + np.array(tip.d0))[..., :2]).max() > 0.05   # the field acts
+    frac, d = check_positions(pos.cpu().numpy().reshape(scan.nz, npix, 4), ref, name, max_traj_only=3)
+    ok = d <= 2e-3
+    assert np.abs(pos.cpu().numpy().reshape(scan.nz, npix, 4)[..., 3] - ref["pos_fz"][..., 3])[ok].max() < 2e-4
+    st = P.read_stats(stats)
+    assert st["n_clamped"] == int(ref["clamped"].sum())
+    assert (st["n_clamped"] > 0) == (not anyper)
+    assert st["n_not_converged"] == int((ref["iters"] < 0).sum())
+    check_iters(iters.cpu().numpy(), ref, d, name)
+    # batch form: two systems (the second with another lateral stiffness), bit for bit the single-system results
+    tip2 = replace(tip, k_lat=(tip.k_lat[0] * 1.3, tip.k_lat[1] * 1.3))
+    posb, itb = run_b(torch.cat([dev.reshape(-1), dev.reshape(-1)]).reshape((2,) + tuple(dev.shape)), [grid, grid],
+                      [tip, tip2], w.fire, [scan, scan])
+    pos2, it2 = run(dev, grid, tip2, w.fire, scan)
+    torch.cuda.synchronize()
+    nps = scan.nz * npix
+    assert torch.equal(posb[:nps], pos.reshape(-1, 4)) and torch.equal(posb[nps:], pos2.reshape(-1, 4))
+    assert torch.equal(itb[:nps], iters.reshape(-1)) and torch.equal(itb[nps:], it2.reshape(-1))
+
+
+def test_relax_asymmetric_tip_cfg0_full_scan_end_to_end(P):
+    """the asymmetric tip on config 0, full scan, against the oracle on its own FP64 grid (end to end) and
+    on the GPU's grid; df too."""
+    w = W.get(0)
+    w = replace(w, tip=replace(w.tip, k_lat=(0.012, 0.019), d0=(0.3, -0.2, -3.98)))
+    ff, pos, iters, df, st = gpu_scan(P, w)
+    npix = w.scan.npx * w.scan.npy
+    pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)
+    ref32 = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan)
+    check_positions(pos_h, ref32, "cfg0 asymmetric tip (GPU grid)")
+    ref64 = oracle.relax_scan(oracle.forcefield(w), w.grid, w.tip, w.fire, w.scan)
+    frac, d = check_positions(pos_h, ref64, "cfg0 asymmetric tip (end to end)")
+    assert np.abs(pos_h[..., 3] - ref64["pos_fz"][..., 3])[d <= 2e-3].max() < 2e-4
+    check_iters(iters.cpu().numpy(), ref64, d, "cfg0 asymmetric tip")
+    check_df_end_to_end(df.cpu().numpy(), ref64, d, w, "cfg0 asymmetric tip")
+    # the deflected equilibrium shows: far from the sample the PP hangs at r_TIP + d0
+    far = pos_h[0].reshape(w.scan.npy, w.scan.npx, 4)[0, 0, :3] - w.scan.p0
+    assert np.allclose(far, w.tip.d0, atol=0.05)
 
 
 def test_relax_zero_field_and_ragged_scan(P):
@@ -371,7 +536,7 @@ def test_relax_uniform_and_linear_field_closed_forms(P):
     pos, _ = P.relax_scan(torch.from_numpy(ffh).cuda(), g, tip, W.Fire(), sc)
     df = P.df(pos, sc.npx, sc.npy, sc.nz, sc.dz, 1.0, 1800.0, 30300.0).cpu().numpy()
     want = -(30300.0 / 3600.0) * 16.02176634 * tip.k_rad * gsl / (tip.k_rad - gsl)
-    assert np.allclose(df, want, rtol=5e-3, atol=1e-2)
+    assert np.allclose(df, want, rtol=5e-3, atol=1e-2)      # north_star's df tolerance (0.5 % or 1e-2 Hz); the oracle's own pin holds 1e-7
 
 
 def test_relax_periodic_wrap_and_clamp(P):

@@ -408,6 +408,29 @@ def test_relaxed_positions_mirror_symmetric_molecule():
     assert np.allclose((pos[..., 1:] - pos[:, :, ::-1, 1:])[ok], 0.0, atol=1e-5)
 
 
+def test_lazy_node_scan_is_the_stored_grid_scan_bit_for_bit():
+    """oracle.relax_scan_atoms (grid nodes evaluated on demand from the atoms and memoised per pixel) must be the
+    scan on the stored FP64 grid, bit for bit: config 0 sampled pixels, a periodic skewed grid with 9 images (nodes
+    reached across the seam), and a non-periodic grid the probe particle leaves (clamping)."""
+    w = W.get(0)
+    pix = W.sample_indices(w.scan.npx * w.scan.npy, 25, 3)
+    a = oracle.relax_scan(oracle.forcefield(w), w.grid, w.tip, w.fire, w.scan, pix=pix)
+    b = oracle.relax_scan_atoms(w, pix=pix)
+    for k in ("pos_fz", "iters", "lam_min", "clamped", "lam_traj"):
+        assert np.array_equal(a[k], b[k]), k
+    assert np.all(b["nodes"] > 8) and np.all(b["nodes"] < 0.2 * w.npoints)        # a small part of the grid
+    w2 = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(5, 4), scan_nz=6)
+    step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
+    w2 = replace(w2, grid=replace(w2.grid, step=step), scan=replace(w2.scan, p0=np.array([-3.0, 20.0, 9.0])))
+    for per, p0 in (((1, 1, 0), [-3.0, 20.0, 9.0]), ((0, 0, 0), [-1.0, 23.0, 12.5])):
+        w3 = replace(w2, grid=replace(w2.grid, periodic=per), scan=replace(w2.scan, p0=np.array(p0)))
+        a = oracle.relax_scan(oracle.forcefield(w3), w3.grid, w3.tip, w3.fire, w3.scan)
+        b = oracle.relax_scan_atoms(w3)
+        for k in ("pos_fz", "iters", "lam_min", "clamped", "lam_traj"):
+            assert np.array_equal(a[k], b[k]), (per, k)
+    assert int(b["clamped"].sum()) > 0
+
+
 def test_max_iter_flag():
     g, ff = _flat_grid()
     ff[..., 2] = 0.03
