@@ -1,18 +1,19 @@
 #!/usr/bin/env python
 """bench.py — one "step" = one pass of the whole hot path (force-field grid -> FIRE relaxation scan -> df) over one
-seeded synthetic workload (BASELINE.json configs; default configs[1]).  Prints ONE JSON line (rank 0).
+seeded synthetic workload of BASELINE.json.  Prints ONE JSON line (rank 0).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference] [--no-cpu-baseline]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+                  [--no-cpu-baseline] [--no-per-config]
 
-* `value` (device-resident inputs): relaxed pixel-steps per second over the full scan, CUDA-event timed per step on
-  the launching stream, L2 flushed between steps, max over ranks.  `parts` carries the other two thirds of
-  BASELINE.json's metric (FF pair-interactions/s with its FP32 fraction, seconds per full scan) and the
-  relax kernel's own rate.
-* `e2e`: the same scan through the one-call host API ppfm_scan_host with pinned HOST buffers (H2D of the atoms and
-  D2H of positions, iteration counts and df inside the timed region).
-* `roofline`: the step's dominant kernel; `roofline_kernels` all three.  FF is ALU-bound (peak = SMs x 128 FP32
-  lanes x max SM clock), relax is bound by the cache gather rate (peak = the in-run gather
-  micro-benchmark = "achievable L2 bandwidth"), df streams HBM (peak = MEASURED_PEAKS.json hbm_gbs).
+Default workload: configs[4], the largest single-GPU configuration.  The other four configs are measured in the
+same process (3 warm-up + 3 timed steps each) and reported as compact numeric records under `parts.per_config`, so
+that one driver run carries the force-field and relaxation fractions of all five configs.
+
+* `value` (device-resident inputs): relaxed pixel-steps per second over the full scan; CUDA events per step on the
+  launching stream, L2 flushed between steps, max over ranks.
+* `e2e`: the same scan through the one-call host API ppfm_scan_host[_batch|_sweep] with pinned HOST buffers.
+* `roofline`: the step's dominant kernel with the bound that binds it; `roofline_kernels`: ff, relax, df of the
+  headline config.  What the fields mean, the algorithmic counts and the peaks are stated in DESIGN.md §6.
 * `cpu_baseline`: the FP64 oracle, as it stands, timed on this box's host cores on a bounded sample.
 * `--impl reference`: the oracle arm (this tier has no reference implementation to install).
 The oracle is imported ONLY by the cpu_baseline leg and the reference arm.
@@ -20,6 +21,7 @@ The oracle is imported ONLY by the cpu_baseline leg and the reference arm.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import sys
@@ -43,20 +45,16 @@ WORKLOAD_NAME = {0: "configs[0] tiny 10 atoms, 60x60x40 grid, 30x30x40 scan",
                  2: "configs[2] molecule on 500-atom periodic slab (9 images), 250x250x120 grid, 200x200x40 scan x 3 Q",
                  3: "configs[3] ML batch of 64 molecules (20-50 atoms), 128x128x64 grids, 128x128x20 scans",
                  4: "configs[4] 5000 atoms x 9 images, 800x800x200 grid, 400x400x80 scan"}
-# canonical algorithmic work per pair interaction: 19 FP32-pipe instructions, 28 flops
-PAIR_INSTR, PAIR_FLOPS = 19, 28
-# what ff_kernel executes per pair and grid point (ff.cu inner loop, FP32x2-packed): 15 FP32-pipe lane-instructions
-# + 1 MUFU for an atom with a Coulomb factor, 13 + 1 for an LJ-only atom (split kernel: 20 / 14)
+# ---- algorithmic counts ------------------------------------------------------------------------------
+PAIR_INSTR, PAIR_FLOPS = 19, 28        # canonical per pair interaction: FP32-pipe instructions, flops
+# what ff_kernel executes per pair (ff.cu, FP32x2-packed): lane-instructions for an atom with / without a Coulomb factor
 PAIR_EXEC = {"charged": 15, "neutral": 13, "charged_split": 20, "neutral_split": 14}
-# what relax_kernel's cached-cell iteration needs (relax.cu, symmetric tip): 44 FFMA + 13 FMUL + 13 FADD = 70
-# FP32-pipe lane-instructions = 114 flops, + 4 MUFU
-ITER_INSTR, ITER_FLOPS = 70, 114
+ITER_INSTR, ITER_FLOPS = 70, 114       # relax_kernel per FIRE iteration (cached cell, symmetric tip); + 4 MUFU
+TRI_INSTR, TRI_FLOPS = 270, 514        # the tri-cubic instance
 SMS, LANES = 148, 128
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/);
-# None where no capture exists for that kernel and config.
-NCU_TRAFFIC = {(1, "ff"): 6.59e6, (1, "relax"): 13.59e6, (1, "df"): 14.41e6, (1, "stiffness"): 27.43e6,
-               (1, "fft_el"): 2.06e9, (2, "ff"): 188.8e6,
-               (3, "ff"): 1.0149e9, (3, "relax"): 513.8e6, (3, "df"): 454.7e6}      # profiles/r01e_full_cfg{1,2,3}*.txt
+# relax_kernel time (ms) of the committed kernels on a B200 at 1965 MHz; the run reports relax ms against 1.1 x these
+# so that a slower instruction schedule of the same source (DESIGN.md §7 "schedule sensitivity") shows up
+PERF_GUARD_RELAX_MS = {0: 0.49, 1: 0.75, 2: 3.35, 3: 8.5, 4: 4.9}
 
 
 def measured_peaks():
@@ -66,6 +64,31 @@ def measured_peaks():
             d = json.load(f)
         return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+def ncu_traffic(cfg: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+    (profiles/r02_traffic.json, written from the captures named there); None where no capture exists."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f).get(f"cfg{cfg}", {}).get(kernel)
+
+
+def inputs_sha256(ws) -> str:
+    """SHA-256 over the generated inputs of a workload list (atoms, types, and every scalar of grid / scan / tip)."""
+    h = hashlib.sha256()
+    for w in ws:
+        h.update(np.ascontiguousarray(w.xyzq, dtype=np.float32).tobytes())
+        h.update(np.ascontiguousarray(w.types, dtype=np.int32).tobytes())
+        for arr in (w.elem_R, w.elem_e, w.lattice.a, w.lattice.b, w.lattice.c, w.lattice.nimg, w.grid.origin,
+                    w.grid.step, w.grid.n, w.grid.periodic, [w.probe.R, w.probe.e, w.probe.Q], w.tip.k_lat,
+                    [w.tip.k_rad], w.tip.d0, w.scan.p0, w.scan.dx, w.scan.dy,
+                    [w.scan.npx, w.scan.npy, w.scan.nz, w.scan.dz], [w.df.A, w.df.k0, w.df.f0, w.r_min],
+                    w.Q_sweep or []):
+            h.update(np.ascontiguousarray(arr, dtype=np.float64).tobytes())
+    return h.hexdigest()
 
 
 # ------------------------------------------------------------------------------------------------- clock sampling
@@ -100,7 +123,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            self._stop.wait(0.002)      # short timed regions (configs 0, 1: ~20 ms) still get several samples
+            self._stop.wait(0.002)
 
     def start(self):
         if self.nv is not None:
@@ -128,6 +151,7 @@ class DeviceJob:
     """Device-resident buffers of one rank's systems and the step that runs the three entry points on them."""
 
     def __init__(self, P, torch, cfg, ws):
+        import ctypes
         self.P, self.torch, self.cfg, self.ws = P, torch, cfg, ws
         self.batch = len(ws) > 1
         w0 = ws[0]
@@ -153,10 +177,10 @@ class DeviceJob:
         self.c_tip = P.c_array([w.tip for w in ws], P.c_tip)
         self.c_scan = P.c_array([w.scan for w in ws], P.c_scan)
         self.c_fire = P.c_fire(w0.fire)
-        import ctypes
         self.c_off = (ctypes.c_int32 * (len(ws) + 1))(*[int(v) for v in self.off])
         self.pairs = float(sum(w.pairs for w in ws))
-        self.pixel_steps = float(nps * (len(self.sweep) if self.sweep else 1))
+        self.n_runs = len(self.sweep) if self.sweep else 1
+        self.pixel_steps = float(nps * self.n_runs)
         self.points = float(npts)
         self.marks = []
 
@@ -173,7 +197,6 @@ class DeviceJob:
         return tot
 
     def relax_tricubic(self, E, stats):
-        """The scan of step() on the energy-only grid E with tri-cubic interpolation (last Q of a sweep)."""
         P = self.P
         if self.batch:
             P.relax_scan_tricubic_batch(E, self.c_grid, self.c_tip, self.c_fire, self.c_scan, pos_fz=self.pos,
@@ -183,8 +206,7 @@ class DeviceJob:
                                   iters=self.iters, stats=stats)
 
     def stiffness(self, out):
-        """Stiffness map of the scan held in self.pos (last Q of a sweep) on the resident grid."""
-        P, ws = self.P, self.ws
+        P = self.P
         if self.batch:
             P.stiffness_batch(self.ff, self.c_grid, self.c_tip, self.c_scan, self.pos, out=out)
         else:
@@ -196,7 +218,7 @@ class DeviceJob:
         self.marks.append((name, ev))
 
     def step(self):
-        """Enqueue one full scan; event marks separate the kernels (all on torch's current stream)."""
+        """Enqueue one full scan (all on torch's current stream); event marks bracket the whole step."""
         P, ws, w0 = self.P, self.ws, self.ws[0]
         s = w0.scan
         self.marks = []
@@ -204,40 +226,27 @@ class DeviceJob:
         if self.batch:
             P.forcefield_batch(self.c_off, self.xyzq, self.types, w0.elem_R, w0.elem_e, self.c_lat, self.c_probe,
                                self.c_grid, w0.r_min, out=self.ff)
-            self._mark("ff")
             P.relax_scan_batch(self.ff, self.c_grid, self.c_tip, self.c_fire, self.c_scan,
                                pos_fz=self.pos, iters=self.iters, stats=self.stats)
-            self._mark("relax")
             P.df(self.pos, s.npx, s.npy, s.nz, s.dz, w0.df.A, w0.df.k0, w0.df.f0, out=self.df, nsys=len(ws))
-            self._mark("df")
         elif self.sweep:
             P.forcefield_split(self.xyzq, self.types, w0.elem_R, w0.elem_e, self.c_lat[0], self.c_probe[0],
                                self.c_grid[0], w0.r_min, out_lj=self.ff_lj, out_el=self.ff_el)
-            self._mark("ff")
             for Q in self.sweep:
                 P.combine(self.ff_lj, self.ff_el, Q, out=self.ff)
-                self._mark("combine")
                 P.relax_scan(self.ff, self.c_grid[0], self.c_tip[0], self.c_fire, self.c_scan[0], pos_fz=self.pos,
                              iters=self.iters, stats=self.stats)
-                self._mark("relax")
                 P.df(self.pos, s.npx, s.npy, s.nz, s.dz, w0.df.A, w0.df.k0, w0.df.f0, out=self.df)
-                self._mark("df")
         else:
             P.forcefield(self.xyzq, self.types, w0.elem_R, w0.elem_e, self.c_lat[0], self.c_probe[0], self.c_grid[0],
                          w0.r_min, out=self.ff)
-            self._mark("ff")
             P.relax_scan(self.ff, self.c_grid[0], self.c_tip[0], self.c_fire, self.c_scan[0], pos_fz=self.pos,
                          iters=self.iters, stats=self.stats)
-            self._mark("relax")
             P.df(self.pos, s.npx, s.npy, s.nz, s.dz, w0.df.A, w0.df.k0, w0.df.f0, out=self.df)
-            self._mark("df")
+        self._mark("end")
 
-    def durations_ms(self):
-        """After a synchronise: (total ms, {kernel: ms}) of the last step from its event marks."""
-        out = {}
-        for (_, e0), (name, e1) in zip(self.marks[:-1], self.marks[1:]):
-            out[name] = out.get(name, 0.0) + e0.elapsed_time(e1)
-        return self.marks[0][1].elapsed_time(self.marks[-1][1]), out
+    def step_ms(self):
+        return self.marks[0][1].elapsed_time(self.marks[-1][1])
 
 
 class HostJob:
@@ -245,7 +254,6 @@ class HostJob:
 
     def __init__(self, P, torch, ws):
         from dataclasses import replace as _replace
-        # argument marshalling done once (as DeviceJob does): ready ctypes structs pass straight through the binding
         ws = [_replace(w, lattice=P.c_lattice(w.lattice), grid=P.c_grid(w.grid), tip=P.c_tip(w.tip),
                        fire=P.c_fire(w.fire), scan=P.c_scan(w.scan)) for w in ws]
         self.P, self.ws = P, ws
@@ -260,9 +268,8 @@ class HostJob:
             hi = torch.empty((nq, s.nz, s.npy, s.npx), dtype=torch.int16).pin_memory()
             hd = torch.empty((nq, s.nz - w.n_df, s.npy, s.npx), dtype=torch.float32).pin_memory()
             self.bufs.append((hx, ht, hp, hi, hd))
-            self.h2d += nq * (hx.numel() * 4 + ht.numel() * 4)
-            self.d2h += nq * (hp.numel() * 4 + hi.numel() * 2 + hd.numel() * 4 + 32)
-
+            self.h2d += hx.numel() * 4 + ht.numel() * 4
+            self.d2h += hp.numel() * 4 + hi.numel() * 2 + hd.numel() * 4 + 56
         if len(ws) > 1:      # batch: one concatenated set of pinned buffers, one ppfm_scan_host_batch call per step
             hx = torch.cat([b[0] for b in self.bufs]).pin_memory()
             ht = torch.cat([b[1] for b in self.bufs]).pin_memory()
@@ -285,13 +292,14 @@ class HostJob:
 
 
 # ------------------------------------------------------------------------------------------------- oracle legs
-def oracle_sample_run(w, n_points: int, n_pixels: int, seed: int = 7, ff_full=None):
+def oracle_sample_run(w, n_points: int, n_pixels: int, seed: int = 7):
     """Time the oracle, as it stands, on a bounded sample of workload `w`: `n_points` seeded grid points of the force
-    field, then the relaxation scan + df of the central `n_pixels` pixels on the oracle's own FP64 grid, built only
-    over the sub-volume those pixels can reach (lateral margin 4 A; building it is not timed).  Where that sub-grid
-    alone would cost more than ~2e9 pair evaluations (configs 2 and 4) and `ff_full` (a full float32 grid, widened to
-    FP64 on access) is given, the relaxation leg runs on it instead — timing only, labelled in `grid_kind`.
-    Returns timings and the extrapolated full-scan rate."""
+    field, then the relaxation scan + df of the central `n_pixels` pixels on the oracle's OWN FP64 force field:
+    * where the sub-grid those pixels can reach (lateral margin 4 Å) costs <= 3e9 pair evaluations it is built first
+      (not timed) and the scan runs on it;
+    * otherwise (configs 2 and 4) the scan evaluates its grid nodes from the atoms on demand (oracle.relax_scan_atoms) and the
+      node evaluations (counted) are taken out of the relaxation time at the pair rate measured in the first leg.
+    Nothing here comes from the CUDA path.  Returns timings and the rate extrapolated to the full workload."""
     from dataclasses import replace
 
     from oracle import oracle
@@ -300,6 +308,7 @@ def oracle_sample_run(w, n_points: int, n_pixels: int, seed: int = 7, ff_full=No
     oracle.forcefield(w, idx=idx)
     t_ff = time.perf_counter() - t0
     ff_pairs = float(len(idx)) * w.natoms * w.nimages
+    ff_rate = ff_pairs / t_ff
     s, g = w.scan, w.grid
     side = max(1, int(round(np.sqrt(n_pixels))))
     side_x, side_y = min(side, s.npx), min(side, s.npy)
@@ -312,18 +321,8 @@ def oracle_sample_run(w, n_points: int, n_pixels: int, seed: int = 7, ff_full=No
     i_hi = np.minimum(np.ceil((hi - g.origin[:2]) / h).astype(int), np.array(g.n[:2]) - 1)
     sub_n = (int(i_hi[0] - i_lo[0] + 1), int(i_hi[1] - i_lo[1] + 1), g.n[2])
     sub_cost = float(sub_n[0]) * sub_n[1] * sub_n[2] * w.natoms * w.nimages
-    if sub_cost > 2e9 and ff_full is not None:
-        grid_kind = "full float32 grid produced by the CUDA path, widened on access (timing only)"
-        iy, ix = np.meshgrid(np.arange(iy0, iy0 + side_y), np.arange(ix0, ix0 + side_x), indexing="ij")
-        pix = (iy * s.npx + ix).ravel()
-        t_grid = 0.0
-        t2 = time.perf_counter()
-        r = oracle.relax_scan(ff_full, g, w.tip, w.fire, s, pix=pix, traj=False)
-        t_relax = time.perf_counter() - t2
-    else:
-        if sub_cost > 2e10:
-            raise RuntimeError("oracle sub-grid for the relaxation sample is not affordable for this config")
-        grid_kind = f"oracle FP64 sub-grid {list(sub_n)}"
+    if sub_cost <= 3e9:
+        grid_kind = f"oracle FP64 sub-grid {list(sub_n)} (built first, not timed)"
         sub_grid = replace(g, origin=g.origin + np.array([i_lo[0] * h[0], i_lo[1] * h[1], 0.0]), n=sub_n,
                            periodic=(0, 0, 0))
         t1 = time.perf_counter()
@@ -332,38 +331,46 @@ def oracle_sample_run(w, n_points: int, n_pixels: int, seed: int = 7, ff_full=No
         t2 = time.perf_counter()
         r = oracle.relax_scan(ff_sub, sub_grid, w.tip, w.fire, sub_scan, traj=False)
         t_relax = time.perf_counter() - t2
+        t_wall = t_relax
+    else:
+        grid_kind = "oracle FP64 grid nodes evaluated from the atoms on demand (their cost taken out at the oracle's pair rate)"
+        t2 = time.perf_counter()
+        r = oracle.relax_scan_atoms(w, scan=sub_scan, traj=False)
+        t_all = time.perf_counter() - t2
+        t_grid = float(r["nodes"].sum()) * w.natoms * w.nimages / ff_rate
+        t_relax = max(t_all - t_grid, 0.05 * t_all)
+        t_wall = t_all
     t3 = time.perf_counter()
     oracle.df(r["pos_fz"][..., 3], s.dz, w.df.A, w.df.k0, w.df.f0)
     t_df = time.perf_counter() - t3
     nq = len(w.Q_sweep) if w.Q_sweep else 1
     pix_n = side_x * side_y
-    ff_rate = ff_pairs / t_ff
     relax_rate = pix_n * s.nz / (t_relax + t_df)
     full_s = w.pairs / ff_rate + nq * w.pixel_steps / relax_rate
     return {"t_ff": t_ff, "t_grid": t_grid, "t_relax": t_relax, "t_df": t_df, "ff_pairs_per_s": ff_rate,
-            "relax_pixel_steps_per_s": relax_rate, "s_per_full_scan_extrapolated": full_s,
+            "relax_pixel_steps_per_s": relax_rate, "relax_wall_pixel_steps_per_s": pix_n * s.nz / (t_wall + t_df),
+            "s_per_full_scan_extrapolated": full_s,
             "value": nq * w.pixel_steps / full_s, "sample_points": int(len(idx)), "sample_pixels": int(pix_n),
             "grid_kind": grid_kind, "iters_per_pixel_step": float(np.abs(r["iters"]).mean()),
             "cores": oracle.num_threads()}
 
 
-def sample_sizes(w, target_s: float, ff_full=None):
+def sample_sizes(w, target_s: float):
     """Sample sizes for about `target_s` seconds of oracle work, from a quick calibration run."""
-    cal = oracle_sample_run(w, 2000, 16, ff_full=ff_full)
+    cal = oracle_sample_run(w, 2000, 16)
     n_points = int(min(w.npoints, max(2000, 0.35 * target_s * cal["ff_pairs_per_s"] / (w.natoms * w.nimages))))
-    n_pixels = int(min(w.scan.npx * w.scan.npy, max(16, 0.45 * target_s * cal["relax_pixel_steps_per_s"] / w.scan.nz)))
+    n_pixels = int(min(w.scan.npx * w.scan.npy, max(16, 0.45 * target_s * cal["relax_wall_pixel_steps_per_s"] / w.scan.nz)))
     return n_points, n_pixels
 
 
-def cpu_baseline(w, target_s: float = 15.0, ff_full=None):
-    n_points, n_pixels = sample_sizes(w, target_s, ff_full)
-    r = oracle_sample_run(w, n_points, n_pixels, ff_full=ff_full)
+def cpu_baseline(w, target_s: float = 15.0):
+    n_points, n_pixels = sample_sizes(w, target_s)
+    r = oracle_sample_run(w, n_points, n_pixels)
     return {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
-            "sample": (f"FP64 oracle (gcc -O2, OpenMP): force field at {r['sample_points']} seeded grid points "
-                       f"({r['t_ff']:.1f} s), relaxation + df of the central {r['sample_pixels']} pixels x all z-steps "
-                       f"on {r['grid_kind']} ({r['t_relax'] + r['t_df']:.1f} s; grid build "
-                       f"{r['t_grid']:.1f} s not counted); value = pixel-steps / (pairs / oracle pair rate + "
-                       f"pixel-steps / oracle relax rate), extrapolated to the full workload"),
+            "sample": (f"unoptimised FP64 oracle (gcc -O2, OpenMP), the checker as it stands: force field at "
+                       f"{r['sample_points']} seeded grid points ({r['t_ff']:.1f} s); relaxation + df of the central "
+                       f"{r['sample_pixels']} pixels x all z-steps on {r['grid_kind']} "
+                       f"({r['t_relax'] + r['t_df']:.1f} s); value extrapolated to the full workload"),
             "ff_pairs_per_s": r["ff_pairs_per_s"], "relax_pixel_steps_per_s": r["relax_pixel_steps_per_s"],
             "s_per_full_scan_extrapolated": r["s_per_full_scan_extrapolated"],
             "iters_per_pixel_step": r["iters_per_pixel_step"]}
@@ -385,8 +392,8 @@ def run_reference(args):
     wall = time.perf_counter() - t0
     value = float(np.mean([r["value"] for r in runs]))
     r = runs[-1]
-    sample = (f"each step: oracle force field at {r['sample_points']} seeded grid points + relaxation/df of the central "
-              f"{r['sample_pixels']} pixels on {r['grid_kind']}; value extrapolated to the full workload")
+    sample = (f"each step: unoptimised FP64 oracle force field at {r['sample_points']} seeded grid points + relaxation/df "
+              f"of the central {r['sample_pixels']} pixels on {r['grid_kind']}; value extrapolated to the full workload")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -398,9 +405,169 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------- our arm
+def measure_config(P, B, torch, cfg, ws, steps, warmup, e2e_steps, flush, env, dist=None, sample_clocks=False):
+    """Run `warmup` + `steps` device-resident steps and `e2e_steps` host-API steps of one config; return the numbers."""
+    peaks, alu_peak = env["peaks"], env["alu_peak"]
+    job = DeviceJob(P, torch, cfg, ws)
+    for _ in range(warmup):
+        flush.zero_()
+        job.stats.zero_()
+        job.step()
+    torch.cuda.synchronize()
+    shard.barrier(dist)
+    sampler = ClockSampler(torch.cuda.current_device()) if sample_clocks else None
+    if sampler:
+        sampler.start()
+    n0 = B.launch_count()
+    B.timing_enable(True)          # per-kernel CUDA events recorded inside the library, directly around each launch
+    tot_ms, iters_total = 0.0, 0
+    t_wall0 = time.perf_counter()
+    for _ in range(steps):
+        flush.zero_()
+        job.stats.zero_()
+        job.step()
+        torch.cuda.synchronize()
+        tot_ms += job.step_ms()
+        iters_total += P.read_stats(job.stats)["total_iters"]
+    torch.cuda.synchronize()
+    shard.barrier(dist)
+    wall_s = time.perf_counter() - t_wall0
+    launches = B.launch_count() - n0
+    clocks = sampler.stop() if sampler else None
+    kern = B.timing_read()
+    B.timing_enable(False)
+    K = max(1, steps)
+    stats = P.read_stats(job.stats)
+    ms = {k: v[0] / K for k, v in kern.items()}
+    n_launch = {k: v[1] / K for k, v in kern.items()}
+    t_local = tot_ms / K * 1e-3
+
+    # ---- end-to-end arm (host buffers through ppfm_scan_host)
+    host = HostJob(P, torch, ws)
+    host.step()
+    torch.cuda.synchronize()
+    shard.barrier(dist)
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        host.step()
+    torch.cuda.synchronize()
+    e2e_local = (time.perf_counter() - t0) / max(1, e2e_steps)
+    shard.barrier(dist)
+    h2d, d2h = host.h2d, host.d2h
+    del host
+
+    (units_ps, units_pairs), t_step = shard.aggregate([job.pixel_steps, job.pairs], t_local, dist)
+    (e2e_units,), e2e_t = shard.aggregate([job.pixel_steps], e2e_local, dist)
+    world = env["world"]
+    ff_s, relax_s, df_s = ms["ff"] * 1e-3, ms["relax"] * 1e-3, ms["df"] * 1e-3
+    iters_per_step = iters_total / K
+    exec_instr = job.pair_exec_instr()
+    relax_bytes = 128.0 * iters_per_step + 18.0 * job.pixel_steps          # SURVEY 8(d) algorithmic bytes
+    gathered = 128.0 * 32.0 * stats["warp_gathers"]                        # bytes the last step really gathered
+    df_bytes = job.pixel_steps * 16.0 + job.df.numel() * 4.0 * job.n_runs
+    rec = {
+        "cfg": cfg, "steps": steps, "ms_per_step": t_step * 1e3, "pixel_steps_per_s": units_ps / t_step,
+        "s_per_full_scan": t_step, "e2e_pixel_steps_per_s": e2e_units / e2e_t, "e2e_ms_per_step": e2e_t * 1e3,
+        "kernel_ms": {k: round(v, 5) for k, v in ms.items() if v > 0},
+        "ff_pairs_per_s": job.pairs / ff_s, "ff_pipe_frac_canonical": job.pairs / ff_s * PAIR_INSTR / alu_peak,
+        "ff_pipe_frac_executed": exec_instr / ff_s / alu_peak,
+        "ff_flop_frac": job.pairs / ff_s * PAIR_FLOPS / (2 * alu_peak),
+        "relax_pixel_steps_per_s": job.pixel_steps / relax_s, "relax_iters_per_s": iters_per_step / relax_s,
+        "relax_iters_per_pixel_step": iters_per_step / job.pixel_steps,
+        "relax_alu_pipe_frac": iters_per_step * ITER_INSTR / relax_s / alu_peak,
+        "relax_issued_pipe_frac": 32.0 * stats["warp_iters"] * ITER_INSTR / relax_s / alu_peak,
+        "relax_lane_utilisation": stats["total_iters"] / max(1, 32 * stats["warp_iters"]),
+        "relax_l2_algorithmic_gbs": relax_bytes / relax_s * 1e-9,
+        "relax_l2_frac_of_cg_probe": relax_bytes / relax_s * 1e-9 / env["gather_cg"],
+        "relax_l2_frac_of_ca_probe": relax_bytes / relax_s * 1e-9 / env["gather_ca"],
+        "relax_gathered_gbs": gathered / relax_s * 1e-9,
+        "relax_ms_guard": {"ms_per_step": ms["relax"], "limit": 1.1 * PERF_GUARD_RELAX_MS[cfg],
+                           "ok": bool(ms["relax"] <= 1.1 * PERF_GUARD_RELAX_MS[cfg])},
+        "df_hbm_frac": df_bytes / df_s * 1e-9 / peaks["hbm_gbs"],
+        "not_converged": stats["n_not_converged"], "clamped": stats["n_clamped"], "max_iters": stats["max_iters"],
+        "inputs_sha256": inputs_sha256(ws),
+    }
+    if cfg == 3:
+        rec["molecules_per_s"] = len(ws) * world / t_step
+    extra = {"job": job, "ms": ms, "n_launch": n_launch, "launches": launches, "clocks": clocks, "wall_s": wall_s,
+             "stats": stats, "iters_per_step": iters_per_step, "exec_instr": exec_instr, "relax_bytes": relax_bytes,
+             "gathered": gathered, "df_bytes": df_bytes, "t_step": t_step, "units_ps": units_ps,
+             "units_pairs": units_pairs, "e2e_units": e2e_units, "e2e_t": e2e_t, "h2d": h2d, "d2h": d2h}
+    return rec, extra
+
+
+def next_rows(P, B, torch, job, ws, flush, env):
+    """The SURVEY 8(f) rows measured beside the step on the headline config's resident grid and scan: stiffness map
+    (N2) and tri-cubic relaxation (N4).  Eq.7 (N3) is measured on the configs[1] grid (see run_ours)."""
+    peaks, alu_peak = env["peaks"], env["alu_peak"]
+    out = {}
+    eig = torch.empty_like(job.pos)
+    for rep in range(2 + 3):
+        if rep == 2:
+            B.timing_enable(True)
+        flush.zero_()
+        job.stiffness(eig)
+    torch.cuda.synchronize()
+    stiff_ms = B.timing_read()["stiffness"][0] / 3.0
+    B.timing_enable(False)
+    del eig
+    n_samples = job.pos.shape[0]
+    out["stiffness"] = {"kernel": "stiffness_kernel", "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"],
+                        "achieved": 32.0 * n_samples / (stiff_ms * 1e-3) * 1e-9,
+                        "frac": 32.0 * n_samples / (stiff_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"], "ms": stiff_ms,
+                        "samples": n_samples, "in_step": False, "traffic": ncu_traffic(job.cfg, "stiffness")}
+    E_only = P.energy_grid(job.ff)
+    tri_stats = P.new_stats()
+    for rep in range(1 + 2):
+        if rep == 1:
+            B.timing_enable(True)
+        flush.zero_()
+        tri_stats.zero_()
+        job.relax_tricubic(E_only, tri_stats)
+    torch.cuda.synchronize()
+    tri_ms = B.timing_read()["relax_tricubic"][0] / 2.0
+    tri = P.read_stats(tri_stats)
+    B.timing_enable(False)
+    del E_only
+    tri_s = tri_ms * 1e-3
+    out["relax_tricubic"] = {"kernel": "relax_kernel<.,.,.,TRICUBIC>", "bound": "alu", "unit": "TFLOP/s",
+                             "achieved": tri["total_iters"] * TRI_FLOPS / tri_s * 1e-12, "peak": 2 * alu_peak * 1e-12,
+                             "frac": tri["total_iters"] * TRI_FLOPS / tri_s / (2 * alu_peak),
+                             "pipe_frac": tri["total_iters"] * TRI_INSTR / tri_s / alu_peak,
+                             "issued_pipe_frac": 32.0 * tri["warp_iters"] * TRI_INSTR / tri_s / alu_peak,
+                             "ms": tri_ms, "pixel_steps_per_s": job.pos.shape[0] / tri_s,
+                             "iters_per_pixel_step": tri["total_iters"] / job.pos.shape[0],
+                             "not_converged": tri["n_not_converged"], "in_step": False, "traffic": None}
+    return out
+
+
+def fft_row(P, B, torch, flush, env):
+    """one Eq.7 call on the configs[1] grid (4 M points), CO-like quadrupole tip; V_S = any potential."""
+    w = W.get(1)
+    peaks = env["peaks"]
+    npts = w.npoints
+    Vs = torch.linspace(-1.0, 1.0, npts, device="cuda", dtype=torch.float32).reshape(w.grid.n[2], w.grid.n[1], w.grid.n[0])
+    ff_fft = torch.empty((npts, 4), dtype=torch.float32, device="cuda")
+    for rep in range(2 + 3):
+        if rep == 2:
+            B.timing_enable(True)
+        flush.zero_()
+        P.forcefield_fft(Vs, w.grid, 0.7, -0.03, 0.0, -0.1, out=ff_fft)
+    torch.cuda.synchronize()
+    fft_ms = B.timing_read()["fft_el"][0] / 3.0
+    B.timing_enable(False)
+    alg = 20.0 * npts       # algorithmic bytes: 4 B potential read + 16 B float4 written per grid point
+    return {"kernel": "ppfm_forcefield_fft (own kernels + cuFFT FP64 transforms)", "bound": "hbm", "unit": "GB/s",
+            "peak": peaks["hbm_gbs"], "achieved": alg / (fft_ms * 1e-3) * 1e-9,
+            "frac": alg / (fft_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"], "ms": fft_ms, "points": npts,
+            "points_per_s": npts / (fft_ms * 1e-3), "in_step": False, "workload": "configs[1] grid",
+            "traffic": ncu_traffic(1, "fft_el")}
+
+
 def run_ours(args):
     import torch
     from paper_2401_14564_b200 import ppfm as P
+    from paper_2401_14564_b200 import ppfm_bench as B
 
     rank, world, local_rank = shard.env_rank_world()
     if not torch.cuda.is_available():
@@ -412,241 +579,100 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", torch.cuda.current_device()))
     peaks = measured_peaks()
+    alu_peak = SMS * LANES * peaks["sm_max_mhz"] * 1e6             # FP32 lane-instructions / s
+    env = {"peaks": peaks, "alu_peak": alu_peak, "world": world,
+           "fma_probe": B.probe_fma(),
+           "gather_ca": B.probe_gather(2 << 20, False),     # 32 MiB volume: L2-resident; through L1 (L1-assisted)
+           "gather_cg": B.probe_gather(2 << 20, True)}      # L1 bypassed: every request served by L2
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     cfg = args.config
     ws = build_workloads(cfg, rank, world)
-    job = DeviceJob(P, torch, cfg, ws)
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-
-    # ---- device-resident arm
-    for _ in range(args.warmup):
-        flush.zero_()
-        job.stats.zero_()
-        job.step()
-    torch.cuda.synchronize()
-    shard.barrier(dist)
-    sampler = ClockSampler(torch.cuda.current_device())
-    sampler.start()
-    n0 = P.launch_count()
-    P.timing_enable(True)          # per-kernel CUDA events recorded inside the library, directly around each launch
-    tot_ms, kern_ms, iters_total = 0.0, {}, 0
-    t_wall0 = time.perf_counter()
-    for _ in range(args.steps):
-        flush.zero_()
-        job.stats.zero_()
-        job.step()
-        torch.cuda.synchronize()
-        t, k = job.durations_ms()
-        tot_ms += t
-        for name, v in k.items():
-            kern_ms[name] = kern_ms.get(name, 0.0) + v
-        iters_total += P.read_stats(job.stats)["total_iters"]
-    torch.cuda.synchronize()
-    shard.barrier(dist)
-    wall_s = time.perf_counter() - t_wall0
-    launches = P.launch_count() - n0
-    clocks = sampler.stop()
-    kern = P.timing_read()
-    P.timing_enable(False)
-    K = max(1, args.steps)
-    stats = P.read_stats(job.stats)
-
-    # ---- stiffness map on the scan just relaxed: measured beside the step, not part of it
-    eig = torch.empty_like(job.pos)
-    stiff_ms = None
-    for rep in range(3 + 5):
-        if rep == 3:
-            P.timing_enable(True)
-        flush.zero_()
-        job.stiffness(eig)
-    torch.cuda.synchronize()
-    stiff_ms = P.timing_read()["stiffness"][0] / 5.0
-    P.timing_enable(False)
-    del eig
-
-    # ---- tri-cubic relaxation of the same scan on the energy-only grid: beside the step
-    E_only = P.energy_grid(job.ff)
-    tri_stats = P.new_stats()
-    for rep in range(2 + 3):
-        if rep == 2:
-            P.timing_enable(True)
-        flush.zero_()
-        tri_stats.zero_()
-        job.relax_tricubic(E_only, tri_stats)
-    torch.cuda.synchronize()
-    tri_ms = P.timing_read()["relax_tricubic"][0] / 3.0
-    tri = P.read_stats(tri_stats)
-    P.timing_enable(False)
-    del E_only
-
-    # ---- Eq.7 electrostatics on the first system's grid: V_S = the .w lane of the resident grid
-    # (any potential serves for timing), CO-like quadrupole tip; measured beside the step, not part of it
-    w0g = ws[0].grid
-    npts0 = ws[0].npoints
-    Vs = job.ff[:npts0, 3].contiguous()
-    ff_fft = torch.empty((npts0, 4), dtype=torch.float32, device="cuda")
-    for rep in range(2 + 3):
-        if rep == 2:
-            P.timing_enable(True)
-        flush.zero_()
-        P.forcefield_fft(Vs, w0g, 0.7, -0.03, 0.0, -0.1, out=ff_fft)
-    torch.cuda.synchronize()
-    fft_ms = P.timing_read()["fft_el"][0] / 3.0
-    P.timing_enable(False)
-    del Vs, ff_fft
+    head, x = measure_config(P, B, torch, cfg, ws, args.steps, args.warmup, max(1, min(args.steps, 5)), flush, env,
+                             dist, sample_clocks=True)
+    job, ms = x["job"], x["ms"]
+    extra_rows = next_rows(P, B, torch, job, ws, flush, env) if rank == 0 or world == 1 else {}
+    del job
+    x["job"] = None
     P.release_scratch()
-    (units_ps, units_pairs), t_step = shard.aggregate([job.pixel_steps, job.pairs], tot_ms / K * 1e-3, dist)
-    value = units_ps / t_step
+    torch.cuda.empty_cache()
 
-    # ---- end-to-end arm (host buffers through ppfm_scan_host)
-    host = HostJob(P, torch, ws)
-    for _ in range(max(1, min(args.warmup, 3))):
-        host.step()
-    torch.cuda.synchronize()
-    shard.barrier(dist)
-    e2e_steps = max(1, min(args.steps, 10))
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        host.step()
-    torch.cuda.synchronize()
-    e2e_local = (time.perf_counter() - t0) / e2e_steps
-    shard.barrier(dist)
-    (e2e_units,), e2e_t = shard.aggregate([job.pixel_steps], e2e_local, dist)
+    per_config = {}
+    if world == 1 and not args.no_per_config:
+        for c in (0, 1, 2, 3, 4):
+            if c == cfg:
+                per_config[str(c)] = head
+                continue
+            rec, xx = measure_config(P, B, torch, c, build_workloads(c, 0, 1), 3, 3, 2, flush, env)
+            xx["job"] = None
+            per_config[str(c)] = rec
+            P.release_scratch()
+            torch.cuda.empty_cache()
+        extra_rows["fft_el"] = fft_row(P, B, torch, flush, env)
+        P.release_scratch()
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
-    # ---- rooflines (rank 0's kernels; every rank runs the same launch configuration)
-    seg_ms = {k: v / K for k, v in kern_ms.items()}          # event marks around the Python calls (with host gaps)
-    ms = {k: v[0] / K for k, v in kern.items()}             # the kernels themselves, per step
-    n_launch = {k: v[1] / K for k, v in kern.items()}
-    n_relax_launches = len(job.sweep) if job.sweep else 1
-    fma_probe = P.probe_fma()
-    gather_ca = P.probe_gather(2 << 20, False)       # 32 MiB volume: L2-resident
-    gather_cg = P.probe_gather(2 << 20, True)
-    alu_peak = SMS * LANES * peaks["sm_max_mhz"] * 1e6             # FP32 lane-instructions / s
-    ff_s = ms["ff"] * 1e-3
-    ff_pairs_s = job.pairs / ff_s
-    exec_instr = job.pair_exec_instr()                            # lane-instructions the kernel really executes
-    rl_ff = {"kernel": "ff_kernel", "bound": "alu", "achieved": ff_pairs_s * PAIR_FLOPS * 1e-12,
-             "peak": 2 * alu_peak * 1e-12, "unit": "TFLOP/s", "frac": ff_pairs_s * PAIR_FLOPS / (2 * alu_peak),
-             "pipe_frac": ff_pairs_s * PAIR_INSTR / alu_peak,
-             "pipe_frac_of_probe": ff_pairs_s * PAIR_INSTR / fma_probe,
-             "pipe_frac_executed": exec_instr / ff_s / alu_peak,
-             "peak_source": f"{SMS} SMs x {LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 (FMA); "
-                            f"in-run FFMA probe {fma_probe * 1e-12:.2f} T lane-instr/s",
-             "algorithmic": f"{PAIR_FLOPS} flops / {PAIR_INSTR} FP32-pipe instructions per pair (SURVEY 8(d) canonical "
-                            f"count) x {job.pairs:.4g} pairs per launch; the kernel's own formulation executes "
-                            f"{exec_instr / job.pairs:.2f} lane-instructions per pair (pipe_frac_executed, comparable "
-                            f"with ncu sm__pipe_fma_cycles_active), so pipe_frac can pass 1",
-             "ms": ms["ff"], "traffic": NCU_TRAFFIC.get((cfg, "ff"))}
-    relax_s = ms["relax"] * 1e-3
-    iters_per_step = iters_total / K
-    relax_bytes = 128.0 * iters_per_step + 18.0 * job.pixel_steps
-    gather_peak = max(gather_ca, gather_cg)
-    gathered = 128.0 * 32.0 * stats["warp_gathers"]                 # bytes the last step's launches really gathered
-    rl_relax = {"kernel": "relax_kernel", "bound": "l2", "achieved": relax_bytes / relax_s * 1e-9,
-                "peak": gather_peak, "unit": "GB/s", "frac": relax_bytes / relax_s * 1e-9 / gather_peak,
-                "peak_source": f"in-run 8-corner float4 gather micro-benchmark over a 32 MiB (L2-resident) volume: "
-                               f"ld.global.ca {gather_ca:.0f} GB/s, ld.global.cg {gather_cg:.0f} GB/s",
-                "algorithmic": f"SURVEY 8(d): 128 B (8 corners x float4) x {iters_per_step:.4g} FIRE iterations + 18 B x "
-                               f"{job.pixel_steps:.4g} pixel-steps per step ({n_relax_launches} launch(es)).  The kernel "
-                               f"holds the current cell in registers and gathers only when the probe particle leaves "
-                               f"it, so it moves a fraction of these bytes (gathered_share_of_algorithmic) and frac can "
-                               f"pass 1 on large scans; what then binds is instruction issue, see alu_view",
-                "gathered_gbs": gathered / relax_s * 1e-9,
-                "gathered_share_of_algorithmic": gathered / max(1.0, 128.0 * iters_per_step),
-                "ms": ms["relax"], "iters_per_pixel_step": iters_per_step / job.pixel_steps,
-                "alu_view": {"bound": "alu", "unit": "TFLOP/s",
-                             "achieved": iters_per_step * ITER_FLOPS / relax_s * 1e-12, "peak": 2 * alu_peak * 1e-12,
-                             "frac": iters_per_step * ITER_FLOPS / relax_s / (2 * alu_peak),
-                             "pipe_frac": iters_per_step * ITER_INSTR / relax_s / alu_peak,
-                             "issued_pipe_frac": 32.0 * stats["warp_iters"] * ITER_INSTR / relax_s / alu_peak,
-                             "algorithmic": f"{ITER_FLOPS} flops / {ITER_INSTR} FP32-pipe lane-instructions (+ 4 MUFU) per "
-                                            f"FIRE iteration in the cached-cell formulation; issued_pipe_frac counts the "
-                                            f"lanes that idle in a warp until its slowest pixel converges",
-                             "peak_source": f"{SMS} SMs x {LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 (FMA)"},
-                "traffic": NCU_TRAFFIC.get((cfg, "relax"))}
-    df_bytes = (job.pixel_steps * 16.0 + job.df.numel() * 4.0 * n_relax_launches)
-    rl_df = {"kernel": "df_kernel", "bound": "hbm", "achieved": df_bytes / (ms["df"] * 1e-3) * 1e-9,
-             "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": df_bytes / (ms["df"] * 1e-3) * 1e-9 / peaks["hbm_gbs"],
-             "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})",
-             "algorithmic": "16 B read per pixel-step (float4 stack, Fz in .w) + 4 B written per df sample",
-             "ms": ms["df"], "traffic": NCU_TRAFFIC.get((cfg, "df"))}
-    n_samples = job.pos.shape[0]
-    rl_stiff = {"kernel": "stiffness_kernel", "bound": "hbm", "achieved": 32.0 * n_samples / (stiff_ms * 1e-3) * 1e-9,
-                "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": 32.0 * n_samples / (stiff_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"],
-                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})",
-                "algorithmic": "16 B position read + 16 B eigenvalues written per (pixel, z-step) sample; the 8-corner "
-                               "gather (128 B per sample) is served by L1/L2 and the touched grid slab is read from "
-                               "HBM once",
-                "ms": stiff_ms, "samples": n_samples, "in_step": False, "traffic": NCU_TRAFFIC.get((cfg, "stiffness"))}
-    # 5 forward + 4 inverse FP64 3-D transforms; each touches its array (16 B per complex point, N/2 of them) about
-    # three times in each direction; plus fill (4 B read, 40 B written), spectral (80 B r/w per complex point on N/2
-    # points), pack (32 B read, 16 B written) -> ~ 9 * 3 * 2 * 8 + 44 + 80 + 48 = 604 B per grid point as the model
-    fft_model_bytes = 604.0 * npts0
-    rl_fft = {"kernel": "ppfm_forcefield_fft (fill + cuFFT D2Z x5 + spectral + cuFFT Z2D x4 + pack)", "bound": "hbm",
-              "achieved": fft_model_bytes / (fft_ms * 1e-3) * 1e-9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-              "frac": fft_model_bytes / (fft_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"],
-              "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})",
-              "algorithmic": "traffic model 604 B per grid point: nine FP64 3-D FFTs at three read+write passes each "
-                             "(8 B per real point per pass) + fill + spectral product + pack; the transforms are "
-                             "cuFFT (library), the three kernels around them are this library's",
-              "ms": fft_ms, "points": npts0, "points_per_s": npts0 / (fft_ms * 1e-3), "in_step": False,
-              "traffic": NCU_TRAFFIC.get((cfg, "fft_el"))}
-    # tri-cubic iteration (relax.cu): weights 42 + x pass 128 + y pass 48 + z pass 12 + metric 3 = 233 FP32-pipe
-    # lane-instructions for the field (tri-linear: 33), the rest of the iteration as above (37): 270 = 2 * 244 + 26
-    TRI_INSTR, TRI_FLOPS = 270, 514
-    tri_s = tri_ms * 1e-3
-    rl_tri = {"kernel": "relax_kernel<.,.,.,TRICUBIC>", "bound": "alu", "unit": "TFLOP/s",
-              "achieved": tri["total_iters"] * TRI_FLOPS / tri_s * 1e-12, "peak": 2 * alu_peak * 1e-12,
-              "frac": tri["total_iters"] * TRI_FLOPS / tri_s / (2 * alu_peak),
-              "pipe_frac": tri["total_iters"] * TRI_INSTR / tri_s / alu_peak,
-              "issued_pipe_frac": 32.0 * tri["warp_iters"] * TRI_INSTR / tri_s / alu_peak,
-              "peak_source": f"{SMS} SMs x {LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 (FMA)",
-              "algorithmic": f"{TRI_FLOPS} flops / {TRI_INSTR} FP32-pipe lane-instructions per FIRE iteration (64-point "
-                             f"stencil held in registers) x {tri['total_iters']:.4g} iterations",
-              "ms": tri_ms, "pixel_steps_per_s": job.pos.shape[0] / tri_s,
-              "iters_per_pixel_step": tri["total_iters"] / job.pos.shape[0], "not_converged": tri["n_not_converged"],
-              "grid_bytes_per_point": 4, "in_step": False, "traffic": NCU_TRAFFIC.get((cfg, "relax_tricubic"))}
-    kernels = {"ff": rl_ff, "relax": rl_relax, "df": rl_df, "stiffness": rl_stiff, "fft_el": rl_fft,
-               "relax_tricubic": rl_tri}
-    for k in kernels:
-        kernels[k]["timing"] = "CUDA events recorded inside libppfm directly around the launch, mean per step"
+    # ---- rooflines of the headline config (rank 0's kernels; every rank runs the same launch configuration)
+    ff_s, relax_s, df_s = ms["ff"] * 1e-3, ms["relax"] * 1e-3, ms["df"] * 1e-3
+    pairs = sum(w.pairs for w in ws)
+    rl_ff = {"kernel": "ff_kernel", "bound": "alu", "unit": "TFLOP/s", "achieved": pairs / ff_s * PAIR_FLOPS * 1e-12,
+             "peak": 2 * alu_peak * 1e-12, "frac": pairs / ff_s * PAIR_FLOPS / (2 * alu_peak),
+             "pipe_frac_canonical": head["ff_pipe_frac_canonical"], "pipe_frac_executed": head["ff_pipe_frac_executed"],
+             "pipe_frac_canonical_of_fma_probe": pairs / ff_s * PAIR_INSTR / env["fma_probe"],
+             "pairs_per_launch": pairs, "flops_per_pair": PAIR_FLOPS, "instr_per_pair_canonical": PAIR_INSTR,
+             "instr_per_pair_executed": x["exec_instr"] / pairs, "ms": ms["ff"], "traffic": ncu_traffic(cfg, "ff")}
+    ips = x["iters_per_step"]
+    n_runs = len(ws[0].Q_sweep) if ws[0].Q_sweep else 1
+    rl_relax = {"kernel": "relax_kernel", "bound": "alu", "unit": "TFLOP/s", "achieved": ips * ITER_FLOPS / relax_s * 1e-12,
+                "peak": 2 * alu_peak * 1e-12, "frac": ips * ITER_FLOPS / relax_s / (2 * alu_peak),
+                "pipe_frac": head["relax_alu_pipe_frac"], "issued_pipe_frac": head["relax_issued_pipe_frac"],
+                "lane_utilisation": head["relax_lane_utilisation"], "iters_per_launch": ips / n_runs,
+                "flops_per_iter": ITER_FLOPS, "instr_per_iter": ITER_INSTR, "ms": ms["relax"],
+                "l2_view": {"bound": "l2", "unit": "GB/s", "algorithmic_bytes_per_step": x["relax_bytes"],
+                            "achieved": head["relax_l2_algorithmic_gbs"], "peak_cg_l2_only": env["gather_cg"],
+                            "peak_ca_l1_assisted": env["gather_ca"], "frac_of_cg": head["relax_l2_frac_of_cg_probe"],
+                            "frac_of_ca": head["relax_l2_frac_of_ca_probe"], "gathered_gbs": head["relax_gathered_gbs"],
+                            "gathered_share_of_algorithmic": x["gathered"] / max(1.0, 128.0 * ips)},
+                "traffic": ncu_traffic(cfg, "relax")}
+    rl_df = {"kernel": "df_kernel", "bound": "hbm", "unit": "GB/s", "achieved": x["df_bytes"] / df_s * 1e-9,
+             "peak": peaks["hbm_gbs"], "frac": head["df_hbm_frac"], "bytes_per_step": x["df_bytes"], "ms": ms["df"],
+             "traffic": ncu_traffic(cfg, "df")}
+    kernels = {"ff": rl_ff, "relax": rl_relax, "df": rl_df}
+    kernels.update(extra_rows)
     dominant = max(("ff", "relax", "df"), key=lambda k: ms[k])
     roof = dict(kernels[dominant])
-    roof["share_of_step"] = ms[dominant] / (tot_ms / K)
+    roof["share_of_step"] = ms[dominant] / (x["t_step"] * 1e3)
+    roof["peak_source"] = (f"{SMS} SMs x {LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 (DESIGN.md 6.1)"
+                           if roof["bound"] == "alu" else f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})")
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak",
+    line = {"metric": METRIC, "value": head["pixel_steps_per_s"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": x["t_step"] * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOAD_NAME[cfg], "seed": BASE_SEED[cfg], "systems_per_gpu": len(ws),
-                       "l2": "flushed between timed steps (512 MiB device write)", "parallelism": f"replicated x{world}"
-                       if world > 1 else "single GPU", "timing": "CUDA events on the launching stream, per step"},
-            "parts": {"ff_pair_interactions_per_s": units_pairs / (ms["ff"] * 1e-3),
-                      "ff_fp32_flop_frac": rl_ff["frac"], "ff_fp32_pipe_frac": rl_ff["pipe_frac"],
-                      "relax_pixel_steps_per_s": units_ps / relax_s,
-                      "relax_fire_iterations_per_s": iters_per_step * world / relax_s,
-                      "s_per_full_scan": t_step, "kernel_ms": ms, "kernel_launches_per_step": n_launch,
-                      "call_ms_incl_host_gaps": seg_ms, "wall_s_timed_region": wall_s,
-                      "not_converged": stats["n_not_converged"], "clamped": stats["n_clamped"],
-                      "max_iters": stats["max_iters"],
-                      "relax_warp_loop_trips": stats["warp_iters"],
-                      "relax_lane_utilisation": stats["total_iters"] / max(1, 32 * stats["warp_iters"]),
-                      "relax_cell_changes_per_iteration": stats["cell_gathers"] / max(1, stats["total_iters"]),
-                      "relax_gather_trips_per_loop_trip": stats["warp_gathers"] / max(1, stats["warp_iters"])},
-            "e2e": {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
-                    "d2h_bytes_per_step": host.d2h, "ms_per_step": e2e_t * 1e3, "steps": e2e_steps,
-                    "api": "ppfm_scan_host[_batch|_sweep] (pinned host buffers: inputs copied in, outputs stored by the kernels straight into host memory)"},
-            "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "roofline_kernels": kernels}
+                       "l2": "flushed between timed steps (512 MiB device write)",
+                       "parallelism": f"replicated x{world}" if world > 1 else "single GPU",
+                       "timing": "CUDA events on the launching stream, per step", "inputs_sha256": head["inputs_sha256"]},
+            "parts": {"ff_pair_interactions_per_s": x["units_pairs"] / ff_s,
+                      "ff_fp32_pipe_frac_canonical": head["ff_pipe_frac_canonical"],
+                      "ff_fp32_pipe_frac_executed": head["ff_pipe_frac_executed"],
+                      "relax_pixel_steps_per_s": x["units_ps"] / relax_s,
+                      "relax_fire_iterations_per_s": ips * world / relax_s, "s_per_full_scan": x["t_step"],
+                      "kernel_ms": {k: round(v, 5) for k, v in ms.items() if v > 0},
+                      "kernel_launches_per_step": {k: v for k, v in x["n_launch"].items() if v > 0},
+                      "wall_s_timed_region": x["wall_s"], "not_converged": head["not_converged"],
+                      "clamped": head["clamped"], "max_iters": head["max_iters"],
+                      "probes": {"fma_lane_instr_per_s": env["fma_probe"], "gather_cg_gbs": env["gather_cg"],
+                                 "gather_ca_gbs": env["gather_ca"]},
+                      "per_config": per_config},
+            "e2e": {"value": x["e2e_units"] / x["e2e_t"], "unit": UNIT, "h2d_bytes_per_step": x["h2d"],
+                    "d2h_bytes_per_step": x["d2h"], "ms_per_step": x["e2e_t"] * 1e3,
+                    "api": "ppfm_scan_host[_batch|_sweep], pinned host buffers"},
+            "gpu_launches": int(x["launches"]), "clocks": x["clocks"], "roofline": roof, "roofline_kernels": kernels}
     if world == 1 and not args.no_cpu_baseline:
-        w0 = ws[0]
-        ff_full = None
-        if not job.batch and w0.npoints * w0.natoms * w0.nimages > 1e10:      # configs 2 and 4 (see oracle_sample_run)
-            ff_full = job.ff.cpu().numpy().reshape(w0.grid.n[2], w0.grid.n[1], w0.grid.n[0], 4)
-        line["cpu_baseline"] = cpu_baseline(w0, ff_full=ff_full)
+        line["cpu_baseline"] = cpu_baseline(ws[0])
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -657,9 +683,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

@@ -22,6 +22,10 @@
  *          Device entry points only enqueue work on `cuda_stream` (a cudaStream_t cast to
  *          void*, NULL = default stream); they never synchronise it and never change the current device.
  *          Host entry points (ppfm_scan_host, _batch, _sweep) synchronise the stream before returning.
+ *   Threads and streams: every entry point may be called from several host threads and on several streams at once.
+ *          Calls on one stream execute in order; calls on different streams may overlap on the device and share
+ *          nothing but read-only caches (the cuFFT plans and tip spectra of (1b)/(1c) are guarded by a mutex on the
+ *          host and by events on the device; each call brings its own cuFFT work area).
  *   Errors: 0 on success, a negative ppfm_status otherwise; no exceptions, no exit(), no output.  Per-pixel
  *          conditions (not converged, PP clamped at a non-periodic grid face) are data (d_iters, d_stats).
  *   Determinism: outputs are bit-reproducible run to run (fixed summation order, no atomics on results).
@@ -40,6 +44,7 @@ extern "C" {
 
 #define PPFM_VERSION 100 /* 0.1.0 */
 #define PPFM_MAX_TYPES 64
+#define PPFM_DF_MAX_N 255 /* largest n = A/dz of ppfm_df */
 
 typedef enum {
     PPFM_OK = 0,
@@ -114,15 +119,22 @@ double ppfm_Nm_to_eVA2(double k_Nm);
 
 /* ---- (1) force-field grid: Eq.5 + Eq.6 summed over atoms and images ------------------
  * d_xyzq   DEVICE float[natoms][4] = (x, y, z, q_i), 16-byte aligned
- * d_type   DEVICE int32[natoms], index into h_R / h_e (validated on the device: out-of-range -> that atom is
- *          skipped and the call's status word, if any, is not affected; validate on the host when you can)
+ * d_type   DEVICE int32[natoms], index into h_R / h_e.  It is device memory, so it is validated on the device: an atom
+ *          whose index is outside [0, ntypes) contributes nothing and is counted in d_status->n_bad_type
  * h_R,h_e  HOST double[ntypes]: element radius R_i (Å) and well depth e_i (eV); mixing R_i + R_PP, sqrt(e_i e_PP)
  * r_min    pair distances are clamped below at r_min (Å) to keep the sum finite on top of an atom; >= 0
  * d_ff     DEVICE float[n2][n1][n0][4], 16-byte aligned, written completely
+ * d_status DEVICE ppfm_ff_status or NULL: per-call conditions that are data, not errors (written, not accumulated;
+ *          batch form: summed over the systems)
  */
+typedef struct {
+    uint32_t n_bad_type;   /* atoms skipped because their type index was outside [0, ntypes)                       */
+    uint32_t n_clamped;    /* systems in which some atom image lies within r_min of the grid's bounding box, i.e.
+                              for which the r_min clamp was compiled into the pair loop                             */
+} ppfm_ff_status;
 int ppfm_forcefield(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes, const double *h_R,
                     const double *h_e, const ppfm_lattice *lattice, const ppfm_probe *probe, const ppfm_grid *grid,
-                    double r_min, float *d_ff, void *cuda_stream);
+                    double r_min, float *d_ff, ppfm_ff_status *d_status, void *cuda_stream);
 
 /* Same pass, two grids (LJ and electrostatic fields are kept separately so the tip charge can
  * change without recomputation): d_ff_lj = Lennard-Jones only, d_ff_el = Coulomb field of a UNIT probe charge
@@ -130,7 +142,7 @@ int ppfm_forcefield(int32_t natoms, const float *d_xyzq, const int32_t *d_type, 
 int ppfm_forcefield_split(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
                           const double *h_R, const double *h_e, const ppfm_lattice *lattice,
                           const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff_lj,
-                          float *d_ff_el, void *cuda_stream);
+                          float *d_ff_el, ppfm_ff_status *d_status, void *cuda_stream);
 
 /* d_out = d_ff_lj + Q * d_ff_el over n_points float4 entries (d_out may alias d_ff_lj). */
 int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q, int64_t n_points, float *d_out,
@@ -142,7 +154,7 @@ int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q, int64_t n
 int ppfm_forcefield_batch(int32_t nsys, const int32_t *h_atom_offset, const float *d_xyzq, const int32_t *d_type,
                           int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
                           const ppfm_probe *probes, const ppfm_grid *grids, double r_min, float *d_ff,
-                          void *cuda_stream);
+                          ppfm_ff_status *d_status, void *cuda_stream);
 
 /* ---- (2) relaxation scan: Eq.1 + Eq.2 + FIRE on the tri-linearly interpolated grid --
  * d_ff      DEVICE grid as written by ppfm_forcefield (read-only)
@@ -231,7 +243,8 @@ int ppfm_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids
 
 /* ---- (3) frequency shift, Giessibl's formula Eq.3 -------------------------------------------
  * Fz is read from the .w lane of d_pos_fz [nz][npy][npx][4].  A = peak-to-peak amplitude (Å); n = A/dz must be an
- * integer >= 1 (within 1e-6) and nz > n.  Eq.3 is integrated exactly for the piecewise-linear interpolant of the
+ * integer (within 1e-6) with 1 <= n <= PPFM_DF_MAX_N (the weights travel as a kernel parameter) and nz > n; the
+ * host entry points check the same before any work is enqueued.  Eq.3 is integrated exactly for the piecewise-linear interpolant of the
  * n+1 samples of each window; output plane k belongs to tip height z0 - (k + n/2) dz.
  * d_df  DEVICE float[nz - n][npy][npx] (Hz).  ppfm_df_weights writes the n+1 quadrature weights to HOST memory.
  * The batch count `nsys` treats d_pos_fz / d_df as nsys consecutive stacks of identical shape.
@@ -271,37 +284,6 @@ int ppfm_scan_host_sweep(int32_t nQ, const double *h_Q, int32_t natoms, const fl
                          const ppfm_probe *probe, const ppfm_grid *grid, double r_min, const ppfm_tip *tip,
                          const ppfm_fire *fire, const ppfm_scan *scan, double A, double k0_Nm, double f0_Hz,
                          float *h_pos_fz, uint16_t *h_iters, float *h_df, ppfm_stats *h_stats, void *cuda_stream);
-
-/* ---- measurement helpers (used by bench.py to define the roofline denominators on the box itself) ------------
- * ppfm_probe_fma:    FFMA-only kernel; returns lane-instructions per second in *h_lane_instr_per_s.
- * ppfm_probe_gather: the relaxation's 8-corner float4 gather over an L2-resident volume of `n_float4` entries
- *                    with no dependent math; `bypass_l1` selects ld.global.cg; returns GB/s in *h_gbs.
- * Both synchronise the stream (they time with CUDA events).
- */
-int ppfm_probe_fma(double *h_lane_instr_per_s, void *cuda_stream);
-int ppfm_probe_gather(int64_t n_float4, int32_t bypass_l1, double *h_gbs, void *cuda_stream);
-
-/* Number of kernels this library has launched on this process so far (for bench.py's gpu_launches). */
-int64_t ppfm_launch_count(void);
-
-/* Per-kernel device timing for the roofline legs of bench.py: while enabled, every launch of the kernels below is
- * bracketed by CUDA events recorded on the launching stream directly around the launch (no host work in between).
- * ppfm_timing_enable(on) clears the accumulators; ppfm_timing_read waits for the recorded events of `kernel_id`
- * (it synchronises on them, not on the stream) and returns the summed milliseconds and the number of launches.
- * Off by default; process-wide. */
-typedef enum {
-    PPFM_K_FF_PREP = 0, /* a1 atom-record packing            */
-    PPFM_K_FF = 1,      /* a2 force-field grid               */
-    PPFM_K_COMBINE = 2, /* a3 F_LJ + Q F_el                  */
-    PPFM_K_RELAX = 3,   /* a4+a5 relaxation scan             */
-    PPFM_K_DF = 4,      /* a6 frequency shift                */
-    PPFM_K_STIFFNESS = 5, /* N2 stiffness map               */
-    PPFM_K_FFT_EL = 6,  /* N3 Eq.7 electrostatics: own kernels + cuFFT, one timed region */
-    PPFM_K_RELAX_TRICUBIC = 7, /* N4 relaxation with tri-cubic interpolation of the potential */
-    PPFM_K_COUNT = 8
-} ppfm_kernel_id;
-int ppfm_timing_enable(int on);
-int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);
 
 /* Scratch memory.  Per-call scratch (packed atom records, job tables; for ppfm_scan_host also the grid and the
  * scan buffers) comes from a library-private stream-ordered pool of the current device, so steady-state calls make

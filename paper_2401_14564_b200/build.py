@@ -15,6 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libppfm.so")
+PROBES_SRC = os.path.join(HERE, "csrc_probes", "probes.cu")
+PROBES_LIB = os.path.join(HERE, "libppfm_probes.so")      # include/ppfm_bench.h (b): measurement only
 NVCC_COMPILE = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
                 "-c"]
 NVCC_LINK = ["-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-Xcompiler", "-fPIC", "-cudart", "static",
@@ -50,6 +52,10 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
                     raise subprocess.CalledProcessError(r.returncode, r.args)
     if jobs or not os.path.exists(lib) or any(os.path.getmtime(lib) < os.path.getmtime(o) for o in objs):
         subprocess.run([nvcc] + NVCC_LINK + ["-o", lib] + objs, check=True)
+    if lib == LIB and (force or not os.path.exists(PROBES_LIB) or
+                       os.path.getmtime(PROBES_LIB) < max(os.path.getmtime(PROBES_SRC), hdr_time)):
+        subprocess.run([nvcc] + [f for f in NVCC_COMPILE if f != "-c"] + ["--shared", "-cudart", "static", "-o",
+                                                                          PROBES_LIB, PROBES_SRC], check=True)
     return lib
 
 

@@ -1,5 +1,5 @@
-// api.cu — the rest of the C ABI: status text, defaults, the one-call host-buffer simulation and the
-// two measurement probes that define the roofline denominators on the box.
+// api.cu — the rest of the C ABI: status text, defaults, scratch pool, the one-call host-buffer simulation
+// and the launch counter / per-kernel timers of include/ppfm_bench.h.
 #include "common.cuh"
 
 #include <mutex>
@@ -13,6 +13,8 @@ static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
 void set_cuda_error(cudaError_t e, const char *where) {
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), where);
+    cudaGetLastError();      // clear the thread's sticky-less last-error state: one failed call must not make the
+                             // next successful launch report a stale error through PPFM_LAUNCH_CHECK
 }
 
 // ---- private scratch pool (one per device, created on first use) ---------------------------------------------------
@@ -82,62 +84,6 @@ static void timing_drain(bool accumulate) {
         cudaEventDestroy(p.e1);
     }
     g_tm_pending.clear();
-}
-
-// ---- probe 1: FP32 FMA issue rate (the denominator of the force-field kernel's pipe utilisation) ----------------
-__global__ void __launch_bounds__(256) probe_fma_kernel(float *out, int iters, float a, float b) {
-    float x[16];
-#pragma unroll
-    for (int i = 0; i < 16; i++) x[i] = (float)(threadIdx.x + i);
-    for (int it = 0; it < iters; it++) {
-#pragma unroll
-        for (int r = 0; r < 8; r++) {
-#pragma unroll
-            for (int i = 0; i < 16; i++) x[i] = fmaf(x[i], a, b);
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; i++) s += x[i];
-    if (s == 123.456f) out[0] = s;   // never true for the arguments used; defeats dead-code elimination
-}
-
-// ---- probe 2: the relaxation's gather pattern with no dependent math ("achievable L2 bandwidth") ------------------
-// A warp covers an 8 x 4 pixel patch (as relax_kernel does); each step it gathers the 8 corners of a cell of an
-// nx x ny x nz float4 volume and moves to a pseudo-random neighbouring cell that does NOT depend on loaded data.
-template <bool BYPASS_L1>
-__global__ void __launch_bounds__(128) probe_gather_kernel(const float4 *__restrict__ g, int nx, int ny, int nz,
-                                                           int steps, float *out) {
-    const int warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    unsigned s = 0x9E3779B9u * (warp_global + 1);
-    float acc = 0.f;
-    for (int it = 0; it < steps; it++) {
-        s = s * 1664525u + 1013904223u;
-        const int bx = (int)((s >> 8) % (unsigned)(nx - 9));
-        const int by = (int)((s >> 4) % (unsigned)(ny - 5));
-        const int bz = (int)((s >> 16) % (unsigned)(nz - 1));
-        const int i0 = bx + (lane & 7), j0 = by + (lane >> 3), k0 = bz;
-#pragma unroll
-        for (int c = 0; c < 8; c++) {
-            const int i = i0 + (c & 1), j = j0 + ((c >> 1) & 1), k = k0 + (c >> 2);
-            const float4 *p = g + ((size_t)k * ny + j) * nx + i;
-            float4 v;
-            if (BYPASS_L1) {
-                asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-            } else {
-                v = __ldg(p);
-            }
-            acc += v.x + v.w;
-        }
-    }
-    if (acc == 123.456f) out[0] = acc;
-}
-
-__global__ void probe_fill_kernel(float4 *g, long long n) {
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-        g[i] = make_float4(1e-3f * (float)(i & 1023), 0.f, 1.f, 2.f);
 }
 
 }  // namespace ppfm
@@ -231,7 +177,7 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
     const ppfm_scan *scan = &scans[0];
     const double nn = (scan->dz > 0) ? A / scan->dz : -1.0;
     const long long n = std::llround(nn);
-    if (h_df && (n < 1 || std::fabs(nn - (double)n) > 1e-6 || scan->nz <= n)) return PPFM_EINVAL;
+    if (h_df && (n < 1 || n > PPFM_DF_MAX_N || std::fabs(nn - (double)n) > 1e-6 || scan->nz <= n)) return PPFM_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t ndf = h_df ? (size_t)nsys * scan->npx * scan->npy * (size_t)(scan->nz - n) : 0;
     const size_t na = (size_t)(natoms > 0 ? natoms : 1);
@@ -273,12 +219,12 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
     if (rc == PPFM_OK) {
         if (nQ > 0)          // S19: F_LJ and unit-charge F_el once, combined per Q
             rc = ppfm_forcefield_split(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min, d_lj,
-                                       d_el, cuda_stream);
+                                       d_el, nullptr, cuda_stream);
         else
             rc = (nsys == 1) ? ppfm_forcefield(natoms, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min,
-                                               d_ff, cuda_stream)
+                                               d_ff, nullptr, cuda_stream)
                              : ppfm_forcefield_batch(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices,
-                                                     probes, grids, r_min, d_ff, cuda_stream);
+                                                     probes, grids, r_min, d_ff, nullptr, cuda_stream);
     }
     for (int run = 0; run < nrun; run++) {
         if (rc == PPFM_OK && nQ > 0) rc = ppfm_combine(d_lj, d_el, h_Q[run], (int64_t)npts, d_ff, cuda_stream);
@@ -332,87 +278,6 @@ extern "C" int ppfm_scan_host_batch(int32_t nsys, const int32_t *h_atom_offset, 
                                     float *h_df, ppfm_stats *h_stats, void *cuda_stream) {
     return scan_host_impl(nsys, h_atom_offset, h_xyzq, h_type, ntypes, h_R, h_e, lattices, probes, grids, r_min, tips,
                           fire, scans, A, k0_Nm, f0_Hz, h_pos_fz, h_iters, h_df, h_stats, cuda_stream);
-}
-
-extern "C" int ppfm_probe_fma(double *h_lane_instr_per_s, void *cuda_stream) {
-    if (!h_lane_instr_per_s) return PPFM_EINVAL;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = 0, sms = 0;
-    PPFM_CUDA(cudaGetDevice(&dev));
-    PPFM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    float *d_out = nullptr;
-    PPFM_CUDA(cudaMallocAsync((void **)&d_out, 4, st));
-    cudaEvent_t e0, e1;
-    PPFM_CUDA(cudaEventCreate(&e0));
-    PPFM_CUDA(cudaEventCreate(&e1));
-    const int iters = 4000, blocks = sms * 8;
-    double best = 0.0;
-    for (int rep = 0; rep < 4; rep++) {
-        PPFM_CUDA(cudaEventRecord(e0, st));
-        probe_fma_kernel<<<blocks, 256, 0, st>>>(d_out, iters, 0.999f, 0.001f);
-        PPFM_LAUNCH_CHECK();
-        PPFM_CUDA(cudaEventRecord(e1, st));
-        PPFM_CUDA(cudaEventSynchronize(e1));
-        float ms = 0.f;
-        PPFM_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-        const double lane_instr = (double)blocks * 256.0 * (double)iters * 8.0 * 16.0;
-        const double rate = lane_instr / (ms * 1e-3);
-        if (rep > 0 && rate > best) best = rate;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    PPFM_CUDA(cudaFreeAsync(d_out, st));
-    PPFM_CUDA(cudaStreamSynchronize(st));
-    *h_lane_instr_per_s = best;
-    return PPFM_OK;
-}
-
-extern "C" int ppfm_probe_gather(int64_t n_float4, int32_t bypass_l1, double *h_gbs, void *cuda_stream) {
-    if (!h_gbs || n_float4 < 64 * 64 * 8) return PPFM_EINVAL;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = 0, sms = 0;
-    PPFM_CUDA(cudaGetDevice(&dev));
-    PPFM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    // volume nx = ny = 256, nz from the requested size (plane = 1 MiB)
-    const int nx = 256, ny = 256;
-    long long nzl = n_float4 / ((long long)nx * ny);
-    if (nzl < 2) nzl = 2;
-    if (nzl > 8192) nzl = 8192;
-    const int nz = (int)nzl;
-    const long long n = (long long)nx * ny * nz;
-    float4 *d_g = nullptr;
-    float *d_out = nullptr;
-    PPFM_CUDA(cudaMallocAsync((void **)&d_g, (size_t)n * 16, st));
-    PPFM_CUDA(cudaMallocAsync((void **)&d_out, 4, st));
-    probe_fill_kernel<<<sms * 8, 256, 0, st>>>(d_g, n);
-    PPFM_LAUNCH_CHECK();
-    cudaEvent_t e0, e1;
-    PPFM_CUDA(cudaEventCreate(&e0));
-    PPFM_CUDA(cudaEventCreate(&e1));
-    const int steps = 2000, blocks = sms * 16;
-    double best = 0.0;
-    for (int rep = 0; rep < 4; rep++) {
-        PPFM_CUDA(cudaEventRecord(e0, st));
-        if (bypass_l1)
-            probe_gather_kernel<true><<<blocks, 128, 0, st>>>(d_g, nx, ny, nz, steps, d_out);
-        else
-            probe_gather_kernel<false><<<blocks, 128, 0, st>>>(d_g, nx, ny, nz, steps, d_out);
-        PPFM_LAUNCH_CHECK();
-        PPFM_CUDA(cudaEventRecord(e1, st));
-        PPFM_CUDA(cudaEventSynchronize(e1));
-        float ms = 0.f;
-        PPFM_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-        const double bytes = (double)blocks * 128.0 * (double)steps * 128.0;
-        const double gbs = bytes / (ms * 1e-3) * 1e-9;
-        if (rep > 0 && gbs > best) best = gbs;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    PPFM_CUDA(cudaFreeAsync(d_g, st));
-    PPFM_CUDA(cudaFreeAsync(d_out, st));
-    PPFM_CUDA(cudaStreamSynchronize(st));
-    *h_gbs = best;
-    return PPFM_OK;
 }
 
 extern "C" int ppfm_scan_host_sweep(int32_t nQ, const double *h_Q, int32_t natoms, const float *h_xyzq,

@@ -11,6 +11,7 @@
 #include <cstring>
 
 #include "../../include/ppfm.h"
+#include "../../include/ppfm_bench.h"
 
 namespace ppfm {
 

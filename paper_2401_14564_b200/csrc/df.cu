@@ -7,7 +7,7 @@
 
 namespace ppfm {
 
-constexpr int DF_MAX_N = 255;
+constexpr int DF_MAX_N = PPFM_DF_MAX_N;
 
 struct DfWeights {
     float w[DF_MAX_N + 1];   // already multiplied by -(f0 / 2 k0) * 16.02176634

@@ -108,22 +108,29 @@ __device__ __forceinline__ bool atom_near_grid(const FFJob &job, float4 a) {
 // summation order is fixed): atoms with a Coulomb factor first, LJ-only atoms after them.
 __device__ __forceinline__ void prep_system(const FFJob &job, const TypeEntry *__restrict__ table, int job_index,
                                             const float4 *__restrict__ xyzq, const int *__restrict__ type,
-                                            AtomRec *__restrict__ recs, FFFlags *__restrict__ flags) {
+                                            AtomRec *__restrict__ recs, FFFlags *__restrict__ flags,
+                                            ppfm_ff_status *__restrict__ status) {
     __shared__ int s_warp[PREP_THREADS / 32];
-    __shared__ int s_total, s_near;
+    __shared__ int s_total, s_near, s_bad;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int n = job.natoms;
     // pass 1: number of charged atoms
-    int cnt = 0;
+    int cnt = 0, bad = 0;
     for (int i = tid; i < n; i += PREP_THREADS) {
-        const AtomRec r = make_record(job, table, xyzq[job.atom_begin + i], type[job.atom_begin + i]);
+        const int t = type[job.atom_begin + i];
+        const AtomRec r = make_record(job, table, xyzq[job.atom_begin + i], t);
         cnt += (r.kq[0] != 0.0f) ? 1 : 0;
+        bad += (t < 0 || t >= job.ntypes) ? 1 : 0;
     }
 #pragma unroll
-    for (int s = 16; s > 0; s >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, s);
-    if (tid == 0) { s_total = 0; s_near = 0; }
+    for (int s = 16; s > 0; s >>= 1) {
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, s);
+        bad += __shfl_xor_sync(0xffffffffu, bad, s);
+    }
+    if (tid == 0) { s_total = 0; s_near = 0; s_bad = 0; }
     __syncthreads();
-    if (lane == 0 && cnt) atomicAdd(&s_total, cnt);      // integer sum: order does not matter
+    if (lane == 0 && cnt) atomicAdd(&s_total, cnt);      // integer sums: order does not matter
+    if (lane == 0 && bad) atomicAdd(&s_bad, bad);
     __syncthreads();
     const int nq = s_total;
     // pass 2: stable partition, PREP_THREADS atoms at a time
@@ -161,20 +168,26 @@ __device__ __forceinline__ void prep_system(const FFJob &job, const TypeEntry *_
     }
     if (near) atomicOr(&s_near, 1);
     __syncthreads();
-    if (tid == 0) { flags[job_index].clamp = s_near; flags[job_index].ncharged = nq; }
+    if (tid == 0) {
+        flags[job_index].clamp = s_near; flags[job_index].ncharged = nq;
+        if (status) {                                   // zeroed by the host on the same stream before this launch
+            if (s_bad) atomicAdd(&status->n_bad_type, (unsigned)s_bad);
+            if (s_near) atomicAdd(&status->n_clamped, 1u);
+        }
+    }
 }
 
 __global__ void __launch_bounds__(PREP_THREADS)
 ff_prep_kernel(const __grid_constant__ FFSingle one, const float4 *__restrict__ xyzq, const int *__restrict__ type,
-               AtomRec *__restrict__ recs, FFFlags *__restrict__ flags) {
-    prep_system(one.job, one.table, 0, xyzq, type, recs, flags);
+               AtomRec *__restrict__ recs, FFFlags *__restrict__ flags, ppfm_ff_status *__restrict__ status) {
+    prep_system(one.job, one.table, 0, xyzq, type, recs, flags, status);
 }
 
 __global__ void __launch_bounds__(PREP_THREADS)
 ff_prep_batch_kernel(const FFJob *__restrict__ jobs, const TypeEntry *__restrict__ table,
                      const float4 *__restrict__ xyzq, const int *__restrict__ type, AtomRec *__restrict__ recs,
-                     FFFlags *__restrict__ flags) {
-    prep_system(jobs[blockIdx.x], table, blockIdx.x, xyzq, type, recs, flags);
+                     FFFlags *__restrict__ flags, ppfm_ff_status *__restrict__ status) {
+    prep_system(jobs[blockIdx.x], table, blockIdx.x, xyzq, type, recs, flags, status);
 }
 
 // ---------------------------------------------------------------------------------------------------- PTX helpers
@@ -569,13 +582,14 @@ static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st
 static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *d_xyzq, const int32_t *d_type,
                            int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
                            const ppfm_probe *probes, const ppfm_grid *grids, double r_min, float *d_a, float *d_b,
-                           bool split, void *cuda_stream) {
+                           bool split, ppfm_ff_status *d_status, void *cuda_stream) {
     if (nsys < 1 || !h_atom_offset || !h_R || !h_e || !lattices || !probes || !grids || !d_a) return PPFM_EINVAL;
     if (h_atom_offset[nsys] > 0 && (!d_xyzq || !d_type)) return PPFM_EINVAL;   // an empty atom list may be NULL
     if (split && !d_b) return PPFM_EINVAL;
     if (ntypes < 1 || ntypes > PPFM_MAX_TYPES) return PPFM_EINVAL;
     if (!(r_min >= 0.0) || !std::isfinite(r_min)) return PPFM_EINVAL;
-    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_a & 15) || (d_b && ((uintptr_t)d_b & 15))) return PPFM_EINVAL;
+    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_a & 15) || (d_b && ((uintptr_t)d_b & 15)) || ((uintptr_t)d_status & 3))
+        return PPFM_EINVAL;
     for (int t = 0; t < ntypes; t++)
         if (!(h_R[t] >= 0.0) || !(h_e[t] >= 0.0) || !std::isfinite(h_R[t]) || !std::isfinite(h_e[t])) return PPFM_EINVAL;
     if (h_atom_offset[0] != 0) return PPFM_EINVAL;
@@ -669,6 +683,7 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
     if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "scratch_alloc"); return PPFM_ENOMEM; }
     if (!single) e = cudaMemcpyAsync(d_buf, h_buf, host_bytes, cudaMemcpyHostToDevice, st);   // pageable: staged before return
     if (e == cudaSuccess) e = cudaMemsetAsync(d_buf + flags_off, 0, flags_bytes, st);
+    if (e == cudaSuccess && d_status) e = cudaMemsetAsync(d_status, 0, sizeof(ppfm_ff_status), st);
     if (e != cudaSuccess) { free(h_buf); set_cuda_error(e, "scratch upload"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
     const FFJob *dj = reinterpret_cast<const FFJob *>(d_buf);
     const TypeEntry *dt = reinterpret_cast<const TypeEntry *>(d_buf + jobs_bytes);
@@ -683,10 +698,10 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
                 one.job = hj[0];
                 memcpy(one.table, ht, (size_t)ntypes * sizeof(TypeEntry));
                 ff_prep_kernel<<<1, PREP_THREADS, 0, st>>>(one, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs,
-                                                           dflags);
+                                                           dflags, d_status);
             } else {
                 ff_prep_batch_kernel<<<nsys, PREP_THREADS, 0, st>>>(
-                    dj, dt, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs, dflags);
+                    dj, dt, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs, dflags, d_status);
             }
         }
         e = cudaGetLastError();
@@ -713,29 +728,29 @@ using namespace ppfm;
 extern "C" int ppfm_forcefield(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
                                const double *h_R, const double *h_e, const ppfm_lattice *lattice,
                                const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
-                               void *cuda_stream) {
+                               ppfm_ff_status *d_status, void *cuda_stream) {
     if (natoms < 0) return PPFM_EINVAL;
     const int32_t off[2] = {0, natoms};
     return forcefield_impl(1, off, d_xyzq, d_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, d_ff, nullptr,
-                           false, cuda_stream);
+                           false, d_status, cuda_stream);
 }
 
 extern "C" int ppfm_forcefield_split(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
                                      const double *h_R, const double *h_e, const ppfm_lattice *lattice,
                                      const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff_lj,
-                                     float *d_ff_el, void *cuda_stream) {
+                                     float *d_ff_el, ppfm_ff_status *d_status, void *cuda_stream) {
     if (natoms < 0) return PPFM_EINVAL;
     const int32_t off[2] = {0, natoms};
     return forcefield_impl(1, off, d_xyzq, d_type, ntypes, h_R, h_e, lattice, probe, grid, r_min, d_ff_lj, d_ff_el,
-                           true, cuda_stream);
+                           true, d_status, cuda_stream);
 }
 
 extern "C" int ppfm_forcefield_batch(int32_t nsys, const int32_t *h_atom_offset, const float *d_xyzq,
                                      const int32_t *d_type, int32_t ntypes, const double *h_R, const double *h_e,
                                      const ppfm_lattice *lattices, const ppfm_probe *probes, const ppfm_grid *grids,
-                                     double r_min, float *d_ff, void *cuda_stream) {
+                                     double r_min, float *d_ff, ppfm_ff_status *d_status, void *cuda_stream) {
     return forcefield_impl(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices, probes, grids, r_min,
-                           d_ff, nullptr, false, cuda_stream);
+                           d_ff, nullptr, false, d_status, cuda_stream);
 }
 
 extern "C" int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q, int64_t n_points, float *d_out,

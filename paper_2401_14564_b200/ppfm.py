@@ -60,13 +60,13 @@ class Stats(C.Structure):
                 ("cell_gathers", C.c_uint64), ("warp_gathers", C.c_uint64)]
 
 
+# the product ABI (include/ppfm.h); the measurement interface of include/ppfm_bench.h is bound in ppfm_bench.py
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
-           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft", "ppfm_forcefield_pauli", "ppfm_relax_scan",
-           "ppfm_relax_scan_batch", "ppfm_relax_scan_tricubic", "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid",
-           "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df", "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch", "ppfm_scan_host_sweep",
-           "ppfm_probe_fma", "ppfm_probe_gather", "ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read",
+           "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft",
+           "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_tricubic",
+           "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid", "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df",
+           "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch", "ppfm_scan_host_sweep",
            "ppfm_release_scratch"]
-KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6, "relax_tricubic": 7}
 
 
 def lib():
@@ -82,7 +82,6 @@ def lib():
         L.ppfm_strerror.argtypes = [C.c_int]
         L.ppfm_Nm_to_eVA2.restype = C.c_double
         L.ppfm_Nm_to_eVA2.argtypes = [C.c_double]
-        L.ppfm_launch_count.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -94,25 +93,6 @@ def _check(rc: int, what: str):
 
 def version() -> int:
     return int(lib().ppfm_version())
-
-
-def launch_count() -> int:
-    return int(lib().ppfm_launch_count())
-
-
-def timing_enable(on: bool = True) -> None:
-    """ppfm_timing_enable: bracket every kernel launch with CUDA events inside the library (clears the totals)."""
-    _check(lib().ppfm_timing_enable(C.c_int(int(on))), "ppfm_timing_enable")
-
-
-def timing_read() -> dict:
-    """ppfm_timing_read for every kernel: {name: (total ms, launches)}."""
-    out = {}
-    for name, kid in KERNEL_IDS.items():
-        ms, n = C.c_double(0.0), C.c_int64(0)
-        _check(lib().ppfm_timing_read(C.c_int(kid), C.byref(ms), C.byref(n)), "ppfm_timing_read")
-        out[name] = (ms.value, int(n.value))
-    return out
 
 
 def release_scratch() -> None:
@@ -216,7 +196,18 @@ def _darr(a):
 
 
 # ---- (1) force field ----------------------------------------------------------------------------------------
-def forcefield(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out=None, Q=None):
+def new_ff_status(device="cuda"):
+    """Device ppfm_ff_status (8 bytes) for the `status` argument of the force-field calls; read with read_ff_status."""
+    torch = _torch()
+    return torch.zeros(2, dtype=torch.int32, device=device)
+
+
+def read_ff_status(status) -> dict:
+    raw = status.cpu().numpy().view(np.uint32)
+    return {"n_bad_type": int(raw[0]), "n_clamped": int(raw[1])}
+
+
+def forcefield(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out=None, Q=None, status=None):
     """ppfm_forcefield: xyzq (N,4) float32 CUDA, types (N,) int32 CUDA -> (nz, ny, nx, 4) float32 CUDA."""
     torch = _torch()
     nx, ny, nz = (int(v) for v in grid.n)
@@ -226,12 +217,14 @@ def forcefield(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out
     e, pe = _darr(elem_e)
     rc = lib().ppfm_forcefield(C.c_int32(xyzq.shape[0]), _dptr(xyzq, torch.float32), _dptr(types, torch.int32),
                                C.c_int32(len(R)), pR, pe, C.byref(c_lattice(lattice)), C.byref(c_probe(probe, Q)),
-                               C.byref(c_grid(grid)), C.c_double(r_min), _dptr(out, torch.float32), _stream())
+                               C.byref(c_grid(grid)), C.c_double(r_min), _dptr(out, torch.float32), _dptr(status),
+                               _stream())
     _check(rc, "ppfm_forcefield")
     return out
 
 
-def forcefield_split(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out_lj=None, out_el=None):
+def forcefield_split(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out_lj=None, out_el=None,
+                     status=None):
     torch = _torch()
     nx, ny, nz = (int(v) for v in grid.n)
     if out_lj is None:
@@ -244,7 +237,7 @@ def forcefield_split(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.
                                      _dptr(types, torch.int32), C.c_int32(len(R)), pR, pe,
                                      C.byref(c_lattice(lattice)), C.byref(c_probe(probe)), C.byref(c_grid(grid)),
                                      C.c_double(r_min), _dptr(out_lj, torch.float32), _dptr(out_el, torch.float32),
-                                     _stream())
+                                     _dptr(status), _stream())
     _check(rc, "ppfm_forcefield_split")
     return out_lj, out_el
 
@@ -260,7 +253,7 @@ def combine(ff_lj, ff_el, Q: float, out=None):
 
 
 def forcefield_batch(atom_offset: Sequence[int], xyzq, types, elem_R, elem_e, lattices, probes, grids, r_min=0.1,
-                     out=None):
+                     out=None, status=None):
     """ppfm_forcefield_batch: concatenated atoms, one launch; returns a flat (sum points, 4) float32 tensor."""
     torch = _torch()
     nsys = len(grids)
@@ -273,7 +266,7 @@ def forcefield_batch(atom_offset: Sequence[int], xyzq, types, elem_R, elem_e, la
     e, pe = _darr(elem_e)
     rc = lib().ppfm_forcefield_batch(C.c_int32(nsys), off, _dptr(xyzq, torch.float32), _dptr(types, torch.int32),
                                      C.c_int32(len(R)), pR, pe, lat, pr, gr, C.c_double(r_min),
-                                     _dptr(out, torch.float32), _stream())
+                                     _dptr(out, torch.float32), _dptr(status), _stream())
     _check(rc, "ppfm_forcefield_batch")
     return out
 
@@ -441,95 +434,71 @@ def df_weights(n: int, dz: float) -> np.ndarray:
 
 
 # ---- whole simulation, host buffers ------------------------------------------------------------------------------
-def scan_host(w, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None, Q=None) -> dict:
-    """ppfm_scan_host on a workload: host (ideally pinned) torch CPU tensors or numpy arrays in and out."""
-    _torch()
+def _hptr(x):
+    """Host pointer of a torch CPU tensor or numpy array (None -> NULL)."""
+    if x is None:
+        return C.c_void_p(0)
+    return C.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data)
 
-    def hp(x):
-        if x is None:
-            return C.c_void_p(0)
-        return C.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data)
 
-    R, pR = _darr(w.elem_R)
-    e, pe = _darr(w.elem_e)
-    st = Stats()
-    rc = lib().ppfm_scan_host(C.c_int32(int(h_xyzq.shape[0])), hp(h_xyzq), hp(h_types), C.c_int32(len(R)), pR, pe,
-                              C.byref(c_lattice(w.lattice)), C.byref(c_probe(w.probe, Q)), C.byref(c_grid(w.grid)),
-                              C.c_double(w.r_min), C.byref(c_tip(w.tip)), C.byref(c_fire(w.fire)),
-                              C.byref(c_scan(w.scan)), C.c_double(w.df.A), C.c_double(w.df.k0), C.c_double(w.df.f0),
-                              hp(h_pos_fz), hp(h_iters), hp(h_df), C.byref(st), _stream())
-    _check(rc, "ppfm_scan_host")
+def _stats_dict(st: Stats) -> dict:
     return {"total_iters": int(st.total_iters), "n_not_converged": int(st.n_not_converged),
             "n_clamped": int(st.n_clamped), "max_iters": int(st.max_iters), "warp_iters": int(st.warp_iters),
             "cell_gathers": int(st.cell_gathers), "warp_gathers": int(st.warp_gathers)}
 
 
-# ---- probes --------------------------------------------------------------------------------------------------------
+def scan_host(w, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None, Q=None) -> dict:
+    """ppfm_scan_host on a workload: host (ideally pinned) torch CPU tensors or numpy arrays in and out."""
+    _torch()
+
+    R, pR = _darr(w.elem_R)
+    e, pe = _darr(w.elem_e)
+    st = Stats()
+    rc = lib().ppfm_scan_host(C.c_int32(int(h_xyzq.shape[0])), _hptr(h_xyzq), _hptr(h_types), C.c_int32(len(R)), pR, pe,
+                              C.byref(c_lattice(w.lattice)), C.byref(c_probe(w.probe, Q)), C.byref(c_grid(w.grid)),
+                              C.c_double(w.r_min), C.byref(c_tip(w.tip)), C.byref(c_fire(w.fire)),
+                              C.byref(c_scan(w.scan)), C.c_double(w.df.A), C.c_double(w.df.k0), C.c_double(w.df.f0),
+                              _hptr(h_pos_fz), _hptr(h_iters), _hptr(h_df), C.byref(st), _stream())
+    _check(rc, "ppfm_scan_host")
+    return _stats_dict(st)
+
+
 def scan_host_sweep(w, Qs, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None) -> dict:
     """ppfm_scan_host_sweep: one split force-field pass, then combine + scan + df per tip charge in Qs; the host
     outputs hold len(Qs) consecutive result sets."""
     _torch()
 
-    def hp(x):
-        if x is None:
-            return C.c_void_p(0)
-        return C.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data)
-
     R, pR = _darr(w.elem_R)
     e, pe = _darr(w.elem_e)
     Q, pQ = _darr(list(Qs))
     st = Stats()
-    rc = lib().ppfm_scan_host_sweep(C.c_int32(len(Q)), pQ, C.c_int32(int(h_xyzq.shape[0])), hp(h_xyzq), hp(h_types),
+    rc = lib().ppfm_scan_host_sweep(C.c_int32(len(Q)), pQ, C.c_int32(int(h_xyzq.shape[0])), _hptr(h_xyzq), _hptr(h_types),
                                     C.c_int32(len(R)), pR, pe, C.byref(c_lattice(w.lattice)), C.byref(c_probe(w.probe)),
                                     C.byref(c_grid(w.grid)), C.c_double(w.r_min), C.byref(c_tip(w.tip)),
                                     C.byref(c_fire(w.fire)), C.byref(c_scan(w.scan)), C.c_double(w.df.A),
-                                    C.c_double(w.df.k0), C.c_double(w.df.f0), hp(h_pos_fz), hp(h_iters), hp(h_df),
+                                    C.c_double(w.df.k0), C.c_double(w.df.f0), _hptr(h_pos_fz), _hptr(h_iters), _hptr(h_df),
                                     C.byref(st), _stream())
     _check(rc, "ppfm_scan_host_sweep")
-    return {"total_iters": int(st.total_iters), "n_not_converged": int(st.n_not_converged),
-            "n_clamped": int(st.n_clamped), "max_iters": int(st.max_iters), "warp_iters": int(st.warp_iters),
-            "cell_gathers": int(st.cell_gathers), "warp_gathers": int(st.warp_gathers)}
+    return _stats_dict(st)
 
 
 def scan_host_batch(ws, h_xyzq, h_types, h_pos_fz=None, h_iters=None, h_df=None) -> dict:
     """ppfm_scan_host_batch on a list of workloads (atoms concatenated in h_xyzq / h_types, outputs concatenated)."""
     _torch()
 
-    def hp(x):
-        if x is None:
-            return C.c_void_p(0)
-        return C.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data)
-
     w0 = ws[0]
     R, pR = _darr(w0.elem_R)
     e, pe = _darr(w0.elem_e)
     off = np.concatenate([[0], np.cumsum([w.natoms for w in ws])]).astype(np.int32)
     st = Stats()
-    rc = lib().ppfm_scan_host_batch(C.c_int32(len(ws)), off.ctypes.data_as(C.c_void_p), hp(h_xyzq), hp(h_types),
+    rc = lib().ppfm_scan_host_batch(C.c_int32(len(ws)), off.ctypes.data_as(C.c_void_p), _hptr(h_xyzq), _hptr(h_types),
                                     C.c_int32(len(R)), pR, pe, c_array([w.lattice for w in ws], c_lattice),
                                     c_array([w.probe for w in ws], c_probe), c_array([w.grid for w in ws], c_grid),
                                     C.c_double(w0.r_min), c_array([w.tip for w in ws], c_tip), C.byref(c_fire(w0.fire)),
                                     c_array([w.scan for w in ws], c_scan), C.c_double(w0.df.A), C.c_double(w0.df.k0),
-                                    C.c_double(w0.df.f0), hp(h_pos_fz), hp(h_iters), hp(h_df), C.byref(st), _stream())
+                                    C.c_double(w0.df.f0), _hptr(h_pos_fz), _hptr(h_iters), _hptr(h_df), C.byref(st), _stream())
     _check(rc, "ppfm_scan_host_batch")
-    return {"total_iters": int(st.total_iters), "n_not_converged": int(st.n_not_converged),
-            "n_clamped": int(st.n_clamped), "max_iters": int(st.max_iters), "warp_iters": int(st.warp_iters),
-            "cell_gathers": int(st.cell_gathers), "warp_gathers": int(st.warp_gathers)}
-
-
-def probe_fma() -> float:
-    _torch()
-    v = C.c_double(0.0)
-    _check(lib().ppfm_probe_fma(C.byref(v), _stream()), "ppfm_probe_fma")
-    return v.value
-
-
-def probe_gather(n_float4: int, bypass_l1: bool) -> float:
-    _torch()
-    v = C.c_double(0.0)
-    _check(lib().ppfm_probe_gather(C.c_int64(n_float4), C.c_int32(int(bypass_l1)), C.byref(v), _stream()),
-           "ppfm_probe_gather")
-    return v.value
+    return _stats_dict(st)
 
 
 # ---- convenience: run a workloads.Workload end to end on device-resident inputs ------------------------------------

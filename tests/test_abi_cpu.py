@@ -1,5 +1,6 @@
-"""CPU-only checks of the C-ABI library: it loads without a GPU, exports every symbol include/ppfm.h declares, its
-ctypes struct mirrors have the header's layout, and argument validation returns PPFM_EINVAL before any CUDA call."""
+"""CPU-only checks of the C-ABI libraries: they load without a GPU, libppfm.so exports every symbol include/ppfm.h
+declares (and the launch counter / timers of include/ppfm_bench.h), libppfm_probes.so exports the probes, the ctypes
+struct mirrors have the header's layout, and argument validation returns PPFM_EINVAL before any CUDA call."""
 import ctypes as C
 import os
 import re
@@ -8,7 +9,7 @@ import numpy as np
 import pytest
 
 from paper_2401_14564_b200 import build as ppfm_build
-from paper_2401_14564_b200 import ppfm
+from paper_2401_14564_b200 import ppfm, ppfm_bench
 from paper_2401_14564_b200 import workloads as W
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -20,8 +21,8 @@ def lib():
     return ppfm.lib()
 
 
-def header_symbols():
-    text = open(os.path.join(ROOT, "include", "ppfm.h")).read()
+def header_symbols(name="ppfm.h"):
+    text = open(os.path.join(ROOT, "include", name)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(ppfm_[A-Za-z0-9_]+)\s*\(", text)))
 
@@ -33,6 +34,15 @@ def test_library_exports_every_declared_symbol(lib):
         assert hasattr(lib, n), f"libppfm.so does not export {n}"
     assert set(names) == set(ppfm.EXPORTS)
     assert lib.ppfm_version() == 100
+    # the measurement interface lives in its own header; the probes in their own library
+    bench = header_symbols("ppfm_bench.h")
+    assert set(bench) == set(ppfm_bench.EXPORTS_LIBPPFM) | set(ppfm_bench.EXPORTS_PROBES)
+    assert not set(bench) & set(names)
+    for n in ppfm_bench.EXPORTS_LIBPPFM:
+        assert hasattr(lib, n), f"libppfm.so does not export {n}"
+    probes = ppfm_bench.probes_lib()
+    for n in ppfm_bench.EXPORTS_PROBES:
+        assert hasattr(probes, n) and not hasattr(lib, n), n
 
 
 def test_struct_layouts_match_header():
@@ -63,23 +73,23 @@ def test_invalid_arguments_are_rejected_on_the_host(lib):
     EINVAL = -1
     ff = lib.ppfm_forcefield
     assert ff(C.c_int32(10), null, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat), C.byref(pr), C.byref(gr),
-              C.c_double(0.1), fake, null) == EINVAL                       # null atoms
+              C.c_double(0.1), fake, null, null) == EINVAL                       # null atoms
     assert ff(C.c_int32(-1), fake, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat), C.byref(pr), C.byref(gr),
-              C.c_double(0.1), fake, null) == EINVAL                       # negative count
+              C.c_double(0.1), fake, null, null) == EINVAL                       # negative count
     assert ff(C.c_int32(10), fake, fake, C.c_int32(0), pd(R), pd(e), C.byref(lat), C.byref(pr), C.byref(gr),
-              C.c_double(0.1), fake, null) == EINVAL                       # no types
+              C.c_double(0.1), fake, null, null) == EINVAL                       # no types
     assert ff(C.c_int32(10), fake, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat), C.byref(pr), C.byref(gr),
-              C.c_double(-1.0), fake, null) == EINVAL                      # negative r_min
+              C.c_double(-1.0), fake, null, null) == EINVAL                      # negative r_min
     bad = ppfm.c_grid(w.grid)
     bad.step[2][2] = 0.0                                                   # singular step matrix
     assert ff(C.c_int32(10), fake, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat), C.byref(pr), C.byref(bad),
-              C.c_double(0.1), fake, null) == EINVAL
+              C.c_double(0.1), fake, null, null) == EINVAL
     bad = ppfm.c_grid(w.grid)
     bad.n[1] = 0
     assert ff(C.c_int32(10), fake, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat), C.byref(pr), C.byref(bad),
-              C.c_double(0.1), fake, null) == EINVAL
+              C.c_double(0.1), fake, null, null) == EINVAL
     assert ff(C.c_int32(10), C.c_void_p(0x1004), fake, C.c_int32(5), pd(R), pd(e), C.byref(lat), C.byref(pr),
-              C.byref(gr), C.c_double(0.1), fake, null) == EINVAL          # misaligned float4 buffer
+              C.byref(gr), C.c_double(0.1), fake, null, null) == EINVAL          # misaligned float4 buffer
 
     tip, fire, sc = ppfm.c_tip(w.tip), ppfm.c_fire(w.fire), ppfm.c_scan(w.scan)
     rx = lib.ppfm_relax_scan
@@ -100,6 +110,7 @@ def test_invalid_arguments_are_rejected_on_the_host(lib):
     assert df(*args(40, 0.1, 0.55)) == EINVAL                              # A/dz not an integer
     assert df(*args(10, 0.1, 1.0)) == EINVAL                               # nz <= n
     assert df(*args(40, 0.0, 1.0)) == EINVAL
+    assert df(*args(4000, 0.001, 1.0)) == EINVAL                           # n = 1000 > PPFM_DF_MAX_N
     # the 8(f) entry points and the host forms validate before any CUDA call too
     td = ppfm.TipDensity(0.0, 1.0, 0.0, 0.0)                               # sigma must be > 0
     assert lib.ppfm_forcefield_fft(fake, C.byref(gr), C.byref(td), fake, null) == EINVAL
@@ -143,4 +154,6 @@ def test_binding_fails_loudly_without_gpu():
     with pytest.raises(ppfm.PpfmError):
         ppfm.upload(w)
     with pytest.raises(ppfm.PpfmError):
-        ppfm.probe_fma()
+        ppfm_bench.probe_fma()
+    with pytest.raises(ppfm.PpfmError):
+        ppfm.new_stats()

@@ -897,7 +897,34 @@ def test_scan_host_batch_equals_per_system_calls(P):
 
 
 def test_probes_run(P):
-    assert P.probe_fma() > 1e12
-    assert P.probe_gather(1 << 20, False) > 10.0
-    assert P.probe_gather(1 << 20, True) > 10.0
-    assert P.launch_count() > 0
+    from paper_2401_14564_b200 import ppfm_bench as B
+    assert B.probe_fma() > 1e12
+    assert B.probe_gather(1 << 20, False) > 10.0
+    assert B.probe_gather(1 << 20, True) > 10.0
+    assert B.launch_count() > 0
+
+
+def test_ff_status_counts_bad_type_indices_and_clamp(P):
+    """include/ppfm.h: an atom whose type index is outside [0, ntypes) contributes nothing and is counted in
+    ppfm_ff_status.n_bad_type (the index array is device memory, so it cannot be validated on the host)."""
+    import torch
+    w = W.shrink(W.get(0), grid_n=(16, 16, 8))
+    types = w.types.copy()
+    types[2], types[7] = 99, -1
+    status = P.new_ff_status()
+    xyzq, _ = P.upload(w)
+    ff = P.forcefield(xyzq, torch.from_numpy(types).cuda(), w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min,
+                      status=status)
+    torch.cuda.synchronize()
+    assert P.read_ff_status(status) == {"n_bad_type": 2, "n_clamped": 0}
+    keep = np.ones(w.natoms, bool)
+    keep[[2, 7]] = False
+    ref = oracle.forcefield(replace(w, xyzq=w.xyzq[keep], types=w.types[keep]))
+    check_ff(ff.cpu().numpy(), ref, "bad types skipped")
+    # status is rewritten by every call; the clamp flag shows when an atom sits inside the grid's box
+    x = w.xyzq.copy()
+    x[0, :3] = [1.0, 1.2, 1.3 + 0.4]
+    P.forcefield(torch.from_numpy(x).cuda(), torch.from_numpy(w.types).cuda(), w.elem_R, w.elem_e, w.lattice, w.probe,
+                 w.grid, 0.5, status=status)
+    torch.cuda.synchronize()
+    assert P.read_ff_status(status) == {"n_bad_type": 0, "n_clamped": 1}
