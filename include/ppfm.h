@@ -17,8 +17,8 @@
  *          passed by pointer are HOST memory and are read before the call returns.
  *   Ownership: every buffer is allocated and freed by the caller.  The library keeps no pointer to caller memory
  *          after return; per-call scratch is stream-ordered (allocated and freed on `cuda_stream` inside the call)
- *          from a library-private pool that caches freed blocks until ppfm_release_scratch(); the cuFFT plans of
- *          (1b)/(1c) are cached per grid size until then too.
+ *          from a library-private pool that caches freed blocks until ppfm_release_scratch(); the cuFFT plans and
+ *          tip spectra of (1b)/(1c) are cached until then too (the one persistent device allocation the library makes).
  *          Device entry points only enqueue work on `cuda_stream` (a cudaStream_t cast to
  *          void*, NULL = default stream); they never synchronise it and never change the current device.
  *          Host entry points (ppfm_scan_host, _batch, _sweep) synchronise the stream before returning.
@@ -185,7 +185,11 @@ int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grid
  * d_V   DEVICE float[nz][ny][nx]: sample potential V_S in eV per unit charge (e.g. the .w lane of the unit-charge
  *       grid of ppfm_forcefield_split, or a Hartree potential)
  * d_ff  DEVICE float[nz][ny][nx][4] = (Fx, Fy, Fz, E_el); add to an LJ grid with ppfm_combine(lj, d_ff, 1.0, ...)
- * The library caches the cuFFT plans (and their work areas) per grid size until ppfm_release_scratch().
+ * The library caches the cuFFT plans per grid size (without work areas: every call binds its own from the scratch
+ * pool) and the four tip spectra of the two most recently used (grid, tip density) pairs (4 x nz*ny*(nx/2+1) complex
+ * doubles each, device memory) until ppfm_release_scratch(): a run of calls on one grid with one tip costs one
+ * forward and four inverse transforms each ("amortized if a batch of simulations is run using the
+ * same grid").
  */
 typedef struct {
     double sigma;   /* Gaussian width (Å)        */
@@ -240,6 +244,18 @@ int ppfm_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip
                    const float *d_pos_fz, float *d_eig, void *cuda_stream);
 int ppfm_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                          const ppfm_scan *scans, const float *d_pos_fz, float *d_eig, void *cuda_stream);
+/* The relaxation scan with the stiffness map folded in: at the end of every z-step the lane that relaxed the pixel
+ * forms J from the grid cell it still holds in registers (no second gather, no second launch) and writes the three
+ * eigenvalues of H at the relaxed point to d_eig (same layout as above; FP32 throughout, the eigenvalues by
+ * deflation on the isolated root so that the two nearly degenerate lateral modes keep full FP32 accuracy).  All other
+ * arguments and outputs as ppfm_relax_scan[_batch]; d_eig must not be NULL.  ppfm_stiffness remains the entry point
+ * for positions that do not come straight from a scan. */
+int ppfm_relax_scan_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_fire *fire,
+                              const ppfm_scan *scan, float *d_pos_fz, uint16_t *d_iters, float *d_eig,
+                              ppfm_stats *d_stats, void *cuda_stream);
+int ppfm_relax_scan_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                                    const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
+                                    float *d_eig, ppfm_stats *d_stats, void *cuda_stream);
 
 /* ---- (3) frequency shift, Giessibl's formula Eq.3 -------------------------------------------
  * Fz is read from the .w lane of d_pos_fz [nz][npy][npx][4].  A = peak-to-peak amplitude (Å); n = A/dz must be an

@@ -39,6 +39,17 @@ typedef enum {
 int ppfm_timing_enable(int on);
 int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);
 
+/* Checked build only (libppfm_chk.so = the same sources compiled with -DPPFM_CHECKS; stands in for compute-sanitizer,
+ * which is closed on the GPU pool this library is developed on).  The kernels then test every global store and gather
+ * index against its buffer's extent and compare each stage of ff_kernel's shared-memory atom ring with the global
+ * records when the stage is acquired and again when it is released.  ppfm_checks_read synchronises the device, writes
+ * the counts since the last call to h_counts[8] and clears them:
+ *   [0] ring stage wrong at acquire (read before the copy landed)   [1] ring stage changed before release (overwritten
+ *   in use)   [2] force-field store out of range   [3] relaxation gather out of range   [4] relaxation store out of
+ *   range   [5] df load out of range   [6] df store out of range   [7] checks executed.
+ * The product build (libppfm.so) returns PPFM_EINVAL. */
+int ppfm_checks_read(uint64_t *h_counts);
+
 /* ---- (b) exported by libppfm_probes.so ------------------------------------------------------------------------
  * ppfm_probe_fma:    FFMA-only kernel; returns lane-instructions per second in *h_lane_instr_per_s.
  * ppfm_probe_gather: the relaxation's 8-corner float4 gather (a warp = 8 x 4 neighbouring cells) over an L2-resident

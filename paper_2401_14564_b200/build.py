@@ -15,6 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libppfm.so")
+CHK_LIB = os.path.join(HERE, "libppfm_chk.so")             # checked build: same sources, -DPPFM_CHECKS (ppfm_bench.h)
+CHK_OBJDIR = os.path.join(HERE, "build", "chk")
 PROBES_SRC = os.path.join(HERE, "csrc_probes", "probes.cu")
 PROBES_LIB = os.path.join(HERE, "libppfm_probes.so")      # include/ppfm_bench.h (b): measurement only
 NVCC_COMPILE = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
@@ -35,6 +37,10 @@ def headers():
 def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str = LIB, objdir: str = OBJDIR) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(objdir, exist_ok=True)
+    chk = None
+    if lib == LIB:            # the checked build compiles alongside
+        chk = ThreadPoolExecutor(max_workers=1)
+        chk_done = chk.submit(build, force, verbose, ("-DPPFM_CHECKS",), CHK_LIB, CHK_OBJDIR)
     hdr_time = max(os.path.getmtime(h) for h in headers())
     jobs, objs = [], []
     for src in sources():
@@ -52,6 +58,9 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
                     raise subprocess.CalledProcessError(r.returncode, r.args)
     if jobs or not os.path.exists(lib) or any(os.path.getmtime(lib) < os.path.getmtime(o) for o in objs):
         subprocess.run([nvcc] + NVCC_LINK + ["-o", lib] + objs, check=True)
+    if chk is not None:
+        chk_done.result()
+        chk.shutdown()
     if lib == LIB and (force or not os.path.exists(PROBES_LIB) or
                        os.path.getmtime(PROBES_LIB) < max(os.path.getmtime(PROBES_SRC), hdr_time)):
         subprocess.run([nvcc] + [f for f in NVCC_COMPILE if f != "-c"] + ["--shared", "-cudart", "static", "-o",

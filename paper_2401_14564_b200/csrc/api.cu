@@ -131,6 +131,21 @@ extern "C" int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_la
     return PPFM_OK;
 }
 
+extern "C" int ppfm_checks_read(uint64_t *h_counts) {
+#ifdef PPFM_CHECKS
+    if (!h_counts) return PPFM_EINVAL;
+    unsigned long long c[PPFM_CHK_KINDS] = {};
+    ff_checks_read(c);
+    relax_checks_read(c);
+    df_checks_read(c);
+    for (int k = 0; k < PPFM_CHK_KINDS; k++) h_counts[k] = (uint64_t)c[k];
+    return PPFM_OK;
+#else
+    (void)h_counts;
+    return PPFM_EINVAL;      // not a checked build
+#endif
+}
+
 extern "C" int ppfm_release_scratch(void) {
     release_fft_plans();
     int dev = 0;

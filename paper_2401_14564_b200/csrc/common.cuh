@@ -55,6 +55,38 @@ struct KernelTimer {
     }
 };
 
+// Checked build (libppfm_chk.so, -DPPFM_CHECKS; compute-sanitizer is closed on the GPU pool this was developed on): every
+// global store / gather index is tested against its buffer's extent and the force-field kernel's shared-memory ring
+// is compared with the global atom records when a chunk is acquired (a stage read before its copy landed) and again
+// when it is released (a stage overwritten while still in use).  Failures are counted per kind, never trapped;
+// ppfm_checks_read (include/ppfm_bench.h) returns the counts.  The product build compiles none of this.
+enum { PPFM_CHK_RING_ACQUIRE = 0, PPFM_CHK_RING_RELEASE = 1, PPFM_CHK_FF_STORE = 2, PPFM_CHK_RELAX_GATHER = 3,
+       PPFM_CHK_RELAX_STORE = 4, PPFM_CHK_DF_LOAD = 5, PPFM_CHK_DF_STORE = 6, PPFM_CHK_VISITS = 7, PPFM_CHK_KINDS = 8 };
+#ifdef PPFM_CHECKS
+#define PPFM_CHK_STORAGE                                                                          \
+    static __device__ unsigned long long g_chk[PPFM_CHK_KINDS];                                   \
+    void PPFM_CHK_READER(unsigned long long *out) {                                               \
+        unsigned long long h[PPFM_CHK_KINDS] = {}, z[PPFM_CHK_KINDS] = {};                        \
+        cudaDeviceSynchronize();                                                                  \
+        cudaMemcpyFromSymbol(h, g_chk, sizeof(h));                                                \
+        cudaMemcpyToSymbol(g_chk, z, sizeof(z));                                                  \
+        for (int k = 0; k < PPFM_CHK_KINDS; k++) out[k] += h[k];                                  \
+    }
+#define PPFM_CHK(kind, cond)                                                  \
+    do {                                                                      \
+        atomicAdd(&g_chk[PPFM_CHK_VISITS], 1ull);                             \
+        if (!(cond)) atomicAdd(&g_chk[kind], 1ull);                           \
+    } while (0)
+#else
+#define PPFM_CHK_STORAGE
+#define PPFM_CHK(kind, cond) \
+    do {                     \
+    } while (0)
+#endif
+void ff_checks_read(unsigned long long *out);
+void relax_checks_read(unsigned long long *out);
+void df_checks_read(unsigned long long *out);
+
 #define PPFM_CUDA(call)                                  \
     do {                                                 \
         cudaError_t _e = (call);                         \

@@ -2,12 +2,21 @@
 //   df = -(f0 / 2k) (8 / (pi A^2)) int_{-A/2}^{A/2} q Fz(z + q) / sqrt(A^2/4 - q^2) dq,
 // integrated exactly for the piecewise-linear interpolant of the n + 1 = A/dz + 1 samples in each window
 // (reading S9).  The n + 1 weights are computed in FP64 on the host and passed by value; the kernel is
-// a streaming weighted sum, one thread per output sample, lanes along x (HBM/L2-bound, trivial next to a2/a5).
+// a streaming weighted sum down each pixel column (HBM-bound: every Fz sample is read once).
 #include "common.cuh"
+
+#include <algorithm>
 
 namespace ppfm {
 
 constexpr int DF_MAX_N = PPFM_DF_MAX_N;
+
+#define PPFM_CHK_READER df_checks_read
+PPFM_CHK_STORAGE
+#undef PPFM_CHK_READER
+#ifndef PPFM_CHECKS
+void df_checks_read(unsigned long long *) {}
+#endif
 
 struct DfWeights {
     float w[DF_MAX_N + 1];   // already multiplied by -(f0 / 2 k0) * 16.02176634
@@ -36,6 +45,55 @@ static void df_weights_host(int n, double dz, double *W) {
 
 // FZ4: Fz is the .w lane of the float4 (x, y, z, Fz) stack; otherwise a plain float stack (ppfm_scan_host keeps one
 // on the device when the float4 stack itself is written straight to mapped host memory).
+//
+// Column kernel (n + 1 <= DF_RING_MAX): one thread per pixel column and chunk of output planes marches down z with the
+// n + 1 samples of the current window in a register ring (slot indices are compile-time constants: the march is
+// unrolled NW = n + 1 deep), so every sample is loaded once per chunk instead of n + 1 times and a warp's loads are
+// 32 consecutive pixels of one plane.  The sum runs in the same order as the gather kernel below (m = 0 .. n).
+constexpr int DF_RING_MAX = 33;
+constexpr int DF_COL_THREADS = 128;
+
+template <int NW, bool FZ4>
+__global__ void __launch_bounds__(DF_COL_THREADS)
+df_column_kernel(const float *__restrict__ fz, long long npix, int nz, int kc, const __grid_constant__ DfWeights W,
+                 float *__restrict__ df) {
+    constexpr int n = NW - 1;
+    constexpr int S = FZ4 ? 4 : 1;
+    const long long col = (long long)blockIdx.x * DF_COL_THREADS + threadIdx.x;
+    if (col >= npix) return;
+    const int nout = nz - n;
+    const int k0 = (int)blockIdx.y * kc;
+    const int cnt = min(kc, nout - k0);                       // output planes of this chunk
+    const long long zs = npix * S;
+    const float *src = fz + (((long long)blockIdx.z * nz + k0) * npix + col) * S + (FZ4 ? 3 : 0);
+    float *dst = df + ((long long)blockIdx.z * nout + k0) * npix + col;
+    float ring[NW];                                           // sample k0 + j lives in slot j % NW
+#pragma unroll
+    for (int j = 0; j < n; j++) ring[j] = __ldg(src + (long long)j * zs);
+    // Each block of NW output planes first loads its NW new samples, unpredicated and back to back (past the chunk's
+    // end the index is clamped to the stack's last plane and the value is not used), then forms the NW sums; only the
+    // stores are guarded.
+    const int jmax = nz - 1 - k0;
+    for (int i0 = 0; i0 < cnt; i0 += NW) {
+        float nxt[NW];
+#pragma unroll
+        for (int r = 0; r < NW; r++) {
+            PPFM_CHK(PPFM_CHK_DF_LOAD, k0 + min(i0 + r + n, jmax) >= 0 && k0 + min(i0 + r + n, jmax) < nz);
+            nxt[r] = __ldg(src + (long long)min(i0 + r + n, jmax) * zs);
+        }
+#pragma unroll
+        for (int r = 0; r < NW; r++) {
+            ring[(r + n) % NW] = nxt[r];
+            float acc = 0.f;
+#pragma unroll
+            for (int m = 0; m <= n; m++) acc = fmaf(W.w[m], ring[(r + n - m) % NW], acc);
+            PPFM_CHK(PPFM_CHK_DF_STORE, i0 + r >= cnt || k0 + i0 + r < nout);
+            if (i0 + r < cnt) dst[(long long)(i0 + r) * npix] = acc;
+        }
+    }
+}
+
+// Gather kernel (any n <= DF_MAX_N): one thread per output sample, n + 1 strided loads each.
 template <bool FZ4>
 __global__ void __launch_bounds__(256)
 df_kernel(const float *__restrict__ fz, long long npix, int nz, int n, int nsys, DfWeights W,
@@ -51,6 +109,17 @@ df_kernel(const float *__restrict__ fz, long long npix, int nz, int n, int nsys,
         float acc = 0.f;
         for (int m = 0; m <= n; m++) acc = fmaf(W.w[m], __ldg(&src[(long long)(n - m) * npix * (FZ4 ? 4 : 1)]), acc);
         df[o] = acc;
+    }
+}
+
+template <int NW>
+static void launch_df_column(int nw, bool fz4, dim3 grid, cudaStream_t st, const float *fz, long long npix, int nz,
+                             int kc, const DfWeights &W, float *df) {
+    if (nw == NW) {
+        if (fz4) df_column_kernel<NW, true><<<grid, DF_COL_THREADS, 0, st>>>(fz, npix, nz, kc, W, df);
+        else df_column_kernel<NW, false><<<grid, DF_COL_THREADS, 0, st>>>(fz, npix, nz, kc, W, df);
+    } else if constexpr (NW < DF_RING_MAX) {
+        launch_df_column<NW + 1>(nw, fz4, grid, st, fz, npix, nz, kc, W, df);
     }
 }
 
@@ -70,12 +139,26 @@ static int df_impl(int nsys, const float *d_pos_fz, int npx, int npy, int nz, do
     for (int m = 0; m <= DF_MAX_N; m++) W.w[m] = (m <= n) ? (float)(pref * Wd[m]) : 0.f;
     const long long npix = (long long)npx * npy;
     const long long total = (long long)(nz - n) * npix * nsys;
-    long long blocks = (total + 255) / 256;
-    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    const int nout = nz - (int)n;
+    const long long col_blocks = (npix + DF_COL_THREADS - 1) / DF_COL_THREADS;
     {
         KernelTimer kt(PPFM_K_DF, (cudaStream_t)cuda_stream);
-        if (fz4) df_kernel<true><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(d_pos_fz, npix, nz, (int)n, nsys, W, d_df);
-        else df_kernel<false><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(d_pos_fz, npix, nz, (int)n, nsys, W, d_df);
+        if (n + 1 <= DF_RING_MAX && nsys <= 65535 && col_blocks <= 0x7fffffffLL) {
+            // chunks of output planes per column: one chunk when the columns alone fill the GPU, otherwise enough chunks
+            // for ~512 threads per SM, each at least one window long (a chunk re-reads n samples of its neighbour)
+            const long long want = 148LL * 512;
+            long long nchunks = (want + npix * nsys - 1) / (npix * nsys);
+            const long long max_chunks = std::max<long long>(1, nout / std::max<long long>(n + 1, 8));
+            nchunks = std::min(std::max<long long>(nchunks, 1), std::min<long long>(max_chunks, 65535));
+            const int kc = (int)((nout + nchunks - 1) / nchunks);
+            const dim3 grid((unsigned)col_blocks, (unsigned)((nout + kc - 1) / kc), (unsigned)nsys);
+            launch_df_column<2>((int)n + 1, fz4, grid, (cudaStream_t)cuda_stream, d_pos_fz, npix, nz, kc, W, d_df);
+        } else {
+            long long blocks = (total + 255) / 256;
+            if (blocks > 148LL * 32) blocks = 148LL * 32;
+            if (fz4) df_kernel<true><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(d_pos_fz, npix, nz, (int)n, nsys, W, d_df);
+            else df_kernel<false><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(d_pos_fz, npix, nz, (int)n, nsys, W, d_df);
+        }
     }
     PPFM_LAUNCH_CHECK();
     return PPFM_OK;

@@ -56,6 +56,13 @@ struct TypeEntry {
     float c6, c12;
 };
 
+#define PPFM_CHK_READER ff_checks_read
+PPFM_CHK_STORAGE
+#undef PPFM_CHK_READER
+#ifndef PPFM_CHECKS
+void ff_checks_read(unsigned long long *) {}
+#endif
+
 // ---------------------------------------------------------------------------------------------------- a1 prep
 struct FFSingle {               // one system: job and per-type table travel as a kernel parameter (constant bank)
     FFJob job;
@@ -433,8 +440,25 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, int ncharged, const At
                     mbar_wait(&full_bar[st], (step / FF_STAGES) & 1);
                     const float4 *s4 = reinterpret_cast<const float4 *>(s_rec + st * FF_CHUNK);
                     const int n = chunk_count(ch);
+#ifdef PPFM_CHECKS
+                    auto ring_matches = [&]() {      // this thread's record of the stage against the global copy
+                        const int a = tid % n;
+                        const float4 *gsrc = reinterpret_cast<const float4 *>(src + chunk_begin(ch) + a);
+                        bool same = true;
+                        for (int q = 0; q < 3; q++) {
+                            const float4 x = s4[3 * a + q], y = gsrc[q];
+                            same = same && __float_as_uint(x.x) == __float_as_uint(y.x) && __float_as_uint(x.y) == __float_as_uint(y.y) &&
+                                   __float_as_uint(x.z) == __float_as_uint(y.z) && __float_as_uint(x.w) == __float_as_uint(y.w);
+                        }
+                        return same;
+                    };
+                    PPFM_CHK(PPFM_CHK_RING_ACQUIRE, ring_matches());
+#endif
                     if (ch < nch_q) run_chunk(s4, n, std::false_type{});
                     else run_chunk(s4, n, std::true_type{});
+#ifdef PPFM_CHECKS
+                    PPFM_CHK(PPFM_CHK_RING_RELEASE, ring_matches());
+#endif
                     __syncwarp();
                     if ((tid & 31) == 0) mbar_arrive(&empty_bar[st]);
 #pragma unroll
@@ -449,6 +473,9 @@ __device__ __forceinline__ void ff_tile(const FFJob &job, int ncharged, const At
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const size_t o = (size_t)job.out_offset + (size_t)(k0 + 2 * h) * job.nxy + col;
+            PPFM_CHK(PPFM_CHK_FF_STORE, k0 + 2 * h >= job.nz ||
+                                            o + (k0 + 2 * h + 1 < job.nz ? job.nxy : 0) <
+                                                (size_t)job.out_offset + (size_t)job.nz * job.nxy);
             if (k0 + 2 * h < job.nz) {
                 out_a[o] = make_float4(Fx[h].x, Fy[h].x, Fz[h].x, Etot[h].x);
                 if (SPLIT) out_b[o] = make_float4(Gx[h].x, Gy[h].x, Gz[h].x, Getot[h].x);

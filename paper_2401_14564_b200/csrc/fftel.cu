@@ -5,10 +5,19 @@
 // cyclic sum over grid nodes times dV = |det(step)|; rho_PP is a Gaussian multipole (monopole q_s, dipole p_z,
 // quadrupole Q_zz) sampled with its analytic gradient at the nodes, minimum image by index.
 //
-// Path: fill_kernel (V -> FP64, rho and grad rho in FP64) -> cuFFT D2Z, batch 5 -> spectral_kernel
-// (conj(rho^_c) V^ dV / N, c = 0..3) -> cuFFT Z2D, batch 4 -> pack_kernel (float4 Fx, Fy, Fz, E).  The FFT itself is
-// the library primitive (cuFFT, FP64: V_S spans several orders of magnitude between the atoms and the scan region,
-// and B200 runs FP64 at half the FP32 rate, so there is no reason to pay FP32's 1e-6 of max|V| everywhere).
+// Path: fill_v_kernel (V -> FP64) -> cuFFT D2Z -> spectral_kernel (conj(rho^_c) V^ dV / N, c = 0..3) -> cuFFT Z2D,
+// batch 4 -> pack_kernel (float4 Fx, Fy, Fz, E).  The four tip spectra rho^_c depend only on (grid, sigma, q_s, p_z,
+// Q_zz): they are computed once (fill_tip_kernel + one batch-4 D2Z) and kept on the device in a small cache next to
+// the plans, so that a run of calls on one grid ("amortized if a batch of simulations is run using the same grid",
+// PAPER.md:298) costs 1 forward + 4 inverse transforms each instead of 5 + 4.  The FFT itself is the library
+// primitive (cuFFT, FP64: V_S spans several orders of magnitude between the atoms and the scan region, and B200 runs
+// FP64 at half the FP32 rate, so there is no reason to pay FP32's 1e-6 of max|V| everywhere).
+//
+// Streams and threads: plans are shared per (device, grid size) but own no work area (cufftSetAutoAllocation off);
+// every call binds its own work area from the stream-ordered scratch pool, and the bind + enqueue sequence on the
+// shared handles runs under one mutex, so calls on different streams or from different host threads neither share
+// scratch nor race on a handle.  A cached tip spectrum carries the event of the stream that produced it; other
+// streams wait on that event before reading it.
 #include "common.cuh"
 
 #include <cufft.h>
@@ -28,7 +37,16 @@ struct FftJob {
 };
 
 __global__ void __launch_bounds__(256)
-fft_fill_kernel(const __grid_constant__ FftJob job, const float *__restrict__ V, double *__restrict__ real5) {
+fft_fill_v_kernel(long long N, double vpow, const float *__restrict__ V, double *__restrict__ real1) {
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= N) return;
+    const double v = (double)V[m];
+    real1[m] = (vpow == 0.0) ? v : pow(fmax(v, 0.0), vpow);
+}
+
+// rho_PP and its analytic gradient at the nodes (minimum image by index): four real fields
+__global__ void __launch_bounds__(256)
+fft_fill_tip_kernel(const __grid_constant__ FftJob job, double *__restrict__ real4) {
     const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= job.N) return;
     const int i = (int)(m % job.nx);
@@ -49,23 +67,22 @@ fft_fill_kernel(const __grid_constant__ FftJob job, const float *__restrict__ V,
     const double dPx = -2.0 * q12 * r[0] * is4, dPy = -2.0 * q12 * r[1] * is4;
     const double dPz = job.p_z * is2 + 4.0 * q12 * r[2] * is4;
     const double Pg = P * g;
-    const double v = (double)V[m];
-    real5[m] = (job.vpow == 0.0) ? v : pow(fmax(v, 0.0), job.vpow);
-    real5[job.N + m] = Pg;
-    real5[2 * job.N + m] = dPx * g - Pg * r[0] * is2;
-    real5[3 * job.N + m] = dPy * g - Pg * r[1] * is2;
-    real5[4 * job.N + m] = dPz * g - Pg * r[2] * is2;
+    real4[m] = Pg;
+    real4[job.N + m] = dPx * g - Pg * r[0] * is2;
+    real4[2 * job.N + m] = dPy * g - Pg * r[1] * is2;
+    real4[3 * job.N + m] = dPz * g - Pg * r[2] * is2;
 }
 
-// in place on the four tip-field spectra: X_c <- conj(X_c) * V^ * scale
+// X_c = conj(T_c) * V^ * scale for the four cached tip spectra T_c
 __global__ void __launch_bounds__(256)
-fft_spectral_kernel(long long Nc, double scale, const double2 *__restrict__ Vh, double2 *__restrict__ X4) {
+fft_spectral_kernel(long long Nc, double scale, const double2 *__restrict__ Vh, const double2 *__restrict__ T4,
+                    double2 *__restrict__ X4) {
     const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= Nc) return;
     const double2 v = Vh[m];
 #pragma unroll
     for (int c = 0; c < 4; c++) {
-        const double2 x = X4[c * Nc + m];
+        const double2 x = T4[c * Nc + m];
         X4[c * Nc + m] = make_double2((x.x * v.x + x.y * v.y) * scale, (x.x * v.y - x.y * v.x) * scale);
     }
 }
@@ -77,36 +94,75 @@ fft_pack_kernel(long long N, const double *__restrict__ real4, float4 *__restric
     ff[m] = make_float4((float)real4[N + m], (float)real4[2 * N + m], (float)real4[3 * N + m], (float)real4[m]);
 }
 
-// ---- cuFFT plans, cached per (device, nx, ny, nz); destroyed by ppfm_release_scratch() ------------------------------
+// ---- cuFFT plans, cached per (device, nx, ny, nz), and tip spectra; destroyed by ppfm_release_scratch() -----------
 struct PlanEntry {
     int dev, nx, ny, nz;
-    cufftHandle fwd, inv;
+    cufftHandle fwd1, fwd4, inv4;
+    size_t work_bytes;          // max over the three plans; bound per call
 };
-static std::mutex g_plan_mu;
+struct TipEntry {
+    int dev, nx, ny, nz;
+    double step[3][3], sigma, q_s, p_z, Q_zz;
+    double2 *spec;              // 4 * Nc spectra (cudaMalloc; freed on eviction / release)
+    cudaEvent_t ready;
+    unsigned long long stamp;
+};
+constexpr int TIP_CACHE_ENTRIES = 2;
+static std::mutex g_fft_mu;     // guards both caches and every bind + enqueue on the shared handles
 static std::vector<PlanEntry> g_plans;
+static std::vector<TipEntry> g_tips;
+static unsigned long long g_tip_clock = 0;
 
-static cufftResult get_plans(int nx, int ny, int nz, cufftHandle *fwd, cufftHandle *inv) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    std::lock_guard<std::mutex> lk(g_plan_mu);
-    for (const PlanEntry &p : g_plans)
-        if (p.dev == dev && p.nx == nx && p.ny == ny && p.nz == nz) { *fwd = p.fwd; *inv = p.inv; return CUFFT_SUCCESS; }
-    PlanEntry e = {dev, nx, ny, nz, 0, 0};
+static cufftResult make_plan(cufftHandle *h, int nx, int ny, int nz, cufftType type, int batch, size_t *work) {
     int dims[3] = {nz, ny, nx};
     const long long N = (long long)nx * ny * nz, Nc = (long long)nz * ny * (nx / 2 + 1);
-    if (N > 0x7fffffffLL) return CUFFT_INVALID_SIZE;
-    cufftResult r = cufftPlanMany(&e.fwd, 3, dims, nullptr, 1, (int)N, nullptr, 1, (int)Nc, CUFFT_D2Z, 5);
+    cufftResult r = cufftCreate(h);
     if (r != CUFFT_SUCCESS) return r;
-    r = cufftPlanMany(&e.inv, 3, dims, nullptr, 1, (int)Nc, nullptr, 1, (int)N, CUFFT_Z2D, 4);
-    if (r != CUFFT_SUCCESS) { cufftDestroy(e.fwd); return r; }
+    r = cufftSetAutoAllocation(*h, 0);
+    const int idist = (type == CUFFT_D2Z) ? (int)N : (int)Nc, odist = (type == CUFFT_D2Z) ? (int)Nc : (int)N;
+    if (r == CUFFT_SUCCESS) r = cufftMakePlanMany(*h, 3, dims, nullptr, 1, idist, nullptr, 1, odist, type, batch, work);
+    if (r != CUFFT_SUCCESS) cufftDestroy(*h);
+    return r;
+}
+
+// caller holds g_fft_mu
+static cufftResult get_plans(int nx, int ny, int nz, PlanEntry *out) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    for (const PlanEntry &p : g_plans)
+        if (p.dev == dev && p.nx == nx && p.ny == ny && p.nz == nz) { *out = p; return CUFFT_SUCCESS; }
+    if ((long long)nx * ny * nz > 0x7fffffffLL) return CUFFT_INVALID_SIZE;
+    PlanEntry e = {dev, nx, ny, nz, 0, 0, 0, 0};
+    size_t w1 = 0, w4 = 0, wi = 0;
+    cufftResult r = make_plan(&e.fwd1, nx, ny, nz, CUFFT_D2Z, 1, &w1);
+    if (r != CUFFT_SUCCESS) return r;
+    r = make_plan(&e.fwd4, nx, ny, nz, CUFFT_D2Z, 4, &w4);
+    if (r != CUFFT_SUCCESS) { cufftDestroy(e.fwd1); return r; }
+    r = make_plan(&e.inv4, nx, ny, nz, CUFFT_Z2D, 4, &wi);
+    if (r != CUFFT_SUCCESS) { cufftDestroy(e.fwd1); cufftDestroy(e.fwd4); return r; }
+    e.work_bytes = w1 > w4 ? w1 : w4;
+    if (wi > e.work_bytes) e.work_bytes = wi;
     g_plans.push_back(e);
-    *fwd = e.fwd; *inv = e.inv;
+    *out = e;
     return CUFFT_SUCCESS;
 }
 
+static bool tip_matches(const TipEntry &t, int dev, const FftJob &job) {
+    if (t.dev != dev || t.nx != job.nx || t.ny != job.ny || t.nz != job.nz) return false;
+    if (t.sigma != job.sigma || t.q_s != job.q_s || t.p_z != job.p_z || t.Q_zz != job.Q_zz) return false;
+    return memcmp(t.step, job.step, sizeof(t.step)) == 0;
+}
+
+static void free_tip(TipEntry &t) {
+    cudaFree(t.spec);           // synchronises the device: no stream still reads the spectra
+    cudaEventDestroy(t.ready);
+}
+
 void release_fft_plans() {
-    std::lock_guard<std::mutex> lk(g_plan_mu);
-    for (const PlanEntry &p : g_plans) { cufftDestroy(p.fwd); cufftDestroy(p.inv); }
+    std::lock_guard<std::mutex> lk(g_fft_mu);
+    for (TipEntry &t : g_tips) free_tip(t);
+    g_tips.clear();
+    for (const PlanEntry &p : g_plans) { cufftDestroy(p.fwd1); cufftDestroy(p.fwd4); cufftDestroy(p.inv4); }
     g_plans.clear();
 }
 
@@ -137,34 +193,93 @@ static int forcefield_fft_impl(const float *d_V, const ppfm_grid *grid, const pp
     job.vpow = vpow;
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    cufftHandle fwd, inv;
-    cufftResult fr = get_plans(job.nx, job.ny, job.nz, &fwd, &inv);
-    if (fr != CUFFT_SUCCESS) { set_cuda_error(cudaErrorUnknown, "cufftPlanMany"); return fr == CUFFT_ALLOC_FAILED ? PPFM_ENOMEM : PPFM_ECUDA; }
-    double *d_real = nullptr;
-    double2 *d_cplx = nullptr;
-    cudaError_t e = scratch_alloc((void **)&d_real, (size_t)5 * job.N * sizeof(double), st);
-    if (e != cudaSuccess) { set_cuda_error(e, "scratch_alloc"); return PPFM_ENOMEM; }
-    e = scratch_alloc((void **)&d_cplx, (size_t)5 * job.Nc * sizeof(double2), st);
-    if (e != cudaSuccess) { set_cuda_error(e, "scratch_alloc"); cudaFreeAsync(d_real, st); return PPFM_ENOMEM; }
-    int rc = PPFM_OK;
+    int dev = 0;
+    cudaGetDevice(&dev);
     const unsigned gN = (unsigned)((job.N + 255) / 256), gC = (unsigned)((job.Nc + 255) / 256);
+    std::lock_guard<std::mutex> lk(g_fft_mu);      // held across bind + enqueue (all asynchronous) on the shared handles
+    PlanEntry pl;
+    cufftResult fr = get_plans(job.nx, job.ny, job.nz, &pl);
+    if (fr != CUFFT_SUCCESS) { set_cuda_error(cudaErrorUnknown, "cufftMakePlanMany"); return fr == CUFFT_ALLOC_FAILED ? PPFM_ENOMEM : PPFM_ECUDA; }
+    double *d_real = nullptr;       // 4 N doubles: V in the first N before the forward transform, the four fields after
+    double2 *d_cplx = nullptr;      // V^ (Nc) | X_c (4 Nc)
+    void *d_work = nullptr;
+    cudaError_t e = scratch_alloc((void **)&d_real, (size_t)4 * job.N * sizeof(double), st);
+    if (e == cudaSuccess) e = scratch_alloc((void **)&d_cplx, (size_t)5 * job.Nc * sizeof(double2), st);
+    if (e == cudaSuccess) e = scratch_alloc(&d_work, pl.work_bytes, st);
+    if (e != cudaSuccess) {
+        set_cuda_error(e, "scratch_alloc");
+        if (d_real) cudaFreeAsync(d_real, st);
+        if (d_cplx) cudaFreeAsync(d_cplx, st);
+        return PPFM_ENOMEM;
+    }
+    int rc = PPFM_OK;
+    int own_launches = 0;
+    auto bind = [&](cufftHandle h) {
+        return cufftSetStream(h, st) == CUFFT_SUCCESS && cufftSetWorkArea(h, d_work) == CUFFT_SUCCESS;
+    };
     {
         KernelTimer kt(PPFM_K_FFT_EL, st);
-        fft_fill_kernel<<<gN, 256, 0, st>>>(job, d_V, d_real);
-        if (cufftSetStream(fwd, st) != CUFFT_SUCCESS || cufftExecD2Z(fwd, d_real, (cufftDoubleComplex *)d_cplx) != CUFFT_SUCCESS)
-            rc = PPFM_ECUDA;
+        // ---- tip spectra: cached, or computed now into a new cache entry
+        TipEntry *te = nullptr;
+        for (TipEntry &t : g_tips)
+            if (tip_matches(t, dev, job)) te = &t;
+        if (!te) {
+            if ((int)g_tips.size() >= TIP_CACHE_ENTRIES) {           // evict the least recently used entry
+                size_t old = 0;
+                for (size_t i = 1; i < g_tips.size(); i++)
+                    if (g_tips[i].stamp < g_tips[old].stamp) old = i;
+                free_tip(g_tips[old]);
+                g_tips.erase(g_tips.begin() + old);
+            }
+            TipEntry t;
+            memset(&t, 0, sizeof(t));
+            t.dev = dev; t.nx = job.nx; t.ny = job.ny; t.nz = job.nz;
+            memcpy(t.step, job.step, sizeof(t.step));
+            t.sigma = job.sigma; t.q_s = job.q_s; t.p_z = job.p_z; t.Q_zz = job.Q_zz;
+            e = cudaMalloc((void **)&t.spec, (size_t)4 * job.Nc * sizeof(double2));
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&t.ready, cudaEventDisableTiming);
+            if (e != cudaSuccess) {
+                if (t.spec) cudaFree(t.spec);
+                set_cuda_error(e, "tip spectrum cache");
+                rc = (e == cudaErrorMemoryAllocation) ? PPFM_ENOMEM : PPFM_ECUDA;
+            } else {
+                fft_fill_tip_kernel<<<gN, 256, 0, st>>>(job, d_real);
+                own_launches++;
+                if (!bind(pl.fwd4) || cufftExecD2Z(pl.fwd4, d_real, (cufftDoubleComplex *)t.spec) != CUFFT_SUCCESS) {
+                    rc = PPFM_ECUDA;
+                    cudaStreamSynchronize(st);
+                    cudaFree(t.spec);
+                    cudaEventDestroy(t.ready);
+                } else {
+                    cudaEventRecord(t.ready, st);
+                    g_tips.push_back(t);
+                    te = &g_tips.back();
+                }
+            }
+        } else {
+            cudaStreamWaitEvent(st, te->ready, 0);                  // produced on another stream, perhaps
+        }
         if (rc == PPFM_OK) {
-            fft_spectral_kernel<<<gC, 256, 0, st>>>(job.Nc, job.scale, d_cplx, d_cplx + job.Nc);
-            if (cufftSetStream(inv, st) != CUFFT_SUCCESS ||
-                cufftExecZ2D(inv, (cufftDoubleComplex *)(d_cplx + job.Nc), d_real) != CUFFT_SUCCESS)
+            te->stamp = ++g_tip_clock;
+            fft_fill_v_kernel<<<gN, 256, 0, st>>>(job.N, job.vpow, d_V, d_real);
+            if (!bind(pl.fwd1) || cufftExecD2Z(pl.fwd1, d_real, (cufftDoubleComplex *)d_cplx) != CUFFT_SUCCESS)
                 rc = PPFM_ECUDA;
         }
-        if (rc == PPFM_OK) fft_pack_kernel<<<gN, 256, 0, st>>>(job.N, d_real, reinterpret_cast<float4 *>(d_ff));
+        if (rc == PPFM_OK) {
+            fft_spectral_kernel<<<gC, 256, 0, st>>>(job.Nc, job.scale, d_cplx, te->spec, d_cplx + job.Nc);
+            if (!bind(pl.inv4) || cufftExecZ2D(pl.inv4, (cufftDoubleComplex *)(d_cplx + job.Nc), d_real) != CUFFT_SUCCESS)
+                rc = PPFM_ECUDA;
+        }
+        if (rc == PPFM_OK) {
+            fft_pack_kernel<<<gN, 256, 0, st>>>(job.N, d_real, reinterpret_cast<float4 *>(d_ff));
+            own_launches += 3;
+        }
     }
     e = cudaGetLastError();
-    if (rc != PPFM_OK) set_cuda_error(cudaErrorUnknown, "cuFFT exec");
-    else if (e != cudaSuccess) { set_cuda_error(e, "fft kernels"); rc = PPFM_ECUDA; }
-    else count_launch(3);
+    if (rc == PPFM_ECUDA && e == cudaSuccess) set_cuda_error(cudaErrorUnknown, "cuFFT exec");
+    else if (rc == PPFM_OK && e != cudaSuccess) { set_cuda_error(e, "fft kernels"); rc = PPFM_ECUDA; }
+    if (rc == PPFM_OK) count_launch(own_launches);
+    cudaFreeAsync(d_work, st);
     cudaFreeAsync(d_cplx, st);
     cudaFreeAsync(d_real, st);
     return rc;

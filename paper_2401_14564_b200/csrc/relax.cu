@@ -51,6 +51,13 @@ struct RelaxJob {
     float d0f[3], R_rest, k_lat[2], k_rad;
 };
 
+#define PPFM_CHK_READER relax_checks_read
+PPFM_CHK_STORAGE
+#undef PPFM_CHK_READER
+#ifndef PPFM_CHECKS
+void relax_checks_read(unsigned long long *) {}
+#endif
+
 struct FireParams {
     float dt0, dt_max, finc, fdec, alpha0, falpha, fconv2;
     int n_min, max_iter;
@@ -134,11 +141,74 @@ __device__ __forceinline__ void axis_cell(float t, float tm, const AxisBase &a, 
     i0 = __float_as_int(zc) - a.K;
 }
 
-template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
+// Eigenvalues (ascending) of a symmetric 3 x 3 matrix in FP32, for the stiffness map folded into the relaxation
+// (SURVEY 8(f) N2).  The two soft lateral modes (~k_xy) are nearly degenerate next to the stiff radial one (~k_R), and
+// any route through all three roots of the characteristic cubic loses the close pair to sqrt(eps).  Instead (the
+// deflation scheme of robust 3 x 3 symmetric solvers): with B = (A - q I)/p, q = tr A/3, p^2 = |A - q I|_F^2/6, the
+// roots of mu^3 - 3 mu - det B = 0 lie in [-2, 2]; the root on the side of sign(det B) is the ISOLATED one
+// (|mu| in [sqrt 3, 2], slope >= 6), found by Newton from |mu| = 2 (monotone: the cubic is convex there).  Its
+// eigenvector is the largest cross product of two rows of A - lambda I; the other two eigenvalues are those of A
+// projected on the plane orthogonal to it, mean +- sqrt(diff^2 + off^2): no cancellation between close roots.
+// Error ~ a few ulp of |A| (2e-7 for k_R = 1.9 eV/A^2; tolerance of the map 1e-5).
+__device__ __forceinline__ void sym3_eigenvalues_f32(float a00, float a11, float a22, float a01, float a02, float a12,
+                                                     float &e0, float &e1, float &e2) {
+    const float q = (a00 + a11 + a22) * (1.0f / 3.0f);
+    const float b00 = a00 - q, b11 = a11 - q, b22 = a22 - q;
+    const float p2 = (fmaf(b00, b00, fmaf(b11, b11, b22 * b22)) + 2.0f * fmaf(a01, a01, fmaf(a02, a02, a12 * a12))) *
+                     (1.0f / 6.0f);
+    if (!(p2 > 1.0e-30f)) { e0 = e1 = e2 = q; return; }
+    const float ip = rsqrtf(p2), p = p2 * ip;
+    const float c00 = b00 * ip, c11 = b11 * ip, c22 = b22 * ip, c01 = a01 * ip, c02 = a02 * ip, c12 = a12 * ip;
+    const float det = c00 * fmaf(c11, c22, -c12 * c12) - c01 * fmaf(c01, c22, -c12 * c02) + c02 * fmaf(c01, c12, -c11 * c02);
+    const float sgn = (det >= 0.0f) ? 1.0f : -1.0f;
+    const float ad = fminf(fabsf(det), 2.0f);
+    float mu = 2.0f;
+#pragma unroll
+    for (int it = 0; it < 6; it++) {
+        const float f = fmaf(mu, fmaf(mu, mu, -3.0f), -ad);
+        mu -= f / fmaf(3.0f * mu, mu, -3.0f);
+    }
+    const float liso = sgn * mu;                       // isolated eigenvalue of C = B/p
+    // eigenvector of liso: largest cross product of two rows of C - liso I
+    const float m00 = c00 - liso, m11 = c11 - liso, m22 = c22 - liso;
+    const float x0 = fmaf(c01, c12, -c02 * m11), y0 = fmaf(c02, c01, -m00 * c12), z0 = fmaf(m00, m11, -c01 * c01);   // r0 x r1
+    const float x1 = fmaf(c01, m22, -c02 * c12), y1 = fmaf(c02, c02, -m00 * m22), z1 = fmaf(m00, c12, -c01 * c02);   // r0 x r2
+    const float x2 = fmaf(m11, m22, -c12 * c12), y2 = fmaf(c12, c02, -c01 * m22), z2 = fmaf(c01, c12, -m11 * c02);   // r1 x r2
+    const float n0 = fmaf(x0, x0, fmaf(y0, y0, z0 * z0)), n1 = fmaf(x1, x1, fmaf(y1, y1, z1 * z1));
+    const float n2 = fmaf(x2, x2, fmaf(y2, y2, z2 * z2));
+    float vx = x0, vy = y0, vz = z0, nn = n0;
+    if (n1 > nn) { vx = x1; vy = y1; vz = z1; nn = n1; }
+    if (n2 > nn) { vx = x2; vy = y2; vz = z2; nn = n2; }
+    const float inn = rsqrtf(nn);
+    vx *= inn; vy *= inn; vz *= inn;
+    // orthonormal a, b spanning the plane orthogonal to v: a = e_k x v for the smallest |v_k|
+    const float ax_ = fabsf(vx), ay_ = fabsf(vy), az_ = fabsf(vz);
+    float ux, uy, uz;
+    if (ax_ <= ay_ && ax_ <= az_) { ux = 0.0f; uy = -vz; uz = vy; }
+    else if (ay_ <= az_) { ux = vz; uy = 0.0f; uz = -vx; }
+    else { ux = -vy; uy = vx; uz = 0.0f; }
+    const float iu = rsqrtf(fmaf(ux, ux, fmaf(uy, uy, uz * uz)));
+    ux *= iu; uy *= iu; uz *= iu;
+    const float wx = fmaf(vy, uz, -vz * uy), wy = fmaf(vz, ux, -vx * uz), wz = fmaf(vx, uy, -vy * ux);
+    // C u, C w and the projected 2 x 2 matrix
+    const float cux = fmaf(c00, ux, fmaf(c01, uy, c02 * uz)), cuy = fmaf(c01, ux, fmaf(c11, uy, c12 * uz));
+    const float cuz = fmaf(c02, ux, fmaf(c12, uy, c22 * uz));
+    const float cwx = fmaf(c00, wx, fmaf(c01, wy, c02 * wz)), cwy = fmaf(c01, wx, fmaf(c11, wy, c12 * wz));
+    const float cwz = fmaf(c02, wx, fmaf(c12, wy, c22 * wz));
+    const float muu = fmaf(ux, cux, fmaf(uy, cuy, uz * cuz)), mww = fmaf(wx, cwx, fmaf(wy, cwy, wz * cwz));
+    const float muw = fmaf(ux, cwx, fmaf(uy, cwy, uz * cwz));
+    const float mean = 0.5f * (muu + mww), hd = 0.5f * (muu - mww);
+    const float sq = sqrtf(fmaf(hd, hd, muw * muw));
+    const float la = fmaf(p, mean - sq, q), lb = fmaf(p, mean + sq, q), li = fmaf(p, liso, q);
+    if (sgn > 0.0f) { e0 = la; e1 = lb; e2 = li; }
+    else { e0 = li; e1 = la; e2 = lb; }
+}
+
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF = false>
 __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FireParams &fp, int lb,
                                              const void *__restrict__ ff, float4 *__restrict__ pos_fz,
                                              uint16_t *__restrict__ iters_out, ppfm_stats *__restrict__ stats,
-                                             float *__restrict__ fz_out) {
+                                             float *__restrict__ fz_out, float4 *__restrict__ eig_out) {
     const int by = lb / job.nbx, bx = lb - by * job.nbx;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ix = bx * RX_TILE_X + (warp & 1) * 8 + (lane & 7);
@@ -315,6 +385,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 const bool inside = (i0 >= 1) & (i0 + 2 <= nx - 1) & (j0 >= 1) & (j0 + 2 <= ny - 1) & (k0 >= 1) &
                                     (k0 + 2 <= nz - 1);
                 if (__all_sync(0xffffffffu, inside)) {
+                    PPFM_CHK(PPFM_CHK_RELAX_GATHER, i0 >= 1 && i0 + 2 <= nx - 1 && j0 >= 1 && j0 + 2 <= ny - 1 && k0 >= 1 && k0 + 2 <= nz - 1);
                     const int base = (int)((k0 - 1) * ny + (j0 - 1)) * nx + (i0 - 1);
 #pragma unroll
                     for (int kk = 0; kk < (TRICUBIC ? 4 : 1); kk++)
@@ -336,6 +407,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                         if (perx) { a -= (a >= nx) ? nx : 0; a += (a < 0) ? nx : 0; } else a = min(max(a, 0), nx - 1);
                         if (pery) { b -= (b >= ny) ? ny : 0; b += (b < 0) ? ny : 0; } else b = min(max(b, 0), ny - 1);
                         if (perz) { c -= (c >= nz) ? nz : 0; c += (c < 0) ? nz : 0; } else c = min(max(c, 0), nz - 1);
+                        PPFM_CHK(PPFM_CHK_RELAX_GATHER, a >= 0 && a < nx && b >= 0 && b < ny && c >= 0 && c < nz);
                         xi[m] = a; yo[m] = b * nx; zo[m] = c * ny * nx;
                     }
 #pragma unroll
@@ -355,6 +427,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 #pragma unroll
                         for (int m = 0; m < (TRICUBIC ? 4 : 1); m++) en[kk][jj][m] -= ref;
             } else if (!ANYPER) {
+                PPFM_CHK(PPFM_CHK_RELAX_GATHER, i0 >= 0 && i0 <= nx - 2 && j0 >= 0 && j0 <= ny - 2 && k0 >= 0 && k0 <= nz - 2);
                 const float4 *p = g + ((long long)(k0 * ny + j0) * nx + i0);
                 c000 = ldg_corner(p);           c001 = ldg_corner(p + 1);
                 c010 = ldg_corner(p + sy);      c011 = ldg_corner(p + sy + 1);
@@ -367,6 +440,8 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 const int i1 = (i0 + 1 == nx) ? 0 : i0 + 1;       // non-periodic axes never reach n - 1
                 const int j1 = (j0 + 1 == ny) ? 0 : j0 + 1;
                 const int k1 = (k0 + 1 == nz) ? 0 : k0 + 1;
+                PPFM_CHK(PPFM_CHK_RELAX_GATHER, i0 >= 0 && i0 < nx && j0 >= 0 && j0 < ny && k0 >= 0 && k0 < nz &&
+                                                    i1 < nx && j1 < ny && k1 < nz);
                 const float4 *r00 = g + (long long)(k0 * ny + j0) * nx, *r01 = g + (long long)(k0 * ny + j1) * nx;
                 const float4 *r10 = g + (long long)(k1 * ny + j0) * nx, *r11 = g + (long long)(k1 * ny + j1) * nx;
                 c000 = ldg_corner(r00 + i0); c001 = ldg_corner(r00 + i1);
@@ -452,9 +527,50 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         outv.y = (float)(rb[1] + job.origin[1] + (double)uy);
         outv.z = (float)(rz + job.origin[2] + (double)uz);
         outv.w = -fr * dzc;                           // Fz_tip = -F_R,z
+        PPFM_CHK(PPFM_CHK_RELAX_STORE, o < (size_t)job.out_offset + (size_t)job.nzs * job.npy * job.npx);
         pos_fz[o] = outv;
         if (fz_out) fz_out[o] = outv.w;
         if (iters_out) iters_out[o] = conv ? (uint16_t)min(moves, 0xFFFE) : (uint16_t)0xFFFF;
+        if (STIFF && !TRICUBIC) {
+            // Stiffness map from the cell this lane still holds: the last FIRE
+            // iteration of a finished lane does not move it, so (c0, cd, fx, fy, fz, fr, dzc) belong to the relaxed
+            // point.  G[c][a] = dF_c/dt_a of the tri-linear interpolant, J = G Minv, H = H_spring - (J + J^T)/2.
+            const float gy = 1.0f - fy, gz = 1.0f - fz;
+            float G[3][3];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const float e00 = fmaf(fx, cd[0][c], c0[0][c]), e10 = fmaf(fx, cd[1][c], c0[1][c]);
+                const float e01 = fmaf(fx, cd[2][c], c0[2][c]), e11 = fmaf(fx, cd[3][c], c0[3][c]);
+                G[c][0] = gz * fmaf(fy, cd[1][c], gy * cd[0][c]) + fz * fmaf(fy, cd[3][c], gy * cd[2][c]);
+                G[c][1] = fmaf(fz, e11 - e01, gz * (e10 - e00));
+                G[c][2] = fmaf(fy, e11 - e10, gy * (e01 - e00));
+            }
+            float J[3][3];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                if (ORTHO) {
+                    J[c][0] = G[c][0] * m00; J[c][1] = G[c][1] * m11; J[c][2] = G[c][2] * m22;
+                } else {
+                    J[c][0] = fmaf(G[c][2], m20, fmaf(G[c][1], m10, G[c][0] * m00));
+                    J[c][1] = fmaf(G[c][2], m21, fmaf(G[c][1], m11, G[c][0] * m01));
+                    J[c][2] = fmaf(G[c][2], m22, fmaf(G[c][1], m12, G[c][0] * m02));
+                }
+            }
+            // H_spring = k_R dd^T/|d|^2 + k_t (I - dd^T/|d|^2) + diag(k_x, k_y, 0), k_t = k_R (|d| - R0)/|d| = -fr
+            const float ddx = SYMTIP ? ux : d0x + ux, ddy = SYMTIP ? uy : d0y + uy, ddz = dzc;
+            const float L2 = fmaf(ddx, ddx, fmaf(ddy, ddy, ddz * ddz));
+            const float kt = -fr;
+            const float kd = (L2 > 0.0f) ? (job.k_rad - kt) / L2 : 0.0f;
+            const float h00 = fmaf(kd * ddx, ddx, kt) - J[0][0] + job.k_lat[0];
+            const float h11 = fmaf(kd * ddy, ddy, kt) - J[1][1] + job.k_lat[1];
+            const float h22 = fmaf(kd * ddz, ddz, kt) - J[2][2];
+            const float h01 = fmaf(kd * ddx, ddy, -0.5f * (J[0][1] + J[1][0]));
+            const float h02 = fmaf(kd * ddx, ddz, -0.5f * (J[0][2] + J[2][0]));
+            const float h12 = fmaf(kd * ddy, ddz, -0.5f * (J[1][2] + J[2][1]));
+            float l0, l1, l2;
+            sym3_eigenvalues_f32(h00, h11, h22, h01, h02, h12, l0, l1, l2);
+            eig_out[o] = make_float4(l0, l1, l2, 0.0f);
+        }
         float tx, ty, tz;
         if (ORTHO) {
             tx = fmaf(m00, ux, ax.tb); ty = fmaf(m11, uy, ay.tb); tz = fmaf(m22, uz, az.tb);
@@ -512,20 +628,21 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 }
 
 // One system: the job travels as a kernel parameter (constant bank), no scratch and no copy.
-template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireParams fp,
              const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
-             ppfm_stats *__restrict__ stats, float *__restrict__ fz_out) {
-    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats, fz_out);
+             ppfm_stats *__restrict__ stats, float *__restrict__ fz_out, float4 *__restrict__ eig_out) {
+    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC, STIFF>(job, fp, blockIdx.x, ff, pos_fz, iters_out, stats, fz_out,
+                                                         eig_out);
 }
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
-template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF>
 __global__ void __launch_bounds__(RX_THREADS)
 relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_constant__ FireParams fp,
                    const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
-                   ppfm_stats *__restrict__ stats, float *__restrict__ fz_out) {
+                   ppfm_stats *__restrict__ stats, float *__restrict__ fz_out, float4 *__restrict__ eig_out) {
     __shared__ RelaxJob s_job;
     const int blk = blockIdx.x;
     int lo = 0, hi = njobs - 1;
@@ -539,17 +656,20 @@ relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_co
         for (int w = threadIdx.x; w < (int)(sizeof(RelaxJob) / sizeof(int)); w += RX_THREADS) dstw[w] = srcw[w];
     }
     __syncthreads();
-    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out, stats, fz_out);
+    relax_pixels<ORTHO, ANYPER, SYMTIP, TRICUBIC, STIFF>(s_job, fp, blk - s_job.block_begin, ff, pos_fz, iters_out,
+                                                         stats, fz_out, eig_out);
 }
 
-template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC>
+template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF>
 static void launch_relax(int nsys, long long blocks, cudaStream_t st, const RelaxJob *hj, const RelaxJob *dj,
                          const FireParams &fp, const void *ff, float4 *pos, uint16_t *it, ppfm_stats *stats,
-                         float *fz) {
+                         float *fz, float4 *eig) {
     if (nsys == 1)
-        relax_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(hj[0], fp, ff, pos, it, stats, fz);
+        relax_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC, STIFF><<<(unsigned)blocks, RX_THREADS, 0, st>>>(
+            hj[0], fp, ff, pos, it, stats, fz, eig);
     else
-        relax_batch_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC><<<(unsigned)blocks, RX_THREADS, 0, st>>>(dj, nsys, fp, ff, pos, it, stats, fz);
+        relax_batch_kernel<ORTHO, ANYPER, SYMTIP, TRICUBIC, STIFF><<<(unsigned)blocks, RX_THREADS, 0, st>>>(
+            dj, nsys, fp, ff, pos, it, stats, fz, eig);
 }
 
 // Host side shared by the relaxation and the stiffness map: validate and pack one RelaxJob per system.
@@ -608,8 +728,10 @@ static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *ti
 
 static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                       const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
-                      ppfm_stats *d_stats, void *cuda_stream, bool tricubic = false, float *d_fz = nullptr) {
+                      ppfm_stats *d_stats, void *cuda_stream, bool tricubic = false, float *d_fz = nullptr,
+                      float *d_eig = nullptr) {
     if (nsys < 1 || !d_ff || !grids || !tips || !fire || !scans || !d_pos_fz) return PPFM_EINVAL;
+    if (d_eig && (tricubic || ((uintptr_t)d_eig & 15))) return PPFM_EINVAL;
     if (((uintptr_t)d_ff & (tricubic ? 3 : 15)) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
         return PPFM_EINVAL;
     if (!(fire->dt > 0) || !(fire->dt_max > 0) || !(fire->finc >= 1.0) || !(fire->fdec > 0 && fire->fdec < 1.0) ||
@@ -641,10 +763,12 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
     float4 *pos4 = reinterpret_cast<float4 *>(d_pos_fz);
     {
         KernelTimer kt(tricubic ? PPFM_K_RELAX_TRICUBIC : PPFM_K_RELAX, st);
+    float4 *eig4 = reinterpret_cast<float4 *>(d_eig);
 #define PPFM_RX(O, A, S) \
     do { \
-        if (tricubic) launch_relax<O, A, S, true>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz); \
-        else launch_relax<O, A, S, false>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz); \
+        if (tricubic) launch_relax<O, A, S, true, false>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz, nullptr); \
+        else if (eig4) launch_relax<O, A, S, false, true>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz, eig4); \
+        else launch_relax<O, A, S, false, false>(nsys, blocks, st, hj, dj, fp, d_ff, pos4, d_iters, d_stats, d_fz, nullptr); \
     } while (0)
         if (symtip) {
             if (ortho && !anyper) PPFM_RX(true, false, true);
@@ -854,6 +978,24 @@ extern "C" int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm
                                      const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz,
                                      uint16_t *d_iters, ppfm_stats *d_stats, void *cuda_stream) {
     return relax_impl(nsys, d_ff, grids, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream);
+}
+
+// relaxation with the stiffness map folded into the end of every z-step: the eigenvalues come
+// from the cell the lane already holds in registers, so the map costs no second gather and no second launch
+extern "C" int ppfm_relax_scan_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip,
+                                         const ppfm_fire *fire, const ppfm_scan *scan, float *d_pos_fz,
+                                         uint16_t *d_iters, float *d_eig, ppfm_stats *d_stats, void *cuda_stream) {
+    if (!d_eig) return PPFM_EINVAL;
+    return relax_impl(1, d_ff, grid, tip, fire, scan, d_pos_fz, d_iters, d_stats, cuda_stream, false, nullptr, d_eig);
+}
+
+extern "C" int ppfm_relax_scan_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids,
+                                               const ppfm_tip *tips, const ppfm_fire *fire, const ppfm_scan *scans,
+                                               float *d_pos_fz, uint16_t *d_iters, float *d_eig, ppfm_stats *d_stats,
+                                               void *cuda_stream) {
+    if (!d_eig) return PPFM_EINVAL;
+    return relax_impl(nsys, d_ff, grids, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream, false, nullptr,
+                      d_eig);
 }
 
 extern "C" int ppfm_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_scan *scan,

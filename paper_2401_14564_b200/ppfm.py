@@ -13,7 +13,8 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libppfm.so")
+# PPFM_LIBRARY selects another build of the same ABI (the checked build libppfm_chk.so, see include/ppfm_bench.h)
+LIB_PATH = os.environ.get("PPFM_LIBRARY") or os.path.join(_HERE, "libppfm.so")
 _lib = None
 
 
@@ -63,7 +64,8 @@ class Stats(C.Structure):
 # the product ABI (include/ppfm.h); the measurement interface of include/ppfm_bench.h is bound in ppfm_bench.py
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft",
-           "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_tricubic",
+           "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_stiffness",
+           "ppfm_relax_scan_stiffness_batch", "ppfm_relax_scan_tricubic",
            "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid", "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df",
            "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch", "ppfm_scan_host_sweep",
            "ppfm_release_scratch"]
@@ -339,6 +341,42 @@ def relax_scan_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, stat
                                      _dptr(pos_fz, torch.float32), _dptr(iters), _dptr(stats), _stream())
     _check(rc, "ppfm_relax_scan_batch")
     return pos_fz, iters
+
+
+def relax_scan_stiffness(ff, grid, tip, fire, scan, pos_fz=None, iters=None, eig=None, stats=None, want_iters=True):
+    """ppfm_relax_scan_stiffness -> (pos_fz, iters, eig (nz, npy, npx, 4) float32): the scan with the stiffness map
+    (Hessian eigenvalues, ascending; 4th lane 0) of every relaxed point written at the end of its z-step."""
+    torch = _torch()
+    shape = (int(scan.nz), int(scan.npy), int(scan.npx))
+    if pos_fz is None:
+        pos_fz = torch.empty(shape + (4,), dtype=torch.float32, device=ff.device)
+    if iters is None and want_iters:
+        iters = torch.empty(shape, dtype=torch.int16, device=ff.device)
+    if eig is None:
+        eig = torch.empty(shape + (4,), dtype=torch.float32, device=ff.device)
+    rc = lib().ppfm_relax_scan_stiffness(_dptr(ff, torch.float32), C.byref(c_grid(grid)), C.byref(c_tip(tip)),
+                                         C.byref(c_fire(fire)), C.byref(c_scan(scan)), _dptr(pos_fz, torch.float32),
+                                         _dptr(iters), _dptr(eig, torch.float32), _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan_stiffness")
+    return pos_fz, iters, eig
+
+
+def relax_scan_stiffness_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, eig=None, stats=None,
+                               want_iters=True):
+    torch = _torch()
+    gr, tp, sc = c_array(grids, c_grid), c_array(tips, c_tip), c_array(scans, c_scan)
+    nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in sc)
+    if pos_fz is None:
+        pos_fz = torch.empty((nps, 4), dtype=torch.float32, device=ff.device)
+    if iters is None and want_iters:
+        iters = torch.empty((nps,), dtype=torch.int16, device=ff.device)
+    if eig is None:
+        eig = torch.empty((nps, 4), dtype=torch.float32, device=ff.device)
+    rc = lib().ppfm_relax_scan_stiffness_batch(C.c_int32(len(grids)), _dptr(ff, torch.float32), gr, tp,
+                                               C.byref(c_fire(fire)), sc, _dptr(pos_fz, torch.float32), _dptr(iters),
+                                               _dptr(eig, torch.float32), _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan_stiffness_batch")
+    return pos_fz, iters, eig
 
 
 # ---- (2a) relaxation on an energy-only grid, tri-cubic interpolation of the potential (PAPER.md:264) ---------------

@@ -9,7 +9,8 @@ import os
 from . import ppfm
 
 PROBES_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libppfm_probes.so")
-EXPORTS_LIBPPFM = ["ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read"]
+EXPORTS_LIBPPFM = ["ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read", "ppfm_checks_read"]
+CHECK_KINDS = ["ring_acquire", "ring_release", "ff_store", "relax_gather", "relax_store", "df_load", "df_store", "visits"]
 EXPORTS_PROBES = ["ppfm_probe_fma", "ppfm_probe_gather"]
 KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6, "relax_tricubic": 7}
 _probes = None
@@ -43,6 +44,15 @@ def timing_read() -> dict:
         ppfm._check(ppfm.lib().ppfm_timing_read(C.c_int(kid), C.byref(ms), C.byref(n)), "ppfm_timing_read")
         out[name] = (ms.value, int(n.value))
     return out
+
+
+def checks_read():
+    """ppfm_checks_read: {kind: count} since the last call, or None when the loaded library is not the checked build."""
+    c = (C.c_uint64 * 8)()
+    rc = ppfm.lib().ppfm_checks_read(c)
+    if rc:
+        return None
+    return {k: int(v) for k, v in zip(CHECK_KINDS, c)}
 
 
 def probe_fma() -> float:

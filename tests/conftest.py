@@ -30,11 +30,24 @@ def pytest_terminal_summary(terminalreporter, exitstatus, config):
         tr.write_line(f"{r['what'][:58]:58s} {r['samples']:9d} {r['fail']:6d} {r['fail_endpoint_flag']:15d} "
                       f"{r['fail_traj_only']:21d} {r['max_ok_dist']:16.2e}")
     out = os.path.join(ROOT, "gpurun_out")
-    if os.path.isdir(out):
+    if os.path.isdir(out) and not os.environ.get("PPFM_CHECKS_OUT"):      # not from the checked build's child session
         import json
         with open(os.path.join(out, "parity_exemptions.jsonl"), "w") as fh:
             for r in PARITY_LOG:
                 fh.write(json.dumps(r) + "\n")
+
+
+def pytest_sessionfinish(session, exitstatus):
+    """Under the checked build (PPFM_LIBRARY=.../libppfm_chk.so, tests/test_checked_build.py) write the kernels' own
+    bounds / ring check counts of this session to the file named by PPFM_CHECKS_OUT."""
+    path = os.environ.get("PPFM_CHECKS_OUT")
+    if not path:
+        return
+    import json
+
+    from paper_2401_14564_b200 import ppfm_bench
+    with open(path, "w") as fh:
+        json.dump({"exitstatus": int(exitstatus), "counts": ppfm_bench.checks_read()}, fh)
 
 
 def pytest_collection_modifyitems(config, items):

@@ -121,6 +121,11 @@ def test_invalid_arguments_are_rejected_on_the_host(lib):
     assert lib.ppfm_relax_scan_tricubic(C.c_void_p(0x1002), C.byref(gr), C.byref(tip), C.byref(fire), C.byref(sc), fake,
                                         null, null, null) == EINVAL        # misaligned float grid
     assert lib.ppfm_energy_grid(fake, C.c_int64(-1), fake, null) == EINVAL
+    rxs = lib.ppfm_relax_scan_stiffness
+    assert rxs(fake, C.byref(gr), C.byref(tip), C.byref(fire), C.byref(sc), fake, null, null, null, null) == EINVAL   # no d_eig
+    assert rxs(fake, C.byref(gr), C.byref(tip), C.byref(fire), C.byref(sc), fake, null, C.c_void_p(0x1004), null,
+               null) == EINVAL                                             # misaligned d_eig
+    assert rxs(fake, C.byref(gr), C.byref(badt), C.byref(fire), C.byref(sc), fake, null, fake, null, null) == EINVAL
     sweep = lib.ppfm_scan_host_sweep
     assert sweep(C.c_int32(0), pd(np.zeros(1)), C.c_int32(10), fake, fake, C.c_int32(5), pd(R), pd(e), C.byref(lat),
                  C.byref(pr), C.byref(gr), C.c_double(0.1), C.byref(tip), C.byref(fire), C.byref(sc), C.c_double(1.0),

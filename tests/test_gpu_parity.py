@@ -718,6 +718,56 @@ def test_fft_pauli_overlap_eq8(P):
         P.forcefield_pauli(torch.from_numpy(rho).cuda(), g, sig, -1.0, A, beta)    # q_tip must be > 0
 
 
+def test_fft_tip_spectrum_cache_streams_and_threads(P):
+    """The cached tip spectra and the shared cuFFT plans (fftel.cu): (a) a second call with the same (grid, tip) -- the
+    cached path -- and a call after ppfm_release_scratch() return the first call's bits; (b) interleaved tips beyond the
+    cache size still do; (c) calls on two streams and from two host threads at once, same grid size, different
+    potentials and tips, each return the bits of the same call made alone (every call brings its own work area)."""
+    import threading
+
+    import torch
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.25, 0.25, 0.25]), n=(48, 40, 36), periodic=(1, 1, 1))
+    rng = np.random.default_rng(5 + SEED0)
+    Vs = [torch.from_numpy(rng.normal(size=(36, 40, 48)).astype(np.float32)).cuda() for _ in range(4)]
+    tips = [(0.7, -0.03, 0.0, -0.1), (0.6, 0.05, 0.01, 0.0), (0.8, 0.0, -0.02, -0.05), (0.7, 0.02, 0.0, 0.0)]
+    alone = []
+    for V, t in zip(Vs, tips):
+        P.release_scratch()
+        alone.append(P.forcefield_fft(V, g, *t).clone())
+    torch.cuda.synchronize()
+    # (a) cached path, then a cold cache again
+    P.release_scratch()
+    first = P.forcefield_fft(Vs[0], g, *tips[0]).clone()
+    again = P.forcefield_fft(Vs[0], g, *tips[0]).clone()
+    other_V = P.forcefield_fft(Vs[1], g, *tips[0]).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(first, alone[0]) and torch.equal(again, alone[0])
+    assert not torch.equal(other_V, alone[0])
+    # (b) four tips through a two-entry cache, twice round
+    for rep in range(2):
+        for V, t, ref in zip(Vs, tips, alone):
+            assert torch.equal(P.forcefield_fft(V, g, *t), ref)
+    # (c) two streams + two host threads, repeated so that the enqueues really interleave
+    out = [None] * 4
+    streams = [torch.cuda.Stream() for _ in range(4)]
+
+    def work(i):
+        with torch.cuda.stream(streams[i]):
+            for _ in range(6):
+                out[i] = P.forcefield_fft(Vs[i], g, *tips[i])
+        streams[i].synchronize()
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(4)]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join()
+    torch.cuda.synchronize()
+    for i in range(4):
+        assert torch.equal(out[i], alone[i]), f"stream/thread {i}"
+    P.release_scratch()
+
+
 def test_fft_electrostatics_rejects_bad_arguments(P):
     import torch
     g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(8, 8, 8), periodic=(1, 1, 1))
@@ -731,12 +781,14 @@ def test_fft_electrostatics_rejects_bad_arguments(P):
 
 
 # ------------------------------------------------------------------------------------------------ stiffness map
-def oracle_inputs(w):
+def oracle_inputs(w, with_iters=False):
     """Inputs for the 8(f) kernels made by the ORACLE (none of them comes from the CUDA path): its force-field grid
     rounded to FP32 and the relaxed scan on that grid, positions rounded to FP32."""
     ff_o = oracle.forcefield(w).astype(np.float32)
     ref = oracle.relax_scan(ff_o, w.grid, w.tip, w.fire, w.scan, traj=False)
     pos_o = np.ascontiguousarray(ref["pos_fz"].astype(np.float32))          # (nz, npix, 4)
+    if with_iters:
+        return ff_o, pos_o, ref["iters"]
     return ff_o, pos_o
 
 
@@ -814,6 +866,126 @@ def test_stiffness_zero_field_periodic_nonorthogonal_and_batch(P):
         one = P.stiffness(ffb[m * npts:(m + 1) * npts], mols[m].grid, mols[m].tip, mols[m].scan,
                           posb[m * nps:(m + 1) * nps])
         assert torch.equal(one.reshape(-1, 4), eigb[m * nps:(m + 1) * nps])
+
+
+def check_stiffness_fused(eig_gpu, pos_gpu, ff_h, w, pos_o, ref_iters, what=""):
+    """Eigenvalues written by the relaxation kernel itself (ppfm_relax_scan_stiffness) against the oracle chain: the
+    oracle's stiffness at the ORACLE's relaxed positions pos_o on the same oracle-made grid.  The kernel evaluates H at
+    its own relaxed point, which differs from pos_o by the FP32 relaxer's |dr| (~1e-6 Å) and is not tied to the FP32
+    rounding of any stored position, so the tolerance is the map's own 1e-5 eV/Å^2 + 1e-5 |lambda| plus the oracle's
+    measured sensitivity of lambda to the position: S_k = |lambda(r + h e_k) - lambda(r)| / h with h = 1e-5 Å,
+    times (|dr_k| + one FP32 ulp of the coordinate).  Compared where both relaxers reached the same point (2e-4 Å)
+    away from cell faces."""
+    rt = oracle.tip_positions(w.scan)
+    rp = pos_o[..., :3].astype(np.float64)
+    ref = oracle.stiffness(ff_h, w.grid, w.tip, rt, rp)
+    h = 1e-5
+    sens = np.zeros(ref.shape[:-1] + (3, 3))
+    for k in range(3):
+        e = np.zeros(3); e[k] = h
+        sens[..., k, :] = np.abs(oracle.stiffness(ff_h, w.grid, w.tip, rt, rp + e) - ref) / h
+    got = np.asarray(eig_gpu, np.float64).reshape(ref.shape[:-1] + (4,))
+    pg = np.asarray(pos_gpu, np.float64).reshape(ref.shape[:-1] + (4,))[..., :3]
+    dr = np.abs(pg - rp)
+    Minv = np.linalg.inv(np.asarray(w.grid.step, float).T)
+    t = (rp - np.asarray(w.grid.origin, float)) @ Minv.T
+    tg = (pg - np.asarray(w.grid.origin, float)) @ Minv.T
+    # the Jacobian of a tri-linear interpolant jumps at cell faces: both relaxed points and the finite-difference
+    # stencil must lie in one cell
+    near_face = (np.abs(t - np.round(t)) <= 1e-3).any(axis=-1) | (np.floor(t) != np.floor(tg)).any(axis=-1)
+    use = (np.linalg.norm(dr, axis=-1) <= 2e-4) & ~near_face & (ref_iters >= 0)
+    assert use.mean() > 0.9, f"{what}: only {use.mean():.4f} of samples comparable"
+    ulp = np.spacing(np.abs(rp).astype(np.float32)).astype(np.float64)
+    tol = 1e-5 + 1e-5 * np.abs(ref) + np.einsum("...k,...kl->...l", dr + ulp, sens)
+    err = np.abs(got[..., :3] - ref)
+    assert np.all(got[..., 3] == 0.0)
+    over = np.where(use[..., None], err - tol, -1.0)
+    worst = np.unravel_index(over.argmax(), over.shape)
+    assert over.max() <= 0, (f"{what}: fused stiffness error {over.max():.3e} over tolerance at {worst}: got {got[worst[:-1]]}, "
+                             f"ref {ref[worst[:-1]]}, dr {dr[worst[:-1]]}, t {t[worst[:-1]]}, sens {sens[worst[:-1]]}")
+    assert np.all(np.diff(got[..., :3], axis=-1) >= 0)
+    return float(err[use].max()), float(np.median(tol[use]))
+
+
+def test_relax_scan_stiffness_fused(P):
+    """SURVEY 8(f) N2 folded into the relaxation (ppfm_relax_scan_stiffness): (a) positions, Fz and move counts are bit
+    for bit those of ppfm_relax_scan; (b) the eigenvalues against the oracle chain (oracle grid -> oracle relaxation
+    -> oracle stiffness); (c) they agree with the stand-alone ppfm_stiffness kernel (FP64 eigen-solver) at the written
+    positions within the position-rounding allowance.  Cases: configs 0 and 1 (symmetric tip, orthogonal clamped
+    grid), an asymmetric tip, and a periodic skewed grid (all four Jacobian / spring code paths)."""
+    import torch
+    cases = []
+    for cfg in (0, 1):
+        cases.append((f"cfg{cfg}", W.get(cfg)))
+    w0 = W.get(0)
+    cases.append(("cfg0 asymmetric tip", replace(w0, tip=replace(w0.tip, d0=np.array([0.3, -0.2, -3.98]),
+                                                               k_lat=np.array([0.012, 0.019])))))
+    wp = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
+    step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
+    cases.append(("periodic skewed", replace(wp, grid=replace(wp.grid, step=step),
+                                             scan=replace(wp.scan, p0=np.array([-3.0, 20.0, 9.0])))))
+    for what, w in cases:
+        ff_o, pos_o, it_o = oracle_inputs(w, with_iters=True)
+        ffd = torch.from_numpy(ff_o).cuda()
+        pos, iters, eig = P.relax_scan_stiffness(ffd, w.grid, w.tip, w.fire, w.scan)
+        pos2, iters2 = P.relax_scan(ffd, w.grid, w.tip, w.fire, w.scan)
+        torch.cuda.synchronize()
+        assert torch.equal(pos, pos2) and torch.equal(iters, iters2), what
+        npix = w.scan.npx * w.scan.npy
+        err, tol = check_stiffness_fused(eig.cpu().numpy(), pos.cpu().numpy(), ff_o, w, pos_o.reshape(w.scan.nz, npix, 4),
+                                         it_o.reshape(w.scan.nz, npix), what)
+        print(f"fused stiffness {what}: max err {err:.2e} (median tolerance {tol:.2e})")
+        alone = P.stiffness(ffd, w.grid, w.tip, w.scan, pos).cpu().numpy().astype(np.float64)
+        d = np.abs(eig.cpu().numpy().astype(np.float64) - alone)[..., :3]
+        assert np.median(d) <= 2e-6 and np.quantile(d, 0.999) <= 2e-4, f"{what}: fused vs stand-alone {np.median(d):.2e} / {d.max():.2e}"
+
+
+def test_relax_scan_stiffness_closed_forms(P):
+    """The folded map on fields with closed forms (the oracle's own pins): zero field -> (k_x, k_y, k_R) for an
+    anisotropic tip; linear field F = -K (r - r0), which tri-linear interpolation reproduces exactly -> the
+    eigenvalues of H_spring(d) + K at the relaxed point; batch form = single calls bit for bit."""
+    import torch
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(20, 20, 60), periodic=(0, 0, 0))
+    sc = W.Scan(p0=np.array([1.0, 1.2, 9.0]), dx=np.array([0.1, 0, 0.0]), dy=np.array([0, 0.1, 0.0]), npx=19, npy=11,
+                nz=7, dz=0.1)
+    tip = replace(W._default_tip(), k_lat=np.array([0.011, 0.023]))
+    ff = torch.zeros((60, 20, 20, 4), dtype=torch.float32, device="cuda")
+    pos, it, eig = P.relax_scan_stiffness(ff, g, tip, W.Fire(), sc)
+    assert np.allclose(eig.cpu().numpy()[..., :3], [0.011, 0.023, tip.k_rad], rtol=2e-6, atol=1e-7)
+    # linear field
+    K = np.array([[0.020, 0.004, -0.003], [0.004, 0.012, 0.002], [-0.003, 0.002, 0.030]])
+    r0 = np.array([2.0, 2.1, 4.6])
+    zz, yy, xx = np.meshgrid(np.arange(60) * 0.2, np.arange(20) * 0.2, np.arange(20) * 0.2, indexing="ij")
+    r = np.stack([xx, yy, zz], axis=-1)
+    F = -(r - r0) @ K.T
+    ffl = np.concatenate([F, np.zeros(F.shape[:-1] + (1,))], axis=-1).astype(np.float32)
+    tip2 = W._default_tip()
+    pos, it, eig = P.relax_scan_stiffness(torch.from_numpy(ffl).cuda(), g, tip2, W.Fire(), sc)
+    torch.cuda.synchronize()
+    ph = pos.cpu().numpy().astype(np.float64)
+    rt = oracle.tip_positions(sc).reshape(ph.shape[:-1] + (3,))
+    d = ph[..., :3] - rt
+    L = np.linalg.norm(d, axis=-1)
+    R0 = np.linalg.norm(tip2.d0)
+    dd = d[..., :, None] * d[..., None, :] / (L ** 2)[..., None, None]
+    kt = tip2.k_rad * (L - R0) / L
+    H = tip2.k_rad * dd + kt[..., None, None] * (np.eye(3) - dd) + np.diag([tip2.k_lat[0], tip2.k_lat[1], 0.0]) + K
+    want = np.linalg.eigvalsh(H)
+    got = eig.cpu().numpy().astype(np.float64)[..., :3]
+    assert np.abs(got - want).max() <= 1e-5, np.abs(got - want).max()
+    # batch == single, bit for bit
+    mols = [W.shrink(m, grid_n=m.grid.n, scan_np=(24, 20), scan_nz=5) for m in W.get(3)[:2]]
+    off = np.concatenate([[0], np.cumsum([m.natoms for m in mols])])
+    xyzq = torch.from_numpy(np.concatenate([m.xyzq for m in mols])).cuda()
+    types = torch.from_numpy(np.concatenate([m.types for m in mols])).cuda()
+    ffb = P.forcefield_batch(off, xyzq, types, mols[0].elem_R, mols[0].elem_e, [m.lattice for m in mols],
+                             [m.probe for m in mols], [m.grid for m in mols], mols[0].r_min)
+    posb, itb, eigb = P.relax_scan_stiffness_batch(ffb, [m.grid for m in mols], [m.tip for m in mols], mols[0].fire,
+                                                   [m.scan for m in mols])
+    nps, npts = mols[0].pixel_steps, mols[0].npoints
+    for m in range(2):
+        p1, i1, e1 = P.relax_scan_stiffness(ffb[m * npts:(m + 1) * npts], mols[m].grid, mols[m].tip, mols[m].fire, mols[m].scan)
+        assert torch.equal(p1.reshape(-1, 4), posb[m * nps:(m + 1) * nps]) and torch.equal(e1.reshape(-1, 4), eigb[m * nps:(m + 1) * nps])
 
 
 # ------------------------------------------------------------------------------------------------ df, host API
@@ -928,3 +1100,23 @@ def test_ff_status_counts_bad_type_indices_and_clamp(P):
                  w.grid, 0.5, status=status)
     torch.cuda.synchronize()
     assert P.read_ff_status(status) == {"n_bad_type": 0, "n_clamped": 1}
+
+
+def test_df_column_and_gather_kernels_all_window_lengths(P):
+    """ppfm_df on the oracle's convention for every window length n = 1 .. 40 (n + 1 <= 33: register-ring column kernel,
+    one instantiation per n; above: gather kernel), ragged pixel counts, several output chunks per column, batch of 3
+    stacks; float4 stacks.  Against the oracle's df of the same FP32 samples."""
+    import torch
+    rng = np.random.default_rng(77 + SEED0)
+    for n in list(range(1, 41)):
+        nz = n + 1 + int(rng.integers(0, 70))
+        npx, npy, nsys = int(rng.integers(1, 45)), int(rng.integers(1, 9)), int(rng.integers(1, 4))
+        dz = 0.05
+        stack = rng.normal(size=(nsys, nz, npy, npx, 4)).astype(np.float32)
+        got = P.df(torch.from_numpy(stack).cuda(), npx, npy, nz, dz, n * dz, 1800.0, 30300.0, nsys=nsys)
+        torch.cuda.synchronize()
+        g = got.cpu().numpy().reshape(nsys, nz - n, npy * npx)
+        for s_ in range(nsys):
+            ref = oracle.df(stack[s_, ..., 3].reshape(nz, -1).astype(np.float64), dz, n * dz, 1800.0, 30300.0)
+            scale = np.abs(ref).max()
+            assert np.abs(g[s_] - ref).max() <= 2e-6 * scale * (n + 1), f"n={n} sys {s_}: {np.abs(g[s_] - ref).max():.3e}"
