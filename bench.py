@@ -68,12 +68,16 @@ def measured_peaks():
 
 def ncu_traffic(cfg: int, kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-    (profiles/r02_traffic.json, written from the captures named there); None where no capture exists."""
-    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    (profiles/r02_traffic.csv: cfg,kernel,dram_read_bytes,dram_write_bytes,capture); None where no capture exists."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.csv")
     if not os.path.exists(p):
         return None
     with open(p) as f:
-        return json.load(f).get(f"cfg{cfg}", {}).get(kernel)
+        for line in f:
+            c = line.strip().split(",")
+            if len(c) >= 4 and c[0] == str(cfg) and c[1] == kernel:
+                return float(c[2]) + float(c[3])
+    return None
 
 
 def inputs_sha256(ws) -> str:
@@ -139,8 +143,15 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------- workloads
-def build_workloads(cfg: int, rank: int, world: int):
-    """This rank's systems (weak scaling: an independent seeded draw of the same config per rank)."""
+def build_workloads(cfg: int, rank: int, world: int, strong: bool = False):
+    """This rank's systems.  Weak scaling (default): an independent seeded draw of the same config per rank.  Strong
+    scaling (--strong): ONE system; rank r takes its rows of the scan and the grid rows under them + 4 Å halo
+    (shard.strong_slab; config 3 splits its 64 molecules instead), no exchange between ranks."""
+    if strong:
+        if cfg == 3:
+            lo, hi = shard.split_batch(64, rank, world)
+            return W.config3(64, seed=BASE_SEED[3])[lo:hi]
+        return [shard.strong_slab(W.get(cfg, seed=BASE_SEED[cfg]), rank, world)[0]]
     seed = shard.rank_seed(BASE_SEED[cfg], rank)
     if cfg == 3:
         return W.config3(64, seed=seed)
@@ -211,6 +222,25 @@ class DeviceJob:
             P.stiffness_batch(self.ff, self.c_grid, self.c_tip, self.c_scan, self.pos, out=out)
         else:
             P.stiffness(self.ff, self.c_grid[0], self.c_tip[0], self.c_scan[0], self.pos, out=out)
+
+    def relax_stiffness(self, eig, stats):
+        """The relaxation scan of step() with the stiffness map folded in (ppfm_relax_scan_stiffness[_batch])."""
+        P = self.P
+        if self.batch:
+            P.relax_scan_stiffness_batch(self.ff, self.c_grid, self.c_tip, self.c_fire, self.c_scan, pos_fz=self.pos,
+                                         iters=self.iters, eig=eig, stats=stats)
+        else:
+            P.relax_scan_stiffness(self.ff, self.c_grid[0], self.c_tip[0], self.c_fire, self.c_scan[0], pos_fz=self.pos,
+                                   iters=self.iters, eig=eig, stats=stats)
+
+    def relax_plain(self, stats):
+        P = self.P
+        if self.batch:
+            P.relax_scan_batch(self.ff, self.c_grid, self.c_tip, self.c_fire, self.c_scan, pos_fz=self.pos,
+                               iters=self.iters, stats=stats)
+        else:
+            P.relax_scan(self.ff, self.c_grid[0], self.c_tip[0], self.c_fire, self.c_scan[0], pos_fz=self.pos,
+                         iters=self.iters, stats=stats)
 
     def _mark(self, name):
         ev = self.torch.cuda.Event(enable_timing=True)
@@ -516,6 +546,29 @@ def next_rows(P, B, torch, job, ws, flush, env):
                         "achieved": 32.0 * n_samples / (stiff_ms * 1e-3) * 1e-9,
                         "frac": 32.0 * n_samples / (stiff_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"], "ms": stiff_ms,
                         "samples": n_samples, "in_step": False, "traffic": ncu_traffic(job.cfg, "stiffness")}
+    # the same map folded into the relaxation: cost = relax_scan_stiffness - relax_scan on the resident grid
+    eig = torch.empty_like(job.pos)
+    st2 = P.new_stats()
+    t_fused = t_plain = 0.0
+    for rep in range(2 + 3):
+        flush.zero_()
+        B.timing_enable(True)
+        job.relax_stiffness(eig, st2)
+        torch.cuda.synchronize()
+        a = B.timing_read()["relax"][0]
+        B.timing_enable(True)
+        flush.zero_()
+        job.relax_plain(st2)
+        torch.cuda.synchronize()
+        b = B.timing_read()["relax"][0]
+        if rep >= 2:
+            t_fused += a / 3.0
+            t_plain += b / 3.0
+    B.timing_enable(False)
+    del eig
+    out["stiffness_fused"] = {"kernel": "relax_kernel<.,.,.,0,STIFF>", "relax_with_map_ms": t_fused, "relax_ms": t_plain,
+                              "extra_ms": t_fused - t_plain, "extra_frac_of_relax": (t_fused - t_plain) / t_plain,
+                              "standalone_kernel_ms": stiff_ms, "samples": n_samples, "in_step": False}
     E_only = P.energy_grid(job.ff)
     tri_stats = P.new_stats()
     for rep in range(1 + 2):
@@ -548,11 +601,20 @@ def fft_row(P, B, torch, flush, env):
     npts = w.npoints
     Vs = torch.linspace(-1.0, 1.0, npts, device="cuda", dtype=torch.float32).reshape(w.grid.n[2], w.grid.n[1], w.grid.n[0])
     ff_fft = torch.empty((npts, 4), dtype=torch.float32, device="cuda")
-    for rep in range(2 + 3):
-        if rep == 2:
-            B.timing_enable(True)
+    P.release_scratch()                      # cold: plans exist after the first call, the tip spectra do not
+    P.forcefield_fft(Vs, w.grid, 0.7, -0.03, 0.0, -0.1, out=ff_fft)
+    P.forcefield_fft(Vs, w.grid, 0.6, -0.03, 0.0, -0.1, out=ff_fft)
+    P.forcefield_fft(Vs, w.grid, 0.5, -0.03, 0.0, -0.1, out=ff_fft)      # evicts the first tip
+    torch.cuda.synchronize()
+    B.timing_enable(True)
+    flush.zero_()
+    P.forcefield_fft(Vs, w.grid, 0.7, -0.03, 0.0, -0.1, out=ff_fft)      # tip spectra recomputed (5 + 4 transforms)
+    torch.cuda.synchronize()
+    miss_ms = B.timing_read()["fft_el"][0]
+    B.timing_enable(True)
+    for rep in range(3):
         flush.zero_()
-        P.forcefield_fft(Vs, w.grid, 0.7, -0.03, 0.0, -0.1, out=ff_fft)
+        P.forcefield_fft(Vs, w.grid, 0.7, -0.03, 0.0, -0.1, out=ff_fft)  # cached tip spectra (1 + 4 transforms)
     torch.cuda.synchronize()
     fft_ms = B.timing_read()["fft_el"][0] / 3.0
     B.timing_enable(False)
@@ -560,7 +622,8 @@ def fft_row(P, B, torch, flush, env):
     return {"kernel": "ppfm_forcefield_fft (own kernels + cuFFT FP64 transforms)", "bound": "hbm", "unit": "GB/s",
             "peak": peaks["hbm_gbs"], "achieved": alg / (fft_ms * 1e-3) * 1e-9,
             "frac": alg / (fft_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"], "ms": fft_ms, "points": npts,
-            "points_per_s": npts / (fft_ms * 1e-3), "in_step": False, "workload": "configs[1] grid",
+            "points_per_s": npts / (fft_ms * 1e-3), "ms_tip_spectra_not_cached": miss_ms, "in_step": False,
+            "workload": "configs[1] grid, cached tip spectra",
             "traffic": ncu_traffic(1, "fft_el")}
 
 
@@ -586,7 +649,7 @@ def run_ours(args):
            "gather_cg": B.probe_gather(2 << 20, True)}      # L1 bypassed: every request served by L2
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     cfg = args.config
-    ws = build_workloads(cfg, rank, world)
+    ws = build_workloads(cfg, rank, world, args.strong)
     head, x = measure_config(P, B, torch, cfg, ws, args.steps, args.warmup, max(1, min(args.steps, 5)), flush, env,
                              dist, sample_clocks=True)
     job, ms = x["job"], x["ms"]
@@ -649,11 +712,13 @@ def run_ours(args):
                            if roof["bound"] == "alu" else f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})")
 
     line = {"metric": METRIC, "value": head["pixel_steps_per_s"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": x["t_step"] * 1e3, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "warmup": args.warmup, "ms_per_step": x["t_step"] * 1e3, "higher_is_better": True,
+            "scaling": "strong" if args.strong else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOAD_NAME[cfg], "seed": BASE_SEED[cfg], "systems_per_gpu": len(ws),
                        "l2": "flushed between timed steps (512 MiB device write)",
-                       "parallelism": f"replicated x{world}" if world > 1 else "single GPU",
+                       "parallelism": ("single GPU" if world == 1 else
+                                       f"one system in {world} row slabs (+4 A halo of grid rows), no exchange" if args.strong
+                                       else f"replicated x{world}"),
                        "timing": "CUDA events on the launching stream, per step", "inputs_sha256": head["inputs_sha256"]},
             "parts": {"ff_pair_interactions_per_s": x["units_pairs"] / ff_s,
                       "ff_fp32_pipe_frac_canonical": head["ff_pipe_frac_canonical"],
@@ -687,6 +752,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--strong", action="store_true",
+                    help="with --gpus N > 1: split ONE system across the ranks (row slabs + halo) instead of replicating")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

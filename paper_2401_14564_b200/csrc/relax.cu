@@ -33,6 +33,13 @@ namespace ppfm {
 
 constexpr int RX_THREADS = 128;     // 4 warps = 2 x 2 patches of 8 x 4 pixels -> 16 x 8 pixels per CTA
 constexpr int RX_TILE_X = 16, RX_TILE_Y = 8;
+// Register budget of the tri-linear kernels: 4 CTAs per SM = up to 128 registers.  Left to itself ptxas cuts some
+// instantiations to 96 registers (5 CTAs) and then sinks the spring chain's MUFU.SQRT next to its MUFU.RCP behind the
+// stale-cell vote: a lone warp then stalls ~17 cycles per iteration (config 1: 0.74 -> 0.85 ms; with the stiffness map
+// folded in, 0.97 ms).  With the budget stated every instantiation gets the schedule with the square root issued
+// ~15 instructions ahead of the vote (checked in the SASS, profiles/r02_sass_summary.txt); the fifth CTA was worth
+// <= 4 % on the large scans and the larger budget is worth that much there too.
+constexpr int RX_MIN_CTAS = 4;
 constexpr float RX_MAGIC = 12582912.0f;      // 1.5 * 2^23: floats in [2^23, 2^24) are the integers
 constexpr int RX_MAGIC_BITS = 0x4B400000;
 constexpr int RX_MAX_N = 1 << 21;            // per-axis grid size limit of the magic-number cell index
@@ -67,6 +74,10 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+__device__ __forceinline__ float rsqrt_refined(float x) {      // MUFU.RSQ + one Newton step: unit vectors to 1 ulp
+    const float y = rsqrt_fast(x);
+    return y * fmaf(-0.5f * x * y, y, 1.5f);
 }
 __device__ __forceinline__ float sqrt_fast(float x) {
     float y;
@@ -157,16 +168,18 @@ __device__ __forceinline__ void sym3_eigenvalues_f32(float a00, float a11, float
     const float p2 = (fmaf(b00, b00, fmaf(b11, b11, b22 * b22)) + 2.0f * fmaf(a01, a01, fmaf(a02, a02, a12 * a12))) *
                      (1.0f / 6.0f);
     if (!(p2 > 1.0e-30f)) { e0 = e1 = e2 = q; return; }
-    const float ip = rsqrtf(p2), p = p2 * ip;
+    const float ip = rsqrt_fast(p2), p = p2 * ip;
     const float c00 = b00 * ip, c11 = b11 * ip, c22 = b22 * ip, c01 = a01 * ip, c02 = a02 * ip, c12 = a12 * ip;
     const float det = c00 * fmaf(c11, c22, -c12 * c12) - c01 * fmaf(c01, c22, -c12 * c02) + c02 * fmaf(c01, c12, -c11 * c02);
     const float sgn = (det >= 0.0f) ? 1.0f : -1.0f;
     const float ad = fminf(fabsf(det), 2.0f);
     float mu = 2.0f;
+    // from mu = 2 the worst case (root sqrt 3) is within 1e-6 after three steps and converged after four; an
+    // approximate reciprocal is enough inside a Newton step (the iteration corrects its own rounding)
 #pragma unroll
-    for (int it = 0; it < 6; it++) {
+    for (int it = 0; it < 5; it++) {
         const float f = fmaf(mu, fmaf(mu, mu, -3.0f), -ad);
-        mu -= f / fmaf(3.0f * mu, mu, -3.0f);
+        mu = fmaf(-f, rcp_fast(fmaf(3.0f * mu, mu, -3.0f)), mu);
     }
     const float liso = sgn * mu;                       // isolated eigenvalue of C = B/p
     // eigenvector of liso: largest cross product of two rows of C - liso I
@@ -179,7 +192,7 @@ __device__ __forceinline__ void sym3_eigenvalues_f32(float a00, float a11, float
     float vx = x0, vy = y0, vz = z0, nn = n0;
     if (n1 > nn) { vx = x1; vy = y1; vz = z1; nn = n1; }
     if (n2 > nn) { vx = x2; vy = y2; vz = z2; nn = n2; }
-    const float inn = rsqrtf(nn);
+    const float inn = rsqrt_refined(nn);
     vx *= inn; vy *= inn; vz *= inn;
     // orthonormal a, b spanning the plane orthogonal to v: a = e_k x v for the smallest |v_k|
     const float ax_ = fabsf(vx), ay_ = fabsf(vy), az_ = fabsf(vz);
@@ -187,7 +200,7 @@ __device__ __forceinline__ void sym3_eigenvalues_f32(float a00, float a11, float
     if (ax_ <= ay_ && ax_ <= az_) { ux = 0.0f; uy = -vz; uz = vy; }
     else if (ay_ <= az_) { ux = vz; uy = 0.0f; uz = -vx; }
     else { ux = -vy; uy = vx; uz = 0.0f; }
-    const float iu = rsqrtf(fmaf(ux, ux, fmaf(uy, uy, uz * uz)));
+    const float iu = rsqrt_refined(fmaf(ux, ux, fmaf(uy, uy, uz * uz)));
     ux *= iu; uy *= iu; uz *= iu;
     const float wx = fmaf(vy, uz, -vz * uy), wy = fmaf(vz, ux, -vx * uz), wz = fmaf(vx, uy, -vy * ux);
     // C u, C w and the projected 2 x 2 matrix
@@ -198,10 +211,59 @@ __device__ __forceinline__ void sym3_eigenvalues_f32(float a00, float a11, float
     const float muu = fmaf(ux, cux, fmaf(uy, cuy, uz * cuz)), mww = fmaf(wx, cwx, fmaf(wy, cwy, wz * cwz));
     const float muw = fmaf(ux, cwx, fmaf(uy, cwy, uz * cwz));
     const float mean = 0.5f * (muu + mww), hd = 0.5f * (muu - mww);
-    const float sq = sqrtf(fmaf(hd, hd, muw * muw));
+    const float sq = sqrt_fast(fmaf(hd, hd, muw * muw));
     const float la = fmaf(p, mean - sq, q), lb = fmaf(p, mean + sq, q), li = fmaf(p, liso, q);
     if (sgn > 0.0f) { e0 = la; e1 = lb; e2 = li; }
     else { e0 = li; e1 = la; e2 = lb; }
+}
+
+// Inputs of the stiffness map at the end of a z-step: the cached cell (corner forces at x0 and their x-differences for
+// the four (y,z) edges), the in-cell fractions, d = r_PP - r_TIP and fr = -k_R (|d| - R0)/|d|.
+struct StiffIn {
+    float c0[4][3], cd[4][3];
+    float f[3], d[3], fr;
+};
+
+// G[c][a] = dF_c/dt_a of the tri-linear interpolant, J = G Minv, H = H_spring - (J + J^T)/2 with
+// H_spring = k_R dd^T/|d|^2 + k_t (I - dd^T/|d|^2) + diag(k_x, k_y, 0), k_t = k_R (|d| - R0)/|d| = -fr; eigenvalues ascending.
+template <bool ORTHO>
+__device__ __noinline__ float4 stiffness_from_cell(const StiffIn in, const RelaxJob &job) {
+    const float fx = in.f[0], fy = in.f[1], fz = in.f[2];
+    const float gy = 1.0f - fy, gz = 1.0f - fz;
+    float G[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const float e00 = fmaf(fx, in.cd[0][c], in.c0[0][c]), e10 = fmaf(fx, in.cd[1][c], in.c0[1][c]);
+        const float e01 = fmaf(fx, in.cd[2][c], in.c0[2][c]), e11 = fmaf(fx, in.cd[3][c], in.c0[3][c]);
+        G[c][0] = gz * fmaf(fy, in.cd[1][c], gy * in.cd[0][c]) + fz * fmaf(fy, in.cd[3][c], gy * in.cd[2][c]);
+        G[c][1] = fmaf(fz, e11 - e01, gz * (e10 - e00));
+        G[c][2] = fmaf(fy, e11 - e10, gy * (e01 - e00));
+    }
+    const float *m = job.Minvf;
+    float J[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if (ORTHO) {
+            J[c][0] = G[c][0] * m[0]; J[c][1] = G[c][1] * m[4]; J[c][2] = G[c][2] * m[8];
+        } else {
+            J[c][0] = fmaf(G[c][2], m[6], fmaf(G[c][1], m[3], G[c][0] * m[0]));
+            J[c][1] = fmaf(G[c][2], m[7], fmaf(G[c][1], m[4], G[c][0] * m[1]));
+            J[c][2] = fmaf(G[c][2], m[8], fmaf(G[c][1], m[5], G[c][0] * m[2]));
+        }
+    }
+    const float ddx = in.d[0], ddy = in.d[1], ddz = in.d[2];
+    const float L2 = fmaf(ddx, ddx, fmaf(ddy, ddy, ddz * ddz));
+    const float kt = -in.fr;
+    const float kd = (L2 > 0.0f) ? (job.k_rad - kt) * rcp_fast(L2) : 0.0f;
+    const float h00 = fmaf(kd * ddx, ddx, kt) - J[0][0] + job.k_lat[0];
+    const float h11 = fmaf(kd * ddy, ddy, kt) - J[1][1] + job.k_lat[1];
+    const float h22 = fmaf(kd * ddz, ddz, kt) - J[2][2];
+    const float h01 = fmaf(kd * ddx, ddy, -0.5f * (J[0][1] + J[1][0]));
+    const float h02 = fmaf(kd * ddx, ddz, -0.5f * (J[0][2] + J[2][0]));
+    const float h12 = fmaf(kd * ddy, ddz, -0.5f * (J[1][2] + J[2][1]));
+    float l0, l1, l2;
+    sym3_eigenvalues_f32(h00, h11, h22, h01, h02, h12, l0, l1, l2);
+    return make_float4(l0, l1, l2, 0.0f);
 }
 
 template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF = false>
@@ -534,42 +596,18 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         if (STIFF && !TRICUBIC) {
             // Stiffness map from the cell this lane still holds: the last FIRE
             // iteration of a finished lane does not move it, so (c0, cd, fx, fy, fz, fr, dzc) belong to the relaxed
-            // point.  G[c][a] = dF_c/dt_a of the tri-linear interpolant, J = G Minv, H = H_spring - (J + J^T)/2.
-            const float gy = 1.0f - fy, gz = 1.0f - fz;
-            float G[3][3];
+            // point.  Done in a function that is NOT inlined: the FIRE loop's instruction schedule and register
+            // allocation then stay those of the plain kernel (inlined, the ~200 extra instructions per z-step cost
+            // config 1 a quarter of its speed through the loop's schedule, DESIGN.md §7 "schedule sensitivity").
+            StiffIn in;
 #pragma unroll
-            for (int c = 0; c < 3; c++) {
-                const float e00 = fmaf(fx, cd[0][c], c0[0][c]), e10 = fmaf(fx, cd[1][c], c0[1][c]);
-                const float e01 = fmaf(fx, cd[2][c], c0[2][c]), e11 = fmaf(fx, cd[3][c], c0[3][c]);
-                G[c][0] = gz * fmaf(fy, cd[1][c], gy * cd[0][c]) + fz * fmaf(fy, cd[3][c], gy * cd[2][c]);
-                G[c][1] = fmaf(fz, e11 - e01, gz * (e10 - e00));
-                G[c][2] = fmaf(fy, e11 - e10, gy * (e01 - e00));
-            }
-            float J[3][3];
+            for (int e = 0; e < 4; e++)
 #pragma unroll
-            for (int c = 0; c < 3; c++) {
-                if (ORTHO) {
-                    J[c][0] = G[c][0] * m00; J[c][1] = G[c][1] * m11; J[c][2] = G[c][2] * m22;
-                } else {
-                    J[c][0] = fmaf(G[c][2], m20, fmaf(G[c][1], m10, G[c][0] * m00));
-                    J[c][1] = fmaf(G[c][2], m21, fmaf(G[c][1], m11, G[c][0] * m01));
-                    J[c][2] = fmaf(G[c][2], m22, fmaf(G[c][1], m12, G[c][0] * m02));
-                }
-            }
-            // H_spring = k_R dd^T/|d|^2 + k_t (I - dd^T/|d|^2) + diag(k_x, k_y, 0), k_t = k_R (|d| - R0)/|d| = -fr
-            const float ddx = SYMTIP ? ux : d0x + ux, ddy = SYMTIP ? uy : d0y + uy, ddz = dzc;
-            const float L2 = fmaf(ddx, ddx, fmaf(ddy, ddy, ddz * ddz));
-            const float kt = -fr;
-            const float kd = (L2 > 0.0f) ? (job.k_rad - kt) / L2 : 0.0f;
-            const float h00 = fmaf(kd * ddx, ddx, kt) - J[0][0] + job.k_lat[0];
-            const float h11 = fmaf(kd * ddy, ddy, kt) - J[1][1] + job.k_lat[1];
-            const float h22 = fmaf(kd * ddz, ddz, kt) - J[2][2];
-            const float h01 = fmaf(kd * ddx, ddy, -0.5f * (J[0][1] + J[1][0]));
-            const float h02 = fmaf(kd * ddx, ddz, -0.5f * (J[0][2] + J[2][0]));
-            const float h12 = fmaf(kd * ddy, ddz, -0.5f * (J[1][2] + J[2][1]));
-            float l0, l1, l2;
-            sym3_eigenvalues_f32(h00, h11, h22, h01, h02, h12, l0, l1, l2);
-            eig_out[o] = make_float4(l0, l1, l2, 0.0f);
+                for (int c = 0; c < 3; c++) { in.c0[e][c] = c0[e][c]; in.cd[e][c] = cd[e][c]; }
+            in.f[0] = fx; in.f[1] = fy; in.f[2] = fz;
+            in.d[0] = SYMTIP ? ux : d0x + ux; in.d[1] = SYMTIP ? uy : d0y + uy; in.d[2] = dzc;
+            in.fr = fr;
+            eig_out[o] = stiffness_from_cell<ORTHO>(in, job);
         }
         float tx, ty, tz;
         if (ORTHO) {
@@ -629,7 +667,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
 
 // One system: the job travels as a kernel parameter (constant bank), no scratch and no copy.
 template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF>
-__global__ void __launch_bounds__(RX_THREADS)
+__global__ void __launch_bounds__(RX_THREADS, TRICUBIC ? 3 : RX_MIN_CTAS)
 relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireParams fp,
              const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
              ppfm_stats *__restrict__ stats, float *__restrict__ fz_out, float4 *__restrict__ eig_out) {
@@ -639,7 +677,7 @@ relax_kernel(const __grid_constant__ RelaxJob job, const __grid_constant__ FireP
 
 // Batch: the CTA finds its system in a device array and keeps a copy in shared memory.
 template <bool ORTHO, bool ANYPER, bool SYMTIP, bool TRICUBIC, bool STIFF>
-__global__ void __launch_bounds__(RX_THREADS)
+__global__ void __launch_bounds__(RX_THREADS, TRICUBIC ? 3 : RX_MIN_CTAS)
 relax_batch_kernel(const RelaxJob *__restrict__ jobs, int njobs, const __grid_constant__ FireParams fp,
                    const void *__restrict__ ff, float4 *__restrict__ pos_fz, uint16_t *__restrict__ iters_out,
                    ppfm_stats *__restrict__ stats, float *__restrict__ fz_out, float4 *__restrict__ eig_out) {
@@ -799,9 +837,9 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
 // and H_spring the second derivative of the tip springs of Eq.2.  Output: the three eigenvalues, ascending.
 //
 // One thread per (pixel, z-step) sample, x fastest so that reads, gathers and the float4 store are coalesced.  Cell
-// lookup and the eigenvalues are FP64 (once per sample; the eigenvalues of interest, ~k_xy = 0.016 eV/A^2, sit next
-// to one of ~k_R = 1.9); the Jacobian is formed in FP32 from the FP32 grid.  Eigenvalues by the closed-form
-// trigonometric solution of the characteristic cubic.
+// lookup and the spring Hessian are FP64 (once per sample); the Jacobian is formed in FP32 from the FP32 grid; the
+// eigenvalues come from the FP32 deflation solver above (the eigenvalues of interest, ~k_xy = 0.016 eV/A^2, sit next to
+// one of ~k_R = 1.9: a route through all three roots of the characteristic cubic would need FP64 trigonometry).
 struct StiffCell {
     int i0, i1;
     float f;
@@ -825,24 +863,6 @@ __device__ __forceinline__ StiffCell stiff_axis(double t, int n, int periodic) {
         c.f = (float)(tc - (double)i);
     }
     return c;
-}
-
-__device__ __forceinline__ void sym3_eigenvalues(double a00, double a11, double a22, double a01, double a02,
-                                                 double a12, double &e0, double &e1, double &e2) {
-    const double p1 = a01 * a01 + a02 * a02 + a12 * a12;
-    const double q = (a00 + a11 + a22) * (1.0 / 3.0);
-    const double b00 = a00 - q, b11 = a11 - q, b22 = a22 - q;
-    const double p2 = b00 * b00 + b11 * b11 + b22 * b22 + 2.0 * p1;
-    if (!(p2 > 0.0)) { e0 = e1 = e2 = q; return; }
-    const double p = sqrt(p2 * (1.0 / 6.0));
-    const double ip = 1.0 / p;
-    const double c00 = b00 * ip, c11 = b11 * ip, c22 = b22 * ip, c01 = a01 * ip, c02 = a02 * ip, c12 = a12 * ip;
-    const double det = c00 * (c11 * c22 - c12 * c12) - c01 * (c01 * c22 - c12 * c02) + c02 * (c01 * c12 - c11 * c02);
-    const double r = fmin(fmax(0.5 * det, -1.0), 1.0);
-    const double phi = acos(r) * (1.0 / 3.0);
-    e2 = q + 2.0 * p * cos(phi);                                          // largest
-    e0 = q + 2.0 * p * cos(phi + 2.0943951023931954923);                 // smallest (phi + 2 pi / 3)
-    e1 = 3.0 * q - e0 - e2;
 }
 
 __global__ void __launch_bounds__(256)
@@ -922,9 +942,10 @@ stiffness_kernel(const RelaxJob *__restrict__ jobs, int njobs, long long nsample
         }
     H[0][0] += (double)job.k_lat[0];
     H[1][1] += (double)job.k_lat[1];
-    double e0, e1, e2;
-    sym3_eigenvalues(H[0][0], H[1][1], H[2][2], H[0][1], H[0][2], H[1][2], e0, e1, e2);
-    eig[s] = make_float4((float)e0, (float)e1, (float)e2, 0.0f);
+    float e0, e1, e2;
+    sym3_eigenvalues_f32((float)H[0][0], (float)H[1][1], (float)H[2][2], (float)H[0][1], (float)H[0][2], (float)H[1][2],
+                         e0, e1, e2);
+    eig[s] = make_float4(e0, e1, e2, 0.0f);
 }
 
 static int stiffness_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,

@@ -838,7 +838,8 @@ def test_stiffness_zero_field_periodic_nonorthogonal_and_batch(P):
     tip = replace(W._default_tip(), k_lat=np.array([0.011, 0.023]))
     pos, _ = P.relax_scan(ff, g, tip, W.Fire(), sc)
     eig = P.stiffness(ff, g, tip, sc, pos).cpu().numpy()
-    assert np.allclose(eig[..., :3], [0.011, 0.023, tip.k_rad], rtol=1e-6, atol=1e-7)
+    # FP32 deflation eigen-solver: error a few ulp of |H| = k_R (1.9 x 6e-8 x 3), far inside the map's 1e-5 tolerance
+    assert np.allclose(eig[..., :3], [0.011, 0.023, tip.k_rad], rtol=1e-6, atol=5e-7)
     # periodic + skewed grid, positions partly outside the cell (wrap) - against the oracle
     w = W.shrink(W.get(2), grid_n=(50, 50, 24), scan_np=(21, 17), scan_nz=6)
     step = np.array([[0.5, 0.02, 0.0], [-0.03, 0.5, 0.0], [0.01, 0.02, 0.25]])
@@ -951,7 +952,7 @@ def test_relax_scan_stiffness_closed_forms(P):
     tip = replace(W._default_tip(), k_lat=np.array([0.011, 0.023]))
     ff = torch.zeros((60, 20, 20, 4), dtype=torch.float32, device="cuda")
     pos, it, eig = P.relax_scan_stiffness(ff, g, tip, W.Fire(), sc)
-    assert np.allclose(eig.cpu().numpy()[..., :3], [0.011, 0.023, tip.k_rad], rtol=2e-6, atol=1e-7)
+    assert np.allclose(eig.cpu().numpy()[..., :3], [0.011, 0.023, tip.k_rad], rtol=1e-6, atol=5e-7)
     # linear field
     K = np.array([[0.020, 0.004, -0.003], [0.004, 0.012, 0.002], [-0.003, 0.002, 0.030]])
     r0 = np.array([2.0, 2.1, 4.6])
@@ -1120,3 +1121,32 @@ def test_df_column_and_gather_kernels_all_window_lengths(P):
             ref = oracle.df(stack[s_, ..., 3].reshape(nz, -1).astype(np.float64), dz, n * dz, 1800.0, 30300.0)
             scale = np.abs(ref).max()
             assert np.abs(g[s_] - ref).max() <= 2e-6 * scale * (n + 1), f"n={n} sys {s_}: {np.abs(g[s_] - ref).max():.3e}"
+
+
+def test_strong_scaling_slabs_match_the_undivided_scan_on_one_gpu(P):
+    """bench.py --strong (shard.strong_slab): the scan of ONE system run as 3 row slabs, each on its own rows of the
+    force-field grid (+ halo), one after the other on this GPU, against the undivided run: same relaxed positions
+    (1e-5 Å: the sub-grid's origin is another FP64 number, so grid coordinates differ in the last bits), same df, no
+    clamping at the slab faces.  Config 1 (clamped grid) and a periodic system whose slabs stay inside the cell."""
+    import torch
+    from paper_2401_14564_b200 import shard
+    w1 = W.shrink(W.get(1), scan_np=(40, 45), scan_nz=14)
+    wp = W.shrink(W.get(2), grid_n=(250, 250, 60), scan_np=(24, 30), scan_nz=12)
+    wp = replace(wp, Q_sweep=None, scan=replace(wp.scan, p0=np.array([9.0, 9.0, wp.scan.p0[2]])))
+    for what, w in (("cfg1", w1), ("periodic", wp)):
+        ff, pos, iters, df, st = gpu_scan(P, w)
+        full = pos.cpu().numpy().reshape(w.scan.nz, w.scan.npy, w.scan.npx, 4)
+        df_full = df.cpu().numpy().reshape(-1, w.scan.npy, w.scan.npx)
+        split = 0
+        for r in range(3):
+            ws, (lo, hi), (j_lo, j_hi) = shard.strong_slab(w, r, 3, halo=3.0)
+            split += (j_hi - j_lo + 1) < w.grid.n[1]
+            ff_s, pos_s, it_s, df_s, st_s = gpu_scan(P, ws)
+            assert st_s["n_clamped"] == 0, what
+            got = pos_s.cpu().numpy().reshape(w.scan.nz, hi - lo, w.scan.npx, 4)
+            d = np.abs(got - full[:, lo:hi]).max(axis=-1)
+            assert np.quantile(d, 0.999) <= 1e-5 and (d <= 2e-3).mean() >= 0.9999, f"{what} slab {r}: {d.max():.3e}"
+            g = df_s.cpu().numpy().reshape(-1, hi - lo, w.scan.npx)
+            err = np.abs(g - df_full[:, lo:hi])
+            assert np.quantile(err, 0.999) <= 1e-2, f"{what} slab {r}: df {err.max():.3e}"
+        assert split == 3, f"{what}: the grid rows were not split"
