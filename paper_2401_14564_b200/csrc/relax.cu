@@ -9,13 +9,14 @@
 // A FIRE iteration is a strictly dependent chain (position -> force -> step), so with few pixels the kernel runs at
 // the latency of that chain and with many pixels at the speed of instruction issue; both want the fewest
 // instructions per iteration:
-//   * the lane keeps the 8 corner forces of its current grid cell in registers (corner values + x-differences) and
-//     the per-axis offset that turns the position into the in-cell fraction with one FFMA; the probe particle leaves
+//   * the lane keeps its current grid cell in registers (per force component the 8 coefficients of the tri-linear
+//     polynomial, evaluated by Horner: 7 FFMA, depth 3) and the per-axis offset that turns the position into the
+//     in-cell fraction with one FFMA; the probe particle leaves
 //     its cell in 2-3 % of iterations, and only then the warp (all lanes, one warp-uniform block entered through
 //     __any_sync) re-locates and re-gathers: cell index and fraction by the magic-number trick (t - 0.5 + 1.5*2^23
 //     rounds to floor(t) in the low mantissa bits; clamps are two FMNMX in that domain), eight LDG.128 issued back
 //     to back;
-//   * the interpolation (nested lerps) is computed speculatively from the cached cell ahead of that branch, the
+//   * the interpolation is computed speculatively from the cached cell ahead of that branch, the
 //     spring chain's two MUFU are pinned ahead of it too (asm volatile: see sqrt_pinned);
 //   * FIRE is branch-free: everything that depends only on the old velocity is computed off the critical path; after
 //     F arrives the chain is F.F -> rsqrt -> one select -> two FMA per component;
@@ -217,10 +218,11 @@ __device__ __forceinline__ void sym3_eigenvalues_f32(float a00, float a11, float
     else { e0 = li; e1 = la; e2 = lb; }
 }
 
-// Inputs of the stiffness map at the end of a z-step: the cached cell (corner forces at x0 and their x-differences for
-// the four (y,z) edges), the in-cell fractions, d = r_PP - r_TIP and fr = -k_R (|d| - R0)/|d|.
+// Inputs of the stiffness map at the end of a z-step: the cached cell (the eight coefficients of the tri-linear
+// polynomial per force component, see relax_pixels), the in-cell fractions, d = r_PP - r_TIP and
+// fr = -k_R (|d| - R0)/|d|.
 struct StiffIn {
-    float c0[4][3], cd[4][3];
+    float a[8][3];
     float f[3], d[3], fr;
 };
 
@@ -229,15 +231,14 @@ struct StiffIn {
 template <bool ORTHO>
 __device__ __noinline__ float4 stiffness_from_cell(const StiffIn in, const RelaxJob &job) {
     const float fx = in.f[0], fy = in.f[1], fz = in.f[2];
-    const float gy = 1.0f - fy, gz = 1.0f - fz;
-    float G[3][3];
+    float G[3][3];               // dF_c/dt_a: derivatives of a0 + a1 x + a2 y + a3 z + a4 xy + a5 xz + a6 yz + a7 xyz
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        const float e00 = fmaf(fx, in.cd[0][c], in.c0[0][c]), e10 = fmaf(fx, in.cd[1][c], in.c0[1][c]);
-        const float e01 = fmaf(fx, in.cd[2][c], in.c0[2][c]), e11 = fmaf(fx, in.cd[3][c], in.c0[3][c]);
-        G[c][0] = gz * fmaf(fy, in.cd[1][c], gy * in.cd[0][c]) + fz * fmaf(fy, in.cd[3][c], gy * in.cd[2][c]);
-        G[c][1] = fmaf(fz, e11 - e01, gz * (e10 - e00));
-        G[c][2] = fmaf(fy, e11 - e10, gy * (e01 - e00));
+        const float a1 = in.a[1][c], a2 = in.a[2][c], a3 = in.a[3][c], a4 = in.a[4][c], a5 = in.a[5][c], a6 = in.a[6][c],
+                    a7 = in.a[7][c];
+        G[c][0] = fmaf(fz, fmaf(fy, a7, a5), fmaf(fy, a4, a1));
+        G[c][1] = fmaf(fz, fmaf(fx, a7, a6), fmaf(fx, a4, a2));
+        G[c][2] = fmaf(fy, fmaf(fx, a7, a6), fmaf(fx, a5, a3));
     }
     const float *m = job.Minvf;
     float J[3][3];
@@ -307,16 +308,18 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
     int npos = 0, moves = 0;
     bool conv = !valid;
     float fr = 0.f, dzc = d0z, fx = 0.f, fy = 0.f, fz = 0.f;
-    // cached cell: corner forces at x0 and their x-differences for the four (y,z) edges 00, 10 (y+1), 01 (z+1),
-    // 11, and per axis tbf = (fraction of the z-step's base point) - (offset of the cached cell from the base
-    // cell), so that the position inside the cell is one FFMA: f = Minv u + tbf.  An impossible offset makes the
-    // first iteration gather.
+    // cached cell: per force component the eight coefficients of the tri-linear polynomial in the in-cell fractions,
+    //   F = a0 + a1 x + a2 y + a3 z + a4 xy + a5 xz + a6 yz + a7 xyz
+    // (formed from the eight corners when the cell is gathered; evaluated by Horner in 7 FFMA of depth 3, where nested
+    // lerps on the corners take 10 operations of depth 5), and per axis tbf = (fraction of the z-step's base point) -
+    // (offset of the cached cell from the base cell), so that the position inside the cell is one FFMA:
+    // f = Minv u + tbf.  An impossible offset makes the first iteration gather.
     float tbfx = -1.0e30f, tbfy = -1.0e30f, tbfz = -1.0e30f;
-    float c0[4][3], cd[4][3];
+    float ca[8][3];
 #pragma unroll
-    for (int e = 0; e < 4; e++)
+    for (int e = 0; e < 8; e++)
 #pragma unroll
-        for (int c = 0; c < 3; c++) c0[e][c] = cd[e][c] = 0.0f;
+        for (int c = 0; c < 3; c++) ca[e][c] = 0.0f;
     // TRICUBIC: the 4 x 4 x 4 energies around the cell, [z][y][x], minus the value at the cell's own node (the
     // gradient does not see a constant, and differences of ~|F| h keep FP32 rounding far below f_conv)
     float en[TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1][TRICUBIC ? 4 : 1];
@@ -329,7 +332,7 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 for (int c = 0; c < (TRICUBIC ? 4 : 1); c++) en[a][b][c] = 0.0f;
     }
 
-    auto interp = [&](float (&S)[3]) {     // nested lerps x, y, z: 10 FP32 ops per component
+    auto interp = [&](float (&S)[3]) {     // Horner in x, y, z on the cached coefficients: 7 FFMA per component, depth 3
         if (TRICUBIC) {
             // F_S = -grad of the tri-cubic (Catmull-Rom per axis, reading S22) interpolant of the energies:
             // weights w and their derivatives d per axis (Horner), x pass per (z,y) row, y pass per z plane, z pass
@@ -374,13 +377,11 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
         }
 #pragma unroll
         for (int c = 0; c < (TRICUBIC ? 0 : 3); c++) {
-            const float e00 = fmaf(fx, cd[0][c], c0[0][c]);
-            const float e10 = fmaf(fx, cd[1][c], c0[1][c]);
-            const float e01 = fmaf(fx, cd[2][c], c0[2][c]);
-            const float e11 = fmaf(fx, cd[3][c], c0[3][c]);
-            const float g0 = fmaf(fy, e10 - e00, e00);
-            const float g1 = fmaf(fy, e11 - e01, e01);
-            S[c] = fmaf(fz, g1 - g0, g0);
+            const float p0 = fmaf(fx, ca[1][c], ca[0][c]);
+            const float p1 = fmaf(fx, ca[4][c], ca[2][c]);
+            const float p2 = fmaf(fx, ca[5][c], ca[3][c]);
+            const float p3 = fmaf(fx, ca[7][c], ca[6][c]);
+            S[c] = fmaf(fz, fmaf(fy, p3, p2), fmaf(fy, p1, p0));
         }
     };
 
@@ -522,14 +523,16 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                 fz = __saturatef(fmaf(m20, ux, fmaf(m21, uy, fmaf(m22, uz, tbfz))));
             }
             if (!TRICUBIC) {
-            c0[0][0] = c000.x; c0[0][1] = c000.y; c0[0][2] = c000.z;
-            c0[1][0] = c010.x; c0[1][1] = c010.y; c0[1][2] = c010.z;
-            c0[2][0] = c100.x; c0[2][1] = c100.y; c0[2][2] = c100.z;
-            c0[3][0] = c110.x; c0[3][1] = c110.y; c0[3][2] = c110.z;
-            cd[0][0] = c001.x - c000.x; cd[0][1] = c001.y - c000.y; cd[0][2] = c001.z - c000.z;
-            cd[1][0] = c011.x - c010.x; cd[1][1] = c011.y - c010.y; cd[1][2] = c011.z - c010.z;
-            cd[2][0] = c101.x - c100.x; cd[2][1] = c101.y - c100.y; cd[2][2] = c101.z - c100.z;
-            cd[3][0] = c111.x - c110.x; cd[3][1] = c111.y - c110.y; cd[3][2] = c111.z - c110.z;
+#define PPFM_COEF(C, I)                                                              \
+    {                                                                                \
+        const float d0 = c001.C - c000.C, d1 = c011.C - c010.C, d2 = c101.C - c100.C, d3 = c111.C - c110.C; \
+        const float e2 = c010.C - c000.C, e6 = c110.C - c100.C;                      \
+        ca[0][I] = c000.C; ca[1][I] = d0; ca[2][I] = e2; ca[3][I] = c100.C - c000.C; \
+        ca[4][I] = d1 - d0; ca[5][I] = d2 - d0; ca[6][I] = e6 - e2;                  \
+        ca[7][I] = (d3 - d2) - (d1 - d0);                                            \
+    }
+            PPFM_COEF(x, 0) PPFM_COEF(y, 1) PPFM_COEF(z, 2)
+#undef PPFM_COEF
             }
             my_reloads += (worst > 0x3F800000u) ? 1u : 0u;
             my_wreloads++;
@@ -601,9 +604,9 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
             // config 1 a quarter of its speed through the loop's schedule, DESIGN.md §7 "schedule sensitivity").
             StiffIn in;
 #pragma unroll
-            for (int e = 0; e < 4; e++)
+            for (int e = 0; e < 8; e++)
 #pragma unroll
-                for (int c = 0; c < 3; c++) { in.c0[e][c] = c0[e][c]; in.cd[e][c] = cd[e][c]; }
+                for (int c = 0; c < 3; c++) in.a[e][c] = ca[e][c];
             in.f[0] = fx; in.f[1] = fy; in.f[2] = fz;
             in.d[0] = SYMTIP ? ux : d0x + ux; in.d[1] = SYMTIP ? uy : d0y + uy; in.d[2] = dzc;
             in.fr = fr;
