@@ -16,8 +16,8 @@
 //     __any_sync) re-locates and re-gathers: cell index and fraction by the magic-number trick (t - 0.5 + 1.5*2^23
 //     rounds to floor(t) in the low mantissa bits; clamps are two FMNMX in that domain), eight LDG.128 issued back
 //     to back;
-//   * the interpolation is computed speculatively from the cached cell ahead of that branch, the
-//     spring chain's two MUFU are pinned ahead of it too (asm volatile: see sqrt_pinned);
+//   * the interpolation is computed speculatively from the cached cell ahead of that branch; the spring chain's
+//     MUFU.SQRT has to issue well ahead of it too, which the stated register budget secures (see RX_MIN_CTAS);
 //   * FIRE is branch-free: everything that depends only on the old velocity is computed off the critical path; after
 //     F arrives the chain is F.F -> rsqrt -> one select -> two FMA per component;
 //   * the convergence vote (__all_sync) is taken every second iteration: finished lanes do not move.
@@ -85,9 +85,10 @@ __device__ __forceinline__ float sqrt_fast(float x) {
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// The spring chain's two MUFU are pinned in program order (volatile) ahead of the stale-cell vote: whether ptxas
-// hoists them above the branch or sinks them below it changes a lone warp's iteration time by 40 % (measured:
-// 0.75 vs 1.05 ms on config 1 for otherwise identical code), because everything behind the chain waits for it.
+// The spring chain's two MUFU.  `volatile` keeps the front end from merging or moving them, but ptxas still schedules
+// them freely against arithmetic: whether MUFU.SQRT issues ~15 instructions ahead of the stale-cell vote or directly in
+// front of its MUFU.RCP changes a lone warp's iteration time by 15-40 %, and it is the register budget (RX_MIN_CTAS)
+// that decides it.
 __device__ __forceinline__ float sqrt_pinned(float x) {
     float y;
     asm volatile("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
