@@ -249,7 +249,9 @@ int ppfm_stiffness_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids
  * eigenvalues of H at the relaxed point to d_eig (same layout as above; FP32 throughout, the eigenvalues by
  * deflation on the isolated root so that the two nearly degenerate lateral modes keep full FP32 accuracy).  All other
  * arguments and outputs as ppfm_relax_scan[_batch]; d_eig must not be NULL.  ppfm_stiffness remains the entry point
- * for positions that do not come straight from a scan. */
+ * for positions that do not come straight from a scan.  (The Jacobian of a tri-linear interpolant jumps across cell
+ * faces: for a point exactly on a face the folded map uses the cell the relaxation held, ppfm_stiffness the cell
+ * floor() picks from the stored FP32 position; the two can then differ by that jump.) */
 int ppfm_relax_scan_stiffness(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tip, const ppfm_fire *fire,
                               const ppfm_scan *scan, float *d_pos_fz, uint16_t *d_iters, float *d_eig,
                               ppfm_stats *d_stats, void *cuda_stream);

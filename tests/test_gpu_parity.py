@@ -1187,3 +1187,37 @@ def test_scratch_oom_is_reported_and_does_not_poison_the_next_call(P):
     assert np.array_equal(p_pos.reshape(-1, 4), pos.cpu().numpy().reshape(-1, 4))
     ff2 = gpu_ff(P, w)
     assert torch.equal(ff2, ff)
+
+
+def test_df_and_folded_stiffness_edge_cases(P):
+    """df: a single output plane (nz = n + 1), a single pixel, and more stacks than the column kernel's grid takes
+    (nsys > 65535 -> gather kernel), each against the oracle; folded stiffness map with max_iter = 0 (nothing moves: the
+    map is evaluated at the spring equilibrium points, not-converged samples included) = the stand-alone kernel."""
+    import torch
+    rng = np.random.default_rng(99 + SEED0)
+    for (nsys, nz, npy, npx, n) in ((1, 11, 3, 5, 10), (1, 25, 1, 1, 20), (70000, 4, 1, 1, 2)):
+        dz = 0.1
+        stack = rng.normal(size=(nsys, nz, npy, npx, 4)).astype(np.float32)
+        got = P.df(torch.from_numpy(stack).cuda(), npx, npy, nz, dz, n * dz, 1800.0, 30300.0, nsys=nsys)
+        torch.cuda.synchronize()
+        g = got.cpu().numpy().reshape(nsys, nz - n, npy * npx)
+        for s_ in (0, nsys // 2, nsys - 1):
+            ref = oracle.df(stack[s_, ..., 3].reshape(nz, -1).astype(np.float64), dz, n * dz, 1800.0, 30300.0)
+            assert np.abs(g[s_] - ref).max() <= 2e-6 * np.abs(ref).max() * (n + 1), (nsys, nz, n)
+    w = W.get(0)
+    # config 0's pixels sit exactly on grid nodes, where the Jacobian of a tri-linear interpolant jumps and the two kernels
+    # may take different cells: shift the scan off the nodes
+    w = replace(w, scan=replace(w.scan, p0=w.scan.p0 + np.array([0.07, 0.05, 0.03])))
+    ffd = gpu_ff(P, w)
+    fire0 = replace(w.fire, max_iter=0)
+    pos, it, eig = P.relax_scan_stiffness(ffd, w.grid, w.tip, fire0, w.scan)
+    alone = P.stiffness(ffd, w.grid, w.tip, w.scan, pos)
+    torch.cuda.synchronize()
+    assert (it.cpu().numpy().view(np.uint16) == 0xFFFF).mean() > 0.5          # not converged, and flagged so
+    e, a = eig.cpu().numpy().astype(np.float64), alone.cpu().numpy().astype(np.float64)
+    # the stand-alone kernel sees the FP32-rounded position (half an ulp of ~10 Å = 5e-7 Å = 2.4e-6 of a 0.2 Å cell); deep
+    # in the repulsive wall, where nothing has relaxed, J changes by its own size across a cell: allow 1e-5 of the
+    # sample's largest |lambda| on top of the map's tolerance
+    scale = np.abs(a[..., :3]).max(axis=-1, keepdims=True)
+    excess = np.abs(e - a)[..., :3] - (1e-5 + 1e-5 * np.abs(a[..., :3]) + 1e-5 * scale)
+    assert np.all(np.isfinite(e)) and excess.max() <= 0, (excess.max(), np.abs(e - a)[..., :3].max(), scale.max())
