@@ -537,10 +537,21 @@ ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const FFFlags *__rest
     __shared__ FFFlags s_flags;
 
     const long long tile = blockIdx.x;
-    int lo = 0, hi = njobs - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (jobs[mid].tile_begin <= tile) lo = mid; else hi = mid - 1;
+    // the system this tile belongs to: with equal tile counts per system (the usual batch) it is tile * njobs / ntiles,
+    // checked with two independent loads; otherwise a binary search (log2(njobs) dependent loads, ~0.3 us each from
+    // L2, which a CTA of a 35-atom molecule would spend a fifth of its life on)
+    int lo = (int)((tile * njobs) / gridDim.x);
+    {
+        const long long b0 = jobs[lo].tile_begin;
+        const long long b1 = (lo + 1 < njobs) ? jobs[lo + 1].tile_begin : (long long)gridDim.x;
+        if (!(b0 <= tile && tile < b1)) {
+            int hi = njobs - 1;
+            lo = 0;
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (jobs[mid].tile_begin <= tile) lo = mid; else hi = mid - 1;
+            }
+        }
     }
     {
         const int *srcw = reinterpret_cast<const int *>(&jobs[lo]);
@@ -572,11 +583,11 @@ static int pick_P(int nz, long long nxy_tiles, bool split) {
     // padded work ~ ceil(nz/P) * (P + per-atom overhead shared by the column, ~1.2 points: 8 scalar FP32 + 3 LDS +
     // loop control against ~16 issue slots per point).  The split kernel keeps two accumulator sets per point, so
     // it takes fewer points per thread.  Small grids take the smallest P that still gives every SM two CTAs.
-    const int cand_one[3] = {20, 10, 8}, cand_two[3] = {10, 8, 6};
+    const int cand_one[4] = {20, 16, 10, 8}, cand_two[4] = {10, 8, 6, 6};
     const int *cand = split ? cand_two : cand_one;
     int best = cand[0];
     double best_cost = 1e300;
-    for (int c = 0; c < 3; c++) {
+    for (int c = 0; c < 4; c++) {
         const int P = cand[c];
         const long long ctas = nxy_tiles * ((nz + P - 1) / P);
         double cost = (double)((nz + P - 1) / P) * (P + 1.2);
@@ -602,6 +613,7 @@ static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st
     else if (P == 8) launch_ff_one<SPLIT, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else if (P == 10) launch_ff_one<SPLIT, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else if constexpr (SPLIT) launch_ff_one<true, 6, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 16) launch_ff_one<false, 16, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else launch_ff_one<false, 20, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     return cudaGetLastError();
 }
