@@ -169,6 +169,7 @@ __device__ __forceinline__ void prep_system(const FFJob &job, const TypeEntry *_
         if (live) {
             const int q_before = run_q + before + in_warp;             // charged atoms ahead of atom i
             const int pos = charged ? q_before : nq + (i - q_before);
+            PPFM_CHK(PPFM_CHK_FF_STORE, pos >= 0 && pos < n);
             recs[job.atom_begin + pos] = r;
         }
         run_q += chunk_total;

@@ -905,6 +905,9 @@ stiffness_kernel(const RelaxJob *__restrict__ jobs, int njobs, long long nsample
     const long long nx = job.n[0], nxy = (long long)job.n[0] * job.n[1];
     const float4 *r00 = g + cz.i0 * nxy + cy.i0 * nx, *r01 = g + cz.i0 * nxy + cy.i1 * nx;
     const float4 *r10 = g + cz.i1 * nxy + cy.i0 * nx, *r11 = g + cz.i1 * nxy + cy.i1 * nx;
+    PPFM_CHK(PPFM_CHK_RELAX_GATHER, cx.i0 >= 0 && cx.i0 < job.n[0] && cx.i1 >= 0 && cx.i1 < job.n[0] && cy.i0 >= 0 &&
+                                        cy.i0 < job.n[1] && cy.i1 >= 0 && cy.i1 < job.n[1] && cz.i0 >= 0 && cz.i0 < job.n[2] &&
+                                        cz.i1 >= 0 && cz.i1 < job.n[2]);
     const float4 c000 = __ldg(r00 + cx.i0), c001 = __ldg(r00 + cx.i1), c010 = __ldg(r01 + cx.i0), c011 = __ldg(r01 + cx.i1);
     const float4 c100 = __ldg(r10 + cx.i0), c101 = __ldg(r10 + cx.i1), c110 = __ldg(r11 + cx.i0), c111 = __ldg(r11 + cx.i1);
     // G[c][a] = dF_c/dt_a inside the cell (FP32): difference along axis a, tri-linear weights on the other two

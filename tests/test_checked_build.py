@@ -15,7 +15,8 @@ SELECT = ("test_ff_ragged_tiles_and_tails or test_ff_charged_neutral_partition o
           "test_ff_batch_cfg3_matches_oracle_and_single_calls or test_relax_every_kernel_instance or "
           "test_relax_periodic_wrap_and_clamp or test_relax_zero_field_and_ragged_scan or "
           "test_relax_tricubic_periodic_skewed_batch_and_edges or test_df_column_and_gather_kernels_all_window_lengths or "
-          "test_relax_scan_stiffness_closed_forms or test_scan_host_equals_device_path or "
+          "test_relax_scan_stiffness_closed_forms or test_stiffness_zero_field_periodic_nonorthogonal_and_batch or "
+          "test_scan_host_equals_device_path or "
           "(test_relax_and_df_full_scan and 0)")
 
 
