@@ -294,7 +294,9 @@ int ppfm_scan_host_batch(int32_t nsys, const int32_t *h_atom_offset, const float
 
 /* Tip-charge sweep (the LJ and electrostatic grids are separate so that the tip charge can change
  * without recomputation; reading S19): F_LJ and the unit-charge F_el are sampled once, then for each of the nQ
- * charges h_Q[i] the grids are combined and the scan + df run.  Outputs hold nQ consecutive result sets:
+ * charges h_Q[i] the grids are combined and the scan + df run (the nQ scans as one batch launch while the nQ combined
+ * grids fit 8 GiB of scratch, one after the other beyond that; the results do not depend on which).  Outputs hold nQ
+ * consecutive result sets:
  * h_pos_fz float[nQ][nz][npy][npx][4], h_iters uint16[nQ][nz][npy][npx], h_df float[nQ][nz-n][npy][npx]; h_stats
  * accumulates over the sweep.  probe->Q is ignored. */
 int ppfm_scan_host_sweep(int32_t nQ, const double *h_Q, int32_t natoms, const float *h_xyzq, const int32_t *h_type,

@@ -212,19 +212,25 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
 #define TRY(x) if (rc == PPFM_OK && (e = (x)) != cudaSuccess) fail(e, #x)
     TRY(scratch_alloc((void **)&d_xyzq, na * 16, st));
     TRY(scratch_alloc((void **)&d_type, na * 4, st));
-    TRY(scratch_alloc((void **)&d_ff, npts * 16, st));
+    // Q sweep (S19): the nQ combined grids are kept side by side and the nQ scans run as ONE batch launch (a single
+    // 200 x 200 scan cannot fill the GPU: 1250 warps on 592 sub-partitions; three at once can), as long as the grids fit
+    // the budget below; otherwise one scan after the other on one combined grid.
+    const size_t sweep_budget = (size_t)8 << 30;
+    const bool sweep_batched = nQ > 1 && (size_t)nQ * npts * 16 <= sweep_budget;
+    const size_t nff = sweep_batched ? (size_t)nQ : 1;
+    TRY(scratch_alloc((void **)&d_ff, nff * npts * 16, st));
     if (nQ > 0) {
         TRY(scratch_alloc((void **)&d_lj, npts * 16, st));
         TRY(scratch_alloc((void **)&d_el, npts * 16, st));
     }
     TRY(scratch_alloc((void **)&d_stats, sizeof(ppfm_stats), st));
     if (zc) {
-        if (h_df) TRY(scratch_alloc((void **)&d_fz, nps * 4, st));
-        if (h_iters) TRY(scratch_alloc((void **)&d_it, nps * 2, st));
+        if (h_df) TRY(scratch_alloc((void **)&d_fz, nff * nps * 4, st));
+        if (h_iters) TRY(scratch_alloc((void **)&d_it, nff * nps * 2, st));
     } else {
-        TRY(scratch_alloc((void **)&d_pos, nps * 16, st));
-        TRY(scratch_alloc((void **)&d_it, nps * 2, st));
-        if (h_df) TRY(scratch_alloc((void **)&d_df, ndf * 4, st));
+        TRY(scratch_alloc((void **)&d_pos, nff * nps * 16, st));
+        TRY(scratch_alloc((void **)&d_it, nff * nps * 2, st));
+        if (h_df) TRY(scratch_alloc((void **)&d_df, nff * ndf * 4, st));
     }
     if (natoms > 0) {
         TRY(cudaMemcpyAsync(d_xyzq, h_xyzq, (size_t)natoms * 16, cudaMemcpyHostToDevice, st));
@@ -241,26 +247,41 @@ static int scan_host_impl(int nsys, const int32_t *h_atom_offset, const float *h
                              : ppfm_forcefield_batch(nsys, h_atom_offset, d_xyzq, d_type, ntypes, h_R, h_e, lattices,
                                                      probes, grids, r_min, d_ff, nullptr, cuda_stream);
     }
-    for (int run = 0; run < nrun; run++) {
-        if (rc == PPFM_OK && nQ > 0) rc = ppfm_combine(d_lj, d_el, h_Q[run], (int64_t)npts, d_ff, cuda_stream);
-        const size_t op = (size_t)run * nps, od = (size_t)run * ndf;      // this run's slice of the host outputs
+    // one pass of (relaxation, df, copies) over `nb` systems laid out consecutively (grids at d_ff) that together make
+    // `sets` result sets of nps pixel-steps / ndf df samples, written at the host offsets op / od
+    auto scan_pass = [&](int nb, const ppfm_grid *g, const ppfm_tip *t, const ppfm_scan *sc, size_t sets, size_t op, size_t od) {
+        const size_t tot_ps = sets * nps, tot_df = sets * ndf;
         if (zc) {
             if (rc == PPFM_OK)
-                rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, m_pos + 4 * op, h_iters ? d_it : nullptr,
-                                   d_stats, d_fz, cuda_stream);
-            if (h_iters) TRY(cudaMemcpyAsync(h_iters + op, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
+                rc = relax_scan_fz(nb, d_ff, g, t, fire, sc, m_pos + 4 * op, h_iters ? d_it : nullptr, d_stats, d_fz,
+                                   cuda_stream);
+            if (h_iters) TRY(cudaMemcpyAsync(h_iters + op, d_it, tot_ps * 2, cudaMemcpyDeviceToHost, st));
             if (rc == PPFM_OK && h_df)
-                rc = df_from_fz(nsys, d_fz, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, m_df + od,
+                rc = df_from_fz(nb, d_fz, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, m_df + od,
                                 cuda_stream);
         } else {
             if (rc == PPFM_OK)
-                rc = relax_scan_fz(nsys, d_ff, grids, tips, fire, scans, d_pos, d_it, d_stats, nullptr, cuda_stream);
+                rc = relax_scan_fz(nb, d_ff, g, t, fire, sc, d_pos, d_it, d_stats, nullptr, cuda_stream);
             if (rc == PPFM_OK && h_df)
-                rc = ppfm_df_batch(nsys, d_pos, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, d_df,
+                rc = ppfm_df_batch(nb, d_pos, scan->npx, scan->npy, scan->nz, scan->dz, A, k0_Nm, f0_Hz, d_df,
                                    cuda_stream);
-            if (h_pos_fz) TRY(cudaMemcpyAsync(h_pos_fz + 4 * op, d_pos, nps * 16, cudaMemcpyDeviceToHost, st));
-            if (h_iters) TRY(cudaMemcpyAsync(h_iters + op, d_it, nps * 2, cudaMemcpyDeviceToHost, st));
-            if (h_df) TRY(cudaMemcpyAsync(h_df + od, d_df, ndf * 4, cudaMemcpyDeviceToHost, st));
+            if (h_pos_fz) TRY(cudaMemcpyAsync(h_pos_fz + 4 * op, d_pos, tot_ps * 16, cudaMemcpyDeviceToHost, st));
+            if (h_iters) TRY(cudaMemcpyAsync(h_iters + op, d_it, tot_ps * 2, cudaMemcpyDeviceToHost, st));
+            if (h_df) TRY(cudaMemcpyAsync(h_df + od, d_df, tot_df * 4, cudaMemcpyDeviceToHost, st));
+        }
+    };
+    if (sweep_batched) {
+        std::vector<ppfm_grid> gs((size_t)nQ, grids[0]);
+        std::vector<ppfm_tip> ts((size_t)nQ, tips[0]);
+        std::vector<ppfm_scan> ss((size_t)nQ, scans[0]);
+        for (int run = 0; run < nQ; run++)
+            if (rc == PPFM_OK)
+                rc = ppfm_combine(d_lj, d_el, h_Q[run], (int64_t)npts, d_ff + (size_t)run * npts * 4, cuda_stream);
+        scan_pass(nQ, gs.data(), ts.data(), ss.data(), (size_t)nQ, 0, 0);   // nsys == 1: nQ systems = nQ result sets
+    } else {
+        for (int run = 0; run < nrun; run++) {
+            if (rc == PPFM_OK && nQ > 0) rc = ppfm_combine(d_lj, d_el, h_Q[run], (int64_t)npts, d_ff, cuda_stream);
+            scan_pass(nsys, grids, tips, scans, 1, (size_t)run * nps, (size_t)run * ndf);   // this run's slice of the outputs
         }
     }
     if (h_stats) TRY(cudaMemcpyAsync(h_stats, d_stats, sizeof(ppfm_stats), cudaMemcpyDeviceToHost, st));
