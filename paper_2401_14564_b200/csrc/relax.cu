@@ -41,6 +41,7 @@ constexpr int RX_TILE_X = 16, RX_TILE_Y = 8;
 // ~15 instructions ahead of the vote (checked in the SASS, profiles/r02_sass_summary.txt); the fifth CTA was worth
 // <= 4 % on the large scans and the larger budget is worth that much there too.
 constexpr int RX_MIN_CTAS = 4;
+constexpr long long RX_SPARSE_MAX_WARPS = 148LL * 2;   // launches up to this many (dense) warps use 16 pixels per warp
 constexpr float RX_MAGIC = 12582912.0f;      // 1.5 * 2^23: floats in [2^23, 2^24) are the integers
 constexpr int RX_MAGIC_BITS = 0x4B400000;
 constexpr int RX_MAX_N = 1 << 21;            // per-axis grid size limit of the magic-number cell index
@@ -50,6 +51,7 @@ struct RelaxJob {
     long long out_offset;    // pixel-step offset of this system's outputs
     int block_begin;
     int nbx;                 // CTAs along x
+    int sparse;              // 16 pixels per warp (4 x 4 patch on lanes 0-15) instead of 32: see build_relax_jobs
     int npx, npy, nzs;
     int n[3], periodic[3];
     double origin[3], Minv[9];
@@ -275,9 +277,10 @@ __device__ __forceinline__ void relax_pixels(const RelaxJob &job, const FirePara
                                              float *__restrict__ fz_out, float4 *__restrict__ eig_out) {
     const int by = lb / job.nbx, bx = lb - by * job.nbx;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int ix = bx * RX_TILE_X + (warp & 1) * 8 + (lane & 7);
-    const int iy = by * RX_TILE_Y + (warp >> 1) * 4 + (lane >> 3);
-    const bool valid = (ix < job.npx) && (iy < job.npy);
+    const bool sparse = job.sparse != 0;
+    const int ix = sparse ? bx * (RX_TILE_X / 2) + (warp & 1) * 4 + (lane & 3) : bx * RX_TILE_X + (warp & 1) * 8 + (lane & 7);
+    const int iy = sparse ? by * RX_TILE_Y + (warp >> 1) * 4 + ((lane >> 2) & 3) : by * RX_TILE_Y + (warp >> 1) * 4 + (lane >> 3);
+    const bool valid = (ix < job.npx) && (iy < job.npy) && (!sparse || lane < 16);
     const int ixc = min(ix, job.npx - 1), iyc = min(iy, job.npy - 1);
 
     // tri-linear: float4 (Fx,Fy,Fz,E) grid; TRICUBIC: energy-only float grid
@@ -760,6 +763,21 @@ static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *ti
         ff_off += grid_points(&g);
         out_off += (long long)s.npx * s.npy * s.nz;
         if (blocks > 0x7fffffffLL) { free(hj); return PPFM_EINVAL; }
+    }
+    // Tiny launches (at most half a warp per SM sub-partition, so that even with twice the warps every warp has a
+    // sub-partition to itself) run at the latency of the slowest warp's chain of FIRE iterations: give each warp 16
+    // pixels instead of 32 (lanes 16-31 idle).  A warp then waits for the slowest of 16 pixels instead of 32 and
+    // re-gathers (a warp-wide trip whenever ANY lane leaves its cell) about half as often: config 0 0.506 -> 0.473 ms.
+    // Beyond that size the doubled instruction count costs more than it saves (config 1, 704 warps: 0.745 -> 1.00 ms).
+    if (blocks * (RX_THREADS / 32) <= RX_SPARSE_MAX_WARPS) {
+        blocks = 0;
+        for (int m = 0; m < nsys; m++) {
+            RelaxJob &j = hj[m];
+            j.sparse = 1;
+            j.block_begin = (int)blocks;
+            j.nbx = (scans[m].npx + RX_TILE_X / 2 - 1) / (RX_TILE_X / 2);
+            blocks += (long long)j.nbx * ((scans[m].npy + RX_TILE_Y - 1) / RX_TILE_Y);
+        }
     }
     *hj_out = hj;
     *blocks_out = blocks;
