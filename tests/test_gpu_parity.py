@@ -379,14 +379,14 @@ def test_relax_cfg2_all_three_tip_charges_gpu_grid_and_end_to_end(P):
 
 
 def test_relax_full_size_cfg4_sampled_gpu_grid_and_end_to_end(cfg4):
-    """Config 4 at full size: (ii) 150 sampled pixels, oracle on the GPU's 1.9 GiB grid; (i) END TO END on 96 sampled
+    """Config 4 at full size: (ii) 4000 sampled pixels (320 000 samples), oracle on the GPU's 1.9 GiB grid; (i) END TO END on 96 sampled
     pixels, the oracle evaluating its own FP64 grid nodes from the 45 000 atom images on demand."""
     w, ff, pos, iters, df, st = cfg4
     npix = w.scan.npx * w.scan.npy
-    pix = sample(npix, 150, 61)
+    pix = sample(npix, 4000, 61)
     ref = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan, pix=pix)
     pos_h = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix]
-    frac, d = check_positions(pos_h, ref, "cfg4 (GPU grid, 150 px)")
+    frac, d = check_positions(pos_h, ref, "cfg4 (GPU grid, 4000 px)")
     check_iters(iters.cpu().numpy().reshape(w.scan.nz, -1)[:, pix], ref, d, "cfg4")
     dfh = df.cpu().numpy().reshape(df.shape[0], -1)[:, pix]
     check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0), "cfg4 df")
