@@ -1283,3 +1283,38 @@ def test_full_size_full_coverage_cfg2_and_cfg3(P):
     frac, d = check_positions(pos[:nps].cpu().numpy().reshape(w.scan.nz, npix, 4), ref, "cfg2 full scan (end to end)")
     check_iters(iters[:nps].cpu().numpy(), ref, d, "cfg2 full scan")
     check_df_end_to_end(df[0].cpu().numpy(), ref, d, w, "cfg2 full scan")
+
+
+def test_relax_batch_cfg3_all_64_molecules_in_the_bench_launch(P):
+    """Config 3 as bench.py launches it (64 molecules, one batch launch each of a2, a5, a6): every molecule's scan on
+    150 sampled pixels against the oracle on the same grid, move counts and df included (the end-to-end chain on the
+    oracle's own grid is test_relax_batch_cfg3's, the full force-field grids test_full_size_full_coverage's)."""
+    import torch
+    mols = W.get(3)
+    off = np.concatenate([[0], np.cumsum([m.natoms for m in mols])])
+    xyzq = torch.from_numpy(np.concatenate([m.xyzq for m in mols])).cuda()
+    types = torch.from_numpy(np.concatenate([m.types for m in mols])).cuda()
+    ff = P.forcefield_batch(off, xyzq, types, mols[0].elem_R, mols[0].elem_e, [m.lattice for m in mols],
+                            [m.probe for m in mols], [m.grid for m in mols], mols[0].r_min)
+    stats = P.new_stats()
+    pos, iters = P.relax_scan_batch(ff, [m.grid for m in mols], [m.tip for m in mols], mols[0].fire,
+                                    [m.scan for m in mols], stats=stats)
+    s = mols[0].scan
+    df = P.df(pos, s.npx, s.npy, s.nz, s.dz, mols[0].df.A, mols[0].df.k0, mols[0].df.f0, nsys=len(mols))
+    torch.cuda.synchronize()
+    nps, npts = s.npx * s.npy * s.nz, mols[0].npoints
+    fails = 0
+    for m, mol in enumerate(mols):
+        pix = sample(s.npx * s.npy, 150, 700 + m)
+        g = mol.grid
+        grid_h = ff[m * npts:(m + 1) * npts].cpu().numpy().reshape(g.n[2], g.n[1], g.n[0], 4)
+        ref = oracle.relax_scan(grid_h, g, mol.tip, mol.fire, mol.scan, pix=pix)
+        pos_h = pos[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1, 4)[:, pix]
+        frac, d = check_positions(pos_h, ref, f"cfg3 mol {m} of 64 (GPU grid, 150 px)")
+        fails += int((d > 2e-3).sum())
+        check_iters(iters[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1)[:, pix], ref, d, f"cfg3 mol {m}")
+        dfh = df[m].cpu().numpy().reshape(df.shape[1], -1)[:, pix]
+        check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), s.dz, mol.df.A, mol.df.k0, mol.df.f0), f"cfg3 df {m}")
+    st = P.read_stats(stats)
+    assert st["n_clamped"] == 0 and st["n_not_converged"] <= 1e-4 * nps * len(mols)
+    print(f"cfg3: 64 molecules x 150 px x {s.nz} z-steps, {fails} samples outside 2e-3 A (all exempt)")
