@@ -50,7 +50,9 @@ typedef enum {
     PPFM_OK = 0,
     PPFM_EINVAL = -1, /* null pointer, n <= 0, singular step matrix, A/dz not an integer, nz <= n, bad type index */
     PPFM_ECUDA = -2,  /* CUDA runtime / launch error; text via ppfm_strerror(PPFM_ECUDA) (thread-local)          */
-    PPFM_ENOMEM = -3  /* scratch allocation failed                                                              */
+    PPFM_ENOMEM = -3, /* scratch allocation failed                                                              */
+    PPFM_ELIMIT = -4  /* input larger than the fixed scratch of an entry point that allocates nothing
+                         (ppfm_forcefield_noalloc: natoms > PPFM_NOALLOC_MAX_ATOMS)                             */
 } ppfm_status;
 
 /* Supercell vectors (Å) and periodic images: the sum runs over shifts na*a + nb*b + nc*c with
@@ -155,6 +157,44 @@ int ppfm_forcefield_batch(int32_t nsys, const int32_t *h_atom_offset, const floa
                           int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattices,
                           const ppfm_probe *probes, const ppfm_grid *grids, double r_min, float *d_ff,
                           ppfm_ff_status *d_status, void *cuda_stream);
+
+/* ---- (1') the same force-field pass for callers that must not allocate ---------------------------------------
+ * Who this is for.  ppfm_forcefield takes its per-call scratch (the packed atom records and two per-system flags
+ * that its set-up kernel writes and its grid kernel reads) from a stream-ordered memory pool.  Some callers cannot
+ * tolerate that: code that runs under a fixed memory budget where every byte of the device has been handed out
+ * beforehand (an inference / simulation server that pre-allocates its arena and treats any later allocation as a
+ * fault), a real-time acquisition loop next to the microscope that must not hit an allocator lock or a driver call
+ * of unbounded latency, and hosts embedding the library behind an allocator hook that forbids cudaMalloc* outside
+ * start-up.  For them this entry point computes exactly what ppfm_forcefield computes (same kernels, same
+ * summation order, bit-identical grid) but keeps the scratch in a fixed array inside the library image.
+ *
+ *   Limit:     natoms <= PPFM_NOALLOC_MAX_ATOMS (16384; the paper's largest systems are a few thousand atoms).
+ *              More atoms: PPFM_ELIMIT, nothing is launched and nothing is written.  The grid size is not limited
+ *              (the grid is the caller's buffer).
+ *   Cost:      PPFM_NOALLOC_SCRATCH_BYTES (768 KiB + 256 B) of device memory on EVERY GPU on which the library is
+ *              loaded, from the moment its code is loaded there until the process exits, whether or not this
+ *              entry point is ever called.
+ *   No allocation: the call makes no cudaMalloc / cudaMallocAsync / cudaFree / pool call, no host malloc, and calls
+ *              no library routine that allocates; the optional per-kernel timers of ppfm_bench.h do not see its
+ *              launches (they would create events).  It enqueues one 8-byte memset, the status memset if d_status
+ *              is given, and the two kernels on `cuda_stream`, and returns without synchronising.
+ *   First call on a device: looks up the device address of the scratch array (cudaGetSymbolAddress, once per
+ *              device, with that device current — the caller must have made the device current, as for every other
+ *              entry point) and remembers it.  That look-up may load the library's device code; make this first
+ *              call during start-up, before any stream capture is begun.
+ *   Sharing:   there is ONE array per device and every call on that device uses it.  The array keeps what the
+ *              previous call left; the call re-zeroes the flags it depends on and overwrites the records it reads,
+ *              so calls that follow one another on one stream are independent.  Two calls whose kernels can
+ *              overlap on the GPU (different streams, or different host threads on different streams) RACE on the
+ *              array and produce garbage: order them yourself (one stream, or events).  ppfm_forcefield has no
+ *              such restriction.
+ *   Arguments, layouts and the other error codes are those of ppfm_forcefield. */
+#define PPFM_NOALLOC_MAX_ATOMS 16384
+#define PPFM_NOALLOC_SCRATCH_BYTES (256 + 48 * PPFM_NOALLOC_MAX_ATOMS)
+int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                            const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                            const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
+                            ppfm_ff_status *d_status, void *cuda_stream);
 
 /* ---- (2) relaxation scan: Eq.1 + Eq.2 + FIRE on the tri-linearly interpolated grid --
  * d_ff      DEVICE grid as written by ppfm_forcefield (read-only)

@@ -98,6 +98,7 @@ extern "C" const char *ppfm_strerror(int code) {
         case PPFM_EINVAL: return "invalid argument";
         case PPFM_ECUDA: return g_cuda_msg;
         case PPFM_ENOMEM: return "device scratch allocation failed";
+        case PPFM_ELIMIT: return "input exceeds the fixed scratch of a no-allocation entry point (natoms > PPFM_NOALLOC_MAX_ATOMS)";
         default: return "unknown status";
     }
 }

@@ -809,3 +809,158 @@ extern "C" int ppfm_combine(const float *d_ff_lj, const float *d_ff_el, double Q
     PPFM_LAUNCH_CHECK();
     return PPFM_OK;
 }
+
+// ------------------------------------------------------------------------- (1') the pass without any allocation
+// ppfm_forcefield_noalloc (include/ppfm.h): for callers that may not allocate after start-up (a pre-carved device
+// arena, a real-time loop, an allocator hook that forbids cudaMalloc*).  It runs ff_prep_kernel and ff_kernel, the
+// kernels of ppfm_forcefield, but the scratch those two share — the FFFlags the prep kernel writes and the packed
+// AtomRec array — lives in the file-scope device array below instead of a pool allocation.  Every GPU that loads this
+// library's device code holds the array until the process exits.
+//
+// `g_noalloc_scratch` names device memory only inside device code.  In host code the same identifier is a host-side
+// handle of the symbol, NOT a device address: handing it to a kernel would fault (or, on a system where the GPU can
+// reach host memory, quietly read and write the wrong bytes).  The host gets the real address from
+// cudaGetSymbolAddress, once per device with that device current (noalloc_scratch_ptr), and passes that to the kernels.
+namespace ppfm {
+
+constexpr size_t NOALLOC_RECS_OFF = 256;      // [FFFlags, padding to 256 B][AtomRec x PPFM_NOALLOC_MAX_ATOMS]
+static_assert(sizeof(FFFlags) <= NOALLOC_RECS_OFF, "flags must fit ahead of the records");
+static_assert(PPFM_NOALLOC_SCRATCH_BYTES == NOALLOC_RECS_OFF + sizeof(AtomRec) * PPFM_NOALLOC_MAX_ATOMS,
+              "PPFM_NOALLOC_SCRATCH_BYTES (ppfm.h) must describe this layout");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[PPFM_NOALLOC_SCRATCH_BYTES];
+
+static std::atomic<unsigned char *> g_noalloc_ptr[64];      // per device ordinal; zero-initialised (static storage)
+
+// Device address of g_noalloc_scratch on the CURRENT device.  The first call on a device asks the runtime (which may
+// load this library's device code on that device: do it before any stream capture); later calls read the cached
+// pointer.  Two threads racing through the first call both get the same answer from the runtime, so a plain atomic
+// store is enough and no lock is taken on the steady-state path.
+static cudaError_t noalloc_scratch_ptr(unsigned char **out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    unsigned char *p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        void *sym = nullptr;
+        e = cudaGetSymbolAddress(&sym, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!sym) return cudaErrorInvalidSymbol;
+        p = static_cast<unsigned char *>(sym);
+        g_noalloc_ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+// launch_ff's dispatch for one system and one output grid, without its KernelTimer (which creates CUDA events when
+// the ppfm_bench.h timers are on — an allocation this path must not make)
+static cudaError_t launch_ff_noalloc(int P, bool zcol, long long ntiles, cudaStream_t st, const FFJob *hj,
+                                     const FFFlags *flags, const AtomRec *recs, float4 *out) {
+    if (!zcol) launch_ff_one<false, 4, false>(ntiles, st, hj, nullptr, 1, flags, recs, out, nullptr);
+    else if (P == 8) launch_ff_one<false, 8, true>(ntiles, st, hj, nullptr, 1, flags, recs, out, nullptr);
+    else if (P == 10) launch_ff_one<false, 10, true>(ntiles, st, hj, nullptr, 1, flags, recs, out, nullptr);
+    else if (P == 16) launch_ff_one<false, 16, true>(ntiles, st, hj, nullptr, 1, flags, recs, out, nullptr);
+    else launch_ff_one<false, 20, true>(ntiles, st, hj, nullptr, 1, flags, recs, out, nullptr);
+    return cudaGetLastError();
+}
+
+}  // namespace ppfm
+
+extern "C" int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                                       const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                                       const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
+                                       ppfm_ff_status *d_status, void *cuda_stream) {
+    // the argument checks of ppfm_forcefield (forcefield_impl with nsys = 1, one grid)
+    if (natoms < 0 || !h_R || !h_e || !lattice || !probe || !grid || !d_ff) return PPFM_EINVAL;
+    if (natoms > 0 && (!d_xyzq || !d_type)) return PPFM_EINVAL;
+    if (ntypes < 1 || ntypes > PPFM_MAX_TYPES) return PPFM_EINVAL;
+    if (!(r_min >= 0.0) || !std::isfinite(r_min)) return PPFM_EINVAL;
+    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_ff & 15) || ((uintptr_t)d_status & 3)) return PPFM_EINVAL;
+    for (int t = 0; t < ntypes; t++)
+        if (!(h_R[t] >= 0.0) || !(h_e[t] >= 0.0) || !std::isfinite(h_R[t]) || !std::isfinite(h_e[t])) return PPFM_EINVAL;
+    if (!grid_ok(grid)) return PPFM_EINVAL;
+    if (!(probe->R >= 0.0) || !(probe->e >= 0.0) || !std::isfinite(probe->R) || !std::isfinite(probe->e) ||
+        !std::isfinite(probe->Q))
+        return PPFM_EINVAL;
+    for (int a = 0; a < 3; a++)
+        if (lattice->nimg[a] < 0 || lattice->nimg[a] > 64) return PPFM_EINVAL;
+    // the one limit this entry point adds: the records must fit the fixed array
+    if (natoms > PPFM_NOALLOC_MAX_ATOMS) return PPFM_ELIMIT;
+
+    const ppfm_grid &g = *grid;
+    const bool zcol = (g.step[2][0] == 0.0 && g.step[2][1] == 0.0);
+    const long long nxy_tiles = ((long long)g.n[0] * g.n[1] + FF_THREADS - 1) / FF_THREADS;
+    const int P = zcol ? pick_P(g.n[2], nxy_tiles, false) : 4;      // the choice ppfm_forcefield makes: same bits
+
+    // the system's description travels as a kernel parameter: it lives on this stack frame, not on the heap
+    FFSingle one;
+    memset(&one, 0, sizeof(one));
+    FFJob &j = one.job;
+    j.tile_begin = 0;
+    j.out_offset = 0;
+    j.atom_begin = 0;
+    j.natoms = natoms;
+    j.nx = g.n[0]; j.ny = g.n[1]; j.nz = g.n[2]; j.nxy = g.n[0] * g.n[1];
+    j.n_xy_tiles = (j.nxy + FF_THREADS - 1) / FF_THREADS;
+    j.n_z_groups = (j.nz + P - 1) / P;
+    j.table_offset = 0;
+    j.ntypes = ntypes;
+    j.split = 0;
+    for (int a = 0; a < 3; a++) {
+        j.nimg[a] = lattice->nimg[a];
+        j.origin[a] = g.origin[a];
+        for (int c = 0; c < 3; c++) j.step[a][c] = g.step[a][c];
+        j.cell[0][a] = lattice->a[a];
+        j.cell[1][a] = lattice->b[a];
+        j.cell[2][a] = lattice->c[a];
+    }
+    for (int c = 0; c < 3; c++) {      // Cartesian bounding box of the grid (decides whether the r_min clamp is live)
+        double lo = g.origin[c], hi = g.origin[c];
+        for (int corner = 1; corner < 8; corner++) {
+            double x = g.origin[c];
+            for (int a = 0; a < 3; a++)
+                if (corner & (1 << a)) x += (g.n[a] - 1) * g.step[a][c];
+            lo = std::fmin(lo, x); hi = std::fmax(hi, x);
+        }
+        j.bb_lo[c] = lo; j.bb_hi[c] = hi;
+    }
+    j.keQ = (float)(kCoulomb * probe->Q);
+    j.rmin2 = (float)(r_min * r_min);
+    for (int t = 0; t < ntypes; t++) {   // mixing rules
+        const double R0 = h_R[t] + probe->R;
+        const double E0 = std::sqrt(h_e[t] * probe->e);
+        const double R6 = R0 * R0 * R0 * R0 * R0 * R0;
+        one.table[t].c6 = (float)(2.0 * E0 * R6);
+        one.table[t].c12 = (float)(E0 * R6 * R6);
+    }
+    const long long ntiles = (long long)j.n_xy_tiles * j.n_z_groups;
+    if (ntiles > 0x7fffffffLL) return PPFM_EINVAL;
+
+    unsigned char *d_scratch = nullptr;
+    cudaError_t e = noalloc_scratch_ptr(&d_scratch);
+    if (e != cudaSuccess) { set_cuda_error(e, "cudaGetSymbolAddress(g_noalloc_scratch)"); return PPFM_ECUDA; }
+    FFFlags *dflags = reinterpret_cast<FFFlags *>(d_scratch);
+    AtomRec *drecs = reinterpret_cast<AtomRec *>(d_scratch + NOALLOC_RECS_OFF);
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // The array still holds the previous call's flags and records.  The flags must read zero when no prep kernel runs
+    // (natoms = 0), so they are cleared every call; records [0, natoms) are all rewritten by the prep kernel and no
+    // record beyond natoms is ever read.
+    e = cudaMemsetAsync(dflags, 0, sizeof(FFFlags), st);
+    if (e == cudaSuccess && d_status) e = cudaMemsetAsync(d_status, 0, sizeof(ppfm_ff_status), st);
+    if (e != cudaSuccess) { set_cuda_error(e, "noalloc flag reset"); return PPFM_ECUDA; }
+    if (natoms > 0) {
+        ff_prep_kernel<<<1, PREP_THREADS, 0, st>>>(one, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs, dflags,
+                                                   d_status);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { set_cuda_error(e, "ff_prep_kernel (noalloc)"); return PPFM_ECUDA; }
+        count_launch();
+    }
+    if (ntiles > 0) {
+        e = launch_ff_noalloc(P, zcol, ntiles, st, &one.job, dflags, drecs, reinterpret_cast<float4 *>(d_ff));
+        if (e != cudaSuccess) { set_cuda_error(e, "ff_kernel (noalloc)"); return PPFM_ECUDA; }
+        count_launch();
+    }
+    return PPFM_OK;
+}

@@ -63,6 +63,7 @@ class Stats(C.Structure):
 
 # the product ABI (include/ppfm.h); the measurement interface of include/ppfm_bench.h is bound in ppfm_bench.py
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
+           "ppfm_forcefield_noalloc",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft",
            "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_stiffness",
            "ppfm_relax_scan_stiffness_batch", "ppfm_relax_scan_tricubic",
@@ -222,6 +223,37 @@ def forcefield(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out
                                C.byref(c_grid(grid)), C.c_double(r_min), _dptr(out, torch.float32), _dptr(status),
                                _stream())
     _check(rc, "ppfm_forcefield")
+    return out
+
+
+NOALLOC_MAX_ATOMS = 16384       # PPFM_NOALLOC_MAX_ATOMS (include/ppfm.h)
+ELIMIT = -4                     # PPFM_ELIMIT
+
+
+def forcefield_noalloc(xyzq, types, elem_R, elem_e, lattice, probe, grid, out, r_min=0.1, Q=None, status=None):
+    """ppfm_forcefield_noalloc: ppfm_forcefield for callers that must not allocate device memory once they are
+    running (a process whose GPU memory was carved up at start-up, a real-time loop that cannot wait on an allocator
+    or the driver, a host whose allocator hook forbids cudaMalloc* after initialisation).  Same kernels and the same
+    bits as `forcefield`, but the library's scratch is a fixed 768 KiB array inside the library, so:
+
+    * at most NOALLOC_MAX_ATOMS (16384) atoms — more raises PpfmError with PPFM_ELIMIT and nothing runs;
+    * `out` is required (a (nz, ny, nx, 4) float32 CUDA tensor): this wrapper allocates nothing on the device either;
+    * every call on a device shares that one array: calls that can overlap on the GPU (different streams) race —
+      keep them on one stream or order them with events;
+    * the first call on a device looks the array's address up (and may load the library's device code): make it at
+      start-up, outside any stream capture.
+    """
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in grid.n)
+    if out is None or out.numel() != nx * ny * nz * 4 or out.dtype != torch.float32 or not out.is_contiguous():
+        raise PpfmError("forcefield_noalloc needs a contiguous float32 CUDA `out` of nz*ny*nx*4 elements")
+    R, pR = _darr(elem_R)
+    e, pe = _darr(elem_e)
+    rc = lib().ppfm_forcefield_noalloc(C.c_int32(xyzq.shape[0]), _dptr(xyzq, torch.float32),
+                                       _dptr(types, torch.int32), C.c_int32(len(R)), pR, pe,
+                                       C.byref(c_lattice(lattice)), C.byref(c_probe(probe, Q)), C.byref(c_grid(grid)),
+                                       C.c_double(r_min), _dptr(out, torch.float32), _dptr(status), _stream())
+    _check(rc, "ppfm_forcefield_noalloc")
     return out
 
 
