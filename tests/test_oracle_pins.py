@@ -552,6 +552,164 @@ def test_fire_path_move_by_move_against_independent_implementation():
     assert np.linalg.norm(force(traj[n_moves])) < fire.f_conv <= np.linalg.norm(force(traj[n_moves - 1]))
 
 
+# ---------------------------------------------------------------------------------------------------- O7
+def _fire_run(force, r0, fire, kmax, state=None):
+    """One z-step of FIRE in readings S6 / S7, written apart from the oracle AND apart from _fire_reference above in
+    one respect: the FIRE state (v, dt, alpha, n_pos) can be handed in and is handed back, so that a scan that does
+    NOT reset it between z-steps can be played.  Returns (r, moves, converged, state)."""
+    r = np.array(r0, dtype=np.float64)
+    v, dt, alpha, n_pos = (np.zeros(3), fire.dt, fire.alpha0, 0) if state is None else state
+    v = np.array(v, dtype=np.float64)
+    moves = 0
+    while True:
+        F = force(r)
+        Fn = np.sqrt(F @ F)
+        if Fn < fire.f_conv:
+            return r, moves, True, (v, dt, alpha, n_pos)
+        if moves >= kmax:
+            return r, moves, False, (v, dt, alpha, n_pos)
+        if F @ v >= 0.0:
+            v = (1.0 - alpha) * v + alpha * np.sqrt(v @ v) * F / Fn
+            if n_pos > fire.n_min:
+                dt, alpha = min(dt * fire.finc, fire.dt_max), alpha * fire.falpha
+            n_pos += 1
+        else:
+            v, dt, alpha, n_pos = np.zeros(3), dt * fire.fdec, fire.alpha0, 0
+        v = v + F * dt
+        r = r + v * dt
+        moves += 1
+
+
+def _play_scan(force_at, p0, d0, nz, dz, fire, kmax, mode):
+    """A one-pixel scan played with the independent FIRE.  mode 'carry' = reading S8 / O7 (the relaxed
+    displacement d = r_PP - r_TIP of one z-step is the start of the next, FIRE state fresh at every step); 'cold' =
+    every z-step starts again from d0; 'keep' = d carried AND the FIRE state (v, dt, alpha, n_pos) kept;
+    'position' = the relaxed POSITION carried instead of the displacement."""
+    d, state, r_prev = np.array(d0, dtype=np.float64), None, None
+    pos, its = [], []
+    for iz in range(nz):
+        rtip = np.array(p0, dtype=np.float64) - np.array([0.0, 0.0, iz * dz])
+        start = rtip + (np.array(d0) if mode == "cold" else d)
+        if mode == "position" and r_prev is not None:
+            start = r_prev
+        r, moves, conv, st = _fire_run(lambda x: force_at(x, rtip), start, fire, kmax,
+                                       state if mode == "keep" else None)
+        state, d, r_prev = st, r - rtip, r
+        pos.append(r)
+        its.append(moves if conv else -1)
+    return np.array(pos), np.array(its)
+
+
+def _affine_case():
+    """The affine sample field and asymmetric tip of the move-by-move test, as (grid, ff, tip, p0, force_at)."""
+    g = W.Grid(origin=np.zeros(3), step=np.diag([0.2, 0.2, 0.2]), n=(20, 20, 60), periodic=(0, 0, 0))
+    zz, yy, xx = np.meshgrid(np.arange(60) * 0.2, np.arange(20) * 0.2, np.arange(20) * 0.2, indexing="ij")
+    b = np.array([0.004, -0.002, -0.08])
+    M = np.array([[-0.004, 0.001, 0.0], [0.0005, -0.006, 0.002], [0.001, 0.0, 0.01]])
+    ff = np.zeros((60, 20, 20, 4))
+    for c in range(3):
+        ff[..., c] = b[c] + M[c, 0] * xx + M[c, 1] * yy + M[c, 2] * zz
+    tip = replace(W._default_tip(), k_lat=(0.012, 0.019), d0=(0.3, -0.2, -3.98))
+    d0 = np.array(tip.d0)
+    R0 = np.linalg.norm(d0)
+
+    def force_at(r, rtip):
+        d = r - rtip
+        L = np.sqrt(d @ d)
+        return (b + M @ r - tip.k_rad * (L - R0) * d / L -
+                np.array([tip.k_lat[0] * (d[0] - d0[0]), tip.k_lat[1] * (d[1] - d0[1]), 0.0]))
+
+    return g, ff, tip, np.array([1.5, 1.7, 9.0]), force_at
+
+
+def test_warm_start_between_z_steps_is_displacement_carried_with_fresh_fire_state():
+    """O7 / reading S8 ("the tip is moved down step by step and the PP is relaxed from its previous
+    position"; oracle relax_pixel: `dcur` carried, v / dt / alpha / n_pos re-initialised per z-step).  A three-step
+    scan on the affine field, each z-step cut off after k moves so that it ends UNCONVERGED and the start of the next
+    step matters at the 1e-2 Å level: the oracle must sit where the independent FIRE sits when it carries the
+    displacement and starts every step with fresh state, and must NOT sit where any of the three plausible
+    alternatives ends up (cold start from d0, FIRE state kept, position carried instead of displacement).  Then the
+    same scan run to convergence: the move count of EVERY z-step is the independent one's, and differs from the
+    cold-start and kept-state scans' counts."""
+    g, ff, tip, p0, force_at = _affine_case()
+    fire = W.Fire()
+    nz, dz = 3, 0.1
+    sc = W.Scan(p0=p0, dx=np.array([0.3, 0, 0.0]), dy=np.array([0, 0.4, 0.0]), npx=1, npy=1, nz=nz, dz=dz)
+    for k in (3, 9, 17, 40):
+        r = oracle.relax_scan(ff, g, tip, replace(fire, max_iter=k), sc)
+        got = r["pos_fz"][:, 0, :3]
+        want, its = _play_scan(force_at, p0, tip.d0, nz, dz, fire, k, "carry")
+        assert np.all(its == -1) and np.all(r["iters"][:, 0] == -1)
+        assert np.abs(got - want).max() < 1e-13, k
+        for mode in ("cold", "keep", "position"):
+            other, _ = _play_scan(force_at, p0, tip.d0, nz, dz, fire, k, mode)
+            assert np.abs(other[0] - want[0]).max() < 1e-13                      # z-step 0 is the same scan in all readings
+            assert np.linalg.norm(got[1] - other[1]) > 1e-4 and np.linalg.norm(got[2] - other[2]) > 1e-4, (k, mode)
+    # to convergence: per-step move counts
+    r = oracle.relax_scan(ff, g, tip, fire, replace(sc, nz=6))
+    want, its = _play_scan(force_at, p0, tip.d0, 6, dz, fire, 1000, "carry")
+    assert np.all(its > 0) and np.array_equal(r["iters"][:, 0], its)
+    assert np.abs(r["pos_fz"][:, 0, :3] - want).max() < 1e-13
+    assert its[0] > 100 and np.all(its[1:] < its[0])          # a warm start from 0.1 Å away needs fewer moves
+    for mode in ("cold", "keep"):
+        _, other = _play_scan(force_at, p0, tip.d0, 6, dz, fire, 1000, mode)
+        assert other[0] == its[0] and not np.array_equal(other[1:], its[1:]), mode
+
+
+def test_warm_start_keeps_the_branch_on_a_bistable_field():
+    """O7 where it changes the ANSWER, not just the path: a lateral force F_x = A(z) s(x) with s piecewise linear
+    (kinks on grid nodes: a shallow ramp, a steep ramp, then a well around x = 3.0) and A linear in z, which tri-linear
+    interpolation reproduces exactly.  With the tip over the shallow ramp (x = 2.4, k_x = 0.0156 eV/Å^2) the
+    x-equilibria follow from k (x - 2.4) = A s(x): for A > k only the well (x ~ 2.9) is stable, for 0.4 k < A < k the
+    well AND a point on the shallow ramp (x ~ 2.45) are stable, for A < 0.4 k only the ramp point.  A decreases as the
+    tip comes down.  The scan therefore falls into the well at the top, STAYS in it through the bistable window because
+    the displacement is carried (a scan restarted from d0 at every step sits on the ramp there: hysteresis), and snaps
+    back once the well equilibrium is gone.  Every z-step of the oracle is compared with the independent FIRE played
+    with carried displacement and fresh state: end point to 1e-12 Å and exact move count."""
+    h = 0.2
+    nx, ny, nzg = 21, 12, 40
+    g = W.Grid(origin=np.zeros(3), step=np.diag([h, h, h]), n=(nx, ny, nzg), periodic=(0, 0, 0))
+    xs, zs = np.arange(nx) * h, np.arange(nzg) * h
+    s_nodes = np.interp(xs, [2.0, 2.6, 2.8, 3.0, 3.2, 3.4], [0.0, 0.2, 1.0, 0.0, -1.0, 0.0])
+    tip = W._default_tip()
+    k = tip.k_lat[0]
+    a1 = 1.0 * k                                  # A(z) = k (1.6 + (z - 5.0)): 1.6 k at z = 5.0, 0.3 k at z = 3.7
+    A_nodes = k * 1.6 + a1 * (zs - 5.0)
+    ff = np.zeros((nzg, ny, nx, 4))
+    ff[..., 0] = A_nodes[:, None, None] * s_nodes[None, None, :]
+    p0 = np.array([2.4, 1.1, 9.0])
+    nz, dz = 14, 0.1
+    sc = W.Scan(p0=p0, dx=np.array([0.3, 0, 0.0]), dy=np.array([0, 0.4, 0.0]), npx=1, npy=1, nz=nz, dz=dz)
+    d0 = np.array(tip.d0)
+    R0 = np.linalg.norm(d0)
+
+    def force_at(r, rtip):
+        d = r - rtip
+        L = np.sqrt(d @ d)
+        Fs = np.array([(k * 1.6 + a1 * (r[2] - 5.0)) * np.interp(r[0], xs, s_nodes), 0.0, 0.0])
+        return Fs - tip.k_rad * (L - R0) * d / L - np.array([tip.k_lat[0] * d[0], tip.k_lat[1] * d[1], 0.0])
+
+    fire = W.Fire()
+    r = oracle.relax_scan(ff, g, tip, fire, sc)
+    got, its_o = r["pos_fz"][:, 0, :3], r["iters"][:, 0]
+    want, its = _play_scan(force_at, p0, d0, nz, dz, fire, fire.max_iter, "carry")
+    assert np.all(its > 0) and np.array_equal(its_o, its)
+    assert np.abs(got - want).max() < 1e-12
+    cold, _ = _play_scan(force_at, p0, d0, nz, dz, fire, fire.max_iter, "cold")
+    A_at = k * 1.6 + a1 * (got[:, 2] - 5.0)
+    in_well = got[:, 0] > 2.8
+    window = (A_at > 0.45 * k) & (A_at < 0.95 * k)
+    assert in_well[0] and A_at[0] > k                                   # falls into the well at the top
+    assert window.sum() >= 4 and np.all(in_well[window])                # carried: stays through the bistable window
+    assert np.all(cold[window, 0] < 2.6)                                # restarted from d0: sits on the ramp instead
+    assert np.all(np.abs(got[window, 0] - cold[window, 0]) > 0.25)
+    assert not in_well[-1] and A_at[-1] < 0.4 * k                       # the well is gone at the bottom: snapped back
+    assert np.abs(got[-1] - cold[-1]).max() < 1e-4                      # ... to the minimum a cold start finds too
+    # both branches are equilibria of the analytic 1-D balance k (x - 2.4) = A s(x)
+    for x, A in zip(got[:, 0], A_at):
+        assert abs(k * (x - p0[0]) - A * np.interp(x, xs, s_nodes)) < 2 * fire.f_conv
+
+
 def test_df_weights_sum_to_zero_and_match_numerical_quadrature():
     """Eq.3: W_m = (2/(pi a^2)) int q hat_m(q)/sqrt(a^2-q^2) dq, checked with scipy.quad using
     the algebraic end-point weight; sum W = 0 (a constant force gives df = 0)."""
