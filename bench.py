@@ -6,8 +6,11 @@ seeded synthetic workload of BASELINE.json.  Prints ONE JSON line (rank 0).
                   [--no-cpu-baseline] [--no-per-config]
 
 Default workload: configs[4], the largest single-GPU configuration.  The other four configs are measured in the
-same process (3 warm-up + 3 timed steps each) and reported as compact numeric records under `parts.per_config`, so
-that one driver run carries the force-field and relaxation fractions of all five configs.
+same process (3 warm-up + 3 timed steps each) and reported as compact numeric records under `roofline.per_config`
+(full records under `parts.per_config`), so that one driver run carries the force-field and relaxation fractions of
+all five configs.  `--gpus N > 1` launched plainly starts N ranks itself (torch.distributed.run, one process per GPU);
+under torchrun it reads the rank environment.  `roofline.traffic` is a STORED ncu measurement (`traffic_source` names
+the capture and the commit), not something the run measures.
 
 * `value` (device-resident inputs): relaxed pixel-steps per second over the full scan; CUDA events per step on the
   launching stream, L2 flushed between steps, max over ranks.
@@ -66,18 +69,27 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-def ncu_traffic(cfg: int, kernel: str):
+TRAFFIC_CSV = "profiles/r02_traffic.csv"
+# the commit whose kernels the captures in TRAFFIC_CSV ran (round 2's final kernels; `git log -- profiles/r02_traffic.csv`).
+# ff.cu's kernels have not changed since; the number is a stored ncu measurement, NOT something this run measured.
+TRAFFIC_COMMIT = "1427f50"
+
+
+def ncu_traffic(cfg: int, kernel: str, with_source: bool = False):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-    (profiles/r02_traffic.csv: cfg,kernel,dram_read_bytes,dram_write_bytes,capture); None where no capture exists."""
-    p = os.path.join(ROOT, "profiles", "r02_traffic.csv")
-    if not os.path.exists(p):
-        return None
-    with open(p) as f:
-        for line in f:
-            c = line.strip().split(",")
-            if len(c) >= 4 and c[0] == str(cfg) and c[1] == kernel:
-                return float(c[2]) + float(c[3])
-    return None
+    (profiles/r02_traffic.csv: cfg,kernel,dram_read_bytes,dram_write_bytes,capture); None where no capture exists.
+    with_source: (bytes, "ncu capture profiles/<file>, commit <sha>")."""
+    p = os.path.join(ROOT, TRAFFIC_CSV)
+    found, src = None, None
+    if os.path.exists(p):
+        with open(p) as f:
+            for line in f:
+                c = line.strip().split(",")
+                if len(c) >= 4 and c[0] == str(cfg) and c[1] == kernel:
+                    found = float(c[2]) + float(c[3])
+                    src = (f"stored ncu --set full capture profiles/{c[4].split(' ')[0] if len(c) > 4 else '?'} via "
+                           f"{TRAFFIC_CSV}, kernels of commit {TRAFFIC_COMMIT}; not measured in this run")
+    return (found, src) if with_source else found
 
 
 def inputs_sha256(ws) -> str:
@@ -431,7 +443,7 @@ def run_reference(args):
     r = runs[-1]
     sample = (f"each step: unoptimised FP64 oracle force field at {r['sample_points']} seeded grid points + relaxation/df "
               f"of the central {r['sample_pixels']} pixels on {r['grid_kind']}; value extrapolated to the full workload")
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD_NAME[args.config], "seed": BASE_SEED[args.config]},
@@ -715,6 +727,11 @@ def run_ours(args):
     dominant = max(("ff", "relax", "df"), key=lambda k: ms[k])
     roof = dict(kernels[dominant])
     roof["share_of_step"] = ms[dominant] / (x["t_step"] * 1e3)
+    roof["traffic_source"] = ncu_traffic(cfg, dominant, with_source=True)[1]
+    compact = ("ms_per_step", "pixel_steps_per_s", "e2e_ms_per_step", "e2e_pixel_steps_per_s", "kernel_ms",
+               "ff_pipe_frac_executed", "ff_flop_frac", "relax_alu_pipe_frac", "relax_issued_pipe_frac",
+               "relax_lane_utilisation", "df_hbm_frac", "not_converged", "steps")
+    roof["per_config"] = {c: {k: r[k] for k in compact if k in r} for c, r in per_config.items()}
     roof["peak_source"] = (f"{SMS} SMs x {LANES} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 (DESIGN.md 6.1)"
                            if roof["bound"] == "alu" else f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})")
 
@@ -750,6 +767,35 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` launched plainly (no torchrun environment): start N ranks of this same command, one
+    process per GPU, the way the driver does (torch.distributed.run on 127.0.0.1, a free port), and return its exit
+    code.  Rank 0 prints the JSON line; it passes through on the inherited stdout."""
+    import socket
+    import subprocess
+    if args_impl(sys.argv) == "ours":
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < n:
+            raise SystemExit(f"bench.py: --gpus {n} needs {n} CUDA devices on this node, found {have} "
+                             "(one process per GPU; ranks are never stacked on one device)")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd).returncode
+
+
+def args_impl(argv) -> str:
+    for i, a in enumerate(argv):
+        if a == "--impl" and i + 1 < len(argv):
+            return argv[i + 1]
+        if a.startswith("--impl="):
+            return a.split("=", 1)[1]
+    return "ours"
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -763,6 +809,13 @@ def main():
                     help="with --gpus N > 1: split ONE system across the ranks (row slabs + halo) instead of replicating")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        raise SystemExit(spawn_ranks(args.gpus))
+    world = shard.env_rank_world()[1]
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world} ranks")
     if args.impl == "reference":
         run_reference(args)
     else:

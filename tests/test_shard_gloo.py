@@ -3,6 +3,7 @@ aggregation bench.py uses (paper_2401_14564_b200/shard.py).  The data path has n
 batch systems are independent: PAPER.md:266, 280, 248), so this is all the multi-rank logic there is."""
 import os
 import socket
+import sys
 
 import numpy as np
 import pytest
@@ -10,6 +11,8 @@ import torch.multiprocessing as mp
 
 from paper_2401_14564_b200 import shard
 from paper_2401_14564_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _free_port():
@@ -164,3 +167,29 @@ def test_rank_workloads_are_valid_and_same_shape():
     assert a.pairs == b.pairs and a.pixel_steps == b.pixel_steps
     assert not np.array_equal(a.xyzq, b.xyzq)
     assert abs(float(b.xyzq[:, 3].sum())) < 1e-5
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` launched plainly must start two ranks itself (one process per GPU through
+    torch.distributed.run on 127.0.0.1) and report the REAL world size.  Driven here through the host-only oracle arm
+    (`--impl reference`: rank 0 works, rank 1 exits 0), which needs no GPU; the GPU arm of the same launcher refuses
+    to start when the node has fewer devices than ranks instead of stacking ranks on one GPU; and a --gpus value that
+    disagrees with the launcher's WORLD_SIZE is an error, not a silently wrong n_gpus."""
+    import json
+    import subprocess
+    bench = os.path.join(ROOT, "bench.py")
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, bench, "--gpus", "2", "--impl", "reference", "--steps", "1", "--warmup", "0",
+                        "--config", "0"], env=env, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout                       # rank 0 alone prints
+    assert lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2 and lines[0]["gpu_launches"] == 0
+    import torch
+    if not torch.cuda.is_available():
+        r = subprocess.run([sys.executable, bench, "--gpus", "2", "--steps", "1"], env=env, capture_output=True, text=True,
+                           timeout=300, cwd=ROOT)
+        assert r.returncode != 0 and "needs 2 CUDA devices" in r.stderr
+    r = subprocess.run([sys.executable, bench, "--gpus", "2", "--impl", "reference"], env=dict(env, WORLD_SIZE="3", RANK="0"),
+                       capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert r.returncode != 0 and "WORLD_SIZE=3" in r.stderr
