@@ -42,7 +42,12 @@
 extern "C" {
 #endif
 
-#define PPFM_VERSION 100 /* 0.1.0 */
+/* ABI version of THIS header.  ppfm_version() returns the value the loaded library was built with; a client should
+ * compare the two once at start-up (the Python binding and tests/c_abi/scan_c.c do) and refuse to run on a mismatch:
+ * an argument list that differs between header and library is not detectable any other way from C.
+ * 200 (0.2.0): the force-field calls take a ppfm_ff_status* before cuda_stream (incompatible with 100); the probe /
+ *              timing / launch-count exports moved to ppfm_bench.h; ppfm_forcefield_noalloc and PPFM_ELIMIT added. */
+#define PPFM_VERSION 200 /* 0.2.0 */
 #define PPFM_MAX_TYPES 64
 #define PPFM_DF_MAX_N 255 /* largest n = A/dz of ppfm_df */
 
@@ -211,6 +216,17 @@ int ppfm_relax_scan(const float *d_ff, const ppfm_grid *grid, const ppfm_tip *ti
 /* Batch form: nsys scans in one launch; grids concatenated as in ppfm_forcefield_batch, outputs concatenated in
  * order (system m starts at pixel-step offset sum_{l<m} nz*npy*npx).  One fire setting for all. */
 int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
+                          const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
+                          ppfm_stats *d_stats, void *cuda_stream);
+
+/* Sweep form (the stored grids exist "so that" tip parameters "can change without recomputation"):
+ * nscan scans on ONE resident grid in one launch.  `grid` is a single HOST struct and d_ff that one grid; tips[m]
+ * and scans[m] (HOST arrays of length nscan) give scan m its own springs (k_x, k_y, k_R), equilibrium displacement
+ * d0 (length and tilt) and scan geometry.  Outputs are concatenated in order as in the batch form.  Nothing is
+ * replicated: a k_xy / k_R / d0 sweep costs the memory of one grid.  (A tip-CHARGE sweep changes the grid itself:
+ * ppfm_forcefield_split + ppfm_combine per Q, then the batch form.)  Results equal those of ppfm_relax_scan_batch
+ * on nscan copies of the grid bit for bit. */
+int ppfm_relax_scan_sweep(int32_t nscan, const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tips,
                           const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
                           ppfm_stats *d_stats, void *cuda_stream);
 

@@ -6,7 +6,7 @@
 //   * a1  `ff_prep_kernel` (one CTA per system) packs one 48-byte record per atom (x, y, z, - | c12, c12, -c6, -c6 |
 //         6 c6, 6 c6, kq, kq: the pair coefficients twice, so that LDS.128 yields aligned FP32x2 operand pairs) and
 //         stable-partitions the records: atoms with a Coulomb factor first, LJ-only atoms behind them.
-//   * a2  `ff_kernel`: one CTA = 256 columns (consecutive x-fastest (i,j) indices, so a warp's float4 stores are
+//   * a2  `ff_kernel`: one CTA = 128 columns (FF_THREADS) (consecutive x-fastest (i,j) indices, so a warp's float4 stores are
 //         512 contiguous bytes) x P consecutive z planes held in registers as P/2 FP32x2 pairs.  Atom records stream
 //         through a 3-stage shared-memory ring filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx),
 //         one elected thread producing two chunks ahead; every warp reads records as uniform (broadcast) LDS.128.
@@ -22,7 +22,10 @@
 
 namespace ppfm {
 
-constexpr int FF_THREADS = 128;  // columns per CTA
+#ifndef PPFM_FF_THREADS
+#define PPFM_FF_THREADS 128
+#endif
+constexpr int FF_THREADS = PPFM_FF_THREADS;  // columns per CTA
 constexpr int FF_CHUNK = 256;   // atoms per pipeline stage
 constexpr int FF_STAGES = 3;
 constexpr int FF_AHEAD = 2;     // chunks in flight ahead of the consumer
@@ -504,7 +507,7 @@ __device__ __forceinline__ void ff_init_barriers(uint64_t *full_bar, uint64_t *e
 // plus ~40 (two accumulator sets in split mode: ~28 per pair): P = 20 needs the full 255 registers (2 CTAs of 128
 // threads per SM), P <= 10 fits 168 (3 CTAs).  More warps do not help: the loop is bound by issue slots, not latency.
 template <int P, bool SPLIT>
-constexpr int ff_min_ctas() { return SPLIT ? (P >= 10 ? 2 : 3) : (P >= 16 ? 2 : 3); }
+constexpr int ff_min_ctas() { return (SPLIT ? (P >= 10 ? 2 : 3) : (P >= 16 ? 2 : 3)) * (128 / FF_THREADS); }
 
 // One system: job in the constant bank (kernel parameter).
 template <int P, bool SPLIT, bool ZCOL>
@@ -614,6 +617,10 @@ static cudaError_t launch_ff(int P, bool zcol, long long ntiles, cudaStream_t st
     else if (P == 8) launch_ff_one<SPLIT, 8, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else if (P == 10) launch_ff_one<SPLIT, 10, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else if constexpr (SPLIT) launch_ff_one<true, 6, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+#ifdef PPFM_EXPERIMENT
+    else if (P == 12) launch_ff_one<false, 12, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+    else if (P == 14) launch_ff_one<false, 14, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
+#endif
     else if (P == 16) launch_ff_one<false, 16, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     else launch_ff_one<false, 20, true>(ntiles, st, hj, dj, njobs, flags, recs, a, b);
     return cudaGetLastError();
@@ -652,7 +659,10 @@ static int forcefield_impl(int nsys, const int32_t *h_atom_offset, const float *
     long long nxy_tiles_total = 0;
     for (int m = 0; m < nsys; m++)
         nxy_tiles_total += ((long long)grids[m].n[0] * grids[m].n[1] + FF_THREADS - 1) / FF_THREADS;
-    const int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2], nxy_tiles_total, split) : 4;
+    int P = zcol ? pick_P(nz_common > 0 ? nz_common : grids[0].n[2], nxy_tiles_total, split) : 4;
+#ifdef PPFM_EXPERIMENT
+    if (zcol && !split && getenv("PPFM_FF_FORCE_P")) P = atoi(getenv("PPFM_FF_FORCE_P"));
+#endif
 
     const bool single = (nsys == 1);
     const size_t jobs_bytes = (size_t)nsys * sizeof(FFJob);

@@ -720,13 +720,13 @@ static void launch_relax(int nsys, long long blocks, cudaStream_t st, const Rela
 // Host side shared by the relaxation and the stiffness map: validate and pack one RelaxJob per system.
 static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *tips, const ppfm_scan *scans,
                             RelaxJob **hj_out, long long *blocks_out, long long *samples_out, bool *ortho_out,
-                            bool *anyper_out, bool *symtip_out) {
+                            bool *anyper_out, bool *symtip_out, bool shared_grid = false) {
     RelaxJob *hj = (RelaxJob *)calloc((size_t)nsys, sizeof(RelaxJob));
     if (!hj) return PPFM_ENOMEM;
     long long blocks = 0, ff_off = 0, out_off = 0;
     bool ortho = true, anyper = false, symtip = true;
     for (int m = 0; m < nsys; m++) {
-        const ppfm_grid &g = grids[m];
+        const ppfm_grid &g = grids[shared_grid ? 0 : m];     // sweep form: every scan reads the ONE grid at offset 0
         const ppfm_scan &s = scans[m];
         const ppfm_tip &t = tips[m];
         RelaxJob &j = hj[m];
@@ -760,7 +760,7 @@ static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *ti
         j.k_rad = (float)t.k_rad;
         if (t.d0[0] != 0.0 || t.d0[1] != 0.0 || j.k_lat[0] != j.k_lat[1]) symtip = false;
         blocks += (long long)j.nbx * ((s.npy + RX_TILE_Y - 1) / RX_TILE_Y);
-        ff_off += grid_points(&g);
+        if (!shared_grid) ff_off += grid_points(&g);
         out_off += (long long)s.npx * s.npy * s.nz;
         if (blocks > 0x7fffffffLL) { free(hj); return PPFM_EINVAL; }
     }
@@ -789,7 +789,7 @@ static int build_relax_jobs(int nsys, const ppfm_grid *grids, const ppfm_tip *ti
 static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const ppfm_tip *tips,
                       const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz, uint16_t *d_iters,
                       ppfm_stats *d_stats, void *cuda_stream, bool tricubic = false, float *d_fz = nullptr,
-                      float *d_eig = nullptr) {
+                      float *d_eig = nullptr, bool shared_grid = false) {
     if (nsys < 1 || !d_ff || !grids || !tips || !fire || !scans || !d_pos_fz) return PPFM_EINVAL;
     if (d_eig && (tricubic || ((uintptr_t)d_eig & 15))) return PPFM_EINVAL;
     if (((uintptr_t)d_ff & (tricubic ? 3 : 15)) || ((uintptr_t)d_pos_fz & 15) || ((uintptr_t)d_iters & 1) || ((uintptr_t)d_stats & 7))
@@ -802,7 +802,8 @@ static int relax_impl(int nsys, const float *d_ff, const ppfm_grid *grids, const
     long long blocks = 0, samples = 0;
     bool ortho = true, anyper = false, symtip = true;
     {
-        const int rc = build_relax_jobs(nsys, grids, tips, scans, &hj, &blocks, &samples, &ortho, &anyper, &symtip);
+        const int rc = build_relax_jobs(nsys, grids, tips, scans, &hj, &blocks, &samples, &ortho, &anyper, &symtip,
+                                        shared_grid);
         if (rc != PPFM_OK) return rc;
     }
     FireParams fp;
@@ -1024,6 +1025,16 @@ extern "C" int ppfm_relax_scan_batch(int32_t nsys, const float *d_ff, const ppfm
                                      const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz,
                                      uint16_t *d_iters, ppfm_stats *d_stats, void *cuda_stream) {
     return relax_impl(nsys, d_ff, grids, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream);
+}
+
+// Parameter sweep on ONE resident grid ("so the tip ... can change without
+// recomputation"): nscan scans with their own tip (k_x, k_y, k_R, d0) and scan geometry in one launch, all gathering
+// from the same grid.  The batch kernel is used as is; every job's grid offset is 0.
+extern "C" int ppfm_relax_scan_sweep(int32_t nscan, const float *d_ff, const ppfm_grid *grid, const ppfm_tip *tips,
+                                     const ppfm_fire *fire, const ppfm_scan *scans, float *d_pos_fz,
+                                     uint16_t *d_iters, ppfm_stats *d_stats, void *cuda_stream) {
+    return relax_impl(nscan, d_ff, grid, tips, fire, scans, d_pos_fz, d_iters, d_stats, cuda_stream, false, nullptr,
+                      nullptr, true);
 }
 
 // relaxation with the stiffness map folded into the end of every z-step: the eigenvalues come

@@ -65,11 +65,14 @@ class Stats(C.Structure):
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
            "ppfm_forcefield_noalloc",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft",
-           "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_stiffness",
+           "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_sweep", "ppfm_relax_scan_stiffness",
            "ppfm_relax_scan_stiffness_batch", "ppfm_relax_scan_tricubic",
            "ppfm_relax_scan_tricubic_batch", "ppfm_energy_grid", "ppfm_stiffness", "ppfm_stiffness_batch", "ppfm_df",
            "ppfm_df_batch", "ppfm_df_weights", "ppfm_scan_host", "ppfm_scan_host_batch", "ppfm_scan_host_sweep",
            "ppfm_release_scratch"]
+
+
+HEADER_VERSION = 200            # PPFM_VERSION of the include/ppfm.h this binding mirrors
 
 
 def lib():
@@ -81,6 +84,9 @@ def lib():
                             "there is no CPU fallback")
         L = C.CDLL(LIB_PATH)
         L.ppfm_version.restype = C.c_int
+        if int(L.ppfm_version()) != HEADER_VERSION:      # argument lists differ between ABI versions: never guess
+            raise PpfmError(f"{LIB_PATH} is ABI version {int(L.ppfm_version())}, this binding was written against "
+                            f"include/ppfm.h version {HEADER_VERSION}; rebuild with `python -m paper_2401_14564_b200.build`")
         L.ppfm_strerror.restype = C.c_char_p
         L.ppfm_strerror.argtypes = [C.c_int]
         L.ppfm_Nm_to_eVA2.restype = C.c_double
@@ -372,6 +378,24 @@ def relax_scan_batch(ff, grids, tips, fire, scans, pos_fz=None, iters=None, stat
     rc = lib().ppfm_relax_scan_batch(C.c_int32(nsys), _dptr(ff, torch.float32), gr, tp, C.byref(c_fire(fire)), sc,
                                      _dptr(pos_fz, torch.float32), _dptr(iters), _dptr(stats), _stream())
     _check(rc, "ppfm_relax_scan_batch")
+    return pos_fz, iters
+
+
+def relax_scan_sweep(ff, grid, tips, fire, scans, pos_fz=None, iters=None, stats=None, want_iters=True):
+    """ppfm_relax_scan_sweep: len(tips) scans (own springs, d0 and scan geometry each) on ONE resident grid `ff`, one
+    launch, nothing replicated; outputs concatenated as in relax_scan_batch."""
+    torch = _torch()
+    assert len(tips) == len(scans)
+    tp, sc = c_array(tips, c_tip), c_array(scans, c_scan)
+    nps = sum(int(s.nz) * int(s.npy) * int(s.npx) for s in sc)
+    if pos_fz is None:
+        pos_fz = torch.empty((nps, 4), dtype=torch.float32, device=ff.device)
+    if iters is None and want_iters:
+        iters = torch.empty((nps,), dtype=torch.int16, device=ff.device)
+    rc = lib().ppfm_relax_scan_sweep(C.c_int32(len(tips)), _dptr(ff, torch.float32), C.byref(c_grid(grid)), tp,
+                                     C.byref(c_fire(fire)), sc, _dptr(pos_fz, torch.float32), _dptr(iters),
+                                     _dptr(stats), _stream())
+    _check(rc, "ppfm_relax_scan_sweep")
     return pos_fz, iters
 
 

@@ -35,6 +35,11 @@ enum { NATOMS = 6, NX = 40, NY = 36, NZ = 44, NPX = 17, NPY = 13, NZS = 24, NDF 
 
 int main(int argc, char **argv) {
     if (argc < 2) { fprintf(stderr, "usage: scan_c OUTPUT_FILE\n"); return 2; }
+    if (ppfm_version() != PPFM_VERSION) {       /* built against another header than the library: argument lists may differ */
+        fprintf(stderr, "libppfm is version %d, this program was built against ppfm.h version %d\n", ppfm_version(),
+                PPFM_VERSION);
+        return 3;
+    }
     /* a ring of six atoms (types 1 = C, 0 = H alternating), charges summing to zero */
     float xyzq[NATOMS][4];
     int32_t type[NATOMS];

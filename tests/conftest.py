@@ -25,10 +25,11 @@ def pytest_terminal_summary(terminalreporter, exitstatus, config):
     tr = terminalreporter
     tr.write_sep("-", "relaxation parity: samples outside 2e-3 Å and how they are exempt (reading S17)")
     tr.write_line(f"{'case':58s} {'samples':>9s} {'fail':>6s} {'end-point flag':>15s} {'trajectory flag only':>21s} "
-                  f"{'inherited':>10s} {'max |dr| ok (Å)':>16s}")
+                  f"{'inherited':>10s} {'valid minima':>13s} {'saddles':>8s} {'max |dr| ok (Å)':>16s}")
     for r in PARITY_LOG:
         tr.write_line(f"{r['what'][:58]:58s} {r['samples']:9d} {r['fail']:6d} {r['fail_endpoint_flag']:15d} "
-                      f"{r['fail_traj_only']:21d} {r.get('fail_inherited', 0):10d} {r['max_ok_dist']:16.2e}")
+                      f"{r['fail_traj_only']:21d} {r.get('fail_inherited', 0):10d} {r.get('exempt_validated', 0):13d} {r.get('exempt_saddle', 0):8d} "
+                      f"{r['max_ok_dist']:16.2e}")
     out = os.path.join(ROOT, "gpurun_out")
     if os.path.isdir(out) and not os.environ.get("PPFM_CHECKS_OUT"):      # not from the checked build's child session
         import json

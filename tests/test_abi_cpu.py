@@ -33,7 +33,8 @@ def test_library_exports_every_declared_symbol(lib):
     for n in names:
         assert hasattr(lib, n), f"libppfm.so does not export {n}"
     assert set(names) == set(ppfm.EXPORTS)
-    assert lib.ppfm_version() == 100
+    header_version = int(re.search(r"#define\s+PPFM_VERSION\s+(\d+)", open(os.path.join(ROOT, "include", "ppfm.h")).read()).group(1))
+    assert lib.ppfm_version() == header_version == ppfm.HEADER_VERSION == 200
     # the measurement interface lives in its own header; the probes in their own library
     bench = header_symbols("ppfm_bench.h")
     assert set(bench) == set(ppfm_bench.EXPORTS_LIBPPFM) | set(ppfm_bench.EXPORTS_PROBES)

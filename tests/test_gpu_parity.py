@@ -71,8 +71,49 @@ def check_ff(got, ref, what=""):
     return (rel.max() if rel.size else 0.0), (dF[~big].max() if (~big).any() else 0.0)
 
 
-def check_positions(pos_gpu, ref, what="", max_traj_only=None):
+F_VALID = 1e-5      # eV/Å: |F_total| (oracle, FP64) at an exempt GPU position.  f_conv = 1e-6 in the kernel's FP32 plus
+                    # the float32 position's half ulp (5e-7 Å at 8 Å) times k_R = 1.9 eV/Å^2 (1e-6 eV/Å)
+
+
+def validate_exempt(pos_gpu, bad, ref, field, what):
+    """Where several results are correct the rest must still be VALID: every failing (hence exempt) sample of a
+    comparison is checked to be a genuine answer — the oracle's total force (Eq.1, FP64) at the GPU's position, on the
+    float4 grid the kernel relaxed on, is below F_VALID, i.e. the kernel stopped where the method's own criterion
+    (|F_total| < f_conv, reading S7) says to stop, on the same field, just not where the oracle's path stopped.  The
+    oracle's Hessian there tells which kind of point it is: positive definite = a true minimum (counted `validated`);
+    otherwise a stationary point that is not a minimum (counted `saddle`): FIRE run to |F| < f_conv ends on one when
+    the start lies on its stable manifold, which happens on the mirror lines of a symmetric sample (config 2's
+    lattice-perfect slab: a pixel straight above an atom), where the FP64 path falls off through rounding noise and the
+    FP32 path does not, or the reverse.  Those are bounded: at most max(1, 1e-5 x samples) per comparison.  Samples the
+    oracle itself could not converge (iters < 0) have no stationary point to sit on and are only counted.
+    field = (ff, grid, tip, scan, pix): ff the numpy float4 grid, pix the sampled pixel indices or None.
+    Returns (validated, saddle, not_converged, max |F|, min lambda)."""
+    ff, grid, tip, scan, pix = field
+    rt = oracle.tip_positions(scan)
+    n_val, n_sad, n_nc, f_max, lam_lo = 0, 0, 0, 0.0, np.inf
+    for z, m in zip(*np.nonzero(bad)):
+        if ref["iters"][z, m] < 0:
+            n_nc += 1
+            continue
+        rtip = rt[z, m if pix is None else pix[m]]
+        r = np.asarray(pos_gpu[z, m, :3], dtype=np.float64)
+        F = oracle.total_force(ff, grid, tip, rtip, r)
+        _, lam = oracle.hessian(ff, grid, tip, rtip, r)
+        Fn = float(np.linalg.norm(F))
+        assert Fn <= F_VALID, f"{what}: exempt sample (z {z}, column {m}) is no equilibrium: |F| = {Fn:.3e} eV/Å"
+        if lam[0] > 0.0:
+            n_val += 1
+        else:
+            n_sad += 1
+            print(f"{what}: exempt sample (z {z}, column {m}) sits on a saddle: |F| = {Fn:.2e}, lambda = {lam}")
+        f_max, lam_lo = max(f_max, Fn), min(lam_lo, float(lam[0]))
+    assert n_sad <= max(1, math.ceil(1e-5 * bad.size)), f"{what}: {n_sad} exempt samples on saddle points"
+    return n_val, n_sad, n_nc, f_max, (lam_lo if n_val + n_sad else 0.0)
+
+
+def check_positions(pos_gpu, ref, what="", max_traj_only=None, field=None):
     """pos_gpu (nz, npix, 4) vs oracle dict; returns (fraction within 2e-3 Å, distances).
+    `field` (see validate_exempt): when given, every failing sample must be a true minimum of that field.
 
     north_star: within 2e-3 Å on >= 99.9 % of samples, the rest limited to samples the oracle flags near-unstable.
     The failing samples are counted by the way they are exempt and logged (conftest.PARITY_LOG): `inherited` = later
@@ -102,6 +143,12 @@ def check_positions(pos_gpu, ref, what="", max_traj_only=None):
            "fail_unflagged": int((bad & ~exempt).sum()),
            "flagged_endpoint": int(end_flag.sum()), "flagged_any": int(flagged.sum()),
            "max_ok_dist": float(d[ok].max()) if ok.any() else 0.0}
+    if field is not None:
+        nv, nsad, nnc, fmax, lmin = validate_exempt(np.asarray(pos_gpu), bad, ref, field, what)
+        rec.update(exempt_validated=nv, exempt_saddle=nsad, exempt_not_converged=nnc, exempt_max_F=fmax,
+                   exempt_min_lambda=lmin)
+    else:
+        rec.update(exempt_validated=0, exempt_unvalidated=int(bad.sum()))
     PARITY_LOG.append(rec)
     print("parity", rec)
     frac = ok.mean()
@@ -143,7 +190,7 @@ def test_ff_full_grid(P, cfg):
 
 
 def test_ff_ragged_tiles_and_tails(P):
-    """Grid sizes that are not multiples of the CTA tile (256 columns) or of any P, several atom chunks."""
+    """Grid sizes that are not multiples of the CTA tile (128 columns) or of any P, several atom chunks."""
     w = W.get(2)
     w = replace(w, grid=replace(w.grid, n=(37, 23, 13), step=np.diag([0.31, 0.47, 0.53])))
     check_ff(gpu_ff(P, w).cpu().numpy(), oracle.forcefield(w), "ragged")
@@ -275,12 +322,68 @@ def cfg4(P):
 
 
 def test_ff_full_size_cfg4_sampled(cfg4):
+    """Config 4's 1.28e8-point grid (2.05 GB, 95 % of 2^31 bytes) as bench.py launches it: 2e5 random points (SURVEY
+    8(d)) plus points aimed at where an indexing slip would show — the complete last plane (k = 199: the last pair of
+    the last z-group, the last 128-column tile row, the highest flat indices / byte offsets), strided samples of the
+    last z-group's first plane (k = 180) and of plane 198, and the last (ragged-free but final) 128-column tile at every
+    height.  ~1.1e6 points, ~5e10 pair terms for the oracle."""
     import torch
     w, ff = cfg4[0], cfg4[1]
-    idx = sample(w.npoints, 1500, 41)
+    nx, ny, nz = w.grid.n
+    nxy = nx * ny
+    aimed = np.concatenate([
+        (nz - 1) * nxy + np.arange(nxy),                                  # complete last plane
+        (nz - 20) * nxy + np.arange(0, nxy, 7),                           # first plane of the last z-group (P = 20)
+        (nz - 2) * nxy + np.arange(0, nxy, 5),                            # the other plane of the last FP32x2 pair
+        (np.arange(nz)[:, None] * nxy + np.arange(nxy - 128, nxy)[None, :]).ravel(),   # last 128-column tile, every k
+    ])
+    idx = np.unique(np.concatenate([sample(w.npoints, 200_000, 41), aimed])).astype(np.int64)
+    assert idx[-1] == w.npoints - 1 and idx.size > 1_000_000
     got = ff.reshape(-1, 4)[torch.from_numpy(idx).cuda()].cpu().numpy()
-    check_ff(got, oracle.forcefield(w, idx=idx), "cfg4 sampled")
+    rel, _ = check_ff(got, oracle.forcefield(w, idx=idx), "cfg4 sampled")
+    print(f"cfg4: {idx.size} points (2e5 random + aimed), max rel force error {rel:.2e}")
     assert bool(torch.isfinite(ff).all())
+
+
+def test_ff_split_grids_beyond_2_GiB(P):
+    """Index width: config 4's atoms on an 820 x 820 x 200 grid — each float4 grid is 2.15 GB, so byte offsets pass
+    2^31 in the single pass, in the two-grid (split) pass and in ppfm_combine.  2e4 random points and the 1e4 highest
+    flat indices.  The single pass and the unit-charge Coulomb grid are held to north_star's tolerance (S16); the
+    LJ-only grid to S16 plus the stagnation floor of DESIGN.md S16a (far-image r^-8 tails below half an ulp of the
+    FP32 running sum: measured 1.06e-4 relative at |F| = 0.012), and the combined grid, at a tip charge other than the
+    workload's, against the magnitudes of its two parts."""
+    import torch
+    w = W.get(4)
+    w = replace(w, grid=replace(w.grid, n=(820, 820, 200)))
+    assert w.npoints * 16 > 2 ** 31
+    xyzq, types = P.upload(w)
+    Q = 0.07
+    idx = np.unique(np.concatenate([sample(w.npoints, 20_000, 43), np.arange(w.npoints - 10_000, w.npoints)]))
+    sel = torch.from_numpy(idx).cuda()
+    ref, ref_lj = oracle.forcefield(w, idx=idx, Q=Q), oracle.forcefield(w, idx=idx, Q=0.0)
+    ref_el = (ref - ref_lj) / Q                                   # unit-charge Coulomb part (Eq.6 is linear in q_PP)
+    pick = lambda t: t.reshape(-1, 4)[sel].cpu().numpy().astype(np.float64)
+    one = P.forcefield(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min, Q=Q)
+    rel, _ = check_ff(pick(one), ref, "820x820x200 single pass")
+    assert bool(torch.isfinite(one).all())
+    del one
+    lj, el = P.forcefield_split(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min)
+    ff = P.combine(lj, el, Q)
+    torch.cuda.synchronize()
+    rel_el, _ = check_ff(pick(el), ref_el, "820x820x200 unit-charge Coulomb grid")
+    n3 = lambda a: np.linalg.norm(a[:, :3], axis=1)
+    d_lj = n3(pick(lj) - ref_lj)
+    assert np.all(d_lj <= 1e-4 * n3(ref_lj) + 2e-6), f"LJ grid: {(d_lj - 1e-4 * n3(ref_lj)).max():.2e} over 1e-4 |F|"
+    d = n3(pick(ff) - ref)
+    assert np.all(d <= 1e-4 * (n3(ref_lj) + abs(Q) * n3(ref_el)) + 2e-6)
+    dE = np.abs(pick(ff)[:, 3] - ref[:, 3])
+    assert np.all(dE <= 1e-4 * (np.abs(ref_lj[:, 3]) + abs(Q) * np.abs(ref_el[:, 3])) + E_ABS_TOL)
+    print(f"820 x 820 x 200: {idx.size} points; max rel force error single pass {rel:.2e}, Coulomb grid {rel_el:.2e}, "
+          f"LJ grid max |dF| {d_lj.max():.2e} (max over 1e-4|F|: {(d_lj - 1e-4 * n3(ref_lj)).max():.2e}), "
+          f"combined max |dF| {d.max():.2e}")
+    assert bool(torch.isfinite(ff).all())
+    del lj, el, ff
+    torch.cuda.empty_cache()
 
 
 # ------------------------------------------------------------------------------------------------ relaxation
@@ -303,11 +406,13 @@ def test_relax_and_df_full_scan(P, cfg):
     pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)
     it_h = iters.cpu().numpy().view(np.uint16).reshape(w.scan.nz, npix).astype(np.int64)
     # (ii) oracle on the GPU's FP32 grid widened on access: isolates the relaxer from grid rounding
-    ref32 = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan)
-    frac, d = check_positions(pos_h, ref32, f"cfg{cfg} (GPU grid)")
+    ff_h = ff.cpu().numpy()
+    ref32 = oracle.relax_scan(ff_h, w.grid, w.tip, w.fire, w.scan)
+    field = (ff_h, w.grid, w.tip, w.scan, None)          # exempt samples: true minima of the grid the kernel relaxed on
+    frac, d = check_positions(pos_h, ref32, f"cfg{cfg} (GPU grid)", field=field)
     # (i) oracle on its own FP64 grid: end to end
     ref64 = oracle.relax_scan(oracle.forcefield(w), w.grid, w.tip, w.fire, w.scan)
-    check_positions(pos_h, ref64, f"cfg{cfg} (oracle grid)")
+    check_positions(pos_h, ref64, f"cfg{cfg} (oracle grid)", field=field)
     # Fz and df
     ok = np.linalg.norm(pos_h[..., :3] - ref64["pos_fz"][..., :3], axis=-1) <= 2e-3
     assert np.abs(pos_h[..., 3] - ref64["pos_fz"][..., 3])[ok].max() < 2e-4
@@ -362,16 +467,17 @@ def test_relax_cfg2_all_three_tip_charges_gpu_grid_and_end_to_end(P):
         ff = P.combine(lj, el, Q)
         ff, pos, iters, df, st = gpu_scan(P, w, ff=ff)
         pix = sample(npix, 400, 51 + q)
-        ref = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan, pix=pix)
+        ff_h = ff.cpu().numpy()
+        ref = oracle.relax_scan(ff_h, w.grid, w.tip, w.fire, w.scan, pix=pix)
         pos_h = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix]
-        frac, d = check_positions(pos_h, ref, f"cfg2 Q={Q:+.1f} (GPU grid, 400 px)")
+        frac, d = check_positions(pos_h, ref, f"cfg2 Q={Q:+.1f} (GPU grid, 400 px)", field=(ff_h, w.grid, w.tip, w.scan, pix))
         check_iters(iters.cpu().numpy().reshape(w.scan.nz, -1)[:, pix], ref, d, f"cfg2 Q={Q}")
         dfh = df.cpu().numpy().reshape(df.shape[0], -1)[:, pix]
         check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0), f"cfg2 df Q={Q}")
         pix2 = sample(npix, 200, 151 + q)
         ref2 = oracle.relax_scan_atoms(w, pix=pix2, Q=Q)
         pos2 = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix2]
-        frac2, d2 = check_positions(pos2, ref2, f"cfg2 Q={Q:+.1f} (end to end, 200 px)")
+        frac2, d2 = check_positions(pos2, ref2, f"cfg2 Q={Q:+.1f} (end to end, 200 px)", field=(ff_h, w.grid, w.tip, w.scan, pix2))
         assert np.abs(pos2[..., 3] - ref2["pos_fz"][..., 3])[d2 <= 2e-3].max() < 2e-4
         check_df_end_to_end(df.cpu().numpy().reshape(df.shape[0], -1)[:, pix2], ref2, d2, w, f"cfg2 Q={Q}")
         assert st["n_clamped"] == 0 and int(ref2["clamped"].sum()) == 0
@@ -384,16 +490,17 @@ def test_relax_full_size_cfg4_sampled_gpu_grid_and_end_to_end(cfg4):
     w, ff, pos, iters, df, st = cfg4
     npix = w.scan.npx * w.scan.npy
     pix = sample(npix, 4000, 61)
-    ref = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan, pix=pix)
+    ff_h = ff.cpu().numpy()
+    ref = oracle.relax_scan(ff_h, w.grid, w.tip, w.fire, w.scan, pix=pix)
     pos_h = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix]
-    frac, d = check_positions(pos_h, ref, "cfg4 (GPU grid, 4000 px)")
+    frac, d = check_positions(pos_h, ref, "cfg4 (GPU grid, 4000 px)", field=(ff_h, w.grid, w.tip, w.scan, pix))
     check_iters(iters.cpu().numpy().reshape(w.scan.nz, -1)[:, pix], ref, d, "cfg4")
     dfh = df.cpu().numpy().reshape(df.shape[0], -1)[:, pix]
     check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), w.scan.dz, w.df.A, w.df.k0, w.df.f0), "cfg4 df")
     pix2 = sample(npix, 96, 161)
     ref2 = oracle.relax_scan_atoms(w, pix=pix2)
     pos2 = pos.cpu().numpy().reshape(w.scan.nz, -1, 4)[:, pix2]
-    frac2, d2 = check_positions(pos2, ref2, "cfg4 (end to end, 96 px)")
+    frac2, d2 = check_positions(pos2, ref2, "cfg4 (end to end, 96 px)", field=(ff_h, w.grid, w.tip, w.scan, pix2))
     assert np.abs(pos2[..., 3] - ref2["pos_fz"][..., 3])[d2 <= 2e-3].max() < 2e-4
     check_df_end_to_end(df.cpu().numpy().reshape(df.shape[0], -1)[:, pix2], ref2, d2, w, "cfg4")
     assert st["n_clamped"] == 0
@@ -422,7 +529,8 @@ def test_relax_batch_cfg3(P):
                                                                   mols[m].grid.n[0], 4)
         ref = oracle.relax_scan(grid_h, mols[m].grid, mols[m].tip, mols[m].fire, mols[m].scan, pix=pix)
         pos_h = pos[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1, 4)[:, pix]
-        frac, d = check_positions(pos_h, ref, f"cfg3 mol {m} (GPU grid, 300 px)")
+        frac, d = check_positions(pos_h, ref, f"cfg3 mol {m} (GPU grid, 300 px)",
+                                  field=(grid_h, mols[m].grid, mols[m].tip, mols[m].scan, pix))
         check_iters(iters[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1)[:, pix], ref, d, f"cfg3 mol {m}")
         dfh = df[m].cpu().numpy().reshape(df.shape[1], -1)[:, pix]
         check_df(dfh, oracle.df(pos_h[..., 3].astype(np.float64), s.dz, 1.0, 1800.0, 30300.0), f"cfg3 df {m}")
@@ -430,7 +538,8 @@ def test_relax_batch_cfg3(P):
         pix2 = sample(s.npx * s.npy, 300, 171 + m)
         ref2 = oracle.relax_scan_atoms(mols[m], pix=pix2)
         pos2 = pos[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1, 4)[:, pix2]
-        frac2, d2 = check_positions(pos2, ref2, f"cfg3 mol {m} (end to end, 300 px)")
+        frac2, d2 = check_positions(pos2, ref2, f"cfg3 mol {m} (end to end, 300 px)",
+                                    field=(grid_h, mols[m].grid, mols[m].tip, mols[m].scan, pix2))
         check_df_end_to_end(df[m].cpu().numpy().reshape(df.shape[1], -1)[:, pix2], ref2, d2, mols[m], f"cfg3 mol {m}")
 
 
@@ -473,7 +582,8 @@ def test_relax_every_kernel_instance(P, small_system, ortho, anyper, symtip, tri
     npix = scan.npx * scan.npy
     ref = oracle.relax_scan(data, grid, tip, w.fire, scan)
     assert np.abs(ref["pos_fz"][..., :2] - (oracle.tip_positions(scan) + np.array(tip.d0))[..., :2]).max() > 0.05   # the field acts
-    frac, d = check_positions(pos.cpu().numpy().reshape(scan.nz, npix, 4), ref, name, max_traj_only=3)
+    frac, d = check_positions(pos.cpu().numpy().reshape(scan.nz, npix, 4), ref, name, max_traj_only=3,
+                              field=None if tricubic else (data, grid, tip, scan, None))
     ok = d <= 2e-3
     assert np.abs(pos.cpu().numpy().reshape(scan.nz, npix, 4)[..., 3] - ref["pos_fz"][..., 3])[ok].max() < 2e-4
     st = P.read_stats(stats)
@@ -509,6 +619,47 @@ def test_relax_every_kernel_instance(P, small_system, ortho, anyper, symtip, tri
         print(f"{name} STIFF: max err {err:.2e} (median tolerance {tol:.2e})")
 
 
+def test_relax_scan_sweep_on_one_resident_grid(P):
+    """ppfm_relax_scan_sweep (re-scan API for parameter sweeps): five tips — the
+    workload's, a stiffer lateral spring, a softer radial spring, a longer and tilted d0, an asymmetric tip — and two
+    scan geometries on config 1's ONE resident grid in one launch.  Bit for bit the batch form on five copies of the
+    grid (which is what a sweep cost before: 5 x 61 MiB); every scan against the oracle on the same grid, 200 sampled
+    pixels each; a one-scan sweep equals ppfm_relax_scan's batch-of-one bits too."""
+    import torch
+    w = W.get(1)
+    ff = gpu_ff(P, w)
+    k = w.tip.k_lat[0]
+    tips = [w.tip, replace(w.tip, k_lat=(2 * k, 2 * k)), replace(w.tip, k_rad=0.6 * w.tip.k_rad),
+            replace(w.tip, d0=(0.25, -0.15, -4.1)), replace(w.tip, k_lat=(0.012, 0.019), d0=(0.3, -0.2, -3.98))]
+    small = replace(w.scan, npx=61, npy=47, nz=32, p0=w.scan.p0 + np.array([1.3, 2.1, -0.2]))
+    scans = [w.scan, small, w.scan, small, w.scan]
+    stats = P.new_stats()
+    pos, iters = P.relax_scan_sweep(ff, w.grid, tips, w.fire, scans, stats=stats)
+    rep = ff.reshape(-1, 4).repeat(len(tips), 1)
+    pos_b, iters_b = P.relax_scan_batch(rep, [w.grid] * len(tips), tips, w.fire, scans)
+    torch.cuda.synchronize()
+    assert torch.equal(pos.view(torch.int32), pos_b.view(torch.int32)) and torch.equal(iters, iters_b)
+    del rep, pos_b, iters_b
+    st = P.read_stats(stats)
+    assert st["n_clamped"] == 0
+    ff_h = ff.cpu().numpy()
+    off = 0
+    for m, (tip, sc) in enumerate(zip(tips, scans)):
+        nps, npix = sc.nz * sc.npy * sc.npx, sc.npy * sc.npx
+        pix = sample(npix, 200, 300 + m)
+        ref = oracle.relax_scan(ff_h, w.grid, tip, w.fire, sc, pix=pix)
+        pos_h = pos[off:off + nps].cpu().numpy().reshape(sc.nz, npix, 4)[:, pix]
+        frac, d = check_positions(pos_h, ref, f"cfg1 sweep scan {m}", field=(ff_h, w.grid, tip, sc, pix))
+        assert np.abs(pos_h[..., 3] - ref["pos_fz"][..., 3])[d <= 2e-3].max() < 2e-4
+        check_iters(iters[off:off + nps].cpu().numpy().reshape(sc.nz, npix)[:, pix], ref, d, f"cfg1 sweep scan {m}")
+        off += nps
+    one, it1 = P.relax_scan_sweep(ff, w.grid, [tips[3]], w.fire, [small])
+    ref1, itr1 = P.relax_scan(ff, w.grid, tips[3], w.fire, small)
+    torch.cuda.synchronize()
+    assert torch.equal(one.view(torch.int32).reshape(-1), ref1.view(torch.int32).reshape(-1))
+    assert torch.equal(it1.reshape(-1), itr1.reshape(-1))
+
+
 def test_relax_asymmetric_tip_cfg0_full_scan_end_to_end(P):
     """the asymmetric tip on config 0, full scan, against the oracle on its own FP64 grid (end to end) and
     on the GPU's grid; df too."""
@@ -517,10 +668,12 @@ def test_relax_asymmetric_tip_cfg0_full_scan_end_to_end(P):
     ff, pos, iters, df, st = gpu_scan(P, w)
     npix = w.scan.npx * w.scan.npy
     pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)
-    ref32 = oracle.relax_scan(ff.cpu().numpy(), w.grid, w.tip, w.fire, w.scan)
-    check_positions(pos_h, ref32, "cfg0 asymmetric tip (GPU grid)")
+    ff_h = ff.cpu().numpy()
+    ref32 = oracle.relax_scan(ff_h, w.grid, w.tip, w.fire, w.scan)
+    field = (ff_h, w.grid, w.tip, w.scan, None)
+    check_positions(pos_h, ref32, "cfg0 asymmetric tip (GPU grid)", field=field)
     ref64 = oracle.relax_scan(oracle.forcefield(w), w.grid, w.tip, w.fire, w.scan)
-    frac, d = check_positions(pos_h, ref64, "cfg0 asymmetric tip (end to end)")
+    frac, d = check_positions(pos_h, ref64, "cfg0 asymmetric tip (end to end)", field=field)
     assert np.abs(pos_h[..., 3] - ref64["pos_fz"][..., 3])[d <= 2e-3].max() < 2e-4
     check_iters(iters.cpu().numpy(), ref64, d, "cfg0 asymmetric tip")
     check_df_end_to_end(df.cpu().numpy(), ref64, d, w, "cfg0 asymmetric tip")
@@ -585,7 +738,8 @@ def test_relax_periodic_wrap_and_clamp(P):
         pos, iters = P.relax_scan(torch.from_numpy(base).cuda(), g, W._default_tip(), W.Fire(), sc, stats=stats)
         torch.cuda.synchronize()
         ref = oracle.relax_scan(base, g, W._default_tip(), W.Fire(), sc)
-        check_positions(pos.cpu().numpy().reshape(sc.nz, -1, 4), ref, f"periodic={periodic}")
+        check_positions(pos.cpu().numpy().reshape(sc.nz, -1, 4), ref, f"periodic={periodic}",
+                        field=(base, g, W._default_tip(), sc, None))
         assert P.read_stats(stats)["n_clamped"] == int(ref["clamped"].sum())
         assert (P.read_stats(stats)["n_clamped"] > 0) == (periodic == (0, 0, 0))
 
@@ -629,6 +783,70 @@ def test_relax_tricubic_cfg0_full_scan(P):
     pos_lin, _ = P.relax_scan(ff, w.grid, w.tip, w.fire, w.scan)
     dl = np.linalg.norm(pos_lin.cpu().numpy().reshape(w.scan.nz, npix, 4)[..., :3] - pos_h[..., :3], axis=-1)
     assert np.median(dl) < 5e-3                                      # two interpolants of the same field
+
+
+def tricubic_chain_stats(P, w, npx_sample, seed, what, ff=None):
+    """The chain include/ppfm.h documents for N4 — ppfm_forcefield -> ppfm_energy_grid -> ppfm_relax_scan_tricubic —
+    on sampled pixels: (ii) against the oracle's O13 on the SAME (GPU-made, FP32) energies: isolates the relaxer;
+    (i) END TO END against the oracle relaxing on its OWN FP64 energies (`ref_E`; None skips it).  Returns the distance
+    arrays."""
+    import torch
+    if ff is None:
+        ff = gpu_ff(P, w)
+    E = P.energy_grid(ff)
+    stats = P.new_stats()
+    pos, iters = P.relax_scan_tricubic(E, w.grid, w.tip, w.fire, w.scan, stats=stats)
+    torch.cuda.synchronize()
+    npix = w.scan.npx * w.scan.npy
+    pix = sample(npix, npx_sample, seed)
+    pos_h = pos.cpu().numpy().reshape(w.scan.nz, npix, 4)[:, pix]
+    E_h = E.cpu().numpy()
+    ref = oracle.relax_scan(E_h, w.grid, w.tip, w.fire, w.scan, pix=pix)
+    frac, d = check_positions(pos_h, ref, f"{what} tricubic chain (GPU energies)")
+    ok = d <= 2e-3
+    assert np.abs(pos_h[..., 3] - ref["pos_fz"][..., 3])[ok].max() < 2e-4
+    return pos_h, pix, d, E_h
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_relax_tricubic_chain_on_library_made_energies(P, cfg):
+    """N4 end to end: the scan on an energy grid THE LIBRARY produced, configs 1 and 2, 1500 / 600
+    sampled pixels.  (ii) the relaxer against the oracle on the same FP32 energies at the relaxation's tolerance;
+    (i) against the oracle on its own FP64 energies, at the SAME tolerance (2e-3 Å on >= 99.9 % of the samples the
+    oracle does not flag, median well below).  The worry that the FP32 accumulation noise of the `.w` lane (S13), put
+    through the derivative stencil, would cost several 1e-3 Å does not materialise: the noise is smooth from node to
+    node (neighbouring nodes sum the same atoms in the same order).  Measured on B200: config 1 median 7e-6 Å, 99.9 %
+    1.1e-4 Å, max 2.6e-4 Å; the figures are written to gpurun_out/tricubic_chain_cfg*.json."""
+    w = W.get(cfg)
+    pos_h, pix, d, E_h = tricubic_chain_stats(P, w, 1500 if cfg == 1 else 600, 81 + cfg, f"cfg{cfg}")
+    E64 = np.ascontiguousarray(oracle.forcefield(w)[..., 3])
+    dE = np.abs(E_h.astype(np.float64) - E64)
+    assert np.all(dE <= 1e-4 * np.abs(E64) + E_ABS_TOL)
+    ref = oracle.relax_scan(E64, w.grid, w.tip, w.fire, w.scan, pix=pix)
+    stable = ~oracle.flags(ref)
+    d2 = np.linalg.norm(pos_h[..., :3].astype(np.float64) - ref["pos_fz"][..., :3], axis=-1)
+    far = np.abs(E64) < 1.0                                   # away from the repulsive cores, where the PP lives
+    print(f"cfg{cfg} tricubic chain end to end: max |dE| where |E| < 1 eV {dE[far].max():.2e} eV, median |dr| "
+          f"{np.median(d2[stable]):.2e}, 99.9 % {np.quantile(d2[stable], 0.999):.2e}, max {d2[stable].max():.2e} Å, "
+          f"within 2e-3: {(d2[stable] <= 2e-3).mean():.5f}")
+    gp = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(gp) and not os.environ.get("PPFM_CHECKS_OUT"):
+        import json
+        with open(os.path.join(gp, f"tricubic_chain_cfg{cfg}.json"), "w") as fh:
+            json.dump({"cfg": cfg, "pixels": int(len(pix)), "samples": int(stable.sum()),
+                       "max_dE_eV_where_E_below_1eV": float(dE[far].max()),
+                       "median_dr": float(np.median(d2[stable])), "q999_dr": float(np.quantile(d2[stable], 0.999)),
+                       "max_dr": float(d2[stable].max()), "frac_within_2e-3": float((d2[stable] <= 2e-3).mean())}, fh)
+    assert (d2[stable] <= 2e-3).mean() >= 0.999
+    assert np.median(d2[stable]) <= 2e-4
+
+
+def test_relax_tricubic_cfg4_sampled_in_the_bench_launch(cfg4):
+    """The tri-cubic scan bench.py times on config 4 (energy grid extracted from the 1.28e8-point float4 grid, 12.8 M
+    pixel-steps in one launch): 500 sampled pixels against the oracle's O13 on the same energies."""
+    from paper_2401_14564_b200 import ppfm as P
+    w, ff = cfg4[0], cfg4[1]
+    tricubic_chain_stats(P, w, 500, 91, "cfg4", ff=ff)
 
 
 def test_relax_tricubic_periodic_skewed_batch_and_edges(P):
@@ -1280,7 +1498,9 @@ def test_full_size_full_coverage_cfg2_and_cfg3(P):
     ref = oracle.relax_scan(ref_ff, w.grid, w.tip, w.fire, w.scan)
     npix = w.scan.npx * w.scan.npy
     nps = w.scan.nz * npix
-    frac, d = check_positions(pos[:nps].cpu().numpy().reshape(w.scan.nz, npix, 4), ref, "cfg2 full scan (end to end)")
+    frac, d = check_positions(pos[:nps].cpu().numpy().reshape(w.scan.nz, npix, 4), ref, "cfg2 full scan (end to end)",
+                              field=(ffq[:n].cpu().numpy().reshape(w.grid.n[2], w.grid.n[1], w.grid.n[0], 4), w.grid, w.tip,
+                                     w.scan, None))
     check_iters(iters[:nps].cpu().numpy(), ref, d, "cfg2 full scan")
     check_df_end_to_end(df[0].cpu().numpy(), ref, d, w, "cfg2 full scan")
 
@@ -1310,7 +1530,8 @@ def test_relax_batch_cfg3_all_64_molecules_in_the_bench_launch(P):
         grid_h = ff[m * npts:(m + 1) * npts].cpu().numpy().reshape(g.n[2], g.n[1], g.n[0], 4)
         ref = oracle.relax_scan(grid_h, g, mol.tip, mol.fire, mol.scan, pix=pix)
         pos_h = pos[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1, 4)[:, pix]
-        frac, d = check_positions(pos_h, ref, f"cfg3 mol {m} of 64 (GPU grid, 150 px)")
+        frac, d = check_positions(pos_h, ref, f"cfg3 mol {m} of 64 (GPU grid, 150 px)",
+                                  field=(grid_h, g, mol.tip, mol.scan, pix))
         fails += int((d > 2e-3).sum())
         check_iters(iters[m * nps:(m + 1) * nps].cpu().numpy().reshape(s.nz, -1)[:, pix], ref, d, f"cfg3 mol {m}")
         dfh = df[m].cpu().numpy().reshape(df.shape[1], -1)[:, pix]
