@@ -52,6 +52,9 @@ WORKLOAD_NAME = {0: "configs[0] tiny 10 atoms, 60x60x40 grid, 30x30x40 scan",
 PAIR_INSTR, PAIR_FLOPS = 19, 28        # canonical per pair interaction: FP32-pipe instructions, flops
 # what ff_kernel executes per pair (ff.cu, FP32x2-packed): lane-instructions for an atom with / without a Coulomb factor
 PAIR_EXEC = {"charged": 15, "neutral": 13, "charged_split": 20, "neutral_split": 14}
+# ffe_kernel (energy-only pass): 8 packed lane-instructions + 1 MUFU per pair; flops: dz add, r2 fma, ir2, 2 x ir6,
+# t fma, 2 energy fmas = 1 + 2 + 1 + 2 + 2 + 4 = 12 (+ the rsqrt)
+ENERGY_PAIR_INSTR, ENERGY_PAIR_FLOPS = 8, 13
 ITER_INSTR, ITER_FLOPS = 70, 114       # relax_kernel per FIRE iteration (cached cell, symmetric tip); + 4 MUFU
 TRI_INSTR, TRI_FLOPS = 270, 514        # the tri-cubic instance
 SMS, LANES = 148, 128
@@ -610,6 +613,29 @@ def next_rows(P, B, torch, job, ws, flush, env):
                              "ms": tri_ms, "pixel_steps_per_s": job.nps_one / tri_s,
                              "iters_per_pixel_step": tri["total_iters"] / job.nps_one,
                              "not_converged": tri["n_not_converged"], "in_step": False, "traffic": None}
+    # N4's energy-only force-field pass (ppfm_forcefield_energy) on the headline system, beside the float4 pass
+    if len(ws) == 1:
+        w = ws[0]
+        xyzq, types = P.upload(w)
+        E_out = torch.empty((w.grid.n[2], w.grid.n[1], w.grid.n[0]), dtype=torch.float32, device="cuda")
+        for rep in range(1 + 2):
+            if rep == 1:
+                B.timing_enable(True)
+            flush.zero_()
+            P.forcefield_energy(xyzq, types, w.elem_R, w.elem_e, w.lattice, w.probe, w.grid, w.r_min, out=E_out)
+        torch.cuda.synchronize()
+        e_ms = B.timing_read()["ff_energy"][0] / 2.0
+        B.timing_enable(False)
+        del E_out
+        e_s = e_ms * 1e-3
+        out["ff_energy"] = {"kernel": "ffe_kernel", "bound": "alu", "unit": "TFLOP/s",
+                            "achieved": w.pairs / e_s * ENERGY_PAIR_FLOPS * 1e-12, "peak": 2 * alu_peak * 1e-12,
+                            "frac": w.pairs / e_s * ENERGY_PAIR_FLOPS / (2 * alu_peak),
+                            "pipe_frac_executed": w.pairs / e_s * ENERGY_PAIR_INSTR / alu_peak,
+                            "xu_pipe_frac": w.pairs / e_s / (alu_peak / 8.0),      # 1 MUFU.RSQ per pair, 16 XU lanes per SM
+                            "pairs_per_s": w.pairs / e_s, "instr_per_pair_executed": ENERGY_PAIR_INSTR,
+                            "flops_per_pair": ENERGY_PAIR_FLOPS, "ms": e_ms, "bytes_per_point": 4, "in_step": False,
+                            "traffic": None}
     return out
 
 

@@ -201,6 +201,20 @@ int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, const int32_t *
                             const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
                             ppfm_ff_status *d_status, void *cuda_stream);
 
+/* ---- (1e) energy-only grid for the tri-cubic scan ("tri-cubic interpolation of the potential ...
+ * avoid storage of forces (i.e. improve memory efficiency)") ---------------------------------------------------
+ * The same sum as ppfm_forcefield, but only E = E_LJ + E_C is accumulated and stored: d_E is DEVICE
+ * float[n2][n1][n0] (4-byte aligned, 4 bytes per point instead of 16, written completely) in the layout
+ * ppfm_relax_scan_tricubic reads.  The pair loop carries no force arithmetic (8 packed instructions + 2 MUFU per
+ * pair of points against 15 + 2).  Every 256-atom partial sum is folded into an FP64 total per point, so the
+ * node-to-node noise the tri-cubic derivative stencil would amplify stays at the FP32 rounding of one chunk's terms
+ * (measured: <= 3e-7 eV where |E| < 1e-2 eV on configs 0-2; parity |dE| <= 1e-4 |E| + 5e-7 eV there).  All other
+ * arguments, d_status and the error codes are ppfm_forcefield's; probe->Q is the tip charge. */
+int ppfm_forcefield_energy(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                           const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                           const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_E,
+                           ppfm_ff_status *d_status, void *cuda_stream);
+
 /* ---- (2) relaxation scan: Eq.1 + Eq.2 + FIRE on the tri-linearly interpolated grid --
  * d_ff      DEVICE grid as written by ppfm_forcefield (read-only)
  * d_pos_fz  DEVICE float[nz][npy][npx][4] = relaxed PP position and Fz_tip = -F_R,z

@@ -34,7 +34,8 @@ typedef enum {
     PPFM_K_STIFFNESS = 5, /* N2 stiffness map               */
     PPFM_K_FFT_EL = 6,  /* N3 Eq.7 electrostatics: own kernels + cuFFT, one timed region */
     PPFM_K_RELAX_TRICUBIC = 7, /* N4 relaxation with tri-cubic interpolation of the potential */
-    PPFM_K_COUNT = 8
+    PPFM_K_FF_ENERGY = 8, /* N4 energy-only force-field pass (ppfm_forcefield_energy) */
+    PPFM_K_COUNT = 9
 } ppfm_kernel_id;
 int ppfm_timing_enable(int on);
 int ppfm_timing_read(int kernel_id, double *h_ms_total, int64_t *h_launches);

@@ -572,6 +572,184 @@ ff_batch_kernel(const FFJob *__restrict__ jobs, int njobs, const FFFlags *__rest
         ff_tile<P, SPLIT, false, ZCOL>(s_job, s_flags.ncharged, recs, out_a, out_b, s_rec, full_bar, empty_bar, local_tile);
 }
 
+// ------------------------------------------------------------------------------------------- energy-only pass (N4)
+// SURVEY 8(f) N4, PAPER.md:264 ("tri-cubic interpolation of the potential ... avoid storage of forces (i.e. improve
+// memory efficiency)"): the same sum as a2 but only E = E_LJ + E_C per grid point, 4 bytes per point instead of 16,
+// for ppfm_relax_scan_tricubic.  Same tile shape, atom records and TMA ring as ff_tile; the pair body shrinks to
+// 8 packed FP32x2 instructions + 2 MUFU.RSQ per pair of points (no force factor, no three accumulating FMAs), which
+// puts the XU (MUFU) pipe level with the FMA pipe.  The derivative stencil of the tri-cubic interpolant amplifies
+// node-to-node noise, so the per-chunk FP32 partial sums are folded into FP64 totals (P DADDs per 256 atoms).
+template <int P, bool CLAMP, bool ZCOL>
+__device__ __forceinline__ void ffe_tile(const FFJob &job, int ncharged, const AtomRec *__restrict__ recs,
+                                         float *__restrict__ out, AtomRec *s_rec, uint64_t *full_bar,
+                                         uint64_t *empty_bar, long long local_tile) {
+    const int tid = threadIdx.x;
+    const int zg = (int)(local_tile / job.n_xy_tiles);
+    const int xyt = (int)(local_tile - (long long)zg * job.n_xy_tiles);
+    const int col = xyt * FF_THREADS + tid;
+    const bool valid = col < job.nxy;
+    const int colc = valid ? col : job.nxy - 1;
+    const int j = colc / job.nx, i = colc - j * job.nx;
+    const int k0 = zg * P;
+    double pb[3];
+#pragma unroll
+    for (int c = 0; c < 3; c++)
+        pb[c] = job.origin[c] + i * job.step[0][c] + j * job.step[1][c] + k0 * job.step[2][c];
+    constexpr int H = P / 2;
+    static_assert(P % 2 == 0, "P must be even: points are processed as FP32x2 pairs");
+    float2 off[ZCOL ? 1 : 3][H];   // offsets of the points along step[2] (ZCOL: step[2] is parallel to z)
+#pragma unroll
+    for (int h = 0; h < H; h++)
+#pragma unroll
+        for (int c = 0; c < (ZCOL ? 1 : 3); c++) {
+            const int cc = ZCOL ? 2 : c;
+            off[c][h] = make_float2((float)((2 * h) * job.step[2][cc]), (float)((2 * h + 1) * job.step[2][cc]));
+        }
+
+    float2 E[H];
+    double Etot[P];
+    const float2 zero2 = make_float2(0.0f, 0.0f);
+#pragma unroll
+    for (int h = 0; h < H; h++) { E[h] = zero2; Etot[2 * h] = 0.0; Etot[2 * h + 1] = 0.0; }
+
+    const int natoms = job.natoms;
+    const int nq = min(max(ncharged, 0), natoms);
+    const int nch_q = (nq + FF_CHUNK - 1) / FF_CHUNK;
+    const int nchunks = nch_q + (natoms - nq + FF_CHUNK - 1) / FF_CHUNK;
+    auto chunk_begin = [&](int c) { return c < nch_q ? c * FF_CHUNK : nq + (c - nch_q) * FF_CHUNK; };
+    auto chunk_count = [&](int c) {
+        return c < nch_q ? min(FF_CHUNK, nq - c * FF_CHUNK) : min(FF_CHUNK, natoms - nq - (c - nch_q) * FF_CHUNK);
+    };
+    const int nimages = (2 * job.nimg[0] + 1) * (2 * job.nimg[1] + 1) * (2 * job.nimg[2] + 1);
+    const int nsteps = nimages * nchunks;
+    const AtomRec *src = recs + job.atom_begin;
+    const float rmin2 = job.rmin2;
+    auto issue = [&](int t) {
+        const int st = t % FF_STAGES;
+        const int use = t / FF_STAGES;
+        if (use > 0) mbar_wait(&empty_bar[st], (use - 1) & 1);
+        const int c = t % nchunks;
+        const uint32_t bytes = (uint32_t)chunk_count(c) * (uint32_t)sizeof(AtomRec);
+        mbar_expect_tx(&full_bar[st], bytes);
+        tma_load_1d(s_rec + st * FF_CHUNK, src + chunk_begin(c), bytes, &full_bar[st]);
+    };
+    if (tid == 0)
+        for (int t = 0; t < FF_AHEAD && t < nsteps; t++) issue(t);
+
+    float ph[3], pl[3];
+    // two atoms per trip so that one atom's MUFU results are in flight while the other's polynomial runs
+    auto pair_energy = [&](const float4 *s4, int a, auto neutral_tag) {
+        constexpr bool NEUTRAL = decltype(neutral_tag)::value;
+        const float4 r0 = s4[3 * a];
+        const float4 r1 = s4[3 * a + 1];
+        const float4 r2_ = s4[3 * a + 2];
+        const float2 c12 = make_float2(r1.x, r1.y), nc6 = make_float2(r1.z, r1.w), kq = make_float2(r2_.z, r2_.w);
+        const float dx0 = (ph[0] - r0.x) + pl[0];
+        const float dy0 = (ph[1] - r0.y) + pl[1];
+        const float dz0 = (ph[2] - r0.z) + pl[2];
+        const float2 dxx = make_float2(dx0, dx0), dyy = make_float2(dy0, dy0), dzz = make_float2(dz0, dz0);
+        float2 r2[H], ir[H];
+        if (ZCOL) {
+            const float rxy2s = fmaf(dy0, dy0, dx0 * dx0);
+            const float2 rxy2 = make_float2(rxy2s, rxy2s);
+#pragma unroll
+            for (int h = 0; h < H; h++) {
+                const float2 dz = __fadd2_rn(dzz, off[0][h]);
+                r2[h] = __ffma2_rn(dz, dz, rxy2);
+            }
+        } else {
+#pragma unroll
+            for (int h = 0; h < H; h++) {
+                const float2 dx = __fadd2_rn(dxx, off[0][h]), dy = __fadd2_rn(dyy, off[1 % (ZCOL ? 1 : 3)][h]),
+                             dz = __fadd2_rn(dzz, off[2 % (ZCOL ? 1 : 3)][h]);
+                r2[h] = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+            }
+        }
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            if (CLAMP) { r2[h].x = fmaxf(r2[h].x, rmin2); r2[h].y = fmaxf(r2[h].y, rmin2); }
+            ir[h].x = rsqrt_approx(r2[h].x);
+            ir[h].y = rsqrt_approx(r2[h].y);
+        }
+        // (A Newton step on 1/r^2 was measured, round 3: config 1's worst |dE| near E = 0 went 1.97e-7 -> 1.42e-7 eV for
+        // 2 more instructions per pair; what remains is the FP32 rounding of ~60-256 signed Coulomb terms inside a
+        // chunk, so the step was dropped.)
+        float2 ir2[H], ir6[H], t[H];
+#pragma unroll
+        for (int h = 0; h < H; h++) ir2[h] = __fmul2_rn(ir[h], ir[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) ir6[h] = __fmul2_rn(ir2[h], ir2[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) ir6[h] = __fmul2_rn(ir6[h], ir2[h]);
+#pragma unroll
+        for (int h = 0; h < H; h++) t[h] = __ffma2_rn(c12, ir6[h], nc6);              // c12/r^6 - c6
+#pragma unroll
+        for (int h = 0; h < H; h++) E[h] = __ffma2_rn(t[h], ir6[h], E[h]);            // E_LJ (Eq.5)
+        if (!NEUTRAL) {
+#pragma unroll
+            for (int h = 0; h < H; h++) E[h] = __ffma2_rn(kq, ir[h], E[h]);           // E_C = kq / r (Eq.6)
+        }
+    };
+    auto run_chunk = [&](const float4 *s4, int n, auto neutral_tag) {
+#pragma unroll 2
+        for (int a = 0; a < n; a++) pair_energy(s4, a, neutral_tag);
+    };
+
+    int step = 0;
+    for (int ia = -job.nimg[0]; ia <= job.nimg[0]; ia++)
+        for (int ib = -job.nimg[1]; ib <= job.nimg[1]; ib++)
+            for (int ic = -job.nimg[2]; ic <= job.nimg[2]; ic++) {
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    const double s = pb[c] - (ia * job.cell[0][c] + ib * job.cell[1][c] + ic * job.cell[2][c]);
+                    ph[c] = (float)s;
+                    pl[c] = (float)(s - (double)ph[c]);
+                }
+                for (int ch = 0; ch < nchunks; ch++, step++) {
+                    if (tid == 0 && step + FF_AHEAD < nsteps) issue(step + FF_AHEAD);
+                    const int st = step % FF_STAGES;
+                    mbar_wait(&full_bar[st], (step / FF_STAGES) & 1);
+                    const float4 *s4 = reinterpret_cast<const float4 *>(s_rec + st * FF_CHUNK);
+                    const int n = chunk_count(ch);
+                    if (ch < nch_q) run_chunk(s4, n, std::false_type{});
+                    else run_chunk(s4, n, std::true_type{});
+                    __syncwarp();
+                    if ((tid & 31) == 0) mbar_arrive(&empty_bar[st]);
+#pragma unroll
+                    for (int h = 0; h < H; h++) {          // fold the chunk's FP32 partial sums into the FP64 totals
+                        Etot[2 * h] += (double)E[h].x;
+                        Etot[2 * h + 1] += (double)E[h].y;
+                        E[h] = zero2;
+                    }
+                }
+            }
+    if (valid) {
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            const size_t o = (size_t)job.out_offset + (size_t)(k0 + p) * job.nxy + col;
+            PPFM_CHK(PPFM_CHK_FF_STORE, k0 + p >= job.nz || o < (size_t)job.out_offset + (size_t)job.nz * job.nxy);
+            if (k0 + p < job.nz) out[o] = (float)Etot[p];
+        }
+    }
+}
+
+template <int P, bool ZCOL>
+__global__ void __launch_bounds__(FF_THREADS, 2)
+ffe_kernel(const __grid_constant__ FFJob job, const FFFlags *__restrict__ flags, const AtomRec *__restrict__ recs,
+           float *__restrict__ out) {
+    __shared__ __align__(128) AtomRec s_rec[FF_STAGES * FF_CHUNK];
+    __shared__ __align__(8) uint64_t full_bar[FF_STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[FF_STAGES];
+    __shared__ FFFlags s_flags;
+    if (threadIdx.x == 0) s_flags = flags[0];
+    ff_init_barriers(full_bar, empty_bar);
+    __syncthreads();
+    if (s_flags.clamp)
+        ffe_tile<P, true, ZCOL>(job, s_flags.ncharged, recs, out, s_rec, full_bar, empty_bar, (long long)blockIdx.x);
+    else
+        ffe_tile<P, false, ZCOL>(job, s_flags.ncharged, recs, out, s_rec, full_bar, empty_bar, (long long)blockIdx.x);
+}
+
 // ---------------------------------------------------------------------------------------------------- a3 combine
 __global__ void combine_kernel(const float4 *__restrict__ lj, const float4 *__restrict__ el, float Q, long long n,
                                float4 *__restrict__ out) {
@@ -877,16 +1055,16 @@ static cudaError_t launch_ff_noalloc(int P, bool zcol, long long ntiles, cudaStr
 
 }  // namespace ppfm
 
-extern "C" int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
-                                       const double *h_R, const double *h_e, const ppfm_lattice *lattice,
-                                       const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
-                                       ppfm_ff_status *d_status, void *cuda_stream) {
-    // the argument checks of ppfm_forcefield (forcefield_impl with nsys = 1, one grid)
-    if (natoms < 0 || !h_R || !h_e || !lattice || !probe || !grid || !d_ff) return PPFM_EINVAL;
-    if (natoms > 0 && (!d_xyzq || !d_type)) return PPFM_EINVAL;
+namespace ppfm {
+// Validation and job description of ONE system on one grid, for the single-system entry points added in round 3
+// (ppfm_forcefield_noalloc, ppfm_forcefield_energy): the checks and the FFJob / per-type table that forcefield_impl
+// builds for nsys = 1, on the caller's stack (no heap).  P and the column mode are chosen as ppfm_forcefield does.
+static int fill_single_job(FFSingle &one, int *P_out, bool *zcol_out, long long *ntiles_out, int32_t natoms,
+                           int32_t ntypes, const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                           const ppfm_probe *probe, const ppfm_grid *grid, double r_min) {
+    if (natoms < 0 || !h_R || !h_e || !lattice || !probe || !grid) return PPFM_EINVAL;
     if (ntypes < 1 || ntypes > PPFM_MAX_TYPES) return PPFM_EINVAL;
     if (!(r_min >= 0.0) || !std::isfinite(r_min)) return PPFM_EINVAL;
-    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_ff & 15) || ((uintptr_t)d_status & 3)) return PPFM_EINVAL;
     for (int t = 0; t < ntypes; t++)
         if (!(h_R[t] >= 0.0) || !(h_e[t] >= 0.0) || !std::isfinite(h_R[t]) || !std::isfinite(h_e[t])) return PPFM_EINVAL;
     if (!grid_ok(grid)) return PPFM_EINVAL;
@@ -895,28 +1073,17 @@ extern "C" int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, cons
         return PPFM_EINVAL;
     for (int a = 0; a < 3; a++)
         if (lattice->nimg[a] < 0 || lattice->nimg[a] > 64) return PPFM_EINVAL;
-    // the one limit this entry point adds: the records must fit the fixed array
-    if (natoms > PPFM_NOALLOC_MAX_ATOMS) return PPFM_ELIMIT;
-
     const ppfm_grid &g = *grid;
     const bool zcol = (g.step[2][0] == 0.0 && g.step[2][1] == 0.0);
     const long long nxy_tiles = ((long long)g.n[0] * g.n[1] + FF_THREADS - 1) / FF_THREADS;
     const int P = zcol ? pick_P(g.n[2], nxy_tiles, false) : 4;      // the choice ppfm_forcefield makes: same bits
-
-    // the system's description travels as a kernel parameter: it lives on this stack frame, not on the heap
-    FFSingle one;
     memset(&one, 0, sizeof(one));
     FFJob &j = one.job;
-    j.tile_begin = 0;
-    j.out_offset = 0;
-    j.atom_begin = 0;
     j.natoms = natoms;
     j.nx = g.n[0]; j.ny = g.n[1]; j.nz = g.n[2]; j.nxy = g.n[0] * g.n[1];
     j.n_xy_tiles = (j.nxy + FF_THREADS - 1) / FF_THREADS;
     j.n_z_groups = (j.nz + P - 1) / P;
-    j.table_offset = 0;
     j.ntypes = ntypes;
-    j.split = 0;
     for (int a = 0; a < 3; a++) {
         j.nimg[a] = lattice->nimg[a];
         j.origin[a] = g.origin[a];
@@ -946,6 +1113,28 @@ extern "C" int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, cons
     }
     const long long ntiles = (long long)j.n_xy_tiles * j.n_z_groups;
     if (ntiles > 0x7fffffffLL) return PPFM_EINVAL;
+    *P_out = P; *zcol_out = zcol; *ntiles_out = ntiles;
+    return PPFM_OK;
+}
+}  // namespace ppfm
+
+extern "C" int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                                       const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                                       const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_ff,
+                                       ppfm_ff_status *d_status, void *cuda_stream) {
+    // the argument checks of ppfm_forcefield (pointers here, the rest in fill_single_job)
+    if (!d_ff || (natoms > 0 && (!d_xyzq || !d_type))) return PPFM_EINVAL;
+    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_ff & 15) || ((uintptr_t)d_status & 3)) return PPFM_EINVAL;
+    FFSingle one;      // the system's description travels as a kernel parameter: it lives on this stack frame
+    int P = 0;
+    bool zcol = true;
+    long long ntiles = 0;
+    {
+        const int rc = fill_single_job(one, &P, &zcol, &ntiles, natoms, ntypes, h_R, h_e, lattice, probe, grid, r_min);
+        if (rc != PPFM_OK) return rc;
+    }
+    // the one limit this entry point adds: the records must fit the fixed array
+    if (natoms > PPFM_NOALLOC_MAX_ATOMS) return PPFM_ELIMIT;
 
     unsigned char *d_scratch = nullptr;
     cudaError_t e = noalloc_scratch_ptr(&d_scratch);
@@ -972,5 +1161,61 @@ extern "C" int ppfm_forcefield_noalloc(int32_t natoms, const float *d_xyzq, cons
         if (e != cudaSuccess) { set_cuda_error(e, "ff_kernel (noalloc)"); return PPFM_ECUDA; }
         count_launch();
     }
+    return PPFM_OK;
+}
+
+// ------------------------------------------------------------------------------------------- (1e) energy-only grid
+// ppfm_forcefield_energy (include/ppfm.h): E = E_LJ + E_C on the grid, float[nz][ny][nx],
+// for ppfm_relax_scan_tricubic.  Set-up (records, flags, scratch) is ppfm_forcefield's; the grid kernel is ffe_kernel.
+extern "C" int ppfm_forcefield_energy(int32_t natoms, const float *d_xyzq, const int32_t *d_type, int32_t ntypes,
+                                      const double *h_R, const double *h_e, const ppfm_lattice *lattice,
+                                      const ppfm_probe *probe, const ppfm_grid *grid, double r_min, float *d_E,
+                                      ppfm_ff_status *d_status, void *cuda_stream) {
+    if (!d_E || (natoms > 0 && (!d_xyzq || !d_type))) return PPFM_EINVAL;
+    if (((uintptr_t)d_xyzq & 15) || ((uintptr_t)d_E & 3) || ((uintptr_t)d_status & 3)) return PPFM_EINVAL;
+    FFSingle one;
+    int P = 0;
+    bool zcol = true;
+    long long ntiles = 0;
+    {
+        const int rc = fill_single_job(one, &P, &zcol, &ntiles, natoms, ntypes, h_R, h_e, lattice, probe, grid, r_min);
+        if (rc != PPFM_OK) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t recs_off = 16;       // [FFFlags, padded to 16 B][AtomRec x natoms]
+    const size_t total_bytes = recs_off + (size_t)(natoms > 0 ? natoms : 1) * sizeof(AtomRec);
+    unsigned char *d_buf = nullptr;
+    cudaError_t e = scratch_alloc((void **)&d_buf, total_bytes, st);
+    if (e != cudaSuccess) { set_cuda_error(e, "scratch_alloc"); return PPFM_ENOMEM; }
+    FFFlags *dflags = reinterpret_cast<FFFlags *>(d_buf);
+    AtomRec *drecs = reinterpret_cast<AtomRec *>(d_buf + recs_off);
+    e = cudaMemsetAsync(dflags, 0, sizeof(FFFlags), st);
+    if (e == cudaSuccess && d_status) e = cudaMemsetAsync(d_status, 0, sizeof(ppfm_ff_status), st);
+    if (e != cudaSuccess) { set_cuda_error(e, "scratch reset"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+    if (natoms > 0) {
+        {
+            KernelTimer kt(PPFM_K_FF_PREP, st);
+            ff_prep_kernel<<<1, PREP_THREADS, 0, st>>>(one, reinterpret_cast<const float4 *>(d_xyzq), d_type, drecs,
+                                                       dflags, d_status);
+        }
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { set_cuda_error(e, "ff_prep_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+        count_launch();
+    }
+    if (ntiles > 0) {
+        const dim3 gridDim3((unsigned)ntiles), block(FF_THREADS);
+        {
+            KernelTimer kt(PPFM_K_FF_ENERGY, st);
+            if (!zcol) ffe_kernel<4, false><<<gridDim3, block, 0, st>>>(one.job, dflags, drecs, d_E);
+            else if (P == 8) ffe_kernel<8, true><<<gridDim3, block, 0, st>>>(one.job, dflags, drecs, d_E);
+            else if (P == 10) ffe_kernel<10, true><<<gridDim3, block, 0, st>>>(one.job, dflags, drecs, d_E);
+            else if (P == 16) ffe_kernel<16, true><<<gridDim3, block, 0, st>>>(one.job, dflags, drecs, d_E);
+            else ffe_kernel<20, true><<<gridDim3, block, 0, st>>>(one.job, dflags, drecs, d_E);
+        }
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { set_cuda_error(e, "ffe_kernel"); cudaFreeAsync(d_buf, st); return PPFM_ECUDA; }
+        count_launch();
+    }
+    PPFM_CUDA(cudaFreeAsync(d_buf, st));
     return PPFM_OK;
 }

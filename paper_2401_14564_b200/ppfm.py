@@ -63,7 +63,7 @@ class Stats(C.Structure):
 
 # the product ABI (include/ppfm.h); the measurement interface of include/ppfm_bench.h is bound in ppfm_bench.py
 EXPORTS = ["ppfm_version", "ppfm_strerror", "ppfm_fire_default", "ppfm_Nm_to_eVA2", "ppfm_forcefield",
-           "ppfm_forcefield_noalloc",
+           "ppfm_forcefield_noalloc", "ppfm_forcefield_energy",
            "ppfm_forcefield_split", "ppfm_combine", "ppfm_forcefield_batch", "ppfm_forcefield_fft",
            "ppfm_forcefield_pauli", "ppfm_relax_scan", "ppfm_relax_scan_batch", "ppfm_relax_scan_sweep", "ppfm_relax_scan_stiffness",
            "ppfm_relax_scan_stiffness_batch", "ppfm_relax_scan_tricubic",
@@ -260,6 +260,23 @@ def forcefield_noalloc(xyzq, types, elem_R, elem_e, lattice, probe, grid, out, r
                                        C.byref(c_lattice(lattice)), C.byref(c_probe(probe, Q)), C.byref(c_grid(grid)),
                                        C.c_double(r_min), _dptr(out, torch.float32), _dptr(status), _stream())
     _check(rc, "ppfm_forcefield_noalloc")
+    return out
+
+
+def forcefield_energy(xyzq, types, elem_R, elem_e, lattice, probe, grid, r_min=0.1, out=None, Q=None, status=None):
+    """ppfm_forcefield_energy: the energy-only grid (nz, ny, nx) float32 CUDA for relax_scan_tricubic — a quarter of
+    the float4 grid's memory, no force arithmetic, FP64 totals per point."""
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in grid.n)
+    if out is None:
+        out = torch.empty((nz, ny, nx), dtype=torch.float32, device=xyzq.device)
+    R, pR = _darr(elem_R)
+    e, pe = _darr(elem_e)
+    rc = lib().ppfm_forcefield_energy(C.c_int32(xyzq.shape[0]), _dptr(xyzq, torch.float32), _dptr(types, torch.int32),
+                                      C.c_int32(len(R)), pR, pe, C.byref(c_lattice(lattice)),
+                                      C.byref(c_probe(probe, Q)), C.byref(c_grid(grid)), C.c_double(r_min),
+                                      _dptr(out, torch.float32), _dptr(status), _stream())
+    _check(rc, "ppfm_forcefield_energy")
     return out
 
 

@@ -12,7 +12,7 @@ PROBES_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libppfm_
 EXPORTS_LIBPPFM = ["ppfm_launch_count", "ppfm_timing_enable", "ppfm_timing_read", "ppfm_checks_read"]
 CHECK_KINDS = ["ring_acquire", "ring_release", "ff_store", "relax_gather", "relax_store", "df_load", "df_store", "visits"]
 EXPORTS_PROBES = ["ppfm_probe_fma", "ppfm_probe_gather"]
-KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6, "relax_tricubic": 7}
+KERNEL_IDS = {"ff_prep": 0, "ff": 1, "combine": 2, "relax": 3, "df": 4, "stiffness": 5, "fft_el": 6, "relax_tricubic": 7, "ff_energy": 8}
 _probes = None
 
 
